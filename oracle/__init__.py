@@ -1,0 +1,163 @@
+"""fp64 CPU oracle for the PKDGRAV3 gravity list-evaluation path -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The arithmetic lives in
+``pkdg_oracle.c`` (plain C, fp64); this file only builds it with gcc and
+marshals numpy arrays through ctypes.  It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from ctypes import POINTER, c_double, c_float, c_int, c_int32, c_int64, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pkdg_oracle.c")
+_LIB = os.path.join(_HERE, "libpkdg_oracle.so")
+TDIM = 13  # ORC_TDIM in pkdg_oracle.c
+
+
+def build(force: bool = False) -> str:
+    """Compile pkdg_oracle.c -> libpkdg_oracle.so (gcc -O2 -fopenmp)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+        )
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        L.orc_num_threads.restype = c_int
+        L.orc_spline.argtypes = [c_double, POINTER(c_double), POINTER(c_double)]
+        L.orc_pp_pair.argtypes = [c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p]
+        L.orc_taylor_coeffs.argtypes = [c_void_p, c_int, c_void_p]
+        L.orc_pc_pair.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+        L.orc_gravity_eval.restype = c_int
+        L.orc_gravity_eval.argtypes = [c_int64, c_void_p, c_int64, c_void_p, c_int32, c_int64,
+                                       c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                                       c_double, c_void_p, c_int64, c_void_p]
+        L.orc_direct_sum.argtypes = [c_int64, c_void_p, c_double, c_void_p, c_int64, c_void_p]
+        L.orc_pack_tiles.restype = c_int64
+        L.orc_pack_tiles.argtypes = [c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.orc_interactions.restype = c_int64
+        L.orc_interactions.argtypes = [c_int64, c_void_p, c_void_p]
+        L.orc_chunk_bounds.restype = c_int64
+        L.orc_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(c_void_p)
+
+
+def _c(a, dtype):
+    if a is None:
+        return None
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def spline(u: float):
+    """(g(u), w(u)) of the cubic-spline softened pair interaction, u = r/h."""
+    g, w = c_double(), c_double()
+    lib().orc_spline(float(u), ctypes.byref(g), ctypes.byref(w))
+    return g.value, w.value
+
+
+def pp_pair(xt, xs, ms: float, eps: float):
+    """Acceleration[3] and potential on a target at xt from one source (xs, ms)."""
+    xt = _c(xt, np.float64); xs = _c(xs, np.float64)
+    acc = np.zeros(3); pot = np.zeros(1)
+    lib().orc_pp_pair(_p(xt), _p(xs), float(ms), float(eps), _p(acc), _p(pot))
+    return acc, float(pot[0])
+
+
+def taylor_coeffs(r, order: int) -> np.ndarray:
+    """Table t[a,b,c] = d^k(1/|r|)/(a!b!c!) for |k| <= order (order <= 12)."""
+    assert 0 <= order <= TDIM - 1
+    r = _c(r, np.float64)
+    t = np.zeros((TDIM, TDIM, TDIM))
+    lib().orc_taylor_coeffs(_p(r), int(order), _p(t))
+    return t
+
+
+def pc_pair(xt, rec):
+    """Acceleration[3] and potential on a target at xt from one canonical 36-float cell record."""
+    xt = _c(xt, np.float64); rec = _c(rec, np.float32)
+    assert rec.size >= 36
+    acc = np.zeros(3); pot = np.zeros(1)
+    lib().orc_pc_pair(_p(xt), _p(rec), _p(acc), _p(pot))
+    return acc, float(pot[0])
+
+
+def gravity_eval(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, sel=None):
+    """The whole path in fp64.  Returns out[n_particles,4] (ax,ay,az,phi); rows of particles that
+    belong to no evaluated bucket are NaN."""
+    xyzm = _c(xyzm, np.float32)
+    n = xyzm.shape[0]
+    if cells is None:
+        cells = np.zeros((0, 36), np.float32)
+    cells = _c(cells, np.float32)
+    stride = cells.shape[1] if cells.ndim == 2 else 36
+    first = _c(first, np.int32); count = _c(count, np.int32)
+    pp_off = _c(pp_off, np.int64); pp_idx = _c(pp_idx, np.int32)
+    pc_off = _c(pc_off, np.int64); pc_idx = _c(pc_idx, np.int32)
+    sel_a = _c(sel, np.int64)
+    out = np.full((n, 4), np.nan)
+    err = lib().orc_gravity_eval(n, _p(xyzm), cells.shape[0], _p(cells), stride, first.shape[0],
+                                 _p(first), _p(count), _p(pp_off), _p(pp_idx), _p(pc_off),
+                                 _p(pc_idx), float(eps), _p(sel_a),
+                                 0 if sel_a is None else sel_a.shape[0], _p(out))
+    if err:
+        raise ValueError("oracle: index out of range in buckets or lists")
+    return out
+
+
+def direct_sum(xyzm, eps, targets=None):
+    """Softened direct summation over all other particles, for the listed targets (default all)."""
+    xyzm = _c(xyzm, np.float32)
+    n = xyzm.shape[0]
+    t = _c(targets, np.int64)
+    nt = n if t is None else t.shape[0]
+    out = np.zeros((nt, 4))
+    lib().orc_direct_sum(n, _p(xyzm), float(eps), _p(t), nt, _p(out))
+    return out
+
+
+def pack_tiles(off, idx):
+    """Packer spec: (tile_off[n_buckets+1] int64, tiles[n_tiles,32] int32 padded with -1)."""
+    off = _c(off, np.int64); idx = _c(idx, np.int32)
+    nb = off.shape[0] - 1
+    tile_off = np.zeros(nb + 1, np.int64)
+    nt = lib().orc_pack_tiles(nb, _p(off), _p(idx), _p(tile_off), None)
+    tiles = np.empty((nt, 32), np.int32)
+    lib().orc_pack_tiles(nb, _p(off), _p(idx), _p(tile_off), _p(tiles))
+    return tile_off, tiles
+
+
+def interactions(count, off) -> int:
+    count = _c(count, np.int32); off = _c(off, np.int64)
+    return int(lib().orc_interactions(count.shape[0], _p(count), _p(off)))
+
+
+def chunk_bounds(pp_off, pc_off, max_entries: int) -> np.ndarray:
+    pp_off = _c(pp_off, np.int64); pc_off = _c(pc_off, np.int64)
+    nb = pp_off.shape[0] - 1
+    bounds = np.zeros(nb + 2, np.int64)
+    nc = lib().orc_chunk_bounds(nb, _p(pp_off), _p(pc_off), int(max_entries), _p(bounds))
+    return bounds[: nc + 1].copy()

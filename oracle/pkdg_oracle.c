@@ -1,0 +1,309 @@
+/*
+ * pkdg_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of what the gravity hot path of PKDGRAV3
+ * (arXiv 1609.08621, /root/reference/PAPER.md) computes: per-bucket evaluation
+ * of particle-particle (P-P) and particle-cell (P-C) interaction lists.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call this file.  It shares no code, header, table
+ * or constant with paper_1609_08621_b200/csrc (the CUDA path).
+ *
+ * The paper prints no formula for either kernel (SURVEY.md preamble); it fixes
+ * the structure: PP for nearby particles, PC = "multipole expansion of the mass
+ * within a more distant cell" (sec 3.1), centre of mass "always
+ * the center of expansions" (L69), "4th order moments" (L71), softening 1/50 of
+ * the mean separation with multipoles only for boxes >= 2 softenings apart
+ * (L69), fp32 inputs and fp64 accumulation (L83).  The formulas below are the
+ * DESIGN.md readings A1-A18; each function cites its own.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): spline closed forms and
+ * quadrature of the spline density; brute-force pairwise sums written in
+ * numpy; momentum conservation; Legendre series of an off-centre point mass;
+ * (b/d)^5 convergence of a cloud's P-C field towards its direct sum; gradient
+ * versus central differences; rotation covariance; trace invariance; tree +
+ * lists versus direct summation; the paper's 655 -> 640 + 15 tile example.
+ * No function here is "parity unpinned".
+ *
+ * No blocking, fusion or reordering: every loop is the definition written out.
+ * OpenMP is used only to run independent buckets on several cores.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_MAXORD 12 /* highest |k| the Taylor-coefficient table can hold */
+#define ORC_TDIM (ORC_MAXORD + 1)
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ---------------------------------------------------------------------------
+ * Softening (readings A1, A2): cubic-spline (Monaghan-Lattanzio) density of
+ * support h = 2*eps; the pair force and potential of a unit mass smeared with
+ * that density (Hernquist & Katz 1989 form), in units u = r/h:
+ *   acceleration factor  g(u):  a_i -= m_j * d * g(u) / h^3,  d = x_i - x_j
+ *   potential factor     w(u):  phi_i += m_j * w(u) / h
+ * For u >= 1 both are exactly Newtonian (1/u^3, -1/u).
+ * ------------------------------------------------------------------------- */
+void orc_spline(double u, double *g, double *w) {
+    double u2 = u * u, u3 = u2 * u;
+    if (u < 0.5) {
+        *g = 32.0 / 3.0 - (192.0 / 5.0) * u2 + 32.0 * u3;
+        *w = (16.0 / 3.0) * u2 - (48.0 / 5.0) * u2 * u2 + (32.0 / 5.0) * u2 * u3 - 14.0 / 5.0;
+    } else if (u < 1.0) {
+        *g = 64.0 / 3.0 - 48.0 * u + (192.0 / 5.0) * u2 - (32.0 / 3.0) * u3 - 1.0 / (15.0 * u3);
+        *w = 1.0 / (15.0 * u) + (32.0 / 3.0) * u2 - 16.0 * u3 + (48.0 / 5.0) * u2 * u2 -
+             (32.0 / 15.0) * u2 * u3 - 16.0 / 5.0;
+    } else {
+        *g = 1.0 / u3;
+        *w = -1.0 / u;
+    }
+}
+
+/* One P-P interaction: contribution of a source (xs, ms) to a target at xt.
+ * Adds to acc[3], pot[1].  G = 1.  ("PP interactions for nearby
+ * particles"; softening L69; readings A1-A4.) */
+void orc_pp_pair(const double xt[3], const double xs[3], double ms, double eps, double acc[3],
+                 double *pot) {
+    double h = 2.0 * eps;
+    double d[3] = {xt[0] - xs[0], xt[1] - xs[1], xt[2] - xs[2]};
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    if (h > 0.0) {
+        double g, w;
+        orc_spline(r / h, &g, &w);
+        double gh3 = g / (h * h * h);
+        acc[0] -= ms * d[0] * gh3;
+        acc[1] -= ms * d[1] * gh3;
+        acc[2] -= ms * d[2] * gh3;
+        *pot += ms * w / h;
+    } else { /* eps == 0: pure Newtonian; coincident distinct particles are the caller's problem */
+        double ir = 1.0 / r;
+        acc[0] -= ms * d[0] * ir * ir * ir;
+        acc[1] -= ms * d[1] * ir * ir * ir;
+        acc[2] -= ms * d[2] * ir * ir * ir;
+        *pot -= ms * ir;
+    }
+}
+
+/* ---------------------------------------------------------------------------
+ * Taylor coefficients of f(r) = 1/|r|:  t_k = (d^k f)/(a! b! c!), k = (a,b,c),
+ * for all |k| <= order, by the recurrence:
+ *   t_0 = 1/|r|
+ *   n |r|^2 t_k + (2n-1) sum_i r_i t_{k-e_i} + (n-1) sum_i t_{k-2e_i} = 0,  n = |k| >= 1
+ * (terms with a negative index are zero).  t is a dense [ORC_TDIM]^3 table,
+ * entry (a,b,c) at t[(a*ORC_TDIM + b)*ORC_TDIM + c]; entries with |k| > order
+ * and every index <= order + 1 are zero, the rest of the table is untouched.
+ * ------------------------------------------------------------------------- */
+#define TIDX(a, b, c) ((((a) * ORC_TDIM) + (b)) * ORC_TDIM + (c))
+
+void orc_taylor_coeffs(const double r[3], int order, double *t) {
+    int zmax = order + 1 < ORC_MAXORD ? order + 1 : ORC_MAXORD; /* zero what a caller may read */
+    for (int a = 0; a <= zmax; ++a)
+        for (int b = 0; b <= zmax; ++b)
+            for (int c = 0; c <= zmax; ++c) t[TIDX(a, b, c)] = 0.0;
+    double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+    t[TIDX(0, 0, 0)] = 1.0 / sqrt(r2);
+    for (int n = 1; n <= order; ++n) {
+        for (int a = n; a >= 0; --a) {
+            for (int b = n - a; b >= 0; --b) {
+                int c = n - a - b;
+                double s1 = 0.0, s2 = 0.0;
+                if (a >= 1) s1 += r[0] * t[TIDX(a - 1, b, c)];
+                if (b >= 1) s1 += r[1] * t[TIDX(a, b - 1, c)];
+                if (c >= 1) s1 += r[2] * t[TIDX(a, b, c - 1)];
+                if (a >= 2) s2 += t[TIDX(a - 2, b, c)];
+                if (b >= 2) s2 += t[TIDX(a, b - 2, c)];
+                if (c >= 2) s2 += t[TIDX(a, b, c - 2)];
+                t[TIDX(a, b, c)] = -((2.0 * n - 1.0) * s1 + (n - 1.0) * s2) / (n * r2);
+            }
+        }
+    }
+}
+
+/* ---------------------------------------------------------------------------
+ * One P-C interaction (readings A4, A5, A9, A12).
+ * Canonical cell record `rec` (36 fp32):
+ *   [0..2] centre of mass, [3] mass, [4..9] raw 2nd moments, [10..19] raw 3rd,
+ *   [20..34] raw 4th, [35] b_max.  M_k = sum_j m_j s^a s^b s^c about the stored
+ *   centre of mass; for each order n the entries run a = n..0, b = n-a..0,
+ *   c = n-a-b.  The dipole is not stored and not used (A9).
+ * With r = x_target - COM and t_k the Taylor coefficients of 1/|r|:
+ *   phi  += - sum_{|k| in {0,2,3,4}} (-1)^{|k|} M_k t_k
+ *   a_l  +=   sum_{|k| in {0,2,3,4}} (-1)^{|k|} M_k (k_l + 1) t_{k+e_l}
+ * i.e. the acceleration is the exact gradient of the truncated potential.
+ * ------------------------------------------------------------------------- */
+void orc_pc_pair(const double xt[3], const float *rec, double acc[3], double *pot) {
+    double r[3] = {xt[0] - (double)rec[0], xt[1] - (double)rec[1], xt[2] - (double)rec[2]};
+    double t[ORC_TDIM * ORC_TDIM * ORC_TDIM];
+    orc_taylor_coeffs(r, 5, t);
+    int pos = 3; /* rec[3] is M_000 */
+    for (int n = 0; n <= 4; ++n) {
+        if (n == 1) continue; /* dipole about the centre of mass: dropped */
+        double sign = (n % 2 == 0) ? 1.0 : -1.0;
+        for (int a = n; a >= 0; --a) {
+            for (int b = n - a; b >= 0; --b) {
+                int c = n - a - b;
+                double M = (double)rec[pos++];
+                *pot -= sign * M * t[TIDX(a, b, c)];
+                acc[0] += sign * M * (a + 1) * t[TIDX(a + 1, b, c)];
+                acc[1] += sign * M * (b + 1) * t[TIDX(a, b + 1, c)];
+                acc[2] += sign * M * (c + 1) * t[TIDX(a, b, c + 1)];
+            }
+        }
+    }
+}
+
+/* ---------------------------------------------------------------------------
+ * The whole path for a set of buckets (SURVEY.md sec 8(c) "Oracle algorithm").
+ * xyzm: [n_particles][4] fp32 (x,y,z,m), tree order.  cells: [n_cells][stride]
+ * fp32 canonical records.  Bucket b holds targets first[b] .. first[b]+count[b].
+ * Lists are CSR: entries off[b] .. off[b+1] of idx.  A P-P source j equal to the
+ * target's own index is skipped BY INDEX (A11).  Negative indices (tile padding)
+ * are skipped.  If `sel` is non-NULL only the n_sel buckets sel[0..n_sel) are
+ * evaluated.  out: [n_particles][4] fp64 (ax, ay, az, phi); only targets of the
+ * evaluated buckets are written.
+ * ------------------------------------------------------------------------- */
+int orc_gravity_eval(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
+                     int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
+                     const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
+                     const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
+                     double *out) {
+    int64_t nb = sel ? n_sel : n_buckets;
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t ib = 0; ib < nb; ++ib) {
+        int64_t b = sel ? sel[ib] : ib;
+        if (b < 0 || b >= n_buckets) {
+#pragma omp atomic write
+                err = 1;
+                continue;
+            }
+        for (int32_t ti = 0; ti < count[b]; ++ti) {
+            int64_t i = (int64_t)first[b] + ti;
+            if (i < 0 || i >= n_particles) {
+#pragma omp atomic write
+                err = 1;
+                continue;
+            }
+            double xt[3] = {xyzm[4 * i], xyzm[4 * i + 1], xyzm[4 * i + 2]};
+            double acc[3] = {0, 0, 0}, pot = 0;
+            if (pp_off) {
+                for (int64_t e = pp_off[b]; e < pp_off[b + 1]; ++e) {
+                    int64_t j = pp_idx[e];
+                    if (j < 0 || j == i) continue;
+                    if (j >= n_particles) {
+#pragma omp atomic write
+                err = 1;
+                continue;
+            }
+                    double xs[3] = {xyzm[4 * j], xyzm[4 * j + 1], xyzm[4 * j + 2]};
+                    orc_pp_pair(xt, xs, (double)xyzm[4 * j + 3], eps, acc, &pot);
+                }
+            }
+            if (pc_off) {
+                for (int64_t e = pc_off[b]; e < pc_off[b + 1]; ++e) {
+                    int64_t c = pc_idx[e];
+                    if (c < 0) continue;
+                    if (c >= n_cells) {
+#pragma omp atomic write
+                err = 1;
+                continue;
+            }
+                    orc_pc_pair(xt, cells + c * (int64_t)stride, acc, &pot);
+                }
+            }
+            out[4 * i + 0] = acc[0];
+            out[4 * i + 1] = acc[1];
+            out[4 * i + 2] = acc[2];
+            out[4 * i + 3] = pot;
+        }
+    }
+    return err;
+}
+
+/* Direct summation: the plain definition the tree method approximates
+ * (PAPER.md:L57).  For each listed target, the softened sum over ALL other
+ * particles.  Used only to pin the oracle (north_star self-checks 1, 3, 4). */
+void orc_direct_sum(int64_t n_particles, const float *xyzm, double eps, const int64_t *targets,
+                    int64_t n_targets, double *out /* [n_targets][4] */) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t it = 0; it < n_targets; ++it) {
+        int64_t i = targets ? targets[it] : it;
+        double xt[3] = {xyzm[4 * i], xyzm[4 * i + 1], xyzm[4 * i + 2]};
+        double acc[3] = {0, 0, 0}, pot = 0;
+        for (int64_t j = 0; j < n_particles; ++j) {
+            if (j == i) continue;
+            double xs[3] = {xyzm[4 * j], xyzm[4 * j + 1], xyzm[4 * j + 2]};
+            orc_pp_pair(xt, xs, (double)xyzm[4 * j + 3], eps, acc, &pot);
+        }
+        out[4 * it + 0] = acc[0];
+        out[4 * it + 1] = acc[1];
+        out[4 * it + 2] = acc[2];
+        out[4 * it + 3] = pot;
+    }
+}
+
+/* ---------------------------------------------------------------------------
+ * Integer side (SURVEY.md sec 8(c) "Integer side"; PAPER.md:L168, L188 fn 11:
+ * lists are cut at warp multiples -- "655 elements ... 640 ... and 15").
+ * Written spec of the packer: per bucket, tiles of 32 entries in list order,
+ * the last tile padded with -1.  tile_off[b] = first tile of bucket b (int64,
+ * [n_buckets+1]); tiles = [n_tiles][32] int32.  Two-call use: tiles == NULL
+ * only fills tile_off and returns the tile count.
+ * ------------------------------------------------------------------------- */
+int64_t orc_pack_tiles(int64_t n_buckets, const int64_t *off, const int32_t *idx, int64_t *tile_off,
+                       int32_t *tiles) {
+    int64_t nt = 0;
+    for (int64_t b = 0; b < n_buckets; ++b) {
+        tile_off[b] = nt;
+        int64_t len = off[b + 1] - off[b];
+        nt += (len + 31) / 32;
+    }
+    tile_off[n_buckets] = nt;
+    if (!tiles) return nt;
+    for (int64_t b = 0; b < n_buckets; ++b) {
+        int64_t len = off[b + 1] - off[b];
+        int64_t ntile = (len + 31) / 32;
+        for (int64_t k = 0; k < ntile * 32; ++k)
+            tiles[tile_off[b] * 32 + k] = (k < len) ? idx[off[b] + k] : -1;
+    }
+    return nt;
+}
+
+/* Interaction counts: I = sum_b count[b] * len[b] (SURVEY.md sec 8 notation). */
+int64_t orc_interactions(int64_t n_buckets, const int32_t *count, const int64_t *off) {
+    int64_t I = 0;
+    for (int64_t b = 0; b < n_buckets; ++b) I += (int64_t)count[b] * (off[b + 1] - off[b]);
+    return I;
+}
+
+/* Chunk boundaries for the streamed variant: greedy fill in bucket order; a
+ * chunk is closed before the bucket that would push its P-P or its P-C entry
+ * count above max_entries (a single bucket longer than max_entries gets a chunk
+ * of its own).  bounds[0] = 0, bounds[n_chunks] = n_buckets; returns n_chunks.
+ * bounds must have room for n_buckets + 1 values. */
+int64_t orc_chunk_bounds(int64_t n_buckets, const int64_t *pp_off, const int64_t *pc_off,
+                         int64_t max_entries, int64_t *bounds) {
+    int64_t nc = 0, b0 = 0;
+    bounds[0] = 0;
+    if (n_buckets == 0) return 0;
+    for (int64_t b = 0; b < n_buckets; ++b) {
+        int64_t pp = pp_off[b + 1] - pp_off[b0];
+        int64_t pc = pc_off[b + 1] - pc_off[b0];
+        if ((pp > max_entries || pc > max_entries) && b > b0) {
+            bounds[++nc] = b;
+            b0 = b;
+        }
+    }
+    bounds[++nc] = n_buckets;
+    return nc;
+}
