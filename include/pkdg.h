@@ -1,0 +1,162 @@
+/*
+ * pkdg.h -- C ABI of pkdg-b200: per-bucket evaluation of gravity interaction lists on one
+ * NVIDIA B200 (sm_100a), after PKDGRAV3 (Potter, Stadel & Teyssier, arXiv 1609.08621).
+ *
+ * Problem statement: leaf cells ("buckets") hold up to
+ * b ~ 16 sink particles; the tree walk gives every sink a P-P list of source particles and a
+ * P-C list of source cells whose multipole moments (to 4th order, about the cell's centre of
+ * mass) stand for their mass; evaluating the lists gives the acceleration and the potential of
+ * every sink particle.  The paper runs exactly this on the GPU (sec 3.3).  The formulas are not
+ * printed in the paper; DESIGN.md (readings A1-A18) fixes them:
+ *
+ *   P-P: d = x_i - x_j, h = 2 eps, u = |d|/h; a_i -= m_j d g(u)/h^3, phi_i += m_j w(u)/h, with
+ *        g, w of the cubic-spline softened pair (exactly Newtonian for |d| >= 2 eps).  A source
+ *        whose INDEX equals the sink's index is skipped; distinct coincident particles interact.
+ *   P-C: r = x_i - COM_c; phi_i += - sum_{|k| in {0,2,3,4}} (-1)^|k| M_k t_k(r), a_i = -grad of
+ *        that truncated potential, t_k = d^k(1/|r|)/k!; unsoftened; dipole dropped.
+ *
+ * Conventions.  G = 1.  Every pointer is a DEVICE pointer unless its name ends in _host.  The
+ * caller owns every buffer; the library never frees, reallocates or retains caller memory after
+ * the work queued by a call has completed.  Calls are asynchronous on `stream` (a cudaStream_t
+ * passed as void*; NULL = the legacy default stream) unless stated; no exception crosses the
+ * ABI; every function returns a pkdg_status (0 = OK, < 0 = error) and pkdg_last_error() gives
+ * the text.  A pkdg_ctx may be used by one host thread at a time.
+ */
+#ifndef PKDG_H
+#define PKDG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PKDG_VERSION_MAJOR 0
+#define PKDG_VERSION_MINOR 1
+
+#define PKDG_TILE 32          /* list entries per tile = lanes per warp */
+#define PKDG_CELL_FLOATS 36   /* canonical cell record, see pkdg_cells */
+#define PKDG_PAD (-1)         /* index that pads the last tile of a list */
+
+typedef int32_t pkdg_status;
+#define PKDG_OK 0
+#define PKDG_EINVAL (-1)   /* null pointer, negative size, bad stride, misaligned buffer */
+#define PKDG_ECUDA (-2)    /* a CUDA runtime call failed; text in pkdg_last_error() */
+#define PKDG_ENOMEM (-3)   /* workspace allocation failed */
+#define PKDG_EBADLIST (-4) /* validation found a non-monotone offset, an index out of range or a
+                              negative bucket count (only reported by pkdg_get_stats) */
+
+/* flags of pkdg_gravity_eval* */
+#define PKDG_ACCUMULATE 0x1u /* add to out instead of overwriting it */
+#define PKDG_SKIP_PP 0x2u    /* ignore the P-P lists (kernel studies) */
+#define PKDG_SKIP_PC 0x4u    /* ignore the P-C lists */
+#define PKDG_VARIANT_SHIFT 8 /* bits 8..15: kernel tuning variant, 0 = library default */
+
+typedef struct pkdg_ctx pkdg_ctx;
+
+/* Sink and source particles, tree order (buckets are contiguous runs).  xyzm = [n][4] fp32
+ * (x, y, z, mass), 16-byte aligned.  ("hierarchically sorted order"; L83 fp32.) */
+typedef struct { const float *xyzm; int64_t n; } pkdg_particles;
+
+/* Source cells.  rec = [n][stride_floats] fp32, stride_floats >= 36.  Canonical record:
+ * [0..2] centre of mass (the centre of expansion), [3] mass, [4..9] 2nd, [10..19]
+ * 3rd, [20..34] 4th raw moments M_k = sum_j m_j s_x^a s_y^b s_z^c about that centre, for each
+ * order n in the sequence a = n..0, b = n-a..0, c = n-a-b (n = 2: xx xy xz yy yz zz), [35] b_max,
+ * the distance from the centre to the farthest particle (used only as the length
+ * scale of the internal normalised form; <= 0 means "derive a scale from the 2nd moments"). */
+typedef struct { const float *rec; int64_t n; int32_t stride_floats; } pkdg_cells;
+
+/* Buckets: sinks first[b] .. first[b]+count[b]-1.  count >= 0 (tuned for <= 16).
+ * Buckets must not overlap unless PKDG_ACCUMULATE semantics are not needed. */
+typedef struct { const int32_t *first; const int32_t *count; int64_t n; } pkdg_buckets;
+
+/* A CSR interaction list: entries offsets[b] .. offsets[b+1]-1 of idx belong to bucket b
+ * (offsets has n_buckets+1 int64 values, offsets[0] may be non-zero).  idx < 0 is padding and
+ * is ignored.  A NULL pkdg_list* or NULL offsets means "no list of this kind". */
+typedef struct { const int64_t *offsets; const int32_t *idx; } pkdg_list;
+
+/* Counters of the last evaluation on a context (pkdg_get_stats synchronises the stream). */
+typedef struct {
+    int64_t n_buckets;
+    int64_t interactions_pp; /* I_pp = sum_b count[b] * len_pp[b]  (padding entries included)  */
+    int64_t interactions_pc; /* I_pc = sum_b count[b] * len_pc[b]                                */
+    int64_t tiles_pp;        /* sum_b ceil(len_pp[b] / 32)                                       */
+    int64_t tiles_pc;
+    int64_t bad_entries;     /* validation failures (0 when the input is well-formed)            */
+    int64_t chunks;          /* streamed variants: number of chunks issued, else 1              */
+} pkdg_stats;
+
+/* Create / destroy a context on CUDA device `device`.  The context owns only internal workspace
+ * (normalised cell records, bucket descriptors, counters, staging buffers); it grows on demand
+ * (the first call with a larger problem allocates and is therefore synchronous). */
+pkdg_status pkdg_create(pkdg_ctx **ctx, int device);
+pkdg_status pkdg_destroy(pkdg_ctx *ctx);
+
+/* One pass of the whole hot path with everything resident on the device:
+ *   a1 packer       bucket work descriptors, tile counts, validation, I_pp / I_pc
+ *   (cell prep)     canonical raw-moment records -> internal normalised trace-free records
+ *   a2 staging, a3 P-P, a4 P-C, a5 reduction + write-back: one fused kernel, one warp per bucket
+ * out_acc_pot = [particles->n][4] fp32 (ax, ay, az, phi), 16-byte aligned.  Rows of particles in a
+ * listed bucket are overwritten (added to with PKDG_ACCUMULATE); other rows are untouched.
+ * No host synchronisation once the workspace is large enough. */
+pkdg_status pkdg_gravity_eval(pkdg_ctx *ctx, const pkdg_particles *particles, const pkdg_cells *cells,
+                              const pkdg_buckets *buckets, const pkdg_list *pp, const pkdg_list *pc,
+                              float eps, uint32_t flags, float *out_acc_pot, void *stream);
+
+/* Streamed variant (a6; "fully asynchronous", L278 bounded queue): particles, cells
+ * and out are device buffers, buckets and lists are PINNED HOST buffers.  Contiguous bucket ranges
+ * ("chunks", greedy fill to at most max_entries_per_chunk P-P and P-C entries; a longer single
+ * bucket forms its own chunk) are copied host->device and evaluated round-robin on n_streams
+ * internal streams; at most n_streams chunks are in flight.  Returns after the last chunk has been
+ * queued; `stream` waits for all of them. */
+pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx *ctx, const pkdg_particles *particles,
+                                       const pkdg_cells *cells, const pkdg_buckets *buckets_host,
+                                       const pkdg_list *pp_host, const pkdg_list *pc_host, float eps,
+                                       uint32_t flags, float *out_acc_pot, int32_t n_streams,
+                                       int64_t max_entries_per_chunk, void *stream);
+
+/* End-to-end variant: EVERY buffer is a host buffer (pinned for full speed).  Copies particles and
+ * cells to the device, streams the lists as above, copies the result back into out_acc_pot_host and
+ * synchronises before returning.  Rows of particles in no bucket come back as 0 (as the caller's
+ * values with PKDG_ACCUMULATE). */
+pkdg_status pkdg_gravity_eval_host(pkdg_ctx *ctx, const pkdg_particles *particles_host,
+                                   const pkdg_cells *cells_host, const pkdg_buckets *buckets_host,
+                                   const pkdg_list *pp_host, const pkdg_list *pc_host, float eps,
+                                   uint32_t flags, float *out_acc_pot_host, int32_t n_streams,
+                                   int64_t max_entries_per_chunk);
+
+/* Packer made visible for bit-exact checks (SURVEY.md sec 8(c) "Integer side"): the tiles the
+ * evaluation kernel consumes.  tile_offsets = [n_buckets+1] int64 (first tile of each bucket);
+ * tiles = [tile_capacity][32] int32, list order, last tile of a bucket padded with PKDG_PAD.
+ * Either output may be NULL.  If the list needs more than tile_capacity tiles only tile_offsets is
+ * complete (tile_offsets[n_buckets] is the number needed). */
+pkdg_status pkdg_pack_export(pkdg_ctx *ctx, int64_t n_buckets, const pkdg_list *list,
+                             int64_t *tile_offsets, int32_t *tiles, int64_t tile_capacity, void *stream);
+
+/* Chunk boundaries the streamed variants use, from HOST offsets: bounds_host gets n_chunks+1
+ * values (room for n_buckets+1); *n_chunks_host the count.  Pure host code. */
+pkdg_status pkdg_chunk_bounds(int64_t n_buckets, const int64_t *pp_offsets_host,
+                              const int64_t *pc_offsets_host, int64_t max_entries_per_chunk,
+                              int64_t *bounds_host, int64_t *n_chunks_host);
+
+/* Internal normalised cell records made visible for tests: out = [cells->n][32] fp32. */
+pkdg_status pkdg_prepare_cells_export(pkdg_ctx *ctx, const pkdg_cells *cells, float *out, void *stream);
+
+/* Synchronises the stream(s) of the last evaluation and returns its counters. */
+pkdg_status pkdg_get_stats(pkdg_ctx *ctx, pkdg_stats *stats_host);
+
+/* Number of kernel launches this context has made since creation. */
+int64_t pkdg_launch_count(const pkdg_ctx *ctx);
+
+const char *pkdg_status_string(pkdg_status s);
+const char *pkdg_last_error(const pkdg_ctx *ctx);
+void pkdg_version(int32_t *major, int32_t *minor);
+
+/* FP32 FFMA-only micro-benchmark (roofline denominator check): runs `iters` dependent-chain-free
+ * FFMA rounds on every SM and returns the elapsed milliseconds and the flop count. Synchronous. */
+pkdg_status pkdg_fma_peak_probe(pkdg_ctx *ctx, int64_t iters, float *ms_host, double *flops_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PKDG_H */

@@ -1,0 +1,245 @@
+"""Thin ctypes binding over the C ABI of include/pkdg.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libpkdg.so; there is no Python or CPU
+fallback: importing this module raises if the library has not been built
+(``python -m paper_1609_08621_b200.build``) and every call raises ``PkdgError`` on a non-zero
+status.  Device buffers are torch CUDA tensors (torch is used for memory and streams only),
+host buffers are numpy arrays or pinned CPU tensors.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_float, c_int, c_int32, c_int64, c_uint32, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpkdg.so")
+
+ACCUMULATE = 0x1
+SKIP_PP = 0x2
+SKIP_PC = 0x4
+VARIANT_SHIFT = 8
+CELL_FLOATS = 36
+CELLQ_FLOATS = 32
+
+EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_streamed",
+           "pkdg_gravity_eval_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
+           "pkdg_get_stats", "pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version",
+           "pkdg_fma_peak_probe"]
+
+
+class PkdgError(RuntimeError):
+    pass
+
+
+class _Particles(Structure):
+    _fields_ = [("xyzm", c_void_p), ("n", c_int64)]
+
+
+class _Cells(Structure):
+    _fields_ = [("rec", c_void_p), ("n", c_int64), ("stride_floats", c_int32)]
+
+
+class _Buckets(Structure):
+    _fields_ = [("first", c_void_p), ("count", c_void_p), ("n", c_int64)]
+
+
+class _List(Structure):
+    _fields_ = [("offsets", c_void_p), ("idx", c_void_p)]
+
+
+class Stats(Structure):
+    _fields_ = [("n_buckets", c_int64), ("interactions_pp", c_int64), ("interactions_pc", c_int64),
+                ("tiles_pp", c_int64), ("tiles_pc", c_int64), ("bad_entries", c_int64), ("chunks", c_int64)]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise PkdgError(f"{LIB_PATH} is missing: build it with `python -m paper_1609_08621_b200.build` "
+                        "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    L.pkdg_create.argtypes = [POINTER(c_void_p), c_int]
+    L.pkdg_destroy.argtypes = [c_void_p]
+    L.pkdg_gravity_eval.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                    POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_void_p]
+    L.pkdg_gravity_eval_streamed.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                             POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p,
+                                             c_int32, c_int64, c_void_p]
+    L.pkdg_gravity_eval_host.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                         POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_int32,
+                                         c_int64]
+    L.pkdg_pack_export.argtypes = [c_void_p, c_int64, POINTER(_List), c_void_p, c_void_p, c_int64, c_void_p]
+    L.pkdg_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int64)]
+    L.pkdg_prepare_cells_export.argtypes = [c_void_p, POINTER(_Cells), c_void_p, c_void_p]
+    L.pkdg_get_stats.argtypes = [c_void_p, POINTER(Stats)]
+    L.pkdg_launch_count.argtypes = [c_void_p]
+    L.pkdg_launch_count.restype = c_int64
+    L.pkdg_status_string.argtypes = [c_int32]
+    L.pkdg_status_string.restype = c_char_p
+    L.pkdg_last_error.argtypes = [c_void_p]
+    L.pkdg_last_error.restype = c_char_p
+    L.pkdg_version.argtypes = [POINTER(c_int32), POINTER(c_int32)]
+    L.pkdg_fma_peak_probe.argtypes = [c_void_p, c_int64, POINTER(c_float), POINTER(c_double)]
+    for name in EXPORTS:
+        if name not in ("pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version"):
+            getattr(L, name).restype = c_int32
+    return L
+
+
+_lib = _load()
+
+
+def lib():
+    return _lib
+
+
+def version():
+    a, b = c_int32(), c_int32()
+    _lib.pkdg_version(byref(a), byref(b))
+    return a.value, b.value
+
+
+def status_string(s: int) -> str:
+    return _lib.pkdg_status_string(int(s)).decode()
+
+
+def _ptr(a):
+    """Address of a torch tensor (any device) or a numpy array; None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise PkdgError("numpy buffers must be C-contiguous")
+        return a.ctypes.data
+    if not a.is_contiguous():
+        raise PkdgError("tensors must be contiguous")
+    return a.data_ptr()
+
+
+def _dt(a, want, name):
+    if a is None:
+        return
+    got = str(a.dtype).replace("torch.", "")
+    if got != want:
+        raise PkdgError(f"{name}: dtype {got}, expected {want}")
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def chunk_bounds(pp_off, pc_off, max_entries: int) -> np.ndarray:
+    """Chunk boundaries of the streamed variants from HOST offsets (pkdg_chunk_bounds)."""
+    ref = pp_off if pp_off is not None else pc_off
+    nb = int(ref.shape[0]) - 1
+    bounds = np.zeros(nb + 2, np.int64)
+    n = c_int64()
+    s = _lib.pkdg_chunk_bounds(nb, _ptr(pp_off), _ptr(pc_off), int(max_entries), bounds.ctypes.data, byref(n))
+    if s != 0:
+        raise PkdgError(status_string(s))
+    return bounds[: n.value + 1].copy()
+
+
+class Context:
+    """A pkdg_ctx: owns internal workspace only (pkdg_create / pkdg_destroy)."""
+
+    def __init__(self, device: int = 0):
+        self._h = c_void_p()
+        s = _lib.pkdg_create(byref(self._h), int(device))
+        if s != 0:
+            self._h = c_void_p()
+            raise PkdgError(f"pkdg_create: {status_string(s)}")
+        self.device = device
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
+            _lib.pkdg_destroy(self._h)
+            self._h = c_void_p()
+
+    __del__ = close
+
+    def _check(self, s, what):
+        if s != 0:
+            raise PkdgError(f"{what}: {status_string(s)}: {_lib.pkdg_last_error(self._h).decode()}")
+
+    @staticmethod
+    def _structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx):
+        _dt(xyzm, "float32", "xyzm"); _dt(cells, "float32", "cells"); _dt(first, "int32", "first")
+        _dt(count, "int32", "count"); _dt(pp_off, "int64", "pp_off"); _dt(pp_idx, "int32", "pp_idx")
+        _dt(pc_off, "int64", "pc_off"); _dt(pc_idx, "int32", "pc_idx")
+        P = _Particles(_ptr(xyzm), int(xyzm.shape[0]))
+        C = None
+        if cells is not None:
+            C = _Cells(_ptr(cells), int(cells.shape[0]), int(cells.shape[1]) if cells.ndim == 2 else CELL_FLOATS)
+        B = _Buckets(_ptr(first), _ptr(count), int(first.shape[0]))
+        pp = _List(_ptr(pp_off), _ptr(pp_idx)) if pp_off is not None else None
+        pc = _List(_ptr(pc_off), _ptr(pc_idx)) if pc_off is not None else None
+        return P, C, B, pp, pc
+
+    def gravity_eval(self, xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, out, flags=0,
+                     stream=None):
+        """pkdg_gravity_eval: everything resident on the device; asynchronous on `stream`."""
+        P, C, B, pp, pc = self._structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx)
+        _dt(out, "float32", "out")
+        s = _lib.pkdg_gravity_eval(self._h, byref(P), byref(C) if C else None, byref(B), byref(pp) if pp else None,
+                                   byref(pc) if pc else None, float(eps), int(flags), _ptr(out), _stream_ptr(stream))
+        self._check(s, "pkdg_gravity_eval")
+        return out
+
+    def gravity_eval_streamed(self, xyzm, cells, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h, eps, out,
+                              n_streams=3, max_entries_per_chunk=1 << 24, flags=0, stream=None):
+        """pkdg_gravity_eval_streamed: device particles/cells/out, HOST buckets and lists."""
+        P, C, B, pp, pc = self._structs(xyzm, cells, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h)
+        s = _lib.pkdg_gravity_eval_streamed(self._h, byref(P), byref(C) if C else None, byref(B),
+                                            byref(pp) if pp else None, byref(pc) if pc else None, float(eps),
+                                            int(flags), _ptr(out), int(n_streams), int(max_entries_per_chunk),
+                                            _stream_ptr(stream))
+        self._check(s, "pkdg_gravity_eval_streamed")
+        return out
+
+    def gravity_eval_host(self, xyzm_h, cells_h, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h, eps,
+                          out_h, n_streams=3, max_entries_per_chunk=1 << 24, flags=0):
+        """pkdg_gravity_eval_host: every buffer on the host; synchronous."""
+        P, C, B, pp, pc = self._structs(xyzm_h, cells_h, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h)
+        s = _lib.pkdg_gravity_eval_host(self._h, byref(P), byref(C) if C else None, byref(B),
+                                        byref(pp) if pp else None, byref(pc) if pc else None, float(eps), int(flags),
+                                        _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
+        self._check(s, "pkdg_gravity_eval_host")
+        return out_h
+
+    def pack_export(self, n_buckets, off, idx, tile_offsets, tiles, stream=None):
+        """pkdg_pack_export: tile_offsets[n_buckets+1] int64 and tiles[cap,32] int32 (device)."""
+        L = _List(_ptr(off), _ptr(idx))
+        cap = 0 if tiles is None else int(tiles.shape[0])
+        s = _lib.pkdg_pack_export(self._h, int(n_buckets), byref(L), _ptr(tile_offsets), _ptr(tiles), cap,
+                                  _stream_ptr(stream))
+        self._check(s, "pkdg_pack_export")
+
+    def prepare_cells_export(self, cells, out, stream=None):
+        C = _Cells(_ptr(cells), int(cells.shape[0]), int(cells.shape[1]))
+        s = _lib.pkdg_prepare_cells_export(self._h, byref(C), _ptr(out), _stream_ptr(stream))
+        self._check(s, "pkdg_prepare_cells_export")
+        return out
+
+    def get_stats(self, check: bool = True) -> dict:
+        st = Stats()
+        s = _lib.pkdg_get_stats(self._h, byref(st))
+        if check:
+            self._check(s, "pkdg_get_stats")
+        return st.as_dict()
+
+    def launch_count(self) -> int:
+        return int(_lib.pkdg_launch_count(self._h))
+
+    def fma_peak_probe(self, iters: int = 1 << 14):
+        ms, fl = c_float(), c_double()
+        self._check(_lib.pkdg_fma_peak_probe(self._h, int(iters), byref(ms), byref(fl)), "pkdg_fma_peak_probe")
+        return ms.value, fl.value

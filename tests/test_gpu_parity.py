@@ -1,0 +1,268 @@
+"""-m gpu parity tests: the CUDA path, called through the C ABI, against the fp64 oracle on the
+same seeded inputs.  Bars (BASELINE.json north_star): integer work bit-exact; per-particle
+|a_gpu - a_or|/|a_or| <= 2e-5 and |phi_gpu - phi_or|/|phi_or| <= 2e-5."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5
+VARIANTS = [0, 1 << 8, 2 << 8, 3 << 8]
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch):
+    from paper_1609_08621_b200 import binding
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _oracle(p, sel=None):
+    import oracle
+    return oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
+
+
+@pytest.mark.parametrize("flags", VARIANTS)
+def test_config1_full_parity(ctx, torch, cfg1, flags):
+    """configs[0]: N = 4096 uniform, octree, theta = 0.7 -- every particle against the oracle."""
+    from gpu_util import rel_errors, run_resident
+    ref = _oracle(cfg1)
+    out = run_resident(ctx, cfg1, torch, flags=flags)
+    ea, ep = rel_errors(out, ref)
+    assert np.isfinite(out).all()
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+    st = ctx.get_stats()
+    import oracle
+    assert st["interactions_pp"] == oracle.interactions(cfg1.count, cfg1.pp_off) == cfg1.I_pp
+    assert st["interactions_pc"] == oracle.interactions(cfg1.count, cfg1.pc_off) == cfg1.I_pc
+    assert st["bad_entries"] == 0 and st["n_buckets"] == cfg1.n_buckets
+
+
+def test_pp_only_and_pc_only_sum_to_full(ctx, torch, cfg1):
+    from paper_1609_08621_b200 import binding
+    from gpu_util import rel_errors, run_resident
+    import oracle
+    p = cfg1
+    ref_pp = oracle.gravity_eval(p.xyzm, None, p.first, p.count, p.pp_off, p.pp_idx, None, None, p.eps)
+    ref_pc = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, None, None, p.pc_off, p.pc_idx, p.eps)
+    out_pp = run_resident(ctx, p, torch, flags=binding.SKIP_PC)
+    out_pc = run_resident(ctx, p, torch, flags=binding.SKIP_PP)
+    for out, ref in ((out_pp, ref_pp), (out_pc, ref_pc)):
+        ea, ep = rel_errors(out, ref)
+        assert ea.max() <= TOL and ep.max() <= TOL
+
+
+def test_accumulate_flag_adds(ctx, torch, cfg1):
+    from paper_1609_08621_b200 import binding
+    from gpu_util import run_resident
+    base = run_resident(ctx, cfg1, torch)
+    acc = run_resident(ctx, cfg1, torch, flags=binding.ACCUMULATE, fill=1.0)
+    assert np.allclose(acc, base + 1.0, rtol=1e-6, atol=1e-6)
+
+
+def test_pack_export_bit_exact(ctx, torch, cfg1):
+    """a1: tiles and tile offsets equal the oracle's packer spec bit for bit (list order kept)."""
+    import oracle
+    for off, idx in ((cfg1.pp_off, cfg1.pp_idx), (cfg1.pc_off, cfg1.pc_idx)):
+        tile_off, tiles = oracle.pack_tiles(off, idx)
+        d_off = torch.from_numpy(off).cuda(); d_idx = torch.from_numpy(idx).cuda()
+        g_off = torch.zeros(off.shape[0], dtype=torch.int64, device="cuda")
+        g_tiles = torch.full((tiles.shape[0] + 3, 32), -7, dtype=torch.int32, device="cuda")
+        ctx.pack_export(off.shape[0] - 1, d_off, d_idx, g_off, g_tiles)
+        torch.cuda.synchronize()
+        assert np.array_equal(g_off.cpu().numpy(), tile_off)
+        assert np.array_equal(g_tiles.cpu().numpy()[: tiles.shape[0]], tiles)
+        assert np.all(g_tiles.cpu().numpy()[tiles.shape[0]:] == -7)
+
+
+def test_pack_export_ragged_empty_and_paper_example(ctx, torch):
+    import oracle
+    lens = [0, 1, 31, 32, 33, 655, 0, 64, 0]
+    off = np.concatenate([[5], 5 + np.cumsum(lens)]).astype(np.int64)      # offsets[0] != 0
+    idx = (np.arange(off[-1], dtype=np.int64) * 7 % 1000).astype(np.int32)
+    tile_off, tiles = oracle.pack_tiles(off, idx)
+    g_off = torch.zeros(off.shape[0], dtype=torch.int64, device="cuda")
+    g_tiles = torch.zeros((tiles.shape[0], 32), dtype=torch.int32, device="cuda")
+    ctx.pack_export(len(lens), torch.from_numpy(off).cuda(), torch.from_numpy(idx).cuda(), g_off, g_tiles)
+    torch.cuda.synchronize()
+    assert np.array_equal(g_off.cpu().numpy(), tile_off) and np.array_equal(g_tiles.cpu().numpy(), tiles)
+    assert tile_off[6] - tile_off[5] == 21                                 # 655 -> 20 full tiles + 15
+    # capacity too small: offsets still complete
+    g_off.zero_()
+    ctx.pack_export(len(lens), torch.from_numpy(off).cuda(), torch.from_numpy(idx).cuda(), g_off, g_tiles[:3].contiguous())
+    torch.cuda.synchronize()
+    assert np.array_equal(g_off.cpu().numpy(), tile_off)
+
+
+def _edge_problem():
+    """Ragged and degenerate buckets: empty bucket, empty lists, counts 1, 17 and 27 (> 16), padding
+    entries, a coincident pair, softened neighbours, list lengths around the tile size."""
+    from paper_1609_08621_b200 import inputs
+    rng = np.random.default_rng(42)
+    counts = [0, 1, 16, 17, 27, 3, 8, 5]
+    n_t = sum(counts)
+    n_src = 700
+    xyzm = np.empty((n_t + n_src, 4), np.float32)
+    xyzm[:n_t, :3] = 0.5 + 0.01 * rng.standard_normal((n_t, 3))
+    xyzm[n_t:, :3] = rng.random((n_src, 3))
+    xyzm[:, 3] = rng.uniform(0.5, 1.5, n_t + n_src) / (n_t + n_src)
+    xyzm[3, :3] = xyzm[2, :3]                                           # coincident distinct particles
+    first = np.concatenate([[0], np.cumsum(counts)[:-1]]).astype(np.int32)
+    count = np.array(counts, np.int32)
+    pp_lens = [40, 0, 33, 64, 700 + n_t, 31, 1, 0]
+    pp = []
+    for b, L in enumerate(pp_lens):
+        own = np.arange(first[b], first[b] + count[b])
+        if L >= n_src + n_t:
+            l = np.arange(n_t + n_src)
+        else:
+            l = np.concatenate([own, n_t + rng.choice(n_src, max(L - own.size, 0), replace=False)])[:L]
+        l = l.astype(np.int32)
+        if b == 2:
+            l[5] = -1                                                   # padding inside a list is ignored
+        pp.append(l)
+    pp_off = np.concatenate([[0], np.cumsum([len(l) for l in pp])]).astype(np.int64)
+    pp_idx = np.concatenate(pp).astype(np.int32)
+    # cells: clouds well away from the targets
+    ncell = 150
+    com = 0.5 + rng.choice([-1, 1], (ncell, 3)) * rng.uniform(0.15, 0.45, (ncell, 3))
+    pts = np.empty((ncell * 20, 4), np.float32)
+    pts[:, :3] = np.repeat(com, 20, axis=0) + 0.02 * rng.standard_normal((ncell * 20, 3))
+    pts[:, 3] = rng.uniform(0.5, 1.5, ncell * 20) / (ncell * 20)
+    cells = inputs.cloud_records(pts, 20)
+    cells[7, 35] = 0.0                                                  # b_max <= 0: scale from 2nd moments
+    cells[9, 4:35] = 0.0                                                # pure monopole cell
+    pc_lens = [0, 150, 32, 31, 65, 1, 150, 0]
+    pc = [rng.choice(ncell, L, replace=False).astype(np.int32) for L in pc_lens]
+    pc_off = np.concatenate([[0], np.cumsum(pc_lens)]).astype(np.int64)
+    pc_idx = np.concatenate(pc).astype(np.int32)
+    return inputs.Problem(name="edge", xyzm=xyzm, cells=cells, first=first, count=count, pp_off=pp_off,
+                          pp_idx=pp_idx, pc_off=pc_off, pc_idx=pc_idx, eps=0.004)
+
+
+@pytest.mark.parametrize("flags", VARIANTS)
+def test_edge_cases(ctx, torch, flags):
+    from gpu_util import rel_errors, run_resident
+    p = _edge_problem()
+    ref = _oracle(p)
+    out = run_resident(ctx, p, torch, flags=flags)
+    rows = np.arange(int(p.first[7]))                                   # bucket 7 has no lists at all
+    ea, ep = rel_errors(out, ref, rows)
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+    lone = out[p.first[7]: p.first[7] + p.count[7]]
+    assert np.all(lone == 0.0) and np.all(ref[p.first[7]: p.first[7] + p.count[7]] == 0.0)   # overwritten with 0
+    assert np.isnan(out[int(p.count.sum()):]).all()                     # particles in no bucket: untouched
+    assert ctx.get_stats()["bad_entries"] == 0
+
+
+def test_softened_plummer_cores(ctx, torch):
+    """configs[1] recipe at N = 2^15: dense Plummer cores put many pairs inside the spline."""
+    from paper_1609_08621_b200 import inputs
+    from gpu_util import rel_errors, run_resident
+    p = inputs.config2(n=1 << 15)
+    ref = _oracle(p)
+    out = run_resident(ctx, p, torch)
+    ea, ep = rel_errors(out, ref)
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+
+
+def test_out_of_range_indices_are_reported_not_followed(ctx, torch, cfg1):
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import run_resident
+    import copy
+    p = copy.copy(cfg1)
+    p.pp_idx = cfg1.pp_idx.copy(); p.pc_idx = cfg1.pc_idx.copy()
+    p.pp_idx[10] = cfg1.n + 5
+    p.pc_idx[3] = cfg1.cells.shape[0]
+    run_resident(ctx, p, torch)
+    with pytest.raises(binding.PkdgError):
+        ctx.get_stats()
+    assert ctx.get_stats(check=False)["bad_entries"] >= 2
+
+
+def test_invalid_arguments_fail_loudly(ctx, torch, cfg1):
+    from paper_1609_08621_b200 import binding
+    from gpu_util import to_dev
+    d = to_dev(cfg1, torch)
+    out = torch.zeros((cfg1.n, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.PkdgError):
+        ctx.gravity_eval(d["xyzm"], d["cells"][:, :20].contiguous(), d["first"], d["count"], d["pp_off"], d["pp_idx"],
+                         d["pc_off"], d["pc_idx"], cfg1.eps, out)
+    with pytest.raises(binding.PkdgError):
+        ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"],
+                         d["pc_idx"], cfg1.eps, out, flags=200 << 8)
+
+
+def test_streamed_and_host_variants_match_resident(ctx, torch, cfg1):
+    """a6: chunked evaluation from host lists gives the same bits as the resident call."""
+    from paper_1609_08621_b200 import binding
+    from gpu_util import run_resident, to_dev
+    import oracle
+    p = cfg1
+    base = run_resident(ctx, p, torch)
+    d = to_dev(p, torch)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h = dict(first=pin(p.first), count=pin(p.count), pp_off=pin(p.pp_off), pp_idx=pin(p.pp_idx),
+             pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
+    for n_streams, max_entries in ((1, 1 << 30), (3, 5000), (2, 300), (4, 1)):
+        out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda")
+        ctx.gravity_eval_streamed(d["xyzm"], d["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"],
+                                  h["pc_off"], h["pc_idx"], p.eps, out, n_streams=n_streams,
+                                  max_entries_per_chunk=max_entries)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), base)
+        st = ctx.get_stats()
+        b_or = oracle.chunk_bounds(p.pp_off, p.pc_off, max_entries)
+        b_lib = binding.chunk_bounds(p.pp_off, p.pc_off, max_entries)
+        assert np.array_equal(b_or, b_lib) and st["chunks"] == len(b_or) - 1
+        assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc
+    out_h = np.full((p.n, 4), np.nan, np.float32)
+    ctx.gravity_eval_host(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, out_h,
+                          n_streams=3, max_entries_per_chunk=20000)
+    assert np.array_equal(out_h, base)
+
+
+def test_prepared_cells_reproduce_oracle_pc_over_distances(ctx, torch):
+    """P-C alone, one cell, targets from 1.5 to 40 cell radii in many directions."""
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors, run_resident
+    rng = np.random.default_rng(3)
+    pts = np.empty((48, 4), np.float32)
+    pts[:, :3] = 0.3 + 0.01 * rng.standard_normal((48, 3)); pts[:, 3] = rng.uniform(0.5, 1.5, 48) / 48
+    cells = inputs.cloud_records(pts, 48)
+    b = float(cells[0, 35])
+    nt = 16 * 40
+    v = rng.standard_normal((nt, 3)); v /= np.linalg.norm(v, axis=1)[:, None]
+    dist = b * np.exp(rng.uniform(np.log(1.5), np.log(40), nt))
+    xyzm = np.zeros((nt, 4), np.float32)
+    xyzm[:, :3] = cells[0, :3] + dist[:, None] * v
+    xyzm[:, 3] = 1.0 / nt
+    first = np.arange(0, nt, 16, dtype=np.int32); count = np.full(40, 16, np.int32)
+    pc_off = np.arange(41, dtype=np.int64); pc_idx = np.zeros(40, np.int32)
+    p = inputs.Problem(name="pc1", xyzm=xyzm, cells=cells, first=first, count=count, pp_off=None, pp_idx=None,
+                       pc_off=pc_off, pc_idx=pc_idx, eps=0.0)
+    ref = _oracle(p)
+    out = run_resident(ctx, p, torch)
+    ea, ep = rel_errors(out, ref)
+    assert ea.max() <= 5e-6 and ep.max() <= 2e-6, (ea.max(), ep.max())
+
+
+def test_config4_sweep_small(ctx, torch):
+    """configs[3] recipe at 256 buckets: a few (L_pp, L_pc) shapes incl. non-multiples of 32."""
+    from paper_1609_08621_b200 import inputs
+    from gpu_util import rel_errors, run_resident
+    for lpp, lpc in ((32, 32), (128, 0), (0, 128), (100, 70), (512, 512)):
+        p = inputs.config4(256, lpp, lpc)
+        ref = _oracle(p)
+        out = run_resident(ctx, p, torch)
+        ea, ep = rel_errors(out, ref, np.arange(256 * 16))
+        assert ea.max() <= TOL and ep.max() <= TOL, (lpp, lpc, ea.max(), ep.max())
