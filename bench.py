@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of pkdg-b200 (contract: the task's "Measurement" section).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--ng 256]
+
+One "step" = one pass of the whole hot path (cell prep + packer + fused P-P/P-C evaluation +
+reduction/write-back: SURVEY.md sec 8(a)) over one synthetic problem.  Workload at every N:
+BASELINE.json configs[2], the configuration the metric is quoted on (N = 2^24 particles, 256^3
+lattice displaced by a Zel'dovich field, binary tree, bucket 16, theta = 0.7); it fits one GPU.
+With --gpus N > 1 (torchrun) every rank evaluates its own replica of that problem, no data-path
+collective (weak scaling).
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle (oracle/) on the host
+cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# Flops per interaction AS EXECUTED by the kernels (add/sub/mul = 1, FMA = 2, rsqrt = 1); derived
+# line by line in DESIGN.md "Flop audit".  The paper's own convention (Table 3: 53 / 215, rsqrt = 7)
+# is reported beside it as context only.
+F_PP = 19
+F_PC = 203
+PAPER_F_PP, PAPER_F_PC = 53, 215
+SM_COUNT_NOMINAL, FP32_LANES_PER_SM = 148, 128
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons with NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, torch, dev):
+        self.samples, self.reasons, self.max_mhz, self.power = [], set(), None, []
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(dev)
+            self.nv = pynvml
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # no NVML: report that instead of inventing numbers
+            self.nv = None
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def start(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        if not self.nv:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": getattr(self, "err", "no nvml")}
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w_max": round(max(self.power), 1) if self.power else None}
+
+
+def build_workload(ng: int):
+    from paper_1609_08621_b200 import inputs
+    t = time.time()
+    p = inputs.config3(ng)
+    return p, time.time() - t
+
+
+def workload_config(p, ng):
+    list_gb = (p.pp_idx.nbytes + p.pc_idx.nbytes + p.pp_off.nbytes + p.pc_off.nbytes) / 1e9
+    return {"workload": f"configs[2]: N={ng}^3={p.n} Zel'dovich lattice (P(k)~k^-2, rms 0.3 cells), binary tree, "
+                        f"bucket<=16, theta=0.7, order-4 multipoles, eps=1/(50*{ng})",
+            "n_particles": p.n, "n_buckets": p.n_buckets, "n_cells": int(p.cells.shape[0]),
+            "mean_bucket_occupancy": round(float(p.count.mean()), 3),
+            "mean_L_pp": round(float(np.diff(p.pp_off).mean()), 2), "mean_L_pc": round(float(np.diff(p.pc_off).mean()), 2),
+            "I_pp": p.I_pp, "I_pc": p.I_pc, "theta": 0.7, "eps": p.eps,
+            "l2_policy": f"inputs larger than L2: lists {list_gb:.2f} GB + particles/cells "
+                         f"{(p.xyzm.nbytes + p.cells.nbytes) / 1e9:.2f} GB are re-read every step (L2 = 126 MB)"}
+
+
+def oracle_sample(p, target_s: float, seed: int = 0):
+    """Time the oracle, as it stands, on an evenly spread sample of buckets sized for ~target_s."""
+    import oracle
+    nb = p.n_buckets
+    probe = np.linspace(0, nb - 1, 64).astype(np.int64)
+    t = time.perf_counter()
+    oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=probe)
+    t = time.perf_counter()   # second pass: threads and caches are warm
+    oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=probe)
+    dt = max(time.perf_counter() - t, 1e-4)
+    n = int(min(nb, max(64, 64 * target_s / dt)))
+    sel = np.unique(np.linspace(0, nb - 1, n).astype(np.int64))
+    inter = int(np.dot(p.count[sel].astype(np.int64), np.diff(p.pp_off)[sel] + np.diff(p.pc_off)[sel]))
+    t = time.perf_counter()
+    oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
+    dt = time.perf_counter() - t
+    return inter / dt, dt, len(sel), inter, oracle.num_threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    p, gen_s = build_workload(args.ng)
+    per_step = min(10.0, 150.0 / (args.steps + args.warmup))
+    for _ in range(args.warmup):
+        oracle_sample(p, per_step)
+    tot_i, tot_t, nb_s, cores = 0, 0.0, 0, 1
+    for _ in range(args.steps):
+        rate, dt, nsel, inter, cores = oracle_sample(p, per_step)
+        tot_i += inter; tot_t += dt; nb_s = nsel
+    value = tot_i / tot_t
+    sample = f"{nb_s} of {p.n_buckets} buckets (evenly spread in tree order) per step, ~{per_step:.1f} s of CPU work each"
+    line = {"impl": "reference", "metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(p, args.ng),
+            "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_1609_08621_b200 import binding
+    peaks, peak_kind = load_peaks()
+
+    p, gen_s = build_workload(args.ng)
+    dev = torch.device("cuda", local_rank)
+    t = lambda a: torch.from_numpy(a).to(dev)
+    d = dict(xyzm=t(p.xyzm), cells=t(p.cells), first=t(p.first), count=t(p.count), pp_off=t(p.pp_off),
+             pp_idx=t(p.pp_idx), pc_off=t(p.pc_off), pc_idx=t(p.pc_idx))
+    out = torch.zeros((p.n, 4), dtype=torch.float32, device=dev)
+    ctx = binding.Context(local_rank)
+    flags = args.variant << binding.VARIANT_SHIFT
+
+    def step():
+        ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"],
+                         d["pc_idx"], p.eps, out, flags=flags)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    ctx.profile_read()
+    ctx.profile_enable(True)
+    sampler = ClockSampler(torch, local_rank)
+    launches0 = ctx.launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    n_eval, eval_ms_total = ctx.profile_read()
+    ctx.profile_enable(False)
+    launches = (ctx.launch_count() - launches0) // args.steps
+    stats = ctx.get_stats()
+    assert stats["interactions_pp"] == p.I_pp and stats["interactions_pc"] == p.I_pc and stats["bad_entries"] == 0
+    if dist is not None:
+        tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    inter = p.I_pp + p.I_pc
+    value = world * inter / (ms_step * 1e-3)
+    flops = F_PP * p.I_pp + F_PC * p.I_pc
+
+    # ---- end to end: every buffer starts in pinned host memory, result read back every step
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(a).pin_memory()
+        h = dict(xyzm=pin(p.xyzm), cells=pin(p.cells), first=pin(p.first), count=pin(p.count), pp_off=pin(p.pp_off),
+                 pp_idx=pin(p.pp_idx), pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
+        out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+
+        def e2e_step():
+            ctx.gravity_eval_host(h["xyzm"], h["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"], h["pc_off"],
+                                  h["pc_idx"], p.eps, out_h, n_streams=args.e2e_streams,
+                                  max_entries_per_chunk=args.e2e_chunk, flags=flags)
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        k2 = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / k2
+        if dist is not None:
+            tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        h2d = sum(int(v.numel() * v.element_size()) for v in h.values())
+        e2e = {"value": world * inter / dt, "unit": "interactions/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": int(out_h.numel() * 4), "ms_per_step": dt * 1e3, "steps": k2,
+               "api": "pkdg_gravity_eval_host (pinned host buffers, lists streamed in chunks)",
+               "n_streams": args.e2e_streams, "max_entries_per_chunk": args.e2e_chunk}
+        del h, out_h
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (pkdg_eval_kernel): plain FP32 ALU (FFMA pipe) bound
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    peak_tflops = sms * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    eval_ms = eval_ms_total / max(n_eval, 1)
+    achieved = flops / (eval_ms * 1e-3) / 1e12
+    probe_ms, probe_flops = ctx.fma_peak_probe(1 << 15)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"cfg3_ng{args.ng}")
+    roofline = {"bound": "alu", "kernel": "pkdg_eval_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": traffic,
+                "peak_kind": f"{sms} SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json clock)",
+                "kernel_ms": eval_ms, "kernel_share_of_step": eval_ms / ms_step,
+                "ffma_probe_tflops": probe_flops / (probe_ms * 1e-3) / 1e12,
+                "flops_per_interaction": {"pp": F_PP, "pc": F_PC},
+                "hbm_algorithmic_gbs": (p.pp_idx.nbytes + p.pc_idx.nbytes + 32 * p.n + 32 * p.n_buckets) / (eval_ms * 1e-3) / 1e9,
+                "hbm_peak_gbs": peaks.get("hbm_gbs")}
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        rate, dt, nsel, inter_s, cores = oracle_sample(p, args.cpu_seconds)
+        cpu_baseline = {"value": rate, "unit": "interactions/s", "cores": cores, "kind": "oracle",
+                        "sample": f"{nsel} of {p.n_buckets} buckets evenly spread in tree order "
+                                  f"({inter_s} interactions, {dt:.1f} s)"}
+
+    line = {"metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(p, args.ng), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "flops_per_s": world * flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / peak_tflops,
+            "paper_convention_tflops": world * (PAPER_F_PP * p.I_pp + PAPER_F_PC * p.I_pc) / (ms_step * 1e-3) / 1e12,
+            "interactions_per_s": {"pp": world * p.I_pp / (ms_step * 1e-3), "pc": world * p.I_pc / (ms_step * 1e-3)},
+            "gen_seconds": round(gen_s, 1)}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ng", type=int, default=256, help="lattice size per axis (256 = the headline 2^24 config)")
+    ap.add_argument("--variant", type=int, default=0, help="kernel tuning variant (0 = library default)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--e2e-streams", type=int, default=3)
+    ap.add_argument("--e2e-chunk", type=int, default=1 << 25)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

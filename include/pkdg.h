@@ -145,6 +145,13 @@ pkdg_status pkdg_prepare_cells_export(pkdg_ctx *ctx, const pkdg_cells *cells, fl
 /* Synchronises the stream(s) of the last evaluation and returns its counters. */
 pkdg_status pkdg_get_stats(pkdg_ctx *ctx, pkdg_stats *stats_host);
 
+/* Device timing of the evaluation kernel alone (the dominant kernel of the path).  With profiling
+ * on, pkdg_gravity_eval brackets its evaluation-kernel launch with CUDA events on the launching
+ * stream (ring of 256 pairs).  pkdg_profile_read synchronises, returns the number of launches
+ * recorded since the last read and their total duration in milliseconds, and clears the ring. */
+pkdg_status pkdg_profile_enable(pkdg_ctx *ctx, int32_t on);
+pkdg_status pkdg_profile_read(pkdg_ctx *ctx, int64_t *n_launches_host, double *eval_ms_total_host);
+
 /* Number of kernel launches this context has made since creation. */
 int64_t pkdg_launch_count(const pkdg_ctx *ctx);
 

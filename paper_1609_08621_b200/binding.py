@@ -26,7 +26,7 @@ CELLQ_FLOATS = 32
 
 EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
-           "pkdg_get_stats", "pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version",
+           "pkdg_get_stats", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version",
            "pkdg_fma_peak_probe"]
 
 
@@ -77,6 +77,8 @@ def _load():
     L.pkdg_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int64)]
     L.pkdg_prepare_cells_export.argtypes = [c_void_p, POINTER(_Cells), c_void_p, c_void_p]
     L.pkdg_get_stats.argtypes = [c_void_p, POINTER(Stats)]
+    L.pkdg_profile_enable.argtypes = [c_void_p, c_int32]
+    L.pkdg_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_double)]
     L.pkdg_launch_count.argtypes = [c_void_p]
     L.pkdg_launch_count.restype = c_int64
     L.pkdg_status_string.argtypes = [c_int32]
@@ -235,6 +237,15 @@ class Context:
         if check:
             self._check(s, "pkdg_get_stats")
         return st.as_dict()
+
+    def profile_enable(self, on: bool = True):
+        self._check(_lib.pkdg_profile_enable(self._h, 1 if on else 0), "pkdg_profile_enable")
+
+    def profile_read(self):
+        """(n_launches, total_ms) of the evaluation kernel since the last read (synchronises)."""
+        n, ms = c_int64(), c_double()
+        self._check(_lib.pkdg_profile_read(self._h, byref(n), byref(ms)), "pkdg_profile_read")
+        return n.value, ms.value
 
     def launch_count(self) -> int:
         return int(_lib.pkdg_launch_count(self._h))

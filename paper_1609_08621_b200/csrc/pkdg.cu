@@ -51,6 +51,9 @@ struct pkdg_ctx {
     cudaStream_t last_stream = nullptr;
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
+    bool profiling = false;
+    cudaEvent_t prof_ev[512] = {};
+    int prof_n = 0;
     std::string err;
 };
 
@@ -122,9 +125,7 @@ pkdg_status check_common(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cell
         if (!C || C->n < 0 || C->n > 0x7fffffffLL) return fail(ctx, PKDG_EINVAL, "P-C list given without valid cells");
         if (C->n > 0 && !C->rec) return fail(ctx, PKDG_EINVAL, "cells->rec is NULL");
         if (C->stride_floats < PKDG_CELL_FLOATS) return fail(ctx, PKDG_EINVAL, "cells->stride_floats < 36");
-        if (!pc->idx && C->n > 0) return fail(ctx, PKDG_EINVAL, "pc->idx is NULL");
     }
-    if (pp && pp->offsets && !pp->idx && P->n > 0) return fail(ctx, PKDG_EINVAL, "pp->idx is NULL");
     return PKDG_OK;
 }
 
@@ -217,6 +218,8 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
         if (s.st) cudaStreamDestroy(s.st);
         if (s.done) cudaEventDestroy(s.done);
     }
+    for (cudaEvent_t e : ctx->prof_ev)
+        if (e) cudaEventDestroy(e);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->ev_ready) cudaEventDestroy(ctx->ev_ready);
     delete ctx;
@@ -255,7 +258,18 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     p.pc_idx = has_pc ? pc->idx : nullptr;
     p.work_counter = ctx->counters + kMaxSlots;
     p.n_buckets = B->n;
-    return launch_eval(ctx, p, st);
+    const bool prof = ctx->profiling && ctx->prof_n < 256;
+    if (prof) {
+        for (int i = 0; i < 2; ++i)
+            if (!ctx->prof_ev[2 * ctx->prof_n + i]) CK(cudaEventCreate(&ctx->prof_ev[2 * ctx->prof_n + i]));
+        CK(cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n], st));
+    }
+    s = launch_eval(ctx, p, st);
+    if (prof) {
+        CK(cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n + 1], st));
+        ctx->prof_n++;
+    }
+    return s;
 }
 
 pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C,
@@ -438,6 +452,28 @@ pkdg_status pkdg_get_stats(pkdg_ctx* ctx, pkdg_stats* out) {
     out->bad_entries = (int64_t)h.bad_entries;
     out->chunks = ctx->last_chunks;
     return h.bad_entries ? fail(ctx, PKDG_EBADLIST, "validation found malformed buckets or list entries") : PKDG_OK;
+}
+
+pkdg_status pkdg_profile_enable(pkdg_ctx* ctx, int32_t on) {
+    if (!ctx) return PKDG_EINVAL;
+    ctx->profiling = on != 0;
+    return PKDG_OK;
+}
+
+pkdg_status pkdg_profile_read(pkdg_ctx* ctx, int64_t* n, double* ms_total) {
+    if (!ctx || !n || !ms_total) return PKDG_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    double tot = 0;
+    for (int i = 0; i < ctx->prof_n; ++i) {
+        float ms = 0;
+        CK(cudaEventSynchronize(ctx->prof_ev[2 * i + 1]));
+        CK(cudaEventElapsedTime(&ms, ctx->prof_ev[2 * i], ctx->prof_ev[2 * i + 1]));
+        tot += ms;
+    }
+    *n = ctx->prof_n;
+    *ms_total = tot;
+    ctx->prof_n = 0;
+    return PKDG_OK;
 }
 
 int64_t pkdg_launch_count(const pkdg_ctx* ctx) { return ctx ? ctx->launches : 0; }
