@@ -86,28 +86,33 @@ pkdg_status ensure(pkdg_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <int TB, int WARPS, int MINB>
+template <int WARPS, int MINB, bool NEWTON, int UNR>
 pkdg_status launch_eval_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pkdg_eval_kernel<TB, WARPS, MINB>, WARPS * 32, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pkdg_eval_kernel<WARPS, MINB, NEWTON, UNR>, WARPS * 32, 0));
     if (per_sm < 1) per_sm = 1;
     int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
     int64_t grid = (int64_t)ctx->num_sms * per_sm;
     if (grid > want) grid = want;
     if (grid < 1) grid = 1;
-    pkdg_eval_kernel<TB, WARPS, MINB><<<(unsigned)grid, WARPS * 32, 0, st>>>(p);
+    pkdg_eval_kernel<WARPS, MINB, NEWTON, UNR><<<(unsigned)grid, WARPS * 32, 0, st>>>(p);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
 }
 
+// Tuning variants (flags bits 8..15).  0 = library default.
 pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     unsigned variant = (p.flags >> PKDG_VARIANT_SHIFT) & 0xffu;
     switch (variant) {
-        case 1: return launch_eval_t<4, 4, 5>(ctx, p, st);
-        case 3: return launch_eval_t<16, 4, 3>(ctx, p, st);
         case 0:
-        case 2: return launch_eval_t<8, 4, 4>(ctx, p, st);
+        case 1: return launch_eval_t<4, 4, true, 2>(ctx, p, st);
+        case 2: return launch_eval_t<4, 3, true, 2>(ctx, p, st);
+        case 3: return launch_eval_t<4, 4, false, 2>(ctx, p, st);
+        case 4: return launch_eval_t<4, 5, true, 1>(ctx, p, st);
+        case 5: return launch_eval_t<4, 4, true, 1>(ctx, p, st);
+        case 6: return launch_eval_t<4, 5, false, 1>(ctx, p, st);
+        case 7: return launch_eval_t<4, 6, false, 1>(ctx, p, st);
         default: return fail(ctx, PKDG_EINVAL, "unknown kernel variant in flags bits 8..15");
     }
 }
@@ -138,7 +143,8 @@ void fill_params(EvalParams& p, pkdg_ctx* ctx, const float* xyzm, int64_t np, in
     p.n_particles = np;
     p.n_cells = nc;
     float h = 2.0f * eps;
-    p.h2min = fmaxf(h * h, FLT_MIN);
+    p.h2 = h * h;
+    p.h2c = fmaxf(h * h, 1.0e-24f);
     p.hinv = h > 0.0f ? 1.0f / h : 0.0f;
     p.flags = flags;
 }

@@ -28,12 +28,14 @@ struct DevStats {
 
 // ------------------------------------------------------------------------------------------------
 // Cell preparation.  Raw moments M^(n) (n = 2,3,4) -> symmetric trace-free Q^(n) = STF[M^(n)], then
-// q^(n) = c_n Q^(n) / (M s^n) with c_n = (2n-1)!!/n! = 3/2, 5/2, 35/8 and s the cell's length scale
-// (b_max).  With u = r/|r|, t = s/|r|:
-//   phi = -(M/|r|) [1 + sum_n t^n P_n(u)],           P_n = q^(n) . u^n
-//   a   =  (M/|r|^2) [W - S u],  W = sum_n n t^n V_n, V_n = q^(n) . u^(n-1), S = 1 + sum_n (2n+1) t^n P_n
+// q^(n) = n c_n Q^(n) / (M s^n) with c_n = (2n-1)!!/n! = 3/2, 5/2, 35/8 and s the cell's length scale
+// (b_max).  With d = x - COM, r = |d| and the scaled displacement tau = s d / r^2 (|tau| = s/r < 1):
+//   V_n = q^(n) . tau^(n-1)  (vector),   e_n = V_n . tau  (= n c_n Q^(n).d^n / (M r^2n))
+//   phi = -(M/r) [1 + sum_n e_n / n]
+//   a   =  (M/r^3) [s G - S d],   G = sum_n V_n,   S = 1 + sum_n (2n+1)/n e_n
 // which is the truncated Taylor series of include/pkdg.h (d^n(1/r) is trace-free, so contracting the
-// raw moments with it equals contracting their trace-free part with r^n).  Arithmetic in fp64: the
+// raw moments with it equals contracting their trace-free part with d^n; the polynomials are
+// homogeneous, so evaluating them at tau absorbs every power of s/r).  Arithmetic in fp64: the
 // trace removal cancels leading digits.  Layout of the 32 floats:
 //   0-3 COM, M | 4 s | 5-9 q2 xx xy xz yy yz | 10-16 q3 xxx xxy xxz xyy xyz yyy yyz |
 //   17-25 q4 xxxx xxxy xxxz xxyy xxyz xyyy xyyz yyyy yyyz | 26 q2zz 27 q3xzz 28 q3yzz 29 q3zzz
@@ -69,9 +71,9 @@ __global__ void pkdg_prep_cells_kernel(const float* __restrict__ rec, int64_t n,
     if (!(s > 0.0)) s = (M > 0.0 && tr2 > 0.0) ? sqrt(tr2 / M) : 0.0;
     double k2 = 0, k3 = 0, k4 = 0;
     if (s > 0.0 && M != 0.0) {
-        k2 = 1.5 / (M * s * s);
-        k3 = 2.5 / (M * s * s * s);
-        k4 = 4.375 / (M * s * s * s * s);
+        k2 = 2 * 1.5 / (M * s * s);
+        k3 = 3 * 2.5 / (M * s * s * s);
+        k4 = 4 * 4.375 / (M * s * s * s * s);
     }
     float* o = out + c * kCellQFloats;
     o[0] = r[0]; o[1] = r[1]; o[2] = r[2]; o[3] = r[3];
@@ -197,8 +199,21 @@ __global__ void pkdg_tiles_kernel(const int64_t* __restrict__ off, const int32_t
 }
 
 // ------------------------------------------------------------------------------------------------
-// Evaluation kernel.
+// Evaluation kernel (a2-a5).  One warp per bucket, buckets handed out in tree order through an
+// atomic counter.  Lanes stride the SOURCE lists (lists are cut at warp multiples;
+// here the remainder is masked instead of being shunted to the CPU).  Sinks are processed in
+// passes of up to 16:
+//   a2  the pass's sinks are staged in shared memory (broadcast reads);
+//   a3  P-P: each lane keeps ONE source in registers and visits all sinks of the pass, unrolled,
+//       with per-lane register accumulators (8 or 16 sink slots);
+//   a4  P-C: each lane keeps ONE cell (35 registers) and visits the sinks in a run-time loop (one or
+//       two per iteration, software-pipelined); per-lane partial sums live in shared memory (s_acc[sink][lane], float4), so
+//       the body is not unrolled 16 times (instruction cache) and any sink count works;
+//   a5  the 32 per-lane partials of every (sink, component) are reduced with a butterfly
+//       transpose-reduction and written as float4 {ax, ay, az, phi}.
 // ------------------------------------------------------------------------------------------------
+constexpr int kTMax = 16;  // sinks per pass
+
 struct EvalParams {
     const float4* xyzm;
     const float4* cellq;  // 8 float4 per cell
@@ -209,48 +224,60 @@ struct EvalParams {
     DevStats* stats;
     unsigned int* work_counter;
     int64_t n_buckets, n_particles, n_cells;
-    float h2min;  // max(h^2, FLT_MIN): pairs with r^2 < h2min leave the Newtonian fast path
+    float h2;     // (2 eps)^2
+    float h2c;    // clamp of r^2 in the Newtonian fast path: max(h2, 1e-24)
     float hinv;   // 1/h, 0 if eps == 0
     uint32_t flags;
 };
 
-// One P-P interaction: sink (tx,ty,tz) with source s (x,y,z,m).  `self` = the source IS the sink.
-// Newtonian fast path: 3 sub, 1 mul + 2 fma, rsqrt, 3 mul, 3 fma, 1 fma = 19 flops (rsqrt = 1).
-__device__ __forceinline__ void pp_interact(const float4 t, const float4 s, bool self, float h2min,
-                                            float hinv, float& ax, float& ay, float& az, float& ph) {
+// Softened pair factors for r^2 < h^2 (cubic spline of support h, u = r/h): a -= m d g, phi += m w.
+__device__ __noinline__ void pp_soft_factors(float r2, float hinv, float& g, float& w) {
+    float u = sqrtf(r2) * hinv;
+    float u2 = u * u;
+    if (u < 0.5f) {
+        g = fmaf(u2, fmaf(32.0f, u, -38.4f), 10.666666667f);
+        w = fmaf(u2, fmaf(u2, fmaf(6.4f, u, -9.6f), 5.3333333333f), -2.8f);
+    } else {
+        float iu = 1.0f / u;
+        float iu3 = iu * iu * iu;
+        g = fmaf(u, fmaf(u, fmaf(-10.666666667f, u, 38.4f), -48.0f), 21.333333333f) - 0.066666666667f * iu3;
+        w = fmaf(u2, fmaf(u, fmaf(u, fmaf(-2.1333333333f, u, 9.6f), -16.0f), 10.666666667f), -3.2f) +
+            0.066666666667f * iu;
+    }
+    g *= hinv * hinv * hinv;
+    w *= hinv;
+}
+
+// MUFU.RSQ without the denormal pre-/post-scaling rsqrtf() emits (inputs here are never denormal).
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Newtonian fast path of one P-P interaction with r^2 clamped from below at h2c (so it is finite
+// for softened and coincident pairs; those are corrected afterwards, see pp_phase).  With SELF the
+// accumulation is masked for the sink's own index (used only for tiles that hold own particles).
+// 3 sub | 1 mul 2 fma | max, min | rsqrt | 3 mul | 3 fma 1 sub  = 19 flops (FMA = 2, rsqrt = 1, min/max 0)
+template <bool SELF>
+__device__ __forceinline__ void pp_fast(const float4 t, const float4 s, bool self, float h2c, float& minr2,
+                                        float4& a) {
     float dx = t.x - s.x, dy = t.y - s.y, dz = t.z - s.z;
     float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    float g, w;  // a -= m d g ; phi += m w
-    if (r2 < h2min) {
-        // softened (or coincident) pair: cubic-spline kernel of support h, u = r/h   (rare path)
-        float r = sqrtf(r2);
-        float u = r * hinv;
-        float u2 = u * u;
-        if (self || hinv == 0.0f) {
-            g = 0.0f; w = 0.0f;  // own index: skipped.  eps == 0 and r == 0: undefined, skipped.
-        } else if (u < 0.5f) {
-            g = fmaf(u2, fmaf(32.0f, u, -38.4f), 10.666666667f);
-            w = fmaf(u2, fmaf(u2, fmaf(6.4f, u, -9.6f), 5.3333333333f), -2.8f);
-        } else {
-            float iu = 1.0f / u;
-            float iu3 = iu * iu * iu;
-            g = fmaf(u, fmaf(u, fmaf(-10.666666667f, u, 38.4f), -48.0f), 21.333333333f) - 0.066666666667f * iu3;
-            w = fmaf(u2, fmaf(u, fmaf(u, fmaf(-2.1333333333f, u, 9.6f), -16.0f), 10.666666667f), -3.2f) +
-                0.066666666667f * iu;
-        }
-        g *= hinv * hinv * hinv;
-        w *= hinv;
-    } else {
-        float ri = rsqrtf(r2);
-        float ri2 = ri * ri;
-        g = ri * ri2;
-        w = -ri;
+    float ri = rsqrt_approx(fmaxf(r2, h2c));
+    float ri2 = ri * ri;
+    float m = s.w;
+    if (SELF) {
+        m = self ? 0.0f : m;
+        r2 = self ? 3.0e38f : r2;
     }
-    float mg = s.w * g;
-    ax = fmaf(-mg, dx, ax);
-    ay = fmaf(-mg, dy, ay);
-    az = fmaf(-mg, dz, az);
-    ph = fmaf(s.w, w, ph);
+    minr2 = fminf(minr2, r2);
+    float mri = m * ri;
+    float mg = mri * ri2;
+    a.x = fmaf(-mg, dx, a.x);
+    a.y = fmaf(-mg, dy, a.y);
+    a.z = fmaf(-mg, dz, a.z);
+    a.w -= mri;
 }
 
 // A cell held in registers by one lane (35 values; COM/M/s + 6 + 10 + 15 normalised components).
@@ -278,23 +305,35 @@ __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const 
     c.zzzz = -(c.xxzz + c.yyzz);
 }
 
-// One P-C interaction (see the formulas above pkdg_prep_cells_kernel).  ~130 FP32-pipe
-// instructions + 1 MUFU; audited flop count in DESIGN.md.
-__device__ __forceinline__ void pc_interact(const float4 t, const CellRegs& c, float& ax, float& ay,
-                                            float& az, float& ph) {
-    float dx = t.x - c.cx, dy = t.y - c.cy, dz = t.z - c.cz;
-    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    float ri = rsqrtf(r2);
-    // one Newton step: MUFU.RSQ is good to ~2^-22.9, and the result enters as ri^2..ri^6
-    float hy = 0.5f * r2 * ri;
-    ri = ri * fmaf(-hy, ri, 1.5f);
-    float x = dx * ri, y = dy * ri, z = dz * ri;
-    float tt = c.s * ri;
+// One P-C interaction (formulas above pkdg_prep_cells_kernel); flop audit in DESIGN.md.  Split in two
+// so that the evaluation loop can software-pipeline it: pc_pre (sink load, displacement, rsqrt: a
+// serial chain of long-latency steps) for the NEXT sinks is issued under pc_body of the current ones.
+struct PcPre { float dx, dy, dz, ri; };
+
+template <bool NEWTON>
+__device__ __forceinline__ PcPre pc_pre(const float4 t, const CellRegs& c) {
+    PcPre q;
+    q.dx = t.x - c.cx; q.dy = t.y - c.cy; q.dz = t.z - c.cz;
+    float r2 = fmaf(q.dz, q.dz, fmaf(q.dy, q.dy, q.dx * q.dx));
+    float ri = rsqrt_approx(r2);
+    if (NEWTON) {  // one Newton step on MUFU.RSQ (2^-22.9): the result enters as ri^2 .. ri^3
+        float hy = 0.5f * r2 * ri;
+        ri = ri * fmaf(-hy, ri, 1.5f);
+    }
+    q.ri = ri;
+    return q;
+}
+
+__device__ __forceinline__ void pc_body(const PcPre q, const CellRegs& c, float4& a) {
+    const float dx = q.dx, dy = q.dy, dz = q.dz, ri = q.ri;
+    float ri2 = ri * ri;
+    float sr = c.s * ri2;
+    float x = dx * sr, y = dy * sr, z = dz * sr;  // tau
     // order 2
     float v2x = fmaf(c.xz, z, fmaf(c.xy, y, c.xx * x));
     float v2y = fmaf(c.yz, z, fmaf(c.yy, y, c.xy * x));
     float v2z = fmaf(c.zz, z, fmaf(c.yz, y, c.xz * x));
-    float p2 = fmaf(v2z, z, fmaf(v2y, y, v2x * x));
+    float e2 = fmaf(v2z, z, fmaf(v2y, y, v2x * x));
     // order 3: quadratic monomials, cross terms carry their multiplicity 2
     float xx = x * x, yy = y * y, zz = z * z;
     float x2 = x + x, y2 = y + y;
@@ -302,7 +341,7 @@ __device__ __forceinline__ void pc_interact(const float4 t, const CellRegs& c, f
     float v3x = fmaf(c.xyz, yz, fmaf(c.xxz, xz, fmaf(c.xxy, xy, fmaf(c.xzz, zz, fmaf(c.xyy, yy, c.xxx * xx)))));
     float v3y = fmaf(c.yyz, yz, fmaf(c.xyz, xz, fmaf(c.xyy, xy, fmaf(c.yzz, zz, fmaf(c.yyy, yy, c.xxy * xx)))));
     float v3z = fmaf(c.yzz, yz, fmaf(c.xzz, xz, fmaf(c.xyz, xy, fmaf(c.zzz, zz, fmaf(c.yyz, yy, c.xxz * xx)))));
-    float p3 = fmaf(v3z, z, fmaf(v3y, y, v3x * x));
+    float e3 = fmaf(v3z, z, fmaf(v3y, y, v3x * x));
     // order 4: cubic monomials with multiplicities 1, 3, 6
     float x3 = 3.0f * x, y3 = 3.0f * y, z3 = 3.0f * z;
     float mxxx = xx * x, myyy = yy * y, mzzz = zz * z;
@@ -314,39 +353,30 @@ __device__ __forceinline__ void pc_interact(const float4 t, const CellRegs& c, f
                 fmaf(c.xyyz, mxyz, fmaf(c.xyyy, mxyy, fmaf(c.xxyz, mxxz, fmaf(c.xxyy, mxxy, c.xxxy * mxxx)))))))));
     float v4z = fmaf(c.zzzz, mzzz, fmaf(c.yzzz, myzz, fmaf(c.yyzz, myyz, fmaf(c.yyyz, myyy, fmaf(c.xzzz, mxzz,
                 fmaf(c.xyzz, mxyz, fmaf(c.xyyz, mxyy, fmaf(c.xxzz, mxxz, fmaf(c.xxyz, mxxy, c.xxxz * mxxx)))))))));
-    float p4 = fmaf(v4z, z, fmaf(v4y, y, v4x * x));
+    float e4 = fmaf(v4z, z, fmaf(v4y, y, v4x * x));
     // combine
-    float t2 = tt * tt, t3 = t2 * tt, t4 = t2 * t2;
-    float e2 = t2 * p2, e3 = t3 * p3, e4 = t4 * p4;
-    float fs = 1.0f + e2 + e3 + e4;                                      // potential series
-    float S = fmaf(9.0f, e4, fmaf(7.0f, e3, fmaf(5.0f, e2, 1.0f)));      // radial part of the force
-    float w2 = t2 + t2, w3 = 3.0f * t3, w4 = 4.0f * t4;
-    float wx = fmaf(w4, v4x, fmaf(w3, v3x, w2 * v2x));
-    float wy = fmaf(w4, v4y, fmaf(w3, v3y, w2 * v2y));
-    float wz = fmaf(w4, v4z, fmaf(w3, v3z, w2 * v2z));
+    float fs = fmaf(0.25f, e4, fmaf(0.33333333333f, e3, fmaf(0.5f, e2, 1.0f)));   // potential series
+    float S = fmaf(2.25f, e4, fmaf(2.3333333333f, e3, fmaf(2.5f, e2, 1.0f)));     // radial part of the force
+    float gx = v2x + v3x + v4x, gy = v2y + v3y + v4y, gz = v2z + v3z + v4z;
     float mr = c.M * ri;
-    float mr2 = mr * ri;
-    ph = fmaf(-mr, fs, ph);
-    ax = fmaf(mr2, fmaf(-S, x, wx), ax);
-    ay = fmaf(mr2, fmaf(-S, y, wy), ay);
-    az = fmaf(mr2, fmaf(-S, z, wz), az);
+    float k3 = mr * ri2;
+    float sk = c.s * k3, Sk = S * k3;
+    a.w = fmaf(-mr, fs, a.w);
+    a.x = fmaf(sk, gx, fmaf(-Sk, dx, a.x));
+    a.y = fmaf(sk, gy, fmaf(-Sk, dy, a.y));
+    a.z = fmaf(sk, gz, fmaf(-Sk, dz, a.z));
 }
 
 // Butterfly transpose-reduction of NV per-lane partial sums across the 32 lanes: log2(32) rounds, in
-// round with partner lane^mask each lane hands over the half of its values the partner keeps.
-// NV = 64: lane l ends with the totals of values 2l, 2l+1 in v[0], v[1];  NV = 32: value l in v[0];
-// NV = 16: value (l & 15) in v[0].   NV - NV/32 shuffles instead of 5 NV.
+// the round with partner lane^mask each lane hands over the half of its values the partner keeps.
+// NV = 64: lane l ends with the totals of values 2l, 2l+1 in v[0], v[1];  NV = 32: value l in v[0].
+// NV - NV/32 shuffles instead of 5 NV.
 template <int NV>
 __device__ __forceinline__ void warp_transpose_reduce(float (&v)[NV], int lane) {
-    static_assert(NV == 16 || NV == 32 || NV == 64, "NV");
-    if (NV == 16) {
-#pragma unroll
-        for (int i = 0; i < NV; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], 16);
-    }
-    constexpr int kFirstMask = (NV == 16) ? 8 : 16;
+    static_assert(NV == 32 || NV == 64, "NV");
     int n = NV / 2;
 #pragma unroll
-    for (int mask = kFirstMask; mask >= 1; mask >>= 1) {
+    for (int mask = 16; mask >= 1; mask >>= 1) {
         bool up = (lane & mask) != 0;
 #pragma unroll
         for (int i = 0; i < NV / 2; ++i) {
@@ -360,12 +390,88 @@ __device__ __forceinline__ void warp_transpose_reduce(float (&v)[NV], int lane) 
     }
 }
 
-template <int TB, int WARPS, int MINB>
+// a3 for one pass: NS sink slots (8 or 16), register accumulators, result stored to (or added into)
+// the per-lane shared accumulators.  Returns with s_acc[t][lane] holding the lane's P-P partials.
+template <int NS>
+__device__ __forceinline__ void pp_phase(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
+                                         const float4* __restrict__ s_tgt, float4* __restrict__ s_acc, int lane,
+                                         unsigned& bad) {
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    float4 acc[NS];
+#pragma unroll
+    for (int t = 0; t < NS; ++t) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
+    const int ntile = (pp_len + 31) >> 5;
+    const int sink0 = d.first + t0;
+    int32_t j = ntile ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 0, lane) : -1;
+    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
+    int32_t jn = ntile > 1 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 1, lane) : -1;
+    for (int k = 0; k < ntile; ++k) {
+        // the source of the next tile and the index of the one after are in flight during this tile
+        if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
+        const float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
+        const int32_t jnn = (k + 2 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 2, lane) : -1;
+        const int self_t = j - sink0;  // sink slot this source coincides with, if any
+        float minr2 = 3.0e38f;
+        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)NS)) {  // tile holds own particles
+#pragma unroll
+            for (int t = 0; t < NS; ++t) pp_fast<true>(s_tgt[t], s, self_t == t, p.h2c, minr2, acc[t]);
+        } else {
+#pragma unroll
+            for (int t = 0; t < NS; ++t) pp_fast<false>(s_tgt[t], s, false, p.h2c, minr2, acc[t]);
+        }
+        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
+            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
+            // Newtonian contribution by the spline one, through the shared accumulators.
+            if (!smem_live) {
+                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                smem_live = true;
+            }
+            if (minr2 < p.h2c) {
+                for (int t = 0; t < ntp; ++t) {
+                    const float4 tg = s_tgt[t];
+                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
+                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    if (r2 < p.h2c && self_t != t) {
+                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
+                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
+                        float ri = rsqrt_approx(p.h2c);  // what pp_fast used for this pair
+                        float gc = ri * ri * ri, wc = -ri;
+                        float4 a = s_acc[t * 32 + lane];
+                        float mg = s.w * (g - gc);
+                        a.x = fmaf(-mg, dx, a.x); a.y = fmaf(-mg, dy, a.y); a.z = fmaf(-mg, dz, a.z);
+                        a.w = fmaf(s.w, w - wc, a.w);
+                        s_acc[t * 32 + lane] = a;
+                    }
+                }
+            }
+        }
+        s = sn; j = jn; jn = jnn;
+    }
+    if (smem_live) {
+#pragma unroll
+        for (int t = 0; t < NS; ++t) {
+            float4 a = s_acc[t * 32 + lane];
+            a.x += acc[t].x; a.y += acc[t].y; a.z += acc[t].z; a.w += acc[t].w;
+            s_acc[t * 32 + lane] = a;
+        }
+    } else {
+#pragma unroll
+        for (int t = 0; t < NS; ++t) s_acc[t * 32 + lane] = acc[t];
+    }
+}
+
+template <int WARPS, int MINB, bool NEWTON, int UNR>
 __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalParams p) {
-    __shared__ float4 s_tgt[WARPS][TB];
+    __shared__ float4 s_acc_all[WARPS][(kTMax + 1) * 32];  // [sink slot][lane]; slot 16 = scratch
+    __shared__ float4 s_tgt_all[WARPS][kTMax + 2];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    float4* s_acc = s_acc_all[warp];
+    float4* s_tgt = s_tgt_all[warp];
     const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);  // pads sink slots; never meets a source
     const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
     unsigned bad = 0;
 
@@ -377,45 +483,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalP
         const BucketDesc d = p.desc[bu];
         const int pp_len = do_pp ? d.pp_len : 0, pc_len = do_pc ? d.pc_len : 0;
 
-        for (int t0 = 0; t0 < d.count; t0 += TB) {
-            const int ntp = min(TB, d.count - t0);
+        for (int t0 = 0; t0 < d.count; t0 += kTMax) {
+            const int ntp = min(kTMax, d.count - t0);
+            // ---- a2: stage the sinks of this pass (slots >= ntp hold a far-away dummy)
             __syncwarp();
-            if (lane < ntp) s_tgt[warp][lane] = __ldg(p.xyzm + d.first + t0 + lane);
+            if (lane < kTMax + 2) s_tgt[lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
             __syncwarp();
-            float acc[TB * 4];
-#pragma unroll
-            for (int i = 0; i < TB * 4; ++i) acc[i] = 0.0f;
 
-            // ---- a3: P-P tiles; source of the next tile is in flight while this one is evaluated
-            {
-                const int ntile = (pp_len + 31) >> 5;
-                int32_t j = ntile ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 0, lane) : -1;
-                if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
-                float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
-                int32_t jn = ntile > 1 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 1, lane) : -1;
-                for (int k = 0; k < ntile; ++k) {
-                    if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
-                    const float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
-                    const int32_t jnn = (k + 2 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 2, lane) : -1;
-                    const int self_t = j - (d.first + t0);  // sink slot this source coincides with
-#pragma unroll
-                    for (int t = 0; t < TB; ++t) {
-                        if (t < ntp) {
-                            const float4 tg = s_tgt[warp][t];
-                            pp_interact(tg, s, self_t == t, p.h2min, p.hinv, acc[4 * t], acc[4 * t + 1],
-                                        acc[4 * t + 2], acc[4 * t + 3]);
-                        }
-                    }
-                    s = sn; j = jn; jn = jnn;
-                }
-            }
-            // ---- a4: P-C tiles; the lane's cell stays in registers for all sinks of the pass
+            // ---- a3: P-P
+            if (ntp <= 8) pp_phase<8>(p, d, pp_len, t0, ntp, s_tgt, s_acc, lane, bad);
+            else pp_phase<16>(p, d, pp_len, t0, ntp, s_tgt, s_acc, lane, bad);
+
+            // ---- a4: P-C.  Two sinks per iteration; the lane's cell stays in registers for the tile.
             {
                 const int ntile = (pc_len + 31) >> 5;
+                const int nte = (ntp + 1) & ~1;  // odd count: the last iteration also visits the dummy slot
                 int32_t c = ntile ? tile_entry(p.pc_idx, d.pc_begin, pc_len, 0, lane) : -1;
+                int32_t c1 = ntile > 1 ? tile_entry(p.pc_idx, d.pc_begin, pc_len, 1, lane) : -1;
                 for (int k = 0; k < ntile; ++k) {
                     if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
-                    const int32_t cn = (k + 1 < ntile) ? tile_entry(p.pc_idx, d.pc_begin, pc_len, k + 1, lane) : -1;
+                    // next tile's record -> L1 while this tile is evaluated; index two tiles ahead in flight
+                    if ((uint32_t)c1 < (uint64_t)p.n_cells)
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(p.cellq + (int64_t)c1 * 8));
+                    const int32_t c2 = (k + 2 < ntile) ? tile_entry(p.pc_idx, d.pc_begin, pc_len, k + 2, lane) : -1;
                     CellRegs cr;
                     if (c >= 0) {
                         const float4* q = p.cellq + (int64_t)c * 8;
@@ -425,33 +515,60 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalP
                         const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
                         cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
                     }
-#pragma unroll
-                    for (int t = 0; t < TB; ++t) {
-                        if (t < ntp) {
-                            const float4 tg = s_tgt[warp][t];
-                            pc_interact(tg, cr, acc[4 * t], acc[4 * t + 1], acc[4 * t + 2], acc[4 * t + 3]);
+                    if (UNR == 2) {
+                        PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr), pB = pc_pre<NEWTON>(s_tgt[1], cr);
+#pragma unroll 1
+                        for (int t = 0; t < nte; t += 2) {
+                            const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 2], cr), nB = pc_pre<NEWTON>(s_tgt[t + 3], cr);
+                            float4 aA = s_acc[t * 32 + lane], aB = s_acc[(t + 1) * 32 + lane];
+                            pc_body(pA, cr, aA);
+                            pc_body(pB, cr, aB);
+                            s_acc[t * 32 + lane] = aA;
+                            s_acc[(t + 1) * 32 + lane] = aB;
+                            pA = nA; pB = nB;
+                        }
+                    } else {
+                        PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr);
+#pragma unroll 1
+                        for (int t = 0; t < ntp; ++t) {
+                            const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 1], cr);
+                            float4 aA = s_acc[t * 32 + lane];
+                            pc_body(pA, cr, aA);
+                            s_acc[t * 32 + lane] = aA;
+                            pA = nA;
                         }
                     }
-                    c = cn;
+                    c = c1; c1 = c2;
                 }
             }
             // ---- a5: cross-lane reduction and write-back
-            warp_transpose_reduce<TB * 4>(acc, lane);
             float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
-            if (TB == 16) {
-                const int t = lane >> 1;
-                if (t < ntp) {
-                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
-                    float2 r = make_float2(acc[0], acc[1]);
-                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
-                    *o2 = r;
+            if (ntp <= 8) {
+                float v[32];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const float4 a = s_acc[t * 32 + lane];
+                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
+                }
+                warp_transpose_reduce<32>(v, lane);
+                if ((lane >> 2) < ntp) {
+                    float r = v[0];
+                    if (accumulate) r += outf[lane];
+                    outf[lane] = r;
                 }
             } else {
-                const int slot = (TB == 8) ? lane : (lane & 15);
-                if ((slot >> 2) < ntp && (TB == 8 || lane < 16)) {
-                    float r = acc[0];
-                    if (accumulate) r += outf[slot];
-                    outf[slot] = r;
+                float v[64];
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    const float4 a = s_acc[t * 32 + lane];
+                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
+                }
+                warp_transpose_reduce<64>(v, lane);
+                if ((lane >> 1) < ntp) {
+                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
+                    float2 r = make_float2(v[0], v[1]);
+                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
+                    *o2 = r;
                 }
             }
         }

@@ -7,7 +7,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 TOL = 2e-5
-VARIANTS = [0, 1 << 8, 2 << 8, 3 << 8]
+VARIANTS = [0, 1 << 8, 2 << 8, 3 << 8, 4 << 8]
 
 
 @pytest.fixture(scope="module")
