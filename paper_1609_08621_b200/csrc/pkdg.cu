@@ -101,6 +101,52 @@ pkdg_status launch_eval_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     return PKDG_OK;
 }
 
+template <int WARPS, int MINB, bool NEWTON>
+pkdg_status launch_eval2_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    auto kern = pkdg_eval2_kernel<WARPS, MINB, NEWTON>;
+    const int smem = WARPS * (int)sizeof(WarpSmem);
+    static bool configured = false;  // per instantiation; the attribute is per function and sticky
+    if (!configured) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        configured = true;
+    }
+    int per_sm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
+    int64_t grid = (int64_t)ctx->num_sms * per_sm;
+    if (grid > want) grid = want;
+    if (grid < 1) grid = 1;
+    kern<<<(unsigned)grid, WARPS * 32, smem, st>>>(p);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+template <int WARPS, int MINB, bool NEWTON>
+pkdg_status launch_eval3_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    auto kern = pkdg_eval3_kernel<WARPS, MINB, NEWTON>;
+    const int smem = WARPS * (int)sizeof(WarpSmem3);
+    static bool configured = false;  // per instantiation; the attribute is per function and sticky
+    if (!configured) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        configured = true;
+    }
+    int per_sm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
+    int64_t grid = (int64_t)ctx->num_sms * per_sm;
+    if (grid > want) grid = want;
+    if (grid < 1) grid = 1;
+    kern<<<(unsigned)grid, WARPS * 32, smem, st>>>(p);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
 // Tuning variants (flags bits 8..15).  0 = library default.
 pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     unsigned variant = (p.flags >> PKDG_VARIANT_SHIFT) & 0xffu;
@@ -113,6 +159,13 @@ pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
         case 5: return launch_eval_t<4, 4, true, 1>(ctx, p, st);
         case 6: return launch_eval_t<4, 5, false, 1>(ctx, p, st);
         case 7: return launch_eval_t<4, 6, false, 1>(ctx, p, st);
+        case 8: return launch_eval2_t<4, 4, true>(ctx, p, st);
+        case 9: return launch_eval2_t<4, 4, false>(ctx, p, st);
+        case 10: return launch_eval2_t<4, 3, false>(ctx, p, st);
+        case 11: return launch_eval3_t<4, 3, false>(ctx, p, st);
+        case 12: return launch_eval3_t<4, 4, false>(ctx, p, st);
+        case 13: return launch_eval3_t<4, 3, true>(ctx, p, st);
+        case 14: return launch_eval3_t<4, 2, false>(ctx, p, st);
         default: return fail(ctx, PKDG_EINVAL, "unknown kernel variant in flags bits 8..15");
     }
 }

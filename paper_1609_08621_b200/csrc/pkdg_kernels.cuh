@@ -576,6 +576,693 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalP
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Evaluation kernel, generation 2 (the library default).  Same mapping and arithmetic as above; what
+// changes is WHEN data moves (profiles/r01_eval_ng128_v1.md: 45 % of warp time was spent waiting on
+// dependent global loads in the per-bucket and per-tile prologues, the FP loops got only 48 %):
+//   * the cell records of P-C tile k+1 are fetched with cp.async into a per-lane shared-memory slot
+//     while tile k is evaluated (tile 0: during the P-P phase) -- a guaranteed landing spot instead
+//     of an L1 prefetch that 16 warps x 4 KB evict before use;
+//   * the NEXT bucket is claimed (atomic) at the start of the current one; its descriptor, its sinks
+//     and the first two tiles of both index lists are fetched with cp.async during the current
+//     bucket's P-C phase, so a bucket starts with one exposed global round trip instead of four;
+//   * P-P sources are gathered two tiles ahead, indices three.
+// ------------------------------------------------------------------------------------------------
+struct __align__(16) WarpSmem {
+    float4 acc[kTMax * 32];       // [sink slot][lane] per-lane partial sums
+    float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
+    float4 tgt[2][kTMax + 2];     // sinks of the current / the next bucket
+    int32_t nidx[4][32];          // tiles 0, 1 of the P-P list and tiles 0, 1 of the P-C list
+    BucketDesc ndesc;             // descriptor of the next bucket
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* q) { return (uint32_t)__cvta_generic_to_shared(q); }
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+struct ListLens { int pp, pc; };
+__device__ __forceinline__ ListLens eff_lens(const BucketDesc& d, bool do_pp, bool do_pc) {
+    ListLens l;
+    l.pp = (do_pp && d.count > 0) ? d.pp_len : 0;
+    l.pc = (do_pc && d.count > 0) ? d.pc_len : 0;
+    return l;
+}
+
+// Sinks of pass t0 and index tiles 0, 1 of both lists by plain loads (first bucket of a warp, passes > 0).
+__device__ __forceinline__ void fill_direct(WarpSmem& S, const EvalParams& p, const BucketDesc& d, ListLens L, int t0,
+                                            int buf, int lane) {
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+    __syncwarp();
+    const int ntp = max(0, min(kTMax, d.count - t0));
+    if (lane < kTMax + 2) S.tgt[buf][lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
+    S.nidx[0][lane] = L.pp > 0 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 0, lane) : -1;
+    S.nidx[1][lane] = L.pp > 32 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 1, lane) : -1;
+    S.nidx[2][lane] = L.pc > 0 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 0, lane) : -1;
+    S.nidx[3][lane] = L.pc > 32 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 1, lane) : -1;
+    __syncwarp();
+}
+
+// The same for the NEXT bucket (descriptor already in S.ndesc), asynchronously.
+__device__ __forceinline__ void stage_next_bucket(WarpSmem& S, const EvalParams& p, int nbuf, bool do_pp, bool do_pc,
+                                                  int lane) {
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+    const BucketDesc nd = S.ndesc;
+    const ListLens L = eff_lens(nd, do_pp, do_pc);
+    const int ntp = max(0, min(kTMax, nd.count));
+    if (lane < kTMax + 2) {
+        if (lane < ntp) cp_async16(&S.tgt[nbuf][lane], p.xyzm + nd.first + lane);
+        else S.tgt[nbuf][lane] = dummy_tgt;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int e = (q & 1) * 32 + lane;
+        const int len = q < 2 ? L.pp : L.pc;
+        const int32_t* src = q < 2 ? p.pp_idx + nd.pp_begin : p.pc_idx + nd.pc_begin;
+        if (e < len) cp_async4(&S.nidx[q][lane], src + e);
+        else S.nidx[q][lane] = -1;
+    }
+}
+
+template <int NS>
+__device__ __forceinline__ void pp_phase2(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
+                                          const float4* __restrict__ s_tgt, float4* __restrict__ s_acc,
+                                          const WarpSmem& S, int lane, unsigned& bad) {
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    float4 acc[NS];
+#pragma unroll
+    for (int t = 0; t < NS; ++t) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
+    const int ntile = (pp_len + 31) >> 5;
+    const int sink0 = d.first + t0;
+    int32_t j = ntile > 0 ? S.nidx[0][lane] : -1;
+    int32_t jn = ntile > 1 ? S.nidx[1][lane] : -1;
+    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+    if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
+    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
+    float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
+    int32_t jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
+    for (int k = 0; k < ntile; ++k) {
+        // sources of the next two tiles and the index of the third are in flight during this tile
+        if ((uint32_t)jnn >= (uint64_t)p.n_particles) { bad += (jnn >= 0); jnn = -1; }
+        const float4 snn = jnn >= 0 ? __ldg(p.xyzm + jnn) : far4;
+        const int32_t jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
+        const int self_t = j - sink0;  // sink slot this source coincides with, if any
+        float minr2 = 3.0e38f;
+        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)NS)) {  // tile holds own particles
+#pragma unroll
+            for (int t = 0; t < NS; ++t) pp_fast<true>(s_tgt[t], s, self_t == t, p.h2c, minr2, acc[t]);
+        } else {
+#pragma unroll
+            for (int t = 0; t < NS; ++t) pp_fast<false>(s_tgt[t], s, false, p.h2c, minr2, acc[t]);
+        }
+        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
+            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
+            // Newtonian contribution by the spline one, through the shared accumulators.
+            if (!smem_live) {
+                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                smem_live = true;
+            }
+            if (minr2 < p.h2c) {
+                for (int t = 0; t < ntp; ++t) {
+                    const float4 tg = s_tgt[t];
+                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
+                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    if (r2 < p.h2c && self_t != t) {
+                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
+                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
+                        float ri = rsqrt_approx(p.h2c);  // what pp_fast used for this pair
+                        float gc = ri * ri * ri, wc = -ri;
+                        float4 a = s_acc[t * 32 + lane];
+                        float mg = s.w * (g - gc);
+                        a.x = fmaf(-mg, dx, a.x); a.y = fmaf(-mg, dy, a.y); a.z = fmaf(-mg, dz, a.z);
+                        a.w = fmaf(s.w, w - wc, a.w);
+                        s_acc[t * 32 + lane] = a;
+                    }
+                }
+            }
+        }
+        s = sn; sn = snn; j = jn; jn = jnn; jnn = jn3;
+    }
+    if (smem_live) {
+#pragma unroll
+        for (int t = 0; t < NS; ++t) {
+            float4 a = s_acc[t * 32 + lane];
+            a.x += acc[t].x; a.y += acc[t].y; a.z += acc[t].z; a.w += acc[t].w;
+            s_acc[t * 32 + lane] = a;
+        }
+    } else {
+#pragma unroll
+        for (int t = 0; t < NS; ++t) s_acc[t * 32 + lane] = acc[t];
+    }
+}
+
+template <int WARPS, int MINB, bool NEWTON>
+__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval2_kernel(const EvalParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+    float4* s_acc = S.acc;
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
+    unsigned bad = 0;
+
+    unsigned cur = 0;
+    if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
+    cur = __shfl_sync(0xffffffffu, cur, 0);
+    if ((int64_t)cur >= p.n_buckets) return;
+    BucketDesc d = p.desc[cur];
+    int buf = 0;
+    fill_direct(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
+
+    for (;;) {
+        unsigned nxt = 0xffffffffu;
+        if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
+        bool has_next = false;
+        const ListLens L = eff_lens(d, do_pp, do_pc);
+        const int npass = max(1, (d.count + kTMax - 1) / kTMax);
+
+        for (int pass = 0; pass < npass; ++pass) {
+            const int t0 = pass * kTMax;
+            const int ntp = max(0, min(kTMax, d.count - t0));
+            const bool last = pass == npass - 1;
+            if (pass > 0) fill_direct(S, p, d, L, t0, buf, lane);
+            const float4* s_tgt = S.tgt[buf];
+
+            // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
+            const int pc_ntile = (L.pc + 31) >> 5;
+            int32_t c = pc_ntile > 0 ? S.nidx[2][lane] : -1;
+            int32_t cn = pc_ntile > 1 ? S.nidx[3][lane] : -1;
+            if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
+            if (c >= 0) {
+                const float4* q = p.cellq + (int64_t)c * 8;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
+            }
+            cp_async_commit();
+
+            // ---- a3: P-P
+            if (ntp <= 8) pp_phase2<8>(p, d, L.pp, t0, ntp, s_tgt, s_acc, S, lane, bad);
+            else pp_phase2<16>(p, d, L.pp, t0, ntp, s_tgt, s_acc, S, lane, bad);
+
+            // ---- next bucket, stage 1: its descriptor
+            if (last) {
+                const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
+                has_next = (int64_t)nb < p.n_buckets;
+                if (has_next && lane < 2)
+                    cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
+                               reinterpret_cast<const char*>(p.desc + nb) + 16 * lane);
+                cp_async_commit();
+            }
+
+            // ---- a4: P-C.  Two sinks per iteration; the lane's cell stays in registers for the tile.
+            {
+                const int nte = (ntp + 1) & ~1;  // odd count: the last iteration also visits the dummy slot
+                for (int k = 0; k < pc_ntile; ++k) {
+                    const int32_t c2 = (k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
+                    cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
+                    CellRegs cr;
+                    if (c >= 0) {
+                        cell_unpack(cr, S.stage[lane], S.stage[32 + lane], S.stage[64 + lane], S.stage[96 + lane],
+                                    S.stage[128 + lane], S.stage[160 + lane], S.stage[192 + lane], S.stage[224 + lane]);
+                    } else {
+                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
+                    }
+                    if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
+                    if (cn >= 0) {  // next tile's record; the slot was read into registers just above
+                        const float4* q = p.cellq + (int64_t)cn * 8;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
+                    }
+                    if (last && k == pc_ntile - 1 && has_next) {  // next bucket, stage 2
+                        __syncwarp();
+                        stage_next_bucket(S, p, buf ^ 1, do_pp, do_pc, lane);
+                    }
+                    cp_async_commit();
+                    PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr), pB = pc_pre<NEWTON>(s_tgt[1], cr);
+#pragma unroll 1
+                    for (int t = 0; t < nte; t += 2) {
+                        const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 2], cr), nB = pc_pre<NEWTON>(s_tgt[t + 3], cr);
+                        float4 aA = s_acc[t * 32 + lane], aB = s_acc[(t + 1) * 32 + lane];
+                        pc_body(pA, cr, aA);
+                        pc_body(pB, cr, aB);
+                        s_acc[t * 32 + lane] = aA;
+                        s_acc[(t + 1) * 32 + lane] = aB;
+                        pA = nA; pB = nB;
+                    }
+                    c = cn; cn = c2;
+                }
+                if (last && pc_ntile == 0 && has_next) {
+                    cp_async_wait_all();
+                    __syncwarp();
+                    stage_next_bucket(S, p, buf ^ 1, do_pp, do_pc, lane);
+                    cp_async_commit();
+                }
+            }
+            // ---- a5: cross-lane reduction and write-back
+            float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
+            if (ntp <= 8) {
+                float v[32];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const float4 a = s_acc[t * 32 + lane];
+                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
+                }
+                warp_transpose_reduce<32>(v, lane);
+                if ((lane >> 2) < ntp) {
+                    float r = v[0];
+                    if (accumulate) r += outf[lane];
+                    outf[lane] = r;
+                }
+            } else {
+                float v[64];
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    const float4 a = s_acc[t * 32 + lane];
+                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
+                }
+                warp_transpose_reduce<64>(v, lane);
+                if ((lane >> 1) < ntp) {
+                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
+                    float2 r = make_float2(v[0], v[1]);
+                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
+                    *o2 = r;
+                }
+            }
+        }
+        if (!has_next) break;
+        cp_async_wait_all();
+        __syncwarp();
+        d = S.ndesc;
+        buf ^= 1;
+    }
+    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generation 3: packed FP32x2 arithmetic (sm_100 FFMA2 / FMUL2 / FADD2).
+//
+// Measured on B200 (profiles/r01_ubench_regfile.md): the register file delivers one 32-bit operand
+// per bank (even / odd register) per clock, so a scalar FFMA with three distinct register operands
+// issues every 1.5 clocks (0.66 of the FMA peak) and the scalar P-C body tops out at 0.76.  A packed
+// FFMA2 computes two FMAs in two clocks from 64-bit register pairs (one read of each bank per
+// operand) and accepts a scalar register broadcast to both halves: coefficient (scalar) x monomial
+// (pair) + accumulator (pair) needs <= 2 reads per bank whenever one operand is reused from the
+// previous instruction -- full FMA rate with half the issue slots, independent of register allocation.
+// So one lane still holds ONE source (particle or cell) in scalar registers, and the two halves of
+// every packed value are two SINKS of the bucket (sink pair p = sinks 2p, 2p+1).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 sp(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 f2mul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 f2add(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 f2fma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+
+constexpr int kPMax = kTMax / 2;  // sink pairs per pass
+
+struct __align__(16) WarpSmem3 {
+    float4 acc[kTMax * 32];       // [pair][half][lane]: {axA, axB, ayA, ayB}, {azA, azB, phiA, phiB}
+    float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
+    float4 tgt[2][kTMax];         // raw sinks (x, y, z, m) of the current / the next bucket
+    float4 tp[(kPMax + 1) * 2];   // current pass, pair layout: {xA, xB, yA, yB}, {zA, zB, -, -}; +1 dummy pair
+    int32_t nidx[4][32];          // tiles 0, 1 of the P-P list and tiles 0, 1 of the P-C list
+    BucketDesc ndesc;             // descriptor of the next bucket
+};
+
+// per-lane partial sums of sink t in the pair layout, as scalars (correction path, reduction)
+__device__ __forceinline__ int acc_idx(int t, int comp, int lane) {  // comp 0..3 = ax ay az phi
+    return (((t >> 1) * 2 + (comp >> 1)) * 32 + lane) * 4 + (comp & 1) * 2 + (t & 1);
+}
+
+// One source against one sink pair, Newtonian with r^2 clamped from below at h2c (see pp_fast).
+// 13 packed FP instructions + 2 MUFU + min/max for 2 interactions; flops as pp_fast (19 each).
+template <bool SELF>
+__device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, const float4 s, bool selfA, bool selfB,
+                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw) {
+    const float2 dx = f2add(make_float2(txy.x, txy.y), sp(-s.x));
+    const float2 dy = f2add(make_float2(txy.z, txy.w), sp(-s.y));
+    const float2 dz = f2add(make_float2(tz.x, tz.y), sp(-s.z));
+    float2 r2 = f2fma(dz, dz, f2fma(dy, dy, f2mul(dx, dx)));
+    const float2 ri = make_float2(rsqrt_approx(fmaxf(r2.x, h2c)), rsqrt_approx(fmaxf(r2.y, h2c)));
+    const float2 ri2 = f2mul(ri, ri);
+    float2 nm = sp(-s.w);
+    if (SELF) {
+        nm.x = selfA ? 0.0f : nm.x; nm.y = selfB ? 0.0f : nm.y;
+        r2.x = selfA ? 3.0e38f : r2.x; r2.y = selfB ? 3.0e38f : r2.y;
+    }
+    minr2 = fminf(minr2, fminf(r2.x, r2.y));
+    const float2 nmri = f2mul(nm, ri);
+    const float2 nmg = f2mul(nmri, ri2);
+    ax = f2fma(nmg, dx, ax);
+    ay = f2fma(nmg, dy, ay);
+    az = f2fma(nmg, dz, az);
+    aw = f2add(aw, nmri);
+}
+
+struct PcPre2 { float2 dx, dy, dz, ri; };
+
+template <bool NEWTON>
+__device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, const CellRegs& c) {
+    PcPre2 q;
+    q.dx = f2add(make_float2(txy.x, txy.y), sp(-c.cx));
+    q.dy = f2add(make_float2(txy.z, txy.w), sp(-c.cy));
+    q.dz = f2add(make_float2(tz.x, tz.y), sp(-c.cz));
+    const float2 r2 = f2fma(q.dz, q.dz, f2fma(q.dy, q.dy, f2mul(q.dx, q.dx)));
+    float2 ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
+    if (NEWTON) {  // one Newton step on MUFU.RSQ: ri <- ri (1.5 - 0.5 r2 ri^2)
+        const float2 hy = f2mul(f2mul(sp(-0.5f), r2), ri);
+        ri = f2mul(ri, f2fma(hy, ri, sp(1.5f)));
+    }
+    q.ri = ri;
+    return q;
+}
+
+// One cell against one sink pair; the formulas of pc_body on packed values.  Each group of three FFMA2
+// shares its monomial operand (register reuse): the contraction runs at the FMA rate.
+#define PKDG_T0(CX, CY, CZ, M) vx = f2mul(sp(CX), M); vy = f2mul(sp(CY), M); vz = f2mul(sp(CZ), M);
+#define PKDG_T1(CX, CY, CZ, M) vx = f2fma(sp(CX), M, vx); vy = f2fma(sp(CY), M, vy); vz = f2fma(sp(CZ), M, vz);
+__device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1) {
+    const float2 ri2 = f2mul(q.ri, q.ri);
+    const float2 sr = f2mul(sp(c.s), ri2);
+    const float2 x = f2mul(q.dx, sr), y = f2mul(q.dy, sr), z = f2mul(q.dz, sr);  // tau
+    float2 vx, vy, vz;
+    PKDG_T0(c.xx, c.xy, c.xz, x) PKDG_T1(c.xy, c.yy, c.yz, y) PKDG_T1(c.xz, c.yz, c.zz, z)
+    const float2 v2x = vx, v2y = vy, v2z = vz;
+    const float2 xx = f2mul(x, x), yy = f2mul(y, y), zz = f2mul(z, z);
+    const float2 x2 = f2add(x, x), y2 = f2add(y, y);
+    const float2 xy = f2mul(x2, y), xz = f2mul(x2, z), yz = f2mul(y2, z);
+    PKDG_T0(c.xxx, c.xxy, c.xxz, xx) PKDG_T1(c.xyy, c.yyy, c.yyz, yy) PKDG_T1(c.xzz, c.yzz, c.zzz, zz)
+    PKDG_T1(c.xxy, c.xyy, c.xyz, xy) PKDG_T1(c.xxz, c.xyz, c.xzz, xz) PKDG_T1(c.xyz, c.yyz, c.yzz, yz)
+    const float2 v3x = vx, v3y = vy, v3z = vz;
+    const float2 x3 = f2mul(sp(3.0f), x), y3 = f2mul(sp(3.0f), y), z3 = f2mul(sp(3.0f), z);
+    const float2 m0 = f2mul(xx, x), m1 = f2mul(yy, y), m2 = f2mul(zz, z);
+    const float2 m3 = f2mul(xx, y3), m4 = f2mul(xx, z3), m5 = f2mul(yy, x3), m6 = f2mul(yy, z3);
+    const float2 m7 = f2mul(zz, x3), m8 = f2mul(zz, y3), m9 = f2mul(xy, z3);
+    PKDG_T0(c.xxxx, c.xxxy, c.xxxz, m0) PKDG_T1(c.xxxy, c.xxyy, c.xxyz, m3) PKDG_T1(c.xxxz, c.xxyz, c.xxzz, m4)
+    PKDG_T1(c.xxyy, c.xyyy, c.xyyz, m5) PKDG_T1(c.xxyz, c.xyyz, c.xyzz, m9) PKDG_T1(c.xxzz, c.xyzz, c.xzzz, m7)
+    PKDG_T1(c.xyyy, c.yyyy, c.yyyz, m1) PKDG_T1(c.xyyz, c.yyyz, c.yyzz, m6) PKDG_T1(c.xyzz, c.yyzz, c.yzzz, m8)
+    PKDG_T1(c.xzzz, c.yzzz, c.zzzz, m2)
+    float2 e2 = f2mul(v2x, x), e3 = f2mul(v3x, x), e4 = f2mul(vx, x);
+    e2 = f2fma(v2y, y, e2); e3 = f2fma(v3y, y, e3); e4 = f2fma(vy, y, e4);
+    e2 = f2fma(v2z, z, e2); e3 = f2fma(v3z, z, e3); e4 = f2fma(vz, z, e4);
+    const float2 fs = f2fma(sp(0.25f), e4, f2fma(sp(0.33333333333f), e3, f2fma(sp(0.5f), e2, sp(1.0f))));
+    const float2 S = f2fma(sp(2.25f), e4, f2fma(sp(2.3333333333f), e3, f2fma(sp(2.5f), e2, sp(1.0f))));
+    const float2 gx = f2add(f2add(v2x, v3x), vx), gy = f2add(f2add(v2y, v3y), vy), gz = f2add(f2add(v2z, v3z), vz);
+    const float2 mr = f2mul(sp(c.M), q.ri);
+    const float2 k3 = f2mul(mr, ri2);
+    const float2 sk = f2mul(sp(c.s), k3), Sk = f2mul(S, k3);
+    float2 ax = make_float2(a0.x, a0.y), ay = make_float2(a0.z, a0.w), az = make_float2(a1.x, a1.y),
+           aw = make_float2(a1.z, a1.w);
+    aw = f2fma(neg2(mr), fs, aw);
+    ax = f2fma(sk, gx, f2fma(neg2(Sk), q.dx, ax));
+    ay = f2fma(sk, gy, f2fma(neg2(Sk), q.dy, ay));
+    az = f2fma(sk, gz, f2fma(neg2(Sk), q.dz, az));
+    a0 = make_float4(ax.x, ax.y, ay.x, ay.y);
+    a1 = make_float4(az.x, az.y, aw.x, aw.y);
+}
+#undef PKDG_T0
+#undef PKDG_T1
+
+// Raw sinks of pass t0 and index tiles 0, 1 of both lists by plain loads (first bucket of a warp, passes > 0).
+__device__ __forceinline__ void fill_direct3(WarpSmem3& S, const EvalParams& p, const BucketDesc& d, ListLens L, int t0,
+                                             int buf, int lane) {
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+    __syncwarp();
+    const int ntp = max(0, min(kTMax, d.count - t0));
+    if (lane < kTMax) S.tgt[buf][lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
+    S.nidx[0][lane] = L.pp > 0 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 0, lane) : -1;
+    S.nidx[1][lane] = L.pp > 32 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 1, lane) : -1;
+    S.nidx[2][lane] = L.pc > 0 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 0, lane) : -1;
+    S.nidx[3][lane] = L.pc > 32 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 1, lane) : -1;
+    __syncwarp();
+}
+
+// The same for the NEXT bucket (descriptor already in S.ndesc), asynchronously.
+__device__ __forceinline__ void stage_next_bucket3(WarpSmem3& S, const EvalParams& p, int nbuf, bool do_pp, bool do_pc,
+                                                   int lane) {
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+    const BucketDesc nd = S.ndesc;
+    const ListLens L = eff_lens(nd, do_pp, do_pc);
+    const int ntp = max(0, min(kTMax, nd.count));
+    if (lane < kTMax) {
+        if (lane < ntp) cp_async16(&S.tgt[nbuf][lane], p.xyzm + nd.first + lane);
+        else S.tgt[nbuf][lane] = dummy_tgt;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int e = (q & 1) * 32 + lane;
+        const int len = q < 2 ? L.pp : L.pc;
+        const int32_t* src = q < 2 ? p.pp_idx + nd.pp_begin : p.pc_idx + nd.pc_begin;
+        if (e < len) cp_async4(&S.nidx[q][lane], src + e);
+        else S.nidx[q][lane] = -1;
+    }
+}
+
+// a2: raw sinks (visible to the warp) -> pair layout; pair kPMax is a dummy pair for the P-C pipeline.
+__device__ __forceinline__ void make_pairs(WarpSmem3& S, int buf, int lane) {
+    if (lane <= kPMax) {
+        const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+        const float4 A = lane < kPMax ? S.tgt[buf][2 * lane] : dummy_tgt;
+        const float4 B = lane < kPMax ? S.tgt[buf][2 * lane + 1] : dummy_tgt;
+        S.tp[2 * lane] = make_float4(A.x, B.x, A.y, B.y);
+        S.tp[2 * lane + 1] = make_float4(A.z, B.z, 0.0f, 0.0f);
+    }
+    __syncwarp();
+}
+
+// a3 for one pass, packed: NP sink pairs (4 or 8) in register accumulators.
+template <int NP>
+__device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
+                                          const float4* __restrict__ s_tgt, WarpSmem3& S, int lane, unsigned& bad) {
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const float4* __restrict__ tp = S.tp;
+    float4* __restrict__ s_acc = S.acc;
+    float* __restrict__ s_accf = reinterpret_cast<float*>(S.acc);
+    float2 ax[NP], ay[NP], az[NP], aw[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = make_float2(0.f, 0.f);
+    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
+    const int ntile = (pp_len + 31) >> 5;
+    const int sink0 = d.first + t0;
+    int32_t j = ntile > 0 ? S.nidx[0][lane] : -1;
+    int32_t jn = ntile > 1 ? S.nidx[1][lane] : -1;
+    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+    if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
+    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
+    float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
+    int32_t jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
+    for (int k = 0; k < ntile; ++k) {
+        // sources of the next two tiles and the index of the third are in flight during this tile
+        if ((uint32_t)jnn >= (uint64_t)p.n_particles) { bad += (jnn >= 0); jnn = -1; }
+        const float4 snn = jnn >= 0 ? __ldg(p.xyzm + jnn) : far4;
+        const int32_t jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
+        const int self_t = j - sink0;  // sink slot this source coincides with, if any
+        float minr2 = 3.0e38f;
+        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)(2 * NP))) {  // tile holds own particles
+#pragma unroll
+            for (int q = 0; q < NP; ++q)
+                pp_fast2<true>(tp[2 * q], tp[2 * q + 1], s, self_t == 2 * q, self_t == 2 * q + 1, p.h2c, minr2, ax[q],
+                               ay[q], az[q], aw[q]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < NP; ++q)
+                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q]);
+        }
+        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
+            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
+            // Newtonian contribution by the spline one, through the shared accumulators.
+            if (!smem_live) {
+                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                smem_live = true;
+            }
+            if (minr2 < p.h2c) {
+                for (int t = 0; t < ntp; ++t) {
+                    const float4 tg = s_tgt[t];
+                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
+                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    if (r2 < p.h2c && self_t != t) {
+                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
+                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
+                        float ri = rsqrt_approx(p.h2c);  // what pp_fast2 used for this pair
+                        float gc = ri * ri * ri, wc = -ri;
+                        float mg = s.w * (g - gc);
+                        s_accf[acc_idx(t, 0, lane)] = fmaf(-mg, dx, s_accf[acc_idx(t, 0, lane)]);
+                        s_accf[acc_idx(t, 1, lane)] = fmaf(-mg, dy, s_accf[acc_idx(t, 1, lane)]);
+                        s_accf[acc_idx(t, 2, lane)] = fmaf(-mg, dz, s_accf[acc_idx(t, 2, lane)]);
+                        s_accf[acc_idx(t, 3, lane)] = fmaf(s.w, w - wc, s_accf[acc_idx(t, 3, lane)]);
+                    }
+                }
+            }
+        }
+        s = sn; sn = snn; j = jn; jn = jnn; jnn = jn3;
+    }
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        float4 a0 = make_float4(ax[q].x, ax[q].y, ay[q].x, ay[q].y), a1 = make_float4(az[q].x, az[q].y, aw[q].x, aw[q].y);
+        if (smem_live) {
+            const float4 b0 = s_acc[(2 * q) * 32 + lane], b1 = s_acc[(2 * q + 1) * 32 + lane];
+            a0.x += b0.x; a0.y += b0.y; a0.z += b0.z; a0.w += b0.w;
+            a1.x += b1.x; a1.y += b1.y; a1.z += b1.z; a1.w += b1.w;
+        }
+        s_acc[(2 * q) * 32 + lane] = a0;
+        s_acc[(2 * q + 1) * 32 + lane] = a1;
+    }
+}
+
+template <int WARPS, int MINB, bool NEWTON>
+__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const EvalParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    WarpSmem3& S = reinterpret_cast<WarpSmem3*>(smem_raw)[warp];
+    float4* s_acc = S.acc;
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
+    unsigned bad = 0;
+
+    unsigned cur = 0;
+    if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
+    cur = __shfl_sync(0xffffffffu, cur, 0);
+    if ((int64_t)cur >= p.n_buckets) return;
+    BucketDesc d = p.desc[cur];
+    int buf = 0;
+    fill_direct3(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
+
+    for (;;) {
+        unsigned nxt = 0xffffffffu;
+        if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
+        bool has_next = false;
+        const ListLens L = eff_lens(d, do_pp, do_pc);
+        const int npass = max(1, (d.count + kTMax - 1) / kTMax);
+
+        for (int pass = 0; pass < npass; ++pass) {
+            const int t0 = pass * kTMax;
+            const int ntp = max(0, min(kTMax, d.count - t0));
+            const bool last = pass == npass - 1;
+            if (pass > 0) fill_direct3(S, p, d, L, t0, buf, lane);
+            const float4* s_tgt = S.tgt[buf];
+
+            // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
+            const int pc_ntile = (L.pc + 31) >> 5;
+            int32_t c = pc_ntile > 0 ? S.nidx[2][lane] : -1;
+            int32_t cn = pc_ntile > 1 ? S.nidx[3][lane] : -1;
+            if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
+            if (c >= 0) {
+                const float4* q = p.cellq + (int64_t)c * 8;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
+            }
+            cp_async_commit();
+
+            // ---- a2: pair layout of the sinks;  a3: P-P
+            make_pairs(S, buf, lane);
+            if (ntp <= 8) pp_phase3<4>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+            else pp_phase3<8>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+
+            // ---- next bucket, stage 1: its descriptor
+            if (last) {
+                const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
+                has_next = (int64_t)nb < p.n_buckets;
+                if (has_next && lane < 2)
+                    cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
+                               reinterpret_cast<const char*>(p.desc + nb) + 16 * lane);
+                cp_async_commit();
+            }
+
+            // ---- a4: P-C.  One sink pair per iteration; the lane's cell stays in registers for the tile.
+            {
+                const int npair = (ntp + 1) >> 1;  // odd count: the last pair's second half is a dummy sink
+                const float4* tp = S.tp;
+                for (int k = 0; k < pc_ntile; ++k) {
+                    const int32_t c2 = (k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
+                    cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
+                    CellRegs cr;
+                    if (c >= 0) {
+                        cell_unpack(cr, S.stage[lane], S.stage[32 + lane], S.stage[64 + lane], S.stage[96 + lane],
+                                    S.stage[128 + lane], S.stage[160 + lane], S.stage[192 + lane], S.stage[224 + lane]);
+                    } else {
+                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
+                    }
+                    if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
+                    if (cn >= 0) {  // next tile's record; the slot was read into registers just above
+                        const float4* q = p.cellq + (int64_t)cn * 8;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
+                    }
+                    if (last && k == pc_ntile - 1 && has_next) {  // next bucket, stage 2
+                        __syncwarp();
+                        stage_next_bucket3(S, p, buf ^ 1, do_pp, do_pc, lane);
+                    }
+                    cp_async_commit();
+                    PcPre2 pA = pc_pre2<NEWTON>(tp[0], tp[1], cr);
+#pragma unroll 1
+                    for (int q = 0; q < npair; ++q) {
+                        const PcPre2 nA = pc_pre2<NEWTON>(tp[2 * q + 2], tp[2 * q + 3], cr);
+                        float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
+                        pc_body2(pA, cr, a0, a1);
+                        s_acc[(2 * q) * 32 + lane] = a0;
+                        s_acc[(2 * q + 1) * 32 + lane] = a1;
+                        pA = nA;
+                    }
+                    c = cn; cn = c2;
+                }
+                if (last && pc_ntile == 0 && has_next) {
+                    cp_async_wait_all();
+                    __syncwarp();
+                    stage_next_bucket3(S, p, buf ^ 1, do_pp, do_pc, lane);
+                    cp_async_commit();
+                }
+            }
+            // ---- a5: cross-lane reduction and write-back
+            float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
+            if (ntp <= 8) {
+                float v[32];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
+                    v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
+                    v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
+                }
+                warp_transpose_reduce<32>(v, lane);
+                if ((lane >> 2) < ntp) {
+                    float r = v[0];
+                    if (accumulate) r += outf[lane];
+                    outf[lane] = r;
+                }
+            } else {
+                float v[64];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
+                    v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
+                    v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
+                }
+                warp_transpose_reduce<64>(v, lane);
+                if ((lane >> 1) < ntp) {
+                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
+                    float2 r = make_float2(v[0], v[1]);
+                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
+                    *o2 = r;
+                }
+            }
+        }
+        if (!has_next) break;
+        cp_async_wait_all();
+        __syncwarp();
+        d = S.ndesc;
+        buf ^= 1;
+    }
+    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
+}
+
 // FFMA-only probe: 8 independent chains per thread, `iters` rounds of 8 FFMA.
 __global__ void pkdg_fma_probe_kernel(float* out, int64_t iters, float a, float b) {
     float v0 = threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5, v6 = v0 + 6, v7 = v0 + 7;
