@@ -31,7 +31,7 @@ sys.path.insert(0, ROOT)
 # line by line in DESIGN.md "Flop audit".  The paper's own convention (Table 3: 53 / 215, rsqrt = 7)
 # is reported beside it as context only.
 F_PP = 19
-F_PC = 196
+F_PC_BY_VARIANT = {0: 187, 1: 196, 2: 187, 3: 192}   # packed default / scalar generation 1 / packed 128-reg / packed + Newton
 PAPER_F_PP, PAPER_F_PC = 53, 215
 SM_COUNT_NOMINAL, FP32_LANES_PER_SM = 148, 128
 
@@ -217,6 +217,7 @@ def run_ours(args, rank, world, local_rank):
     ms_step = ms_total / args.steps
     inter = p.I_pp + p.I_pc
     value = world * inter / (ms_step * 1e-3)
+    F_PC = F_PC_BY_VARIANT[args.variant]
     flops = F_PP * p.I_pp + F_PC * p.I_pc
 
     # ---- end to end: every buffer starts in pinned host memory, result read back every step
@@ -267,7 +268,7 @@ def run_ours(args, rank, world, local_rank):
     if os.path.exists(tpath):
         with open(tpath) as f:
             traffic = json.load(f).get(f"cfg3_ng{args.ng}")
-    roofline = {"bound": "alu", "kernel": "pkdg_eval_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "pkdg_eval3_kernel" if args.variant != 1 else "pkdg_eval_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic,
                 "peak_kind": f"{sms} SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json clock)",
                 "kernel_ms": eval_ms, "kernel_share_of_step": eval_ms / ms_step,
@@ -291,7 +292,7 @@ def run_ours(args, rank, world, local_rank):
             "flops_per_s": world * flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / peak_tflops,
             "paper_convention_tflops": world * (PAPER_F_PP * p.I_pp + PAPER_F_PC * p.I_pc) / (ms_step * 1e-3) / 1e12,
             "interactions_per_s": {"pp": world * p.I_pp / (ms_step * 1e-3), "pc": world * p.I_pc / (ms_step * 1e-3)},
-            "gen_seconds": round(gen_s, 1)}
+            "gen_seconds": round(gen_s, 1), "kernel_variant": args.variant}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -102,29 +102,6 @@ pkdg_status launch_eval_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
 }
 
 template <int WARPS, int MINB, bool NEWTON>
-pkdg_status launch_eval2_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
-    auto kern = pkdg_eval2_kernel<WARPS, MINB, NEWTON>;
-    const int smem = WARPS * (int)sizeof(WarpSmem);
-    static bool configured = false;  // per instantiation; the attribute is per function and sticky
-    if (!configured) {
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        configured = true;
-    }
-    int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
-    if (per_sm < 1) per_sm = 1;
-    int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
-    int64_t grid = (int64_t)ctx->num_sms * per_sm;
-    if (grid > want) grid = want;
-    if (grid < 1) grid = 1;
-    kern<<<(unsigned)grid, WARPS * 32, smem, st>>>(p);
-    ctx->launches++;
-    CK(cudaGetLastError());
-    return PKDG_OK;
-}
-
-template <int WARPS, int MINB, bool NEWTON>
 pkdg_status launch_eval3_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     auto kern = pkdg_eval3_kernel<WARPS, MINB, NEWTON>;
     const int smem = WARPS * (int)sizeof(WarpSmem3);
@@ -151,21 +128,10 @@ pkdg_status launch_eval3_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) 
 pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     unsigned variant = (p.flags >> PKDG_VARIANT_SHIFT) & 0xffu;
     switch (variant) {
-        case 0:
-        case 1: return launch_eval_t<4, 4, true, 2>(ctx, p, st);
-        case 2: return launch_eval_t<4, 3, true, 2>(ctx, p, st);
-        case 3: return launch_eval_t<4, 4, false, 2>(ctx, p, st);
-        case 4: return launch_eval_t<4, 5, true, 1>(ctx, p, st);
-        case 5: return launch_eval_t<4, 4, true, 1>(ctx, p, st);
-        case 6: return launch_eval_t<4, 5, false, 1>(ctx, p, st);
-        case 7: return launch_eval_t<4, 6, false, 1>(ctx, p, st);
-        case 8: return launch_eval2_t<4, 4, true>(ctx, p, st);
-        case 9: return launch_eval2_t<4, 4, false>(ctx, p, st);
-        case 10: return launch_eval2_t<4, 3, false>(ctx, p, st);
-        case 11: return launch_eval3_t<4, 3, false>(ctx, p, st);
-        case 12: return launch_eval3_t<4, 4, false>(ctx, p, st);
-        case 13: return launch_eval3_t<4, 3, true>(ctx, p, st);
-        case 14: return launch_eval3_t<4, 2, false>(ctx, p, st);
+        case 0: return launch_eval3_t<4, 3, false>(ctx, p, st);   // packed FP32x2, 168 registers, 12 warps / SM
+        case 1: return launch_eval_t<4, 4, true, 2>(ctx, p, st);  // generation 1: scalar arithmetic (A/B reference)
+        case 2: return launch_eval3_t<4, 4, false>(ctx, p, st);   // packed, 128 registers, 16 warps / SM
+        case 3: return launch_eval3_t<4, 3, true>(ctx, p, st);    // packed, Newton step on the P-C rsqrt
         default: return fail(ctx, PKDG_EINVAL, "unknown kernel variant in flags bits 8..15");
     }
 }

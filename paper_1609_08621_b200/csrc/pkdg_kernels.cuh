@@ -577,25 +577,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalP
 }
 
 // ------------------------------------------------------------------------------------------------
-// Evaluation kernel, generation 2 (the library default).  Same mapping and arithmetic as above; what
-// changes is WHEN data moves (profiles/r01_eval_ng128_v1.md: 45 % of warp time was spent waiting on
-// dependent global loads in the per-bucket and per-tile prologues, the FP loops got only 48 %):
-//   * the cell records of P-C tile k+1 are fetched with cp.async into a per-lane shared-memory slot
-//     while tile k is evaluated (tile 0: during the P-P phase) -- a guaranteed landing spot instead
-//     of an L1 prefetch that 16 warps x 4 KB evict before use;
-//   * the NEXT bucket is claimed (atomic) at the start of the current one; its descriptor, its sinks
-//     and the first two tiles of both index lists are fetched with cp.async during the current
-//     bucket's P-C phase, so a bucket starts with one exposed global round trip instead of four;
-//   * P-P sources are gathered two tiles ahead, indices three.
+// Asynchronous staging helpers (cp.async = LDGSTS): global -> shared memory without registers.
 // ------------------------------------------------------------------------------------------------
-struct __align__(16) WarpSmem {
-    float4 acc[kTMax * 32];       // [sink slot][lane] per-lane partial sums
-    float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
-    float4 tgt[2][kTMax + 2];     // sinks of the current / the next bucket
-    int32_t nidx[4][32];          // tiles 0, 1 of the P-P list and tiles 0, 1 of the P-C list
-    BucketDesc ndesc;             // descriptor of the next bucket
-};
-
 __device__ __forceinline__ uint32_t smem_u32(const void* q) { return (uint32_t)__cvta_generic_to_shared(q); }
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
@@ -612,258 +595,6 @@ __device__ __forceinline__ ListLens eff_lens(const BucketDesc& d, bool do_pp, bo
     l.pp = (do_pp && d.count > 0) ? d.pp_len : 0;
     l.pc = (do_pc && d.count > 0) ? d.pc_len : 0;
     return l;
-}
-
-// Sinks of pass t0 and index tiles 0, 1 of both lists by plain loads (first bucket of a warp, passes > 0).
-__device__ __forceinline__ void fill_direct(WarpSmem& S, const EvalParams& p, const BucketDesc& d, ListLens L, int t0,
-                                            int buf, int lane) {
-    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-    __syncwarp();
-    const int ntp = max(0, min(kTMax, d.count - t0));
-    if (lane < kTMax + 2) S.tgt[buf][lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
-    S.nidx[0][lane] = L.pp > 0 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 0, lane) : -1;
-    S.nidx[1][lane] = L.pp > 32 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 1, lane) : -1;
-    S.nidx[2][lane] = L.pc > 0 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 0, lane) : -1;
-    S.nidx[3][lane] = L.pc > 32 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 1, lane) : -1;
-    __syncwarp();
-}
-
-// The same for the NEXT bucket (descriptor already in S.ndesc), asynchronously.
-__device__ __forceinline__ void stage_next_bucket(WarpSmem& S, const EvalParams& p, int nbuf, bool do_pp, bool do_pc,
-                                                  int lane) {
-    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-    const BucketDesc nd = S.ndesc;
-    const ListLens L = eff_lens(nd, do_pp, do_pc);
-    const int ntp = max(0, min(kTMax, nd.count));
-    if (lane < kTMax + 2) {
-        if (lane < ntp) cp_async16(&S.tgt[nbuf][lane], p.xyzm + nd.first + lane);
-        else S.tgt[nbuf][lane] = dummy_tgt;
-    }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int e = (q & 1) * 32 + lane;
-        const int len = q < 2 ? L.pp : L.pc;
-        const int32_t* src = q < 2 ? p.pp_idx + nd.pp_begin : p.pc_idx + nd.pc_begin;
-        if (e < len) cp_async4(&S.nidx[q][lane], src + e);
-        else S.nidx[q][lane] = -1;
-    }
-}
-
-template <int NS>
-__device__ __forceinline__ void pp_phase2(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
-                                          const float4* __restrict__ s_tgt, float4* __restrict__ s_acc,
-                                          const WarpSmem& S, int lane, unsigned& bad) {
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    float4 acc[NS];
-#pragma unroll
-    for (int t = 0; t < NS; ++t) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
-    const int ntile = (pp_len + 31) >> 5;
-    const int sink0 = d.first + t0;
-    int32_t j = ntile > 0 ? S.nidx[0][lane] : -1;
-    int32_t jn = ntile > 1 ? S.nidx[1][lane] : -1;
-    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
-    if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
-    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
-    float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
-    int32_t jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
-    for (int k = 0; k < ntile; ++k) {
-        // sources of the next two tiles and the index of the third are in flight during this tile
-        if ((uint32_t)jnn >= (uint64_t)p.n_particles) { bad += (jnn >= 0); jnn = -1; }
-        const float4 snn = jnn >= 0 ? __ldg(p.xyzm + jnn) : far4;
-        const int32_t jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
-        const int self_t = j - sink0;  // sink slot this source coincides with, if any
-        float minr2 = 3.0e38f;
-        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)NS)) {  // tile holds own particles
-#pragma unroll
-            for (int t = 0; t < NS; ++t) pp_fast<true>(s_tgt[t], s, self_t == t, p.h2c, minr2, acc[t]);
-        } else {
-#pragma unroll
-            for (int t = 0; t < NS; ++t) pp_fast<false>(s_tgt[t], s, false, p.h2c, minr2, acc[t]);
-        }
-        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
-            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
-            // Newtonian contribution by the spline one, through the shared accumulators.
-            if (!smem_live) {
-                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-                smem_live = true;
-            }
-            if (minr2 < p.h2c) {
-                for (int t = 0; t < ntp; ++t) {
-                    const float4 tg = s_tgt[t];
-                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
-                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    if (r2 < p.h2c && self_t != t) {
-                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
-                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
-                        float ri = rsqrt_approx(p.h2c);  // what pp_fast used for this pair
-                        float gc = ri * ri * ri, wc = -ri;
-                        float4 a = s_acc[t * 32 + lane];
-                        float mg = s.w * (g - gc);
-                        a.x = fmaf(-mg, dx, a.x); a.y = fmaf(-mg, dy, a.y); a.z = fmaf(-mg, dz, a.z);
-                        a.w = fmaf(s.w, w - wc, a.w);
-                        s_acc[t * 32 + lane] = a;
-                    }
-                }
-            }
-        }
-        s = sn; sn = snn; j = jn; jn = jnn; jnn = jn3;
-    }
-    if (smem_live) {
-#pragma unroll
-        for (int t = 0; t < NS; ++t) {
-            float4 a = s_acc[t * 32 + lane];
-            a.x += acc[t].x; a.y += acc[t].y; a.z += acc[t].z; a.w += acc[t].w;
-            s_acc[t * 32 + lane] = a;
-        }
-    } else {
-#pragma unroll
-        for (int t = 0; t < NS; ++t) s_acc[t * 32 + lane] = acc[t];
-    }
-}
-
-template <int WARPS, int MINB, bool NEWTON>
-__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval2_kernel(const EvalParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
-    float4* s_acc = S.acc;
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
-    unsigned bad = 0;
-
-    unsigned cur = 0;
-    if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
-    cur = __shfl_sync(0xffffffffu, cur, 0);
-    if ((int64_t)cur >= p.n_buckets) return;
-    BucketDesc d = p.desc[cur];
-    int buf = 0;
-    fill_direct(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
-
-    for (;;) {
-        unsigned nxt = 0xffffffffu;
-        if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
-        bool has_next = false;
-        const ListLens L = eff_lens(d, do_pp, do_pc);
-        const int npass = max(1, (d.count + kTMax - 1) / kTMax);
-
-        for (int pass = 0; pass < npass; ++pass) {
-            const int t0 = pass * kTMax;
-            const int ntp = max(0, min(kTMax, d.count - t0));
-            const bool last = pass == npass - 1;
-            if (pass > 0) fill_direct(S, p, d, L, t0, buf, lane);
-            const float4* s_tgt = S.tgt[buf];
-
-            // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
-            const int pc_ntile = (L.pc + 31) >> 5;
-            int32_t c = pc_ntile > 0 ? S.nidx[2][lane] : -1;
-            int32_t cn = pc_ntile > 1 ? S.nidx[3][lane] : -1;
-            if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
-            if (c >= 0) {
-                const float4* q = p.cellq + (int64_t)c * 8;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
-            }
-            cp_async_commit();
-
-            // ---- a3: P-P
-            if (ntp <= 8) pp_phase2<8>(p, d, L.pp, t0, ntp, s_tgt, s_acc, S, lane, bad);
-            else pp_phase2<16>(p, d, L.pp, t0, ntp, s_tgt, s_acc, S, lane, bad);
-
-            // ---- next bucket, stage 1: its descriptor
-            if (last) {
-                const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
-                has_next = (int64_t)nb < p.n_buckets;
-                if (has_next && lane < 2)
-                    cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
-                               reinterpret_cast<const char*>(p.desc + nb) + 16 * lane);
-                cp_async_commit();
-            }
-
-            // ---- a4: P-C.  Two sinks per iteration; the lane's cell stays in registers for the tile.
-            {
-                const int nte = (ntp + 1) & ~1;  // odd count: the last iteration also visits the dummy slot
-                for (int k = 0; k < pc_ntile; ++k) {
-                    const int32_t c2 = (k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
-                    cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
-                    CellRegs cr;
-                    if (c >= 0) {
-                        cell_unpack(cr, S.stage[lane], S.stage[32 + lane], S.stage[64 + lane], S.stage[96 + lane],
-                                    S.stage[128 + lane], S.stage[160 + lane], S.stage[192 + lane], S.stage[224 + lane]);
-                    } else {
-                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
-                    }
-                    if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
-                    if (cn >= 0) {  // next tile's record; the slot was read into registers just above
-                        const float4* q = p.cellq + (int64_t)cn * 8;
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
-                    }
-                    if (last && k == pc_ntile - 1 && has_next) {  // next bucket, stage 2
-                        __syncwarp();
-                        stage_next_bucket(S, p, buf ^ 1, do_pp, do_pc, lane);
-                    }
-                    cp_async_commit();
-                    PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr), pB = pc_pre<NEWTON>(s_tgt[1], cr);
-#pragma unroll 1
-                    for (int t = 0; t < nte; t += 2) {
-                        const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 2], cr), nB = pc_pre<NEWTON>(s_tgt[t + 3], cr);
-                        float4 aA = s_acc[t * 32 + lane], aB = s_acc[(t + 1) * 32 + lane];
-                        pc_body(pA, cr, aA);
-                        pc_body(pB, cr, aB);
-                        s_acc[t * 32 + lane] = aA;
-                        s_acc[(t + 1) * 32 + lane] = aB;
-                        pA = nA; pB = nB;
-                    }
-                    c = cn; cn = c2;
-                }
-                if (last && pc_ntile == 0 && has_next) {
-                    cp_async_wait_all();
-                    __syncwarp();
-                    stage_next_bucket(S, p, buf ^ 1, do_pp, do_pc, lane);
-                    cp_async_commit();
-                }
-            }
-            // ---- a5: cross-lane reduction and write-back
-            float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
-            if (ntp <= 8) {
-                float v[32];
-#pragma unroll
-                for (int t = 0; t < 8; ++t) {
-                    const float4 a = s_acc[t * 32 + lane];
-                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
-                }
-                warp_transpose_reduce<32>(v, lane);
-                if ((lane >> 2) < ntp) {
-                    float r = v[0];
-                    if (accumulate) r += outf[lane];
-                    outf[lane] = r;
-                }
-            } else {
-                float v[64];
-#pragma unroll
-                for (int t = 0; t < 16; ++t) {
-                    const float4 a = s_acc[t * 32 + lane];
-                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
-                }
-                warp_transpose_reduce<64>(v, lane);
-                if ((lane >> 1) < ntp) {
-                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
-                    float2 r = make_float2(v[0], v[1]);
-                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
-                    *o2 = r;
-                }
-            }
-        }
-        if (!has_next) break;
-        cp_async_wait_all();
-        __syncwarp();
-        d = S.ndesc;
-        buf ^= 1;
-    }
-    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
 
 // ------------------------------------------------------------------------------------------------
