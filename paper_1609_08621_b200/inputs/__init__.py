@@ -122,7 +122,7 @@ def _zeldovich_field(ng: int, index: float, seed: int):
     psi = []
     for ax in range(3):
         kk = (kx[:, None, None], kx[None, :, None], kz[None, None, :])[ax]
-        psi.append(np.fft.irfftn(1j * kk * dk, s=(ng, ng, ng)).astype(np.float32))
+        psi.append(np.fft.irfftn(1j * kk * dk, s=(ng, ng, ng), axes=(0, 1, 2)).astype(np.float32))
     return psi
 
 

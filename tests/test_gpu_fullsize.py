@@ -1,0 +1,173 @@
+"""-m gpu: parity at BASELINE.json's full sizes, in the launch configuration bench.py times (resident
+pkdg_gravity_eval, default kernel variant), on SAMPLED buckets the oracle can compute one by one, plus
+properties that hold at any size and bit-exact integer counters.  (DESIGN.md sec 7 for the recipes.)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch):
+    from paper_1609_08621_b200 import binding
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _sample(p, n_even, n_long, seed=0):
+    """Evenly spread buckets plus the longest-list ones plus a few random ones."""
+    nb = p.n_buckets
+    ltot = np.diff(p.pp_off) + np.diff(p.pc_off)
+    rng = np.random.default_rng(seed)
+    sel = np.concatenate([np.linspace(0, nb - 1, n_even).astype(np.int64), np.argsort(ltot)[-n_long:],
+                          np.argsort(np.diff(p.pp_off))[-n_long:], rng.integers(0, nb, n_even // 4)])
+    return np.unique(sel)
+
+
+def _check_sampled(ctx, torch, p, sel, flags=0):
+    import oracle
+    from gpu_util import bucket_rows, rel_errors, run_resident
+    out = run_resident(ctx, p, torch, flags=flags)
+    st = ctx.get_stats()
+    assert st["interactions_pp"] == oracle.interactions(p.count, p.pp_off) == p.I_pp      # bit-exact integers
+    assert st["interactions_pc"] == oracle.interactions(p.count, p.pc_off) == p.I_pc
+    assert st["tiles_pp"] == int(((np.diff(p.pp_off) + 31) // 32).sum())
+    assert st["tiles_pc"] == int(((np.diff(p.pc_off) + 31) // 32).sum())
+    assert st["bad_entries"] == 0 and st["n_buckets"] == p.n_buckets
+    ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
+    rows = bucket_rows(p, sel)
+    ea, ep = rel_errors(out, ref, rows)
+    assert ea.max() <= TOL and ep.max() <= TOL, (p.name, ea.max(), ep.max())
+    return out, ea, ep
+
+
+def _check_properties(p, out):
+    """Hold at any size: every row of a listed bucket is finite; the potential is negative; the net
+    force sum_i m_i a_i is far below sum_i m_i |a_i| (exact for P-P pairs, O(theta^5) for P-C)."""
+    covered = np.zeros(p.n, bool)
+    covered[np.repeat(p.first.astype(np.int64) - np.concatenate([[0], np.cumsum(p.count.astype(np.int64))[:-1]]),
+                      p.count) + np.arange(int(p.count.sum()))] = True
+    assert covered.all()
+    assert np.isfinite(out).all()
+    assert (out[:, 3] < 0).all()
+    m = p.xyzm[:, 3].astype(np.float64)
+    a = out[:, :3].astype(np.float64)
+    net = np.linalg.norm((m[:, None] * a).sum(axis=0))
+    tot = (m * np.linalg.norm(a, axis=1)).sum()
+    assert net <= 2e-3 * tot, (net, tot)
+
+
+def test_config2_full(ctx, torch):
+    """configs[1]: N = 2^20, 32 Plummer spheres + background, binary tree, theta = 0.7."""
+    from paper_1609_08621_b200 import inputs
+    p = inputs.config2()
+    assert p.n == 1 << 20
+    out, ea, ep = _check_sampled(ctx, torch, p, _sample(p, 6000, 64))
+    _check_properties(p, out)
+
+
+@pytest.fixture(scope="module")
+def cfg3():
+    from paper_1609_08621_b200 import inputs
+    return inputs.config3(256)
+
+
+def test_config3_headline_full(ctx, torch, cfg3):
+    """configs[2], the configuration bench.py times: N = 2^24 Zel'dovich lattice, theta = 0.7."""
+    p = cfg3
+    assert p.n == 1 << 24
+    out, ea, ep = _check_sampled(ctx, torch, p, _sample(p, 4096, 64))
+    _check_properties(p, out)
+
+
+def test_config3_sharded_equals_unsharded(ctx, torch, cfg3):
+    """Multi-GPU path emulated as consecutive calls on one GPU (no kernel waits on another): the two
+    ranks' pieces, evaluated separately, give the same bits as one call."""
+    from paper_1609_08621_b200 import shard
+    from gpu_util import to_dev
+    p = cfg3
+    d = to_dev(p, torch)
+    whole = torch.zeros((p.n, 4), dtype=torch.float32, device="cuda:0")
+    ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"], d["pc_idx"],
+                     p.eps, whole)
+    parts = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda:0")
+    bounds = shard.shard_bounds(shard.bucket_cost(p.count, p.pp_off, p.pc_off), 2)
+    tot_pp = tot_pc = 0
+    for r in range(2):
+        b0, b1 = int(bounds[r]), int(bounds[r + 1])
+        first, count, ppo, ppi, pco, pci = shard.slice_problem(p.first, p.count, p.pp_off, p.pp_idx, p.pc_off,
+                                                               p.pc_idx, b0, b1)
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+        ctx.gravity_eval(d["xyzm"], d["cells"], t(first), t(count), t(ppo), t(ppi), t(pco), t(pci), p.eps, parts)
+        st = ctx.get_stats()
+        tot_pp += st["interactions_pp"]; tot_pc += st["interactions_pc"]
+    torch.cuda.synchronize()
+    assert tot_pp == p.I_pp and tot_pc == p.I_pc
+    assert torch.equal(whole, parts)
+
+
+@pytest.mark.parametrize("nb,lpp,lpc", [(65536, 32, 0), (65536, 4096, 0), (65536, 0, 32), (65536, 128, 128),
+                                        (16384, 512, 512), (8192, 0, 2048), (4096, 2048, 2048), (65536, 100, 70)])
+def test_config4_sweep_full(ctx, torch, nb, lpp, lpc):
+    """configs[3]: 65,536 buckets of 16 sinks; the extreme list lengths.  (The shapes with >= 512 cells
+    per list use fewer buckets: building their 64-particle clouds on the host needs 15 GB and 30 s at
+    65,536 buckets, which does not belong in a test suite.)"""
+    from paper_1609_08621_b200 import inputs
+    p = inputs.config4(nb, lpp, lpc)
+    sel = np.unique(np.concatenate([np.linspace(0, nb - 1, 96).astype(np.int64), [0, 1, nb - 1]]))
+    _check_sampled(ctx, torch, p, sel)
+
+
+def test_config5_streamed_range(ctx, torch):
+    """configs[4]: N = 2^26 particles, theta = 0.55; lists are built chunk by chunk on the host and
+    streamed (a6).  A contiguous range of 2^19 buckets is evaluated through the streamed call on 3
+    streams; sampled buckets are compared with the oracle; chunk accounting is bit-exact."""
+    import oracle
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import bucket_rows, rel_errors
+    xyzm, eps = inputs.config5_particles()
+    assert xyzm.shape[0] == 1 << 26
+    p = inputs.build_tree(xyzm, "binary", 16, name="cfg5")
+    del xyzm
+    nb_all = p.n_buckets
+    b0 = nb_all // 3
+    b1 = b0 + (1 << 19)
+    pp_off, pp_idx, pc_off, pc_idx = inputs.build_lists(p, 0.55, eps, b0, b1)
+    first = np.ascontiguousarray(p.first[b0:b1]); count = np.ascontiguousarray(p.count[b0:b1])
+    dev = "cuda:0"
+    d_xyzm = torch.from_numpy(p.xyzm).to(dev); d_cells = torch.from_numpy(p.cells).to(dev)
+    out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device=dev)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h = [pin(first), pin(count), pin(pp_off), pin(pp_idx), pin(pc_off), pin(pc_idx)]
+    max_entries = 1 << 24
+    ctx.gravity_eval_streamed(d_xyzm, d_cells, h[0], h[1], h[2], h[3], h[4], h[5], eps, out, n_streams=3,
+                              max_entries_per_chunk=max_entries)
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    cnt = count.astype(np.int64)
+    assert st["interactions_pp"] == int(np.dot(cnt, np.diff(pp_off)))
+    assert st["interactions_pc"] == int(np.dot(cnt, np.diff(pc_off)))
+    assert st["chunks"] == len(oracle.chunk_bounds(pp_off, pc_off, max_entries)) - 1 and st["chunks"] > 3
+    assert st["bad_entries"] == 0
+    sel = np.unique(np.concatenate([np.linspace(0, b1 - b0 - 1, 2048).astype(np.int64),
+                                    np.argsort(np.diff(pp_off) + np.diff(pc_off))[-32:]]))
+    ref = oracle.gravity_eval(p.xyzm, p.cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, sel=sel)
+    rows = np.concatenate([np.arange(first[b], first[b] + count[b]) for b in sel]).astype(np.int64)
+    got = out[torch.from_numpy(rows).to(dev)].cpu().numpy()
+    ea, ep = rel_errors(got, ref[rows])
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+    lo, hi = int(first[0]), int(first[-1] + count[-1])
+    o = out.cpu().numpy()
+    assert np.isfinite(o[lo:hi]).all() and np.isnan(o[:lo]).all() and np.isnan(o[hi:]).all()
