@@ -163,6 +163,17 @@ void pkdg_version(int32_t *major, int32_t *minor);
  * FFMA rounds on every SM and returns the elapsed milliseconds and the flop count. Synchronous. */
 pkdg_status pkdg_fma_peak_probe(pkdg_ctx *ctx, int64_t iters, float *ms_host, double *flops_host);
 
+/* The same for other operand patterns (DESIGN.md sec 6 "register-file bandwidth"): registers only, no
+ * memory in the timed loop, 4 CTAs of 128 threads per SM.  flops_host counts FMA = 2 and, for modes 4
+ * and 5, the audited flops of the P-C body (196 scalar with Newton step, 187 packed). */
+#define PKDG_PROBE_FFMA_CONST 0   /* FFMA, two constant-bank operands: the FMA-pipe peak               */
+#define PKDG_PROBE_FFMA_3REG 1    /* scalar FFMA, three distinct register operands                      */
+#define PKDG_PROBE_FFMA2_3REG 2   /* packed FFMA2, three distinct register pairs                        */
+#define PKDG_PROBE_FFMA2_REUSE 3  /* FFMA2 scalar x pair + pair, pair shared by 3 consecutive FFMA2     */
+#define PKDG_PROBE_PC_SCALAR 4    /* generation-1 scalar P-C body, two sinks per trip                   */
+#define PKDG_PROBE_PC_PACKED 5    /* packed P-C body of the default kernel, one sink pair per trip      */
+pkdg_status pkdg_fma_probe(pkdg_ctx *ctx, int32_t mode, int64_t iters, float *ms_host, double *flops_host);
+
 #ifdef __cplusplus
 }
 #endif

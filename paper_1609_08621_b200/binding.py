@@ -27,7 +27,7 @@ CELLQ_FLOATS = 32
 EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
            "pkdg_get_stats", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version",
-           "pkdg_fma_peak_probe"]
+           "pkdg_fma_peak_probe", "pkdg_fma_probe"]
 
 
 class PkdgError(RuntimeError):
@@ -87,6 +87,7 @@ def _load():
     L.pkdg_last_error.restype = c_char_p
     L.pkdg_version.argtypes = [POINTER(c_int32), POINTER(c_int32)]
     L.pkdg_fma_peak_probe.argtypes = [c_void_p, c_int64, POINTER(c_float), POINTER(c_double)]
+    L.pkdg_fma_probe.argtypes = [c_void_p, c_int32, c_int64, POINTER(c_float), POINTER(c_double)]
     for name in EXPORTS:
         if name not in ("pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version"):
             getattr(L, name).restype = c_int32
@@ -249,6 +250,13 @@ class Context:
 
     def launch_count(self) -> int:
         return int(_lib.pkdg_launch_count(self._h))
+
+    def fma_probe(self, mode: int, iters: int = 1 << 12):
+        """(ms, flops) of probe `mode` (PKDG_PROBE_*: 0 const-operand FFMA, 1 3-register FFMA, 2 FFMA2,
+        3 FFMA2 with operand reuse, 4 scalar P-C body, 5 packed P-C body)."""
+        ms, fl = c_float(), c_double()
+        self._check(_lib.pkdg_fma_probe(self._h, int(mode), int(iters), byref(ms), byref(fl)), "pkdg_fma_probe")
+        return ms.value, fl.value
 
     def fma_peak_probe(self, iters: int = 1 << 14):
         ms, fl = c_float(), c_double()

@@ -521,26 +521,65 @@ void pkdg_version(int32_t* major, int32_t* minor) {
     if (minor) *minor = PKDG_VERSION_MINOR;
 }
 
-pkdg_status pkdg_fma_peak_probe(pkdg_ctx* ctx, int64_t iters, float* ms_host, double* flops_host) {
+pkdg_status pkdg_fma_probe(pkdg_ctx* ctx, int32_t mode, int64_t iters, float* ms_host, double* flops_host) {
     if (!ctx || !ms_host || !flops_host || iters < 1) return PKDG_EINVAL;
+    if (mode < 0 || mode > 5) return fail(ctx, PKDG_EINVAL, "probe mode must be in 0..5");
     CK(cudaSetDevice(ctx->device));
-    const int threads = 256, blocks = ctx->num_sms * 8;
-    float* buf = nullptr;
-    CK(cudaMalloc((void**)&buf, sizeof(float) * threads * blocks));
+    const int threads = mode == 0 ? 256 : 128, blocks = ctx->num_sms * (mode == 0 ? 8 : 4);
+    float *buf = nullptr, *in = nullptr;
+    CK(cudaMalloc((void**)&buf, sizeof(float4) * threads * blocks));
+    // input: 1024 operands around 0.5; 32 synthetic cell records (COM, M, s, small moments); 2 sinks
+    float h[2048];
+    for (int i = 0; i < 1024; ++i) h[i] = 0.5f + 0.001f * (float)(i % 97);
+    float* hc = h + 1024;
+    for (int i = 0; i < 32 * 32; ++i) hc[i] = 0.01f * (float)(i % 13) - 0.03f;
+    for (int l = 0; l < 32; ++l) {
+        hc[l * 32 + 0] = 0.1f * l; hc[l * 32 + 1] = 0.2f; hc[l * 32 + 2] = 0.3f; hc[l * 32 + 3] = 1.0f;
+        hc[l * 32 + 4] = 0.05f;
+    }
+    const float tgt[8] = {5.f, 6.f, 7.f, 0.f, -5.f, 6.f, -7.f, 0.f};
+    CK(cudaMalloc((void**)&in, sizeof(h) + sizeof(tgt)));
+    CK(cudaMemcpy(in, h, sizeof(h), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(in + 2048, tgt, sizeof(tgt), cudaMemcpyHostToDevice));
+    const float4* cells = reinterpret_cast<const float4*>(in + 1024);
+    const float4* tg = reinterpret_cast<const float4*>(in + 2048);
+    auto launch = [&](int64_t n) {
+        switch (mode) {
+            case 0: pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, n, 0.999f, 0.001f); break;
+            case 1: pkdg_rf_probe_kernel<1><<<blocks, threads>>>(in, buf, n); break;
+            case 2: pkdg_rf_probe_kernel<2><<<blocks, threads>>>(in, buf, n); break;
+            case 3: pkdg_rf_probe_kernel<3><<<blocks, threads>>>(in, buf, n); break;
+            case 4: pkdg_pc_probe_kernel<false><<<blocks, threads>>>(cells, tg, reinterpret_cast<float4*>(buf), n); break;
+            default: pkdg_pc_probe_kernel<true><<<blocks, threads>>>(cells, tg, reinterpret_cast<float4*>(buf), n); break;
+        }
+    };
+    if (mode >= 4) iters = (iters + 1) & ~(int64_t)1;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, 16, 0.999f, 0.001f);  // warm-up
+    launch(16);  // warm-up
     CK(cudaEventRecord(e0, 0));
-    pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, iters, 0.999f, 0.001f);
+    launch(iters);
     CK(cudaEventRecord(e1, 0));
     CK(cudaEventSynchronize(e1));
     ctx->launches += 2;
+    CK(cudaGetLastError());
     CK(cudaEventElapsedTime(ms_host, e0, e1));
-    *flops_host = 2.0 * 64.0 * (double)iters * threads * blocks;
+    const double lanes = (double)threads * blocks;
+    switch (mode) {
+        case 0: case 1: *flops_host = 2.0 * 64.0 * (double)iters * lanes; break;  // 64 FFMA per trip
+        case 2: case 3: *flops_host = 4.0 * 64.0 * (double)iters * lanes; break;  // 64 FFMA2 per trip
+        case 4: *flops_host = 2.0 * 196.0 * (double)iters * lanes; break;         // 2 sinks per trip
+        default: *flops_host = 2.0 * 187.0 * (double)iters * lanes; break;        // 1 sink pair per trip
+    }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     CK(cudaFree(buf));
+    CK(cudaFree(in));
     return PKDG_OK;
+}
+
+pkdg_status pkdg_fma_peak_probe(pkdg_ctx* ctx, int64_t iters, float* ms_host, double* flops_host) {
+    return pkdg_fma_probe(ctx, PKDG_PROBE_FFMA_CONST, iters, ms_host, flops_host);
 }
 
 }  // extern "C"

@@ -1008,7 +1008,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
 
-// FFMA-only probe: 8 independent chains per thread, `iters` rounds of 8 FFMA.
+// ------------------------------------------------------------------------------------------------
+// Probes (pkdg_fma_probe): what the FP32 pipe delivers for a given operand pattern.  Registers only, no
+// memory in the timed loop; 4 CTAs of 128 threads per SM.  Results in DESIGN.md sec 6.
+//   0  FFMA with two constant-bank operands (one register read per FMA): the FMA-pipe peak
+//   1  FFMA, three distinct register operands
+//   2  FFMA2 (packed), three distinct register pairs
+//   3  FFMA2, scalar x pair + pair with the pair operand shared by three consecutive instructions
+//   4  the scalar P-C body of generation 1 (pc_pre + pc_body), two sinks per trip
+//   5  the packed P-C body (pc_pre2 + pc_body2), one sink pair per trip
+// ------------------------------------------------------------------------------------------------
 __global__ void pkdg_fma_probe_kernel(float* out, int64_t iters, float a, float b) {
     float v0 = threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5, v6 = v0 + 6, v7 = v0 + 7;
     for (int64_t i = 0; i < iters; ++i) {
@@ -1019,6 +1028,74 @@ __global__ void pkdg_fma_probe_kernel(float* out, int64_t iters, float a, float 
         }
     }
     out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
+}
+
+// modes 1-3: 64 (packed) FMA instructions per trip; `in` holds >= 1024 floats around 0.5
+template <int MODE>
+__global__ void __launch_bounds__(128, 4) pkdg_rf_probe_kernel(const float* __restrict__ in, float* __restrict__ out,
+                                                               int64_t iters) {
+    float2 x[8], y[8], a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        x[i] = make_float2(in[threadIdx.x + 32 * i], in[threadIdx.x + 32 * i + 1]);
+        y[i] = make_float2(in[threadIdx.x + 32 * i + 256], in[threadIdx.x + 32 * i + 257]);
+        a[i] = make_float2(in[threadIdx.x + 32 * i + 512], in[threadIdx.x + 32 * i + 513]);
+    }
+    for (int64_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (MODE == 1) a[i].x = fmaf(x[i].x, y[(i + u) & 7].x, a[i].x);
+                if (MODE == 2) a[i] = __ffma2_rn(x[i], y[(i + u) & 7], a[i]);
+                if (MODE == 3) a[i] = __ffma2_rn(make_float2(x[i].x, x[i].x), y[(3 * u + i / 3) & 7], a[i]);
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i].x + a[i].y;
+    out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// modes 4, 5: `cells` = 32 internal records (one per lane), `tg` = 2 sinks
+template <bool PACKED>
+__global__ void __launch_bounds__(128, 4) pkdg_pc_probe_kernel(const float4* __restrict__ cells,
+                                                               const float4* __restrict__ tg, float4* __restrict__ out,
+                                                               int64_t iters) {
+    CellRegs cr;
+    const float4* q = cells + (threadIdx.x & 31) * 8;
+    cell_unpack(cr, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7]);
+    float4 tA = tg[0], tB = tg[1];
+    float4 r;
+    if (PACKED) {
+        float4 txy = make_float4(tA.x, tB.x, tA.y, tB.y), tz = make_float4(tA.z, tB.z, 0.f, 0.f);
+        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
+        PcPre2 pA = pc_pre2<false>(txy, tz, cr);
+#pragma unroll 1
+        for (int64_t it = 0; it < iters; it += 2) {
+            txy.x += 1e-3f; txy.w += 1e-3f;
+            const PcPre2 pB = pc_pre2<false>(txy, tz, cr);
+            pc_body2(pA, cr, a0, a1);
+            txy.y += 1e-3f; txy.z += 1e-3f;
+            pA = pc_pre2<false>(txy, tz, cr);
+            pc_body2(pB, cr, a0, a1);
+        }
+        r = make_float4(a0.x + a0.y, a0.z + a0.w, a1.x + a1.y, a1.z + a1.w);
+    } else {
+        float4 aA = make_float4(0.f, 0.f, 0.f, 0.f), aB = aA;
+        PcPre pA = pc_pre<true>(tA, cr), pB = pc_pre<true>(tB, cr);
+#pragma unroll 1
+        for (int64_t it = 0; it < iters; ++it) {
+            tA.x += 1e-3f; tB.y += 1e-3f;
+            const PcPre nA = pc_pre<true>(tA, cr), nB = pc_pre<true>(tB, cr);
+            pc_body(pA, cr, aA);
+            pc_body(pB, cr, aB);
+            pA = nA; pB = nB;
+        }
+        r = make_float4(aA.x + aB.x, aA.y + aB.y, aA.z + aB.z, aA.w + aB.w);
+    }
+    out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = r;
 }
 
 }  // namespace pkdg
