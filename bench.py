@@ -298,6 +298,144 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------
+# --report: every BASELINE.json config through the resident call (kernel-only timing from the
+# library's CUDA events, median of `reps`), the oracle timed and compared on a bounded sample of the
+# same buckets.  One JSON line per case; not the driver's contract line (that is the default mode).
+# ------------------------------------------------------------------------------------------------
+def report_case(name, p, ctx, torch, binding, peak_tflops, reps, variant, cpu_seconds, note=""):
+    dev = torch.device("cuda", 0)
+    t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    has_pc = p.cells is not None and p.cells.shape[0] > 0 and p.pc_off is not None
+    d = dict(xyzm=t(p.xyzm), cells=t(p.cells) if has_pc else None, first=t(p.first), count=t(p.count),
+             pp_off=t(p.pp_off), pp_idx=t(p.pp_idx), pc_off=t(p.pc_off) if has_pc else None,
+             pc_idx=t(p.pc_idx) if has_pc else None)
+    out = torch.zeros((p.n, 4), dtype=torch.float32, device=dev)
+    flags = variant << binding.VARIANT_SHIFT
+    step = lambda: ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"],
+                                    d["pc_off"], d["pc_idx"], p.eps, out, flags=flags)
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    ctx.profile_read(); ctx.profile_enable(True)
+    kms, sms_ = [], []
+    for _ in range(reps):
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(); step(); e1.record(); torch.cuda.synchronize()
+        n, ms = ctx.profile_read()
+        kms.append(ms / max(n, 1)); sms_.append(e0.elapsed_time(e1))
+    ctx.profile_enable(False)
+    st = ctx.get_stats()
+    I_pp, I_pc = p.I_pp, (p.I_pc if has_pc else 0)
+    assert st["interactions_pp"] == I_pp and st["interactions_pc"] == I_pc and st["bad_entries"] == 0
+    k_med, k_best = float(np.median(kms)), float(min(kms))
+    flops = F_PP * I_pp + F_PC_BY_VARIANT[variant] * I_pc
+    line = {"case": name, "n_particles": p.n, "n_buckets": p.n_buckets, "I_pp": I_pp, "I_pc": I_pc,
+            "mean_L_pp": round(float(np.diff(p.pp_off).mean()), 1) if p.pp_off is not None else 0,
+            "mean_L_pc": round(float(np.diff(p.pc_off).mean()), 1) if has_pc else 0,
+            "kernel_ms_median": k_med, "kernel_ms_best": k_best, "step_ms_median": float(np.median(sms_)),
+            "interactions_per_s": (I_pp + I_pc) / (k_med * 1e-3), "tflops": flops / (k_med * 1e-3) / 1e12,
+            "frac_fp32_fma_peak": flops / (k_med * 1e-3) / 1e12 / peak_tflops,
+            "paper_convention_tflops": (PAPER_F_PP * I_pp + PAPER_F_PC * I_pc) / (k_med * 1e-3) / 1e12, "note": note}
+    if cpu_seconds > 0:
+        import oracle
+        nb = p.n_buckets
+        cost = p.count.astype(np.int64) * ((np.diff(p.pp_off) if p.pp_off is not None else 0) +
+                                           (np.diff(p.pc_off) if has_pc else 0))
+        per_bucket = max(float(cost.mean()), 1.0) / 3.0e6 * 1.0      # ~3e6 interactions/s per core-second guess
+        n_s = int(min(nb, max(64, cpu_seconds * oracle.num_threads() / max(per_bucket, 1e-9))))
+        sel = np.unique(np.linspace(0, nb - 1, n_s).astype(np.int64))
+        args = (p.xyzm, p.cells if has_pc else None, p.first, p.count,
+                p.pp_off if p.pp_off is not None else np.zeros(nb + 1, np.int64),
+                p.pp_idx if p.pp_idx is not None else np.zeros(0, np.int32),
+                p.pc_off if has_pc else np.zeros(nb + 1, np.int64), p.pc_idx if has_pc else np.zeros(0, np.int32), p.eps)
+        t0 = time.perf_counter()
+        ref = oracle.gravity_eval(*args, sel=sel)
+        dt = time.perf_counter() - t0
+        rows = np.concatenate([np.arange(p.first[b], p.first[b] + p.count[b]) for b in sel]).astype(np.int64)
+        got = out[torch.from_numpy(rows).to(dev)].cpu().numpy().astype(np.float64)
+        r = ref[rows]
+        ea = np.linalg.norm(got[:, :3] - r[:, :3], axis=1) / np.linalg.norm(r[:, :3], axis=1)
+        ep = np.abs(got[:, 3] - r[:, 3]) / np.abs(r[:, 3])
+        S = oracle.contribution_norms(*args, sel=sel)   # conditioning of each sum
+        kappa = S[rows] / np.linalg.norm(r[:, :3], axis=1)
+        line.update({"kappa_max": float(kappa.max()), "kappa_median": float(np.median(kappa)),
+                     "max_err_over_kappa": float((ea / kappa).max()), "n_sampled_particles": int(len(rows)),
+                     "n_acc_err_above_2e-5": int((ea > 2e-5).sum())})
+        line.update({"oracle_interactions_per_s": float(cost[sel].sum()) / dt, "oracle_cores": oracle.num_threads(),
+                     "oracle_sample": f"{len(sel)} of {nb} buckets, {dt:.1f} s",
+                     "max_rel_err_acc": float(ea.max()), "max_rel_err_pot": float(ep.max())})
+    print(json.dumps(line), flush=True)
+    del d, out
+    torch.cuda.empty_cache()
+    return line
+
+
+def run_report(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --report: no CUDA device; the product path has no CPU fallback")
+    from paper_1609_08621_b200 import binding, inputs
+    peaks, _ = load_peaks()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    peak = sms * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    ctx = binding.Context(0)
+    rc = lambda name, p, note="": report_case(name, p, ctx, torch, binding, peak, args.report_reps, args.variant,
+                                              args.cpu_seconds, note)
+    lines = []
+    want = set(args.report.split(","))
+    if "1" in want or "all" in want:
+        lines.append(rc("cfg1 N=4096 uniform, octree", inputs.config1()))
+    if "2" in want or "all" in want:
+        lines.append(rc("cfg2 N=2^20 Plummer mix", inputs.config2()))
+    if "3" in want or "all" in want:
+        lines.append(rc(f"cfg3 N={args.ng}^3 Zel'dovich (headline)", inputs.config3(args.ng)))
+    if "4" in want or "all" in want:
+        nb = 65536
+        for lpp in (32, 128, 512, 2048, 4096):
+            lines.append(rc(f"cfg4 P-P only L_pp={lpp}", inputs.config4(nb, lpp, 0), "reuse 16"))
+        for lpc, nbc in ((32, 65536), (128, 65536), (512, 16384), (2048, 8192)):
+            lines.append(rc(f"cfg4 P-C only L_pc={lpc}", inputs.config4(nbc, 0, lpc), f"{nbc} buckets, reuse 16"))
+        for l, nbc in ((32, 65536), (128, 65536), (512, 16384), (2048, 4096)):
+            lines.append(rc(f"cfg4 fused L_pp=L_pc={l}", inputs.config4(nbc, l, l), f"{nbc} buckets, reuse 16"))
+    if "5" in want or "all" in want:
+        # N = 2^26: a contiguous range of 2^20 buckets (lists built for that range), resident and streamed
+        xyzm, eps = inputs.config5_particles()
+        p = inputs.build_tree(xyzm, "binary", 16, name="cfg5")
+        del xyzm
+        b0 = p.n_buckets // 3; b1 = b0 + (1 << 20)
+        pp_off, pp_idx, pc_off, pc_idx = inputs.build_lists(p, 0.55, eps, b0, b1)
+        q = inputs.Problem(name="cfg5_range", xyzm=p.xyzm, cells=p.cells, first=np.ascontiguousarray(p.first[b0:b1]),
+                           count=np.ascontiguousarray(p.count[b0:b1]), pp_off=pp_off, pp_idx=pp_idx, pc_off=pc_off,
+                           pc_idx=pc_idx, eps=eps)
+        ln = rc("cfg5 N=2^26 theta=0.55, 2^20 of %d buckets, resident" % p.n_buckets, q)
+        lines.append(ln)
+        dev = torch.device("cuda", 0)
+        d_x = torch.from_numpy(q.xyzm).to(dev); d_c = torch.from_numpy(q.cells).to(dev)
+        out = torch.zeros((q.n, 4), dtype=torch.float32, device=dev)
+        pin = lambda a: torch.from_numpy(a).pin_memory()
+        h = [pin(q.first), pin(q.count), pin(pp_off), pin(pp_idx), pin(pc_off), pin(pc_idx)]
+        for ns, chunk in ((1, 1 << 24), (3, 1 << 24), (3, 1 << 26)):
+            ts = []
+            for _ in range(4):
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                ctx.gravity_eval_streamed(d_x, d_c, h[0], h[1], h[2], h[3], h[4], h[5], eps, out, n_streams=ns,
+                                          max_entries_per_chunk=chunk, flags=args.variant << binding.VARIANT_SHIFT)
+                e1.record(); torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            st = ctx.get_stats()
+            ms = float(np.median(ts[1:]))
+            sl = {"case": f"cfg5 streamed lists, {ns} stream(s), chunk {chunk} entries", "chunks": st["chunks"],
+                  "ms": ms, "interactions_per_s": (q.I_pp + q.I_pc) / (ms * 1e-3),
+                  "h2d_gb": (pp_idx.nbytes + pc_idx.nbytes + pp_off.nbytes + pc_off.nbytes + 8 * q.n_buckets) / 1e9,
+                  "resident_kernel_ms": ln["kernel_ms_median"]}
+            print(json.dumps(sl), flush=True)
+            lines.append(sl)
+    ctx.close()
+    return lines
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -311,10 +449,16 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=3)
     ap.add_argument("--e2e-chunk", type=int, default=1 << 25)
+    ap.add_argument("--report", default="", help="comma list of configs (1,2,3,4,5 or all): per-case report lines "
+                                                  "instead of the contract line")
+    ap.add_argument("--report-reps", type=int, default=10)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.report:
+        if rank == 0:
+            run_report(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

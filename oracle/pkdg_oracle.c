@@ -230,6 +230,59 @@ int orc_gravity_eval(int64_t n_particles, const float *xyzm, int64_t n_cells, co
     return err;
 }
 
+/* ---------------------------------------------------------------------------
+ * Conditioning of the sum (reading A17): for each target of the
+ * evaluated buckets, S_i = sum over its list entries of |a_ij| (the Euclidean norm
+ * of each entry's acceleration contribution, from the same pair functions as
+ * above).  kappa_i = S_i / |a_i| measures the cancellation in a_i; a relative
+ * error of any finite-precision evaluation grows in proportion to it.  Diagnostic
+ * only: no evaluation result depends on it.  out_abs: [n_particles] fp64.
+ * ------------------------------------------------------------------------- */
+int orc_contribution_norms(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
+                           int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
+                           const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
+                           const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
+                           double *out_abs) {
+    int64_t nb = sel ? n_sel : n_buckets;
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t ib = 0; ib < nb; ++ib) {
+        int64_t b = sel ? sel[ib] : ib;
+        if (b < 0 || b >= n_buckets) {
+#pragma omp atomic write
+            err = 1;
+            continue;
+        }
+        for (int32_t ti = 0; ti < count[b]; ++ti) {
+            int64_t i = (int64_t)first[b] + ti;
+            if (i < 0 || i >= n_particles) continue;
+            double xt[3] = {xyzm[4 * i], xyzm[4 * i + 1], xyzm[4 * i + 2]};
+            double S = 0.0;
+            if (pp_off) {
+                for (int64_t e = pp_off[b]; e < pp_off[b + 1]; ++e) {
+                    int64_t j = pp_idx[e];
+                    if (j < 0 || j == i || j >= n_particles) continue;
+                    double xs[3] = {xyzm[4 * j], xyzm[4 * j + 1], xyzm[4 * j + 2]};
+                    double a[3] = {0, 0, 0}, pot = 0;
+                    orc_pp_pair(xt, xs, (double)xyzm[4 * j + 3], eps, a, &pot);
+                    S += sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+                }
+            }
+            if (pc_off) {
+                for (int64_t e = pc_off[b]; e < pc_off[b + 1]; ++e) {
+                    int64_t c = pc_idx[e];
+                    if (c < 0 || c >= n_cells) continue;
+                    double a[3] = {0, 0, 0}, pot = 0;
+                    orc_pc_pair(xt, cells + c * (int64_t)stride, a, &pot);
+                    S += sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+                }
+            }
+            out_abs[i] = S;
+        }
+    }
+    return err;
+}
+
 /* Direct summation: the plain definition the tree method approximates
  * (PAPER.md:L57).  For each listed target, the softened sum over ALL other
  * particles.  Used only to pin the oracle (north_star self-checks 1, 3, 4). */

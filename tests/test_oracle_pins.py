@@ -448,3 +448,28 @@ def test_chunk_bounds_greedy():
         if hi < 8:                                               # greedy: one more bucket would not fit
             assert pp_off[hi + 1] - pp_off[lo] > 30 or pc_off[hi + 1] - pc_off[lo] > 30
     assert list(oracle.chunk_bounds(np.array([0]), np.array([0]), 10)) == [0]
+
+
+def test_contribution_norms_diagnostic():
+    """S_i = sum_j |a_ij| (conditioning diagnostic): one source -> |a|; two equal sources on opposite
+    sides -> a = 0 but S = 2 |a_1|; always S >= |a|."""
+    xyzm = np.array([[0.5, 0.5, 0.5, 1.0], [0.7, 0.5, 0.5, 2.0], [0.3, 0.5, 0.5, 2.0]], np.float32)
+    first = np.array([0], np.int32); count = np.array([1], np.int32)
+    z = np.zeros(2, np.int64); e = np.zeros(0, np.int32)
+    a1 = 2.0 / np.float64(np.float32(0.7) - np.float32(0.5)) ** 2
+    for idx, want_a, want_s in (([1], a1, a1), ([1, 2], None, None)):
+        off = np.array([0, len(idx)], np.int64); ii = np.array(idx, np.int32)
+        ref = oracle.gravity_eval(xyzm, None, first, count, off, ii, z, e, 0.0)
+        S = oracle.contribution_norms(xyzm, None, first, count, off, ii, z, e, 0.0)
+        an = np.linalg.norm(ref[0, :3])
+        assert S[0] >= an * (1 - 1e-15) and np.isnan(S[1:]).all()
+        if want_a is not None:
+            assert abs(an - want_a) < 1e-12 * want_a and abs(S[0] - want_s) < 1e-12 * want_s
+        else:
+            d1 = np.float64(np.float32(0.7)) - 0.5; d2 = 0.5 - np.float64(np.float32(0.3))
+            assert abs(S[0] - (2.0 / d1 ** 2 + 2.0 / d2 ** 2)) < 1e-12 * S[0]
+            assert an < 1e-5 * S[0]
+    p = inputs.config1(512, seed=5)
+    ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
+    S = oracle.contribution_norms(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
+    assert (S >= np.linalg.norm(ref[:, :3], axis=1) * (1 - 1e-12)).all()
