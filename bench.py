@@ -447,8 +447,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
-    ap.add_argument("--e2e-streams", type=int, default=3)
-    ap.add_argument("--e2e-chunk", type=int, default=1 << 25)
+    ap.add_argument("--e2e-streams", type=int, default=4)
+    ap.add_argument("--e2e-chunk", type=int, default=1 << 23)
     ap.add_argument("--report", default="", help="comma list of configs (1,2,3,4,5 or all): per-case report lines "
                                                   "instead of the contract line")
     ap.add_argument("--report-reps", type=int, default=10)

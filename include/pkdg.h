@@ -118,7 +118,10 @@ pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx *ctx, const pkdg_particles *part
 /* End-to-end variant: EVERY buffer is a host buffer (pinned for full speed).  Copies particles and
  * cells to the device, streams the lists as above, copies the result back into out_acc_pot_host and
  * synchronises before returning.  Rows of particles in no bucket come back as 0 (as the caller's
- * values with PKDG_ACCUMULATE). */
+ * values with PKDG_ACCUMULATE).  When the buckets tile the particle array (first[0] = 0, every bucket
+ * starts where the previous one ends, the last one ends at n: the tree order of PAPER.md:L63) the rows
+ * of each chunk are copied back on the chunk's stream as soon as its kernel is done, overlapping the
+ * host->device traffic of later chunks. */
 pkdg_status pkdg_gravity_eval_host(pkdg_ctx *ctx, const pkdg_particles *particles_host,
                                    const pkdg_cells *cells_host, const pkdg_buckets *buckets_host,
                                    const pkdg_list *pp_host, const pkdg_list *pc_host, float eps,

@@ -297,10 +297,13 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     return s;
 }
 
-pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C,
-                                       const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
-                                       uint32_t flags, float* out, int32_t n_streams, int64_t max_entries,
-                                       void* stream) {
+// out_host != NULL: the rows of every chunk (buckets are then known to be contiguous runs in ascending
+// order, see pkdg_gravity_eval_host) are copied back on the chunk's stream right after its kernel, so
+// the device->host traffic overlaps the host->device traffic of later chunks (PCIe is full duplex).
+static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C,
+                                 const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
+                                 uint32_t flags, float* out, int32_t n_streams, int64_t max_entries,
+                                 void* stream, float* out_host) {
     pkdg_status s = check_common(ctx, P, C, Bh, pph, pch, out);
     if (s != PKDG_OK) return s;
     if (n_streams < 1 || n_streams > kMaxSlots) return fail(ctx, PKDG_EINVAL, "n_streams must be in 1..8");
@@ -375,6 +378,11 @@ pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, c
         p.work_counter = counter;
         p.n_buckets = cb;
         if ((rc = launch_eval(ctx, p, sl.st)) != PKDG_OK) break;
+        if (out_host) {
+            const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];
+            if (r1 > r0 && cudaMemcpyAsync(out_host + 4 * r0, out + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
+                                           cudaMemcpyDeviceToHost, sl.st) != cudaSuccess) { rc = PKDG_ECUDA; break; }
+        }
         if (cudaEventRecord(sl.done, sl.st) != cudaSuccess) { rc = PKDG_ECUDA; break; }
         sl.busy = true;
     }
@@ -384,6 +392,13 @@ pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, c
             rc = PKDG_ECUDA;
     if (rc == PKDG_ECUDA && ctx->err.empty()) ctx->err = cudaGetErrorString(cudaGetLastError());
     return rc;
+}
+
+pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C,
+                                       const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
+                                       uint32_t flags, float* out, int32_t n_streams, int64_t max_entries,
+                                       void* stream) {
+    return streamed_impl(ctx, P, C, Bh, pph, pch, eps, flags, out, n_streams, max_entries, stream, nullptr);
 }
 
 pkdg_status pkdg_gravity_eval_host(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch,
@@ -410,10 +425,18 @@ pkdg_status pkdg_gravity_eval_host(pkdg_ctx* ctx, const pkdg_particles* Ph, cons
         CK(cudaMemsetAsync(ctx->e2e_out, 0, sizeof(float) * 4 * Ph->n, st));  // rows in no bucket come back as 0
     }
     pkdg_particles Pd = {ctx->e2e_xyzm, Ph->n};
-    s = pkdg_gravity_eval_streamed(ctx, &Pd, has_pc ? &Cd : nullptr, Bh, pph, has_pc ? pch : nullptr, eps, flags,
-                                   ctx->e2e_out, n_streams, max_entries, st);
+    // tree-ordered input (every bucket starts where the previous one ends, together they cover all rows):
+    // each chunk's rows go back as soon as they are done; anything else: one copy at the end
+    bool tiled = Bh->n > 0 && Bh->first[0] == 0;
+    for (int64_t b = 0; tiled && b < Bh->n; ++b) {
+        const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
+        tiled = Bh->count[b] >= 0 && end == (b + 1 < Bh->n ? (int64_t)Bh->first[b + 1] : Ph->n);
+    }
+    s = streamed_impl(ctx, &Pd, has_pc ? &Cd : nullptr, Bh, pph, has_pc ? pch : nullptr, eps, flags, ctx->e2e_out,
+                      n_streams, max_entries, st, tiled ? out_host : nullptr);
     if (s != PKDG_OK) return s;
-    if (Ph->n) CK(cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st));
+    if (!tiled && Ph->n)
+        CK(cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return PKDG_OK;
 }
