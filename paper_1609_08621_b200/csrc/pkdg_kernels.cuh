@@ -2,12 +2,14 @@
 // problem statement and DESIGN.md for the kernel design and its roofline.
 //
 // Kernels:
-//   pkdg_prep_cells_kernel  canonical raw-moment records -> normalised trace-free records (128 B)
-//   pkdg_pack_kernel        a1: bucket work descriptors, tile counts, validation, I_pp / I_pc
-//   pkdg_tiles_kernel       a1: materialised 32-entry tiles (pkdg_pack_export)
-//   pkdg_eval_kernel<TB>    a2-a5: one warp per bucket, lanes stride the source lists, TB sinks
-//                           register-blocked per pass, butterfly transpose-reduction, float4 store
-//   pkdg_fma_probe_kernel   FFMA-only loop (roofline denominator check)
+//   pkdg_prep_cells_kernel   canonical raw-moment records -> normalised trace-free records (128 B)
+//   pkdg_pack_kernel         a1: bucket work descriptors, tile counts, validation, I_pp / I_pc
+//   pkdg_tiles_kernel        a1: materialised 32-entry tiles (pkdg_pack_export)
+//   pkdg_eval3_kernel        a2-a5, library default: one warp per bucket, lanes stride the source
+//                            lists, packed FP32x2 arithmetic over sink pairs, cp.async staging of
+//                            cell records and of the next bucket, butterfly transpose-reduction
+//   pkdg_eval_kernel         generation 1 of the same mapping (scalar FFMA, L1 prefetch): variant 1
+//   pkdg_*_probe_kernel      operand-pattern probes (roofline denominator, register-file study)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
