@@ -50,6 +50,14 @@ typedef int32_t pkdg_status;
 #define PKDG_ACCUMULATE 0x1u /* add to out instead of overwriting it */
 #define PKDG_SKIP_PP 0x2u    /* ignore the P-P lists (kernel studies) */
 #define PKDG_SKIP_PC 0x4u    /* ignore the P-C lists */
+#define PKDG_PP_LEAVES 0x8u  /* the P-P list's entries are BUCKET indices (into `buckets`), each standing for
+                                all particles of that bucket, <= 16 of them (SURVEY.md sec 8(f) NEXT-1,
+                                range-compressed P-P entries; a leaf that fails the
+                                opening test joins the P-P list whole).  16 times fewer list bytes and
+                                contiguous source gathers.  interactions_pp counts the particles the
+                                references stand for, tiles_pp two references per tile.  With the
+                                streamed variants `buckets_host` must hold ALL buckets a reference may
+                                name (it always does: references index it).                           */
 #define PKDG_VARIANT_SHIFT 8 /* bits 8..15: kernel tuning variant, 0 = library default */
 
 typedef struct pkdg_ctx pkdg_ctx;

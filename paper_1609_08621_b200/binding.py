@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libpkdg.so")
 ACCUMULATE = 0x1
 SKIP_PP = 0x2
 SKIP_PC = 0x4
+PP_LEAVES = 0x8
 VARIANT_SHIFT = 8
 CELL_FLOATS = 36
 CELLQ_FLOATS = 32

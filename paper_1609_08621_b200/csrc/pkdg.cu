@@ -48,6 +48,10 @@ struct pkdg_ctx {
     int64_t e2e_np = 0, e2e_nc = 0, e2e_no = 0;
     int64_t* scan_tmp = nullptr;
     int64_t scan_cap = 0;
+    int2* gfc = nullptr;               // PKDG_PP_LEAVES: (first, count) of every bucket
+    int64_t gfc_cap = 0;
+    int32_t *g_first = nullptr, *g_count = nullptr;  // streamed variants: device copy of the bucket arrays
+    int64_t g_first_cap = 0, g_count_cap = 0;
     cudaStream_t last_stream = nullptr;
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
@@ -127,6 +131,8 @@ pkdg_status launch_eval3_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) 
 // Tuning variants (flags bits 8..15).  0 = library default.
 pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     unsigned variant = (p.flags >> PKDG_VARIANT_SHIFT) & 0xffu;
+    if ((p.flags & PKDG_PP_LEAVES) && variant == 1)
+        return fail(ctx, PKDG_EINVAL, "PKDG_PP_LEAVES is not implemented by kernel variant 1 (generation 1)");
     switch (variant) {
         case 0: return launch_eval3_t<4, 3, false>(ctx, p, st);   // packed FP32x2, 168 registers, 12 warps / SM
         case 1: return launch_eval_t<4, 4, true, 2>(ctx, p, st);  // generation 1: scalar arithmetic (A/B reference)
@@ -173,6 +179,17 @@ pkdg_status prep_cells(pkdg_ctx* ctx, const pkdg_cells* C, float* dst, cudaStrea
     int threads = 128;
     int64_t blocks = (C->n + threads - 1) / threads;
     pkdg_prep_cells_kernel<<<(unsigned)blocks, threads, 0, st>>>(C->rec, C->n, C->stride_floats, dst);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+// (first, count) records of all n buckets from DEVICE arrays (PKDG_PP_LEAVES)
+pkdg_status build_gfc(pkdg_ctx* ctx, const int32_t* first, const int32_t* count, int64_t n, int64_t n_particles,
+                      cudaStream_t st) {
+    pkdg_status s = ensure(ctx, &ctx->gfc, &ctx->gfc_cap, n);
+    if (s != PKDG_OK || n == 0) return s;
+    pkdg_fc_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(first, count, n, n_particles, ctx->gfc);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -236,6 +253,7 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
     cudaDeviceSynchronize();
     cudaFree(ctx->cellq); cudaFree(ctx->desc); cudaFree(ctx->stats); cudaFree(ctx->counters);
     cudaFree(ctx->e2e_xyzm); cudaFree(ctx->e2e_cells); cudaFree(ctx->e2e_out); cudaFree(ctx->scan_tmp);
+    cudaFree(ctx->gfc); cudaFree(ctx->g_first); cudaFree(ctx->g_count);
     for (int i = 0; i < ctx->n_slots_live; ++i) {
         Slot& s = ctx->slots[i];
         cudaFree(s.pp_idx); cudaFree(s.pc_idx); cudaFree(s.first); cudaFree(s.count);
@@ -270,9 +288,12 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     {
         int threads = 256;
         int64_t blocks = (B->n + threads - 1) / threads;
+        const bool leaves = has_pp && (flags & PKDG_PP_LEAVES);
+        if (leaves && (s = build_gfc(ctx, B->first, B->count, B->n, P->n, st)) != PKDG_OK) return s;
         pkdg_pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(B->first, B->count, has_pp ? pp->offsets : nullptr,
                                                              has_pc ? pc->offsets : nullptr, B->n, P->n, 0, 0,
-                                                             ctx->desc, ctx->stats, ctx->counters + kMaxSlots);
+                                                             ctx->desc, ctx->stats, ctx->counters + kMaxSlots,
+                                                             leaves ? pp->idx : nullptr, ctx->gfc, B->n);
         ctx->launches++;
         CK(cudaGetLastError());
     }
@@ -283,6 +304,8 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     p.pc_idx = has_pc ? pc->idx : nullptr;
     p.work_counter = ctx->counters + kMaxSlots;
     p.n_buckets = B->n;
+    p.gfc = ctx->gfc;
+    p.n_gbuckets = B->n;
     const bool prof = ctx->profiling && ctx->prof_n < 256;
     if (prof) {
         for (int i = 0; i < 2; ++i)
@@ -319,6 +342,14 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     if (has_pc) {
         if ((s = ensure(ctx, &ctx->cellq, &ctx->cellq_cap, C->n * kCellQFloats)) != PKDG_OK) return s;
         if ((s = prep_cells(ctx, C, ctx->cellq, st)) != PKDG_OK) return s;
+    }
+    const bool leaves = has_pp && (flags & PKDG_PP_LEAVES);
+    if (leaves) {  // leaf references may point at any bucket: all (first, count) pairs go to the device first
+        if ((s = ensure(ctx, &ctx->g_first, &ctx->g_first_cap, nb)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->g_count, &ctx->g_count_cap, nb)) != PKDG_OK) return s;
+        CK(cudaMemcpyAsync(ctx->g_first, Bh->first, sizeof(int32_t) * nb, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->g_count, Bh->count, sizeof(int32_t) * nb, cudaMemcpyHostToDevice, st));
+        if ((s = build_gfc(ctx, ctx->g_first, ctx->g_count, nb, P->n, st)) != PKDG_OK) return s;
     }
     CK(cudaEventRecord(ctx->ev_ready, st));
     int64_t* bounds = (int64_t*)malloc(sizeof(int64_t) * (size_t)(nb + 1));
@@ -368,7 +399,7 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
         int threads = 256;
         pkdg_pack_kernel<<<(unsigned)((cb + threads - 1) / threads), threads, 0, sl.st>>>(
             sl.first, sl.count, has_pp ? sl.pp_off : nullptr, has_pc ? sl.pc_off : nullptr, cb, P->n, pbase, cbase,
-            sl.desc, ctx->stats, counter);
+            sl.desc, ctx->stats, counter, leaves ? sl.pp_idx : nullptr, ctx->gfc, nb);
         ctx->launches++;
         EvalParams p;
         fill_params(p, ctx, P->xyzm, P->n, has_pc ? C->n : 0, eps, flags, out);
@@ -377,6 +408,8 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
         p.pc_idx = sl.pc_idx;
         p.work_counter = counter;
         p.n_buckets = cb;
+        p.gfc = ctx->gfc;
+        p.n_gbuckets = nb;
         if ((rc = launch_eval(ctx, p, sl.st)) != PKDG_OK) break;
         if (out_host) {
             const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];

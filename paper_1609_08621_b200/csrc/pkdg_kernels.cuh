@@ -103,11 +103,15 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
     return v;
 }
 
+// With leaf_idx != NULL (PKDG_PP_LEAVES) the P-P entries are references into gfc[n_g] = (first, count) of all
+// buckets: I_pp counts the particles they stand for, tiles_pp two references per tile; a reference out of
+// range or to a bucket of more than 16 particles is a bad entry.
 __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ count,
                                  const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
                                  int64_t n_buckets, int64_t n_particles, int64_t pp_base, int64_t pc_base,
                                  BucketDesc* __restrict__ desc, DevStats* __restrict__ stats,
-                                 unsigned int* __restrict__ work_counter) {
+                                 unsigned int* __restrict__ work_counter, const int32_t* __restrict__ leaf_idx,
+                                 const int2* __restrict__ gfc, int64_t n_g) {
     int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long ipp = 0, ipc = 0, tpp = 0, tpc = 0, bad = 0;
     if (b == 0) *work_counter = 0u;
@@ -127,6 +131,19 @@ __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_
         ipp = (unsigned long long)d.count * (unsigned long long)lp;
         ipc = (unsigned long long)d.count * (unsigned long long)lc;
         tpp = (unsigned long long)((lp + 31) >> 5);
+        if (leaf_idx) {
+            unsigned long long np = 0;
+            for (int64_t e = 0; e < lp; ++e) {
+                const int32_t g = leaf_idx[p0 - pp_base + e];
+                if (g < 0) continue;  // padding
+                if (g >= n_g) { bad++; continue; }
+                const int2 fc = gfc[g];
+                if (fc.y > 16 || fc.y < 0) { bad++; continue; }
+                np += (unsigned long long)fc.y;
+            }
+            ipp = (unsigned long long)d.count * np;
+            tpp = (unsigned long long)((lp + 1) >> 1);
+        }
         tpc = (unsigned long long)((lc + 31) >> 5);
     }
     ipp = warp_sum_u64(ipp); ipc = warp_sum_u64(ipc); tpp = warp_sum_u64(tpp); tpc = warp_sum_u64(tpc);
@@ -138,6 +155,16 @@ __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_
         if (tpc) atomicAdd(&stats->tiles_pc, tpc);
         if (bad) atomicAdd(&stats->bad_entries, bad);
     }
+}
+
+// (first, count) of every bucket as one 8-byte record: what a P-P leaf reference is resolved against.
+__global__ void pkdg_fc_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ count, int64_t n,
+                               int64_t n_particles, int2* __restrict__ out) {
+    int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n) return;
+    int2 fc = make_int2(first[b], count[b]);
+    if (fc.y < 0 || fc.x < 0 || (int64_t)fc.x + fc.y > n_particles) fc = make_int2(0, 0);
+    out[b] = fc;
 }
 
 // The tile view of a list, shared by the evaluation kernel and pkdg_pack_export: entry `lane` of
@@ -222,6 +249,8 @@ struct EvalParams {
     const BucketDesc* desc;
     const int32_t* pp_idx;
     const int32_t* pc_idx;
+    const int2* gfc;      // PKDG_PP_LEAVES: (first, count) of EVERY bucket a P-P entry may refer to
+    int64_t n_gbuckets;
     float4* out;
     DevStats* stats;
     unsigned int* work_counter;
@@ -775,7 +804,10 @@ __device__ __forceinline__ void make_pairs(WarpSmem3& S, int buf, int lane) {
 }
 
 // a3 for one pass, packed: NP sink pairs (4 or 8) in register accumulators.
-template <int NP>
+// LEAF (PKDG_PP_LEAVES): the list's entries are references to whole buckets.  A tile is then TWO
+// references: lanes 0-15 hold the particles of the first, lanes 16-31 those of the second (a bucket holds
+// at most 16), so the source gather is two contiguous runs and the list is 16 times shorter.
+template <int NP, bool LEAF>
 __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
                                           const float4* __restrict__ s_tgt, WarpSmem3& S, int lane, unsigned& bad) {
     const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
@@ -786,20 +818,49 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
 #pragma unroll
     for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = make_float2(0.f, 0.f);
     bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
-    const int ntile = (pp_len + 31) >> 5;
+    const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
     const int sink0 = d.first + t0;
-    int32_t j = ntile > 0 ? S.nidx[0][lane] : -1;
-    int32_t jn = ntile > 1 ? S.nidx[1][lane] : -1;
+    const int half = lane >> 4, slot = lane & 15;
+    // LEAF helpers: reference of tile k for this half-warp (the first 64 are staged in shared memory),
+    // its (first, count), and the lane's particle in it
+    auto leaf_ref = [&](int k) -> int32_t {
+        const int r = 2 * k + half;
+        if (r >= pp_len) return -1;
+        return r < 64 ? S.nidx[r >> 5][r & 31] : __ldg(p.pp_idx + d.pp_begin + r);
+    };
+    auto leaf_fc = [&](int32_t g) -> int2 {
+        if ((uint32_t)g >= (uint64_t)p.n_gbuckets) { bad += (g >= 0 && slot == 0); return make_int2(0, 0); }
+        return __ldg(p.gfc + g);
+    };
+    auto leaf_j = [&](int2 fc) -> int32_t { return slot < fc.y ? fc.x + slot : -1; };
+    int32_t j, jn, jnn = -1, gB = -1;
+    int2 fcA = make_int2(0, 0);
+    if (LEAF) {
+        j = ntile > 0 ? leaf_j(leaf_fc(leaf_ref(0))) : -1;
+        jn = ntile > 1 ? leaf_j(leaf_fc(leaf_ref(1))) : -1;
+        fcA = ntile > 2 ? leaf_fc(leaf_ref(2)) : make_int2(0, 0);
+        gB = ntile > 3 ? leaf_ref(3) : -1;
+    } else {
+        j = ntile > 0 ? S.nidx[0][lane] : -1;
+        jn = ntile > 1 ? S.nidx[1][lane] : -1;
+        jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
+    }
     if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
     if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
     float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
     float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
-    int32_t jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
     for (int k = 0; k < ntile; ++k) {
         // sources of the next two tiles and the index of the third are in flight during this tile
+        int32_t jn3 = -1;
+        if (LEAF) {
+            jnn = leaf_j(fcA);                                   // tile k+2
+            fcA = (k + 3 < ntile) ? leaf_fc(gB) : make_int2(0, 0);  // tile k+3
+            gB = (k + 4 < ntile) ? leaf_ref(k + 4) : -1;          // tile k+4
+        } else {
+            jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
+        }
         if ((uint32_t)jnn >= (uint64_t)p.n_particles) { bad += (jnn >= 0); jnn = -1; }
         const float4 snn = jnn >= 0 ? __ldg(p.xyzm + jnn) : far4;
-        const int32_t jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
         const int self_t = j - sink0;  // sink slot this source coincides with, if any
         float minr2 = 3.0e38f;
         if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)(2 * NP))) {  // tile holds own particles
@@ -862,6 +923,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
     float4* s_acc = S.acc;
     const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
     const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
+    const bool pp_leaves = (p.flags & 0x8u) != 0;
     unsigned bad = 0;
 
     unsigned cur = 0;
@@ -900,8 +962,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
 
             // ---- a2: pair layout of the sinks;  a3: P-P
             make_pairs(S, buf, lane);
-            if (ntp <= 8) pp_phase3<4>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
-            else pp_phase3<8>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+            if (pp_leaves) {
+                if (ntp <= 8) pp_phase3<4, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+                else pp_phase3<8, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+            } else {
+                if (ntp <= 8) pp_phase3<4, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+                else pp_phase3<8, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+            }
 
             // ---- next bucket, stage 1: its descriptor
             if (last) {

@@ -53,6 +53,9 @@ def _L():
         L.tg_lists_totals.argtypes = [c_void_p, c_void_p, c_void_p]
         L.tg_lists_export_free.argtypes = [c_void_p] * 5
         L.tg_cloud_records.argtypes = [c_int64, c_int64, c_void_p, c_void_p]
+        L.tg_pp_to_leaves.restype = c_int64
+        L.tg_pp_to_leaves.argtypes = [c_int64, c_int64, c_void_p, c_void_p, c_int64, c_void_p, c_void_p, c_void_p,
+                                      c_void_p]
         L.tg_num_threads.restype = c_int
         _lib = L
     return _lib
@@ -254,6 +257,34 @@ def with_lists(p: Problem, theta: float, eps: float) -> Problem:
     p.pp_off, p.pp_idx, p.pc_off, p.pc_idx = build_lists(p, theta, eps)
     p.theta = theta; p.eps = eps
     return p
+
+
+def pp_leaves(n_particles: int, gfirst: np.ndarray, gcount: np.ndarray, pp_off: np.ndarray, pp_idx: np.ndarray):
+    """P-P lists in leaf form (PKDG_PP_LEAVES): every run of a whole bucket's particles becomes one
+    reference to that bucket (index into the GLOBAL bucket arrays gfirst / gcount).  Returns
+    (leaf_off int64[n_b+1], leaf_idx int32)."""
+    L = _L()
+    gfirst = np.ascontiguousarray(gfirst, np.int32); gcount = np.ascontiguousarray(gcount, np.int32)
+    pp_off = np.ascontiguousarray(pp_off, np.int64); pp_idx = np.ascontiguousarray(pp_idx, np.int32)
+    nb = pp_off.shape[0] - 1
+    off = np.empty(nb + 1, np.int64)
+    n = L.tg_pp_to_leaves(n_particles, gfirst.shape[0], _p(gfirst), _p(gcount), nb, _p(pp_off), _p(pp_idx), _p(off), None)
+    if n < 0:
+        raise ValueError("a P-P list is not a sequence of whole buckets")
+    idx = np.empty(n, np.int32)
+    L.tg_pp_to_leaves(n_particles, gfirst.shape[0], _p(gfirst), _p(gcount), nb, _p(pp_off), _p(pp_idx), _p(off), _p(idx))
+    return off, idx
+
+
+def expand_leaves(gfirst: np.ndarray, gcount: np.ndarray, leaf_off: np.ndarray, leaf_idx: np.ndarray):
+    """Inverse of pp_leaves (numpy): the particle-index lists the leaf references stand for."""
+    c = gcount[leaf_idx].astype(np.int64)
+    per_bucket = np.add.reduceat(np.concatenate([c, [0]]), np.minimum(leaf_off[:-1], c.shape[0]))[: leaf_off.shape[0] - 1]
+    per_bucket[np.diff(leaf_off) == 0] = 0
+    off = np.concatenate([[0], np.cumsum(per_bucket)]).astype(np.int64)
+    start = np.repeat(gfirst[leaf_idx].astype(np.int64) - np.concatenate([[0], np.cumsum(c)[:-1]]), c)
+    idx = (start + np.arange(int(c.sum()), dtype=np.int64)).astype(np.int32)
+    return off, idx
 
 
 def cloud_records(pts: np.ndarray, k: int) -> np.ndarray:

@@ -286,6 +286,38 @@ void tg_cloud_records(int64_t nclouds, int64_t k, const float *pts, float *rec) 
     }
 }
 
+/* P-P lists in LEAF form (PKDG_PP_LEAVES): the tree walk adds a rejected leaf to the P-P list whole, so
+ * every P-P list is a sequence of complete buckets.  map[i] = bucket of particle i (from the GLOBAL bucket
+ * arrays gfirst / gcount, ng buckets); entry e is replaced by its bucket wherever e is the bucket's first
+ * particle.  Two passes: count (leaf_off), then fill (leaf_idx).  Returns -1 if a list is not made of
+ * whole buckets in order, else the number of references. */
+int64_t tg_pp_to_leaves(int64_t n_particles, int64_t ng, const int32_t *gfirst, const int32_t *gcount, int64_t nb,
+                        const int64_t *pp_off, const int32_t *pp_idx, int64_t *leaf_off, int32_t *leaf_idx) {
+    int32_t *map = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_particles > 0 ? n_particles : 1));
+    if (!map) return -1;
+    for (int64_t i = 0; i < n_particles; ++i) map[i] = -1;
+    for (int64_t g = 0; g < ng; ++g)
+        for (int32_t t = 0; t < gcount[g]; ++t) map[gfirst[g] + t] = (int32_t)g;
+    int bad = 0;
+    leaf_off[0] = 0;
+    for (int64_t b = 0; b < nb; ++b) {     /* serial prefix: cheap next to the list build itself */
+        int64_t n = 0;
+        for (int64_t e = pp_off[b]; e < pp_off[b + 1];) {
+            int32_t j = pp_idx[e];
+            int32_t g = (j >= 0 && j < n_particles) ? map[j] : -1;
+            if (g < 0 || gfirst[g] != j || e + gcount[g] > pp_off[b + 1]) { bad = 1; break; }
+            for (int32_t t = 0; t < gcount[g]; ++t)
+                if (pp_idx[e + t] != j + t) bad = 1;
+            if (leaf_idx) leaf_idx[leaf_off[b] + n] = g;
+            ++n;
+            e += gcount[g];
+        }
+        leaf_off[b + 1] = leaf_off[b] + n;
+    }
+    free(map);
+    return bad ? -1 : leaf_off[nb];
+}
+
 int tg_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

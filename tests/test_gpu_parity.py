@@ -266,3 +266,67 @@ def test_config4_sweep_small(ctx, torch):
         out = run_resident(ctx, p, torch)
         ea, ep = rel_errors(out, ref, np.arange(256 * 16))
         assert ea.max() <= TOL and ep.max() <= TOL, (lpp, lpc, ea.max(), ep.max())
+
+
+def _leaf_problem(p):
+    """The same problem with its P-P lists in leaf form (references to whole buckets)."""
+    import copy
+    from paper_1609_08621_b200 import inputs
+    q = copy.copy(p)
+    q.pp_off, q.pp_idx = inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+    eo, ei = inputs.expand_leaves(p.first, p.count, q.pp_off, q.pp_idx)
+    assert np.array_equal(eo, p.pp_off) and np.array_equal(ei, p.pp_idx)      # the references stand for the same lists
+    return q
+
+
+@pytest.mark.parametrize("flags", [0, 2 << 8, 3 << 8])
+def test_pp_leaves_resident(ctx, torch, cfg1, flags):
+    """PKDG_PP_LEAVES: leaf references give the oracle's result of the expanded lists, and the same
+    interaction count; tiles_pp counts two references per tile."""
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors, run_resident
+    for p in (cfg1, inputs.config2(n=1 << 15), inputs.config3(32)):
+        q = _leaf_problem(p)
+        ref = _oracle(p)
+        out = run_resident(ctx, q, torch, flags=flags | binding.PP_LEAVES)
+        st = ctx.get_stats()
+        ea, ep = rel_errors(out, ref)
+        assert ea.max() <= TOL and ep.max() <= TOL, (p.name, ea.max(), ep.max())
+        assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
+        assert st["tiles_pp"] == int(((np.diff(q.pp_off) + 1) // 2).sum())
+        base = run_resident(ctx, p, torch, flags=flags)                       # particle lists: same sums, other order
+        eb, epb = rel_errors(out, base.astype(np.float64))
+        assert eb.max() <= 1e-5 and epb.max() <= 2e-6
+
+
+def test_pp_leaves_streamed_host_and_bad_references(ctx, torch, cfg1):
+    from paper_1609_08621_b200 import binding
+    from gpu_util import run_resident, to_dev
+    p = cfg1
+    q = _leaf_problem(p)
+    base = run_resident(ctx, q, torch, flags=binding.PP_LEAVES)
+    d = to_dev(q, torch)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h = dict(first=pin(q.first), count=pin(q.count), pp_off=pin(q.pp_off), pp_idx=pin(q.pp_idx),
+             pc_off=pin(q.pc_off), pc_idx=pin(q.pc_idx))
+    for n_streams, max_entries in ((1, 1 << 30), (3, 700), (2, 40)):
+        out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda")
+        ctx.gravity_eval_streamed(d["xyzm"], d["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"],
+                                  h["pc_off"], h["pc_idx"], p.eps, out, n_streams=n_streams,
+                                  max_entries_per_chunk=max_entries, flags=binding.PP_LEAVES)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), base)
+        st = ctx.get_stats()
+        assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["chunks"] >= 1
+    out_h = np.full((p.n, 4), np.nan, np.float32)
+    ctx.gravity_eval_host(q.xyzm, q.cells, q.first, q.count, q.pp_off, q.pp_idx, q.pc_off, q.pc_idx, p.eps, out_h,
+                          n_streams=3, max_entries_per_chunk=5000, flags=binding.PP_LEAVES)
+    assert np.array_equal(out_h, base)
+    # a reference out of range is reported, not followed; variant 1 does not implement leaves
+    bad = _leaf_problem(p)
+    bad.pp_idx = bad.pp_idx.copy(); bad.pp_idx[3] = p.n_buckets + 5
+    out = run_resident(ctx, bad, torch, flags=binding.PP_LEAVES)
+    assert np.isfinite(out).all()
+    assert ctx.get_stats(check=False)["bad_entries"] > 0
+    with pytest.raises(binding.PkdgError):
+        run_resident(ctx, q, torch, flags=binding.PP_LEAVES | (1 << 8))
