@@ -252,6 +252,59 @@ def run_ours(args, rank, world, local_rank):
                "n_streams": args.e2e_streams, "max_entries_per_chunk": args.e2e_chunk}
         del h, out_h
 
+    # ---- the same workload with the P-P lists in leaf form (PKDG_PP_LEAVES): extra key
+    leaves = None
+    if not args.no_leaves:
+        from paper_1609_08621_b200 import inputs as _inputs
+        lo, li = _inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+        lflags = flags | binding.PP_LEAVES
+        d_lo, d_li = t(lo), t(li)
+
+        def lstep():
+            ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d_lo, d_li, d["pc_off"], d["pc_idx"], p.eps,
+                             out, flags=lflags)
+        for _ in range(3):
+            lstep()
+        barrier()
+        ctx.profile_read(); ctx.profile_enable(True)
+        l0 = torch.cuda.Event(enable_timing=True); l1 = torch.cuda.Event(enable_timing=True)
+        l0.record()
+        for _ in range(args.steps):
+            lstep()
+        l1.record()
+        barrier()
+        ln, lk = ctx.profile_read(); ctx.profile_enable(False)
+        lst = ctx.get_stats()
+        assert lst["interactions_pp"] == p.I_pp and lst["interactions_pc"] == p.I_pc and lst["bad_entries"] == 0
+        lms = l0.elapsed_time(l1) / args.steps
+        leaves = {"value": world * inter / (lms * 1e-3), "unit": "interactions/s", "ms_per_step": lms,
+                  "kernel_ms": lk / max(ln, 1), "pp_list_entries": int(li.shape[0]),
+                  "frac_fp32_fma_peak_kernel": None}
+        if not args.no_e2e:
+            pin = lambda a: torch.from_numpy(a).pin_memory()
+            h = dict(xyzm=pin(p.xyzm), cells=pin(p.cells), first=pin(p.first), count=pin(p.count), pp_off=pin(lo),
+                     pp_idx=pin(li), pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
+            out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+
+            def le2e():
+                ctx.gravity_eval_host(h["xyzm"], h["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"],
+                                      h["pc_off"], h["pc_idx"], p.eps, out_h, n_streams=args.e2e_streams,
+                                      max_entries_per_chunk=args.e2e_chunk, flags=lflags)
+            for _ in range(2):
+                le2e()
+            barrier()
+            k2 = max(2, min(args.steps, 5))
+            t0 = time.perf_counter()
+            for _ in range(k2):
+                le2e()
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) / k2
+            leaves["e2e"] = {"value": world * inter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3,
+                             "h2d_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in h.values()),
+                             "d2h_bytes_per_step": int(out_h.numel() * 4)}
+            del h, out_h
+        del d_lo, d_li
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -292,7 +345,9 @@ def run_ours(args, rank, world, local_rank):
             "flops_per_s": world * flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / peak_tflops,
             "paper_convention_tflops": world * (PAPER_F_PP * p.I_pp + PAPER_F_PC * p.I_pc) / (ms_step * 1e-3) / 1e12,
             "interactions_per_s": {"pp": world * p.I_pp / (ms_step * 1e-3), "pc": world * p.I_pc / (ms_step * 1e-3)},
-            "gen_seconds": round(gen_s, 1), "kernel_variant": args.variant}
+            "gen_seconds": round(gen_s, 1), "kernel_variant": args.variant, "pp_leaves": leaves}
+    if leaves is not None:
+        leaves["frac_fp32_fma_peak_kernel"] = flops / (leaves["kernel_ms"] * 1e-3) / 1e12 / peak_tflops
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -446,6 +501,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="kernel tuning variant (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-leaves", action="store_true", help="skip the extra PKDG_PP_LEAVES measurement")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-chunk", type=int, default=1 << 23)

@@ -109,6 +109,26 @@ def test_config3_headline_full(ctx, torch, cfg3):
     _check_properties(p, out)
 
 
+def test_config3_headline_pp_leaves(ctx, torch, cfg3):
+    """The headline configuration with its P-P lists as bucket references (PKDG_PP_LEAVES)."""
+    import copy
+    from paper_1609_08621_b200 import binding, inputs
+    p = cfg3
+    q = copy.copy(p)
+    q.pp_off, q.pp_idx = inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+    assert q.pp_idx.shape[0] * 8 < p.pp_idx.shape[0]
+    import oracle
+    from gpu_util import bucket_rows, rel_errors, run_resident
+    out = run_resident(ctx, q, torch, flags=binding.PP_LEAVES)
+    st = ctx.get_stats()
+    assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
+    sel = _sample(p, 2048, 32, seed=1)
+    ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
+    ea, ep = rel_errors(out, ref, bucket_rows(p, sel))
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+    _check_properties(p, out)
+
+
 def test_config3_sharded_equals_unsharded(ctx, torch, cfg3):
     """Multi-GPU path emulated as consecutive calls on one GPU (no kernel waits on another): the two
     ranks' pieces, evaluated separately, give the same bits as one call."""
