@@ -987,10 +987,25 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                 for (int k = 0; k < pc_ntile; ++k) {
                     const int32_t c2 = (k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
                     cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
+                    // A last tile that is at most half (a quarter) full is shared out: 2 (4) groups of lanes take
+                    // the same cells and each group a half (a quarter) of the sink pairs, so the tile costs a
+                    // half (a quarter) of a full one.  Per-lane partial sums stay in the lane's own column.
+                    const int valid = min(32, L.pc - 32 * k);              // warp-uniform
+                    const int rep = (valid <= 8 && npair >= 4) ? 4 : (valid <= 16 && npair >= 2) ? 2 : 1;
+                    int src = lane, q0 = 0, q1 = npair;
+                    int32_t cs = c;
+                    if (rep > 1) {
+                        const int width = 32 / rep, chunk = (npair + rep - 1) / rep;
+                        src = lane & (width - 1);
+                        q0 = min(npair, (lane / width) * chunk);
+                        q1 = min(npair, q0 + chunk);
+                        cs = __shfl_sync(0xffffffffu, c, src);
+                        __syncwarp();  // the record of lane `src` was copied by lane `src`
+                    }
                     CellRegs cr;
-                    if (c >= 0) {
-                        cell_unpack(cr, S.stage[lane], S.stage[32 + lane], S.stage[64 + lane], S.stage[96 + lane],
-                                    S.stage[128 + lane], S.stage[160 + lane], S.stage[192 + lane], S.stage[224 + lane]);
+                    if (cs >= 0) {
+                        cell_unpack(cr, S.stage[src], S.stage[32 + src], S.stage[64 + src], S.stage[96 + src],
+                                    S.stage[128 + src], S.stage[160 + src], S.stage[192 + src], S.stage[224 + src]);
                     } else {
                         const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
                         cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
@@ -1008,9 +1023,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     cp_async_commit();
                     // software pipeline, two pairs per trip so that no register copies are needed: the
                     // displacement / rsqrt of the next pair is issued under the body of the current one
-                    PcPre2 pA = pc_pre2<NEWTON>(tp[0], tp[1], cr);
+                    PcPre2 pA = pc_pre2<NEWTON>(tp[2 * q0], tp[2 * q0 + 1], cr);
 #pragma unroll 1
-                    for (int q = 0; q < npair; q += 2) {
+                    for (int q = q0; q < q1; q += 2) {
                         const PcPre2 pB = pc_pre2<NEWTON>(tp[2 * q + 2], tp[2 * q + 3], cr);
                         {
                             float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
@@ -1018,7 +1033,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                             s_acc[(2 * q) * 32 + lane] = a0;
                             s_acc[(2 * q + 1) * 32 + lane] = a1;
                         }
-                        if (q + 1 < npair) {
+                        if (q + 1 < q1) {
                             pA = pc_pre2<NEWTON>(tp[2 * q + 4], tp[2 * q + 5], cr);
                             float4 a0 = s_acc[(2 * q + 2) * 32 + lane], a1 = s_acc[(2 * q + 3) * 32 + lane];
                             pc_body2(pB, cr, a0, a1);
