@@ -176,7 +176,7 @@ void fill_params(EvalParams& p, pkdg_ctx* ctx, const float* xyzm, int64_t np, in
 
 pkdg_status prep_cells(pkdg_ctx* ctx, const pkdg_cells* C, float* dst, cudaStream_t st) {
     if (!C || C->n == 0) return PKDG_OK;
-    int threads = 128;
+    const int threads = kPrepThreads;
     int64_t blocks = (C->n + threads - 1) / threads;
     pkdg_prep_cells_kernel<<<(unsigned)blocks, threads, 0, st>>>(C->rec, C->n, C->stride_floats, dst);
     ctx->launches++;
