@@ -21,6 +21,11 @@
  * passed as void*; NULL = the legacy default stream) unless stated; no exception crosses the
  * ABI; every function returns a pkdg_status (0 = OK, < 0 = error) and pkdg_last_error() gives
  * the text.  A pkdg_ctx may be used by one host thread at a time.
+ *
+ * Value range.  Coordinates must satisfy |x| <= 1e12 and masses must be finite: the kernels park
+ * masked list entries (padding, out-of-range indices) at +1e15 with mass 0 and unused sink slots at
+ * -1e15, and rely on those never coming within fp32 range of a real particle.  Cell records must
+ * have b_max / |x_sink - COM| < 1 for every listed pair (any sensible opening criterion does).
  */
 #ifndef PKDG_H
 #define PKDG_H
