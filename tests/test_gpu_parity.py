@@ -330,3 +330,23 @@ def test_pp_leaves_streamed_host_and_bad_references(ctx, torch, cfg1):
     assert ctx.get_stats(check=False)["bad_entries"] > 0
     with pytest.raises(binding.PkdgError):
         run_resident(ctx, q, torch, flags=binding.PP_LEAVES | (1 << 8))
+
+
+def test_probes_report_sane_rates(ctx, torch):
+    """pkdg_fma_probe: the operand-pattern probes behind DESIGN.md sec 6 run and order as documented
+    (constant-operand FFMA near the FMA peak; three-register FFMA and FFMA2 well below it; FFMA2 with
+    a reused operand in between; the packed P-C body above the scalar one)."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    clock_ghz = torch.cuda.get_device_properties(0).clock_rate / 1e6 if hasattr(torch.cuda.get_device_properties(0), "clock_rate") else 1.965
+    peak = sms * 128 * 2 * clock_ghz / 1e3                       # Tflop/s
+    rate = {}
+    for mode in range(6):
+        ms, fl = ctx.fma_probe(mode, 1 << 11)
+        assert ms > 0 and fl > 0
+        rate[mode] = fl / ms / 1e9
+    assert 0.8 * peak < rate[0] < 1.05 * peak, (rate, peak)
+    assert rate[1] < 0.75 * rate[0] and rate[2] < 0.8 * rate[0]      # register-file bandwidth
+    assert rate[3] > rate[2] * 1.2                                   # operand reuse lifts FFMA2
+    assert rate[5] > rate[4] * 1.1                                   # packed P-C body beats the scalar one
+    with pytest.raises(Exception):
+        ctx.fma_probe(17, 16)
