@@ -45,3 +45,29 @@ def test_product_arm_fails_loudly_without_a_gpu():
     r = _run(["--ng", "16", "--steps", "1", "--warmup", "0"])
     assert r.returncode != 0
     assert "no CUDA device" in (r.stderr + r.stdout)
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_product_arm_line_on_gpu():
+    """The product arm at a small lattice (same code path as the headline run): one JSON line with the
+    keys the measurement contract asks for, a roofline fraction in (0, 1.05) and a counted launch number."""
+    r = _run(["--ng", "64", "--steps", "3", "--warmup", "3", "--cpu-seconds", "1"], timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["dtype"] == "f32" and d["data"] == "synthetic" and d["scaling"] == "weak" and d["vs_baseline"] is None
+    assert d["gpu_launches"] == 3 and d["warmup"] >= 3
+    rf = d["roofline"]
+    assert rf["bound"] == "alu" and rf["unit"] == "TFLOP/s" and 0.0 < rf["frac"] < 1.05
+    assert abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-12
+    assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] == 16 * d["config"]["n_particles"]
+    assert d["e2e"]["value"] < d["value"]
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["pp_leaves"]["e2e"]["h2d_bytes_per_step"] < d["e2e"]["h2d_bytes_per_step"]
