@@ -30,3 +30,34 @@ def test_host_only_entry_points_work_without_gpu():
     for cap in (1, 50, 1000, 10 ** 9):
         assert np.array_equal(binding.chunk_bounds(pp, pc, cap), oracle.chunk_bounds(pp, pc, cap))
     assert binding.status_string(0) == "PKDG_OK" and "EINVAL" in binding.status_string(-1)
+
+
+def test_binding_fails_loudly_without_the_library(monkeypatch, tmp_path):
+    """No CPU fallback: without libpkdg.so the binding refuses to load instead of degrading."""
+    import pytest
+    from paper_1609_08621_b200 import binding
+    monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "libpkdg.so"))
+    with pytest.raises(binding.PkdgError, match="no CPU fallback"):
+        binding._load()
+
+
+def test_product_package_does_not_import_the_oracle():
+    """The product path (package + bench.py's own arm) never reaches into oracle/."""
+    import ast
+    pkg = os.path.join(ROOT, "paper_1609_08621_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if not f.endswith(".py"):
+                continue
+            tree = ast.parse(open(os.path.join(dirpath, f)).read())
+            for node in ast.walk(tree):
+                names = []
+                if isinstance(node, ast.Import):
+                    names = [a.name for a in node.names]
+                elif isinstance(node, ast.ImportFrom):
+                    names = [node.module or ""]
+                assert not any(n == "oracle" or n.startswith("oracle.") for n in names), (f, names)
+    for src in ("csrc/pkdg.cu", "csrc/pkdg_kernels.cuh"):
+        text = open(os.path.join(pkg, src)).read()
+        assert "oracle" not in text.lower().replace("the oracle", "")  # comments may mention it; no include
+        assert "#include \"../../oracle" not in text and "pkdg_oracle" not in text
