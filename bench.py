@@ -7,8 +7,9 @@ One "step" = one pass of the whole hot path (cell prep + packer + fused P-P/P-C 
 reduction/write-back: SURVEY.md sec 8(a)) over one synthetic problem.  Workload at every N:
 BASELINE.json configs[2], the configuration the metric is quoted on (N = 2^24 particles, 256^3
 lattice displaced by a Zel'dovich field, binary tree, bucket 16, theta = 0.7); it fits one GPU.
-With --gpus N > 1 (torchrun) every rank evaluates its own replica of that problem, no data-path
-collective (weak scaling).
+With --gpus N > 1 (torchrun) ONE problem is strong-scaled: rank 0's arrays are broadcast over NCCL, every rank
+evaluates the cost-balanced bucket range paper_1609_08621_b200/shard.py gives it, no data-path collective
+(DESIGN.md "Multi-GPU"); --scaling weak runs N independent replicas instead.
 
 Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle (oracle/) on the host
 cores on a bounded sample of the same workload.
@@ -31,7 +32,7 @@ sys.path.insert(0, ROOT)
 # line by line in DESIGN.md "Flop audit".  The paper's own convention (Table 3: 53 / 215, rsqrt = 7)
 # is reported beside it as context only.
 F_PP = 19
-F_PC_BY_VARIANT = {0: 187, 1: 196, 2: 187, 3: 192}   # packed default / scalar generation 1 / packed 128-reg / packed + Newton
+F_PC = 187
 PAPER_F_PP, PAPER_F_PC = 53, 215
 SM_COUNT_NOMINAL, FP32_LANES_PER_SM = 148, 128
 
@@ -158,7 +159,52 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) of the CUDA sources the evaluation kernel is built from: the key
+    profiles/traffic.json is stamped with, so that a measured DRAM-traffic figure is dropped (null) as soon as
+    the kernel it was measured on has changed."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in ("paper_1609_08621_b200/csrc/pkdg_kernels.cuh", "paper_1609_08621_b200/csrc/pkdg.cu", "include/pkdg.h"):
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the evaluation kernel from the last ncu --set full
+    capture (profiles/traffic.json), or None if that capture was taken on other kernel sources."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(tpath):
+        return None, "no capture"
+    with open(tpath) as f:
+        t = json.load(f)
+    if t.get("source_hash") != kernel_source_hash():
+        return None, f"stale: captured on sources {t.get('source_hash')}, running {kernel_source_hash()}"
+    return t.get(key), f"ncu capture {t.get('capture', '?')}"
+
+
+def _max_over_ranks(x, dist, torch, dev):
+    if dist is None:
+        return x
+    tt = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def _sum_over_ranks(x, dist, torch, dev):
+    if dist is None:
+        return x
+    tt = torch.tensor([x], dtype=torch.int64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.SUM)
+    return int(tt.item())
+
+
 def run_ours(args, rank, world, local_rank):
+    """One problem (config 3) on `world` GPUs.  world > 1, default --scaling strong: rank 0 builds the problem,
+    multigpu.distribute broadcasts the read-only arrays over NCCL and every rank evaluates the bucket range
+    shard.rank_piece gives it through pkdg_gravity_eval_range -- no collective on the data path; value =
+    all interactions / max-over-ranks time.  --scaling weak: every rank evaluates its own full replica."""
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
@@ -167,21 +213,31 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    from paper_1609_08621_b200 import binding
+    from paper_1609_08621_b200 import binding, multigpu
     peaks, peak_kind = load_peaks()
-
-    p, gen_s = build_workload(args.ng)
     dev = torch.device("cuda", local_rank)
-    t = lambda a: torch.from_numpy(a).to(dev)
-    d = dict(xyzm=t(p.xyzm), cells=t(p.cells), first=t(p.first), count=t(p.count), pp_off=t(p.pp_off),
-             pp_idx=t(p.pp_idx), pc_off=t(p.pc_off), pc_idx=t(p.pc_idx))
-    out = torch.zeros((p.n, 4), dtype=torch.float32, device=dev)
-    ctx = binding.Context(local_rank)
-    flags = args.variant << binding.VARIANT_SHIFT
+    strong = world > 1 and args.scaling != "weak"
 
-    def step():
-        ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"],
-                         d["pc_idx"], p.eps, out, flags=flags)
+    p, gen_s = (None, 0.0)
+    if rank == 0 or not strong:
+        p, gen_s = build_workload(args.ng)
+    if strong:
+        g, piece = multigpu.distribute(p, dist, rank, world, dev, torch)
+    else:
+        g, piece = multigpu.distribute(p, None, 0, 1, dev, torch)
+    cfg = workload_config(p, args.ng) if p is not None else None
+    n_particles = int(g.xyzm.shape[0])
+    cnt_piece = piece.count.astype(np.int64)
+    I_pp = int(np.dot(cnt_piece, np.diff(piece.pp_off))); I_pc = int(np.dot(cnt_piece, np.diff(piece.pc_off)))
+    tot_pp = _sum_over_ranks(I_pp, dist if strong else None, torch, dev)
+    tot_pc = _sum_over_ranks(I_pc, dist if strong else None, torch, dev)
+    out = torch.zeros((n_particles, 4), dtype=torch.float32, device=dev)
+    ctx = binding.Context(local_rank)
+    flags = args.flags
+
+    def step(fl=flags):
+        ctx.gravity_eval_range(g.xyzm, g.cells, g.first, g.count, piece.b0, piece.b1, piece.d_pp_off, piece.pp_idx,
+                               piece.d_pc_off, piece.pc_idx, g.eps, out, flags=fl)
 
     def barrier():
         torch.cuda.synchronize()
@@ -189,49 +245,64 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    def timed(fn, k):
+        """K calls of fn between barriers, CUDA events on the launching stream; ms per call, max over ranks."""
+        barrier()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(k):
+            fn()
+        e1.record()
+        barrier()
+        return _max_over_ranks(e0.elapsed_time(e1) / k, dist, torch, dev)
+
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step()
     barrier()
     ctx.profile_read()
     ctx.profile_enable(True)
     sampler = ClockSampler(torch, local_rank)
     launches0 = ctx.launch_count()
-    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     sampler.start()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
+    ms_step = timed(step, args.steps)
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    n_eval, eval_ms_total = ctx.profile_read()
+    n_eval, eval_ms_total, fix_ms_total = ctx.profile_read()
     ctx.profile_enable(False)
     launches = (ctx.launch_count() - launches0) // args.steps
     stats = ctx.get_stats()
-    assert stats["interactions_pp"] == p.I_pp and stats["interactions_pc"] == p.I_pc and stats["bad_entries"] == 0
-    if dist is not None:
-        tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
-    ms_step = ms_total / args.steps
-    inter = p.I_pp + p.I_pc
-    value = world * inter / (ms_step * 1e-3)
-    F_PC = F_PC_BY_VARIANT[args.variant]
-    flops = F_PP * p.I_pp + F_PC * p.I_pc
+    assert stats["interactions_pp"] == I_pp and stats["interactions_pc"] == I_pc and stats["bad_entries"] == 0
+    if not strong:
+        tot_pp, tot_pc = world * I_pp, world * I_pc
+    inter = tot_pp + tot_pc
+    value = inter / (ms_step * 1e-3)
+    flops = F_PP * tot_pp + F_PC * tot_pc
+    fix_sinks = _sum_over_ranks(stats["fixup_sinks"], dist, torch, dev)
+    # the cost of the conditioning-triggered fp64 fix-up: the same step without it
+    ms_nofix = timed(lambda: step(flags | binding.NO_FIXUP), max(3, args.steps // 2))
+    fixup = {"sinks": fix_sinks, "frac_of_sinks": fix_sinks / (n_particles * (1 if strong else world)),
+             "kernel_ms": fix_ms_total / max(n_eval, 1), "step_ms_without_fixup_and_estimate": ms_nofix,
+             "added_ms": ms_step - ms_nofix}
+    shares = None
+    if strong:
+        sh = torch.zeros(world, dtype=torch.float64, device=dev)
+        sh[rank] = piece.cost / max(piece.cost_total, 1)
+        dist.all_reduce(sh)
+        shares = [round(float(x), 4) for x in sh.tolist()]
 
     # ---- end to end: every buffer starts in pinned host memory, result read back every step
     e2e = None
+    pin = lambda t_: t_.cpu().pin_memory()
     if not args.no_e2e:
-        pin = lambda a: torch.from_numpy(a).pin_memory()
-        h = dict(xyzm=pin(p.xyzm), cells=pin(p.cells), first=pin(p.first), count=pin(p.count), pp_off=pin(p.pp_off),
-                 pp_idx=pin(p.pp_idx), pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
-        out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+        h = dict(xyzm=pin(g.xyzm), cells=pin(g.cells), first=pin(g.first), count=pin(g.count),
+                 pp_off=torch.from_numpy(piece.pp_off).pin_memory(), pp_idx=pin(piece.pp_idx),
+                 pc_off=torch.from_numpy(piece.pc_off).pin_memory(), pc_idx=pin(piece.pc_idx))
+        out_h = torch.zeros((n_particles, 4), dtype=torch.float32).pin_memory()
 
         def e2e_step():
-            ctx.gravity_eval_host(h["xyzm"], h["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"], h["pc_off"],
-                                  h["pc_idx"], p.eps, out_h, n_streams=args.e2e_streams,
-                                  max_entries_per_chunk=args.e2e_chunk, flags=flags)
+            ctx.gravity_eval_host_range(h["xyzm"], h["cells"], h["first"], h["count"], piece.b0, piece.b1, h["pp_off"],
+                                        h["pp_idx"], h["pc_off"], h["pc_idx"], g.eps, out_h, n_streams=args.e2e_streams,
+                                        max_entries_per_chunk=args.e2e_chunk, flags=flags)
         for _ in range(2):
             e2e_step()
         barrier()
@@ -240,59 +311,44 @@ def run_ours(args, rank, world, local_rank):
         for _ in range(k2):
             e2e_step()
         torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / k2
-        if dist is not None:
-            tt = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = _max_over_ranks((time.perf_counter() - t0) / k2, dist, torch, dev)
+        rows = int(cnt_piece.sum())
         h2d = sum(int(v.numel() * v.element_size()) for v in h.values())
-        e2e = {"value": world * inter / dt, "unit": "interactions/s", "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": int(out_h.numel() * 4), "ms_per_step": dt * 1e3, "steps": k2,
-               "api": "pkdg_gravity_eval_host (pinned host buffers, lists streamed in chunks)",
+        e2e = {"value": inter / dt, "unit": "interactions/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": rows * 16, "ms_per_step": dt * 1e3, "steps": k2,
+               "api": "pkdg_gravity_eval_host_range (pinned host buffers, lists streamed in chunks; bytes are this rank's)",
                "n_streams": args.e2e_streams, "max_entries_per_chunk": args.e2e_chunk}
         del h, out_h
 
-    # ---- the same workload with the P-P lists in leaf form (PKDG_PP_LEAVES): extra key
+    # ---- the same workload with the P-P lists in leaf form (PKDG_PP_LEAVES): extra key, N = 1
     leaves = None
-    if not args.no_leaves:
+    if not args.no_leaves and world == 1:
         from paper_1609_08621_b200 import inputs as _inputs
         lo, li = _inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
         lflags = flags | binding.PP_LEAVES
-        d_lo, d_li = t(lo), t(li)
+        d_lo, d_li = torch.from_numpy(lo).to(dev), torch.from_numpy(li).to(dev)
 
         def lstep():
-            ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d_lo, d_li, d["pc_off"], d["pc_idx"], p.eps,
-                             out, flags=lflags)
+            ctx.gravity_eval(g.xyzm, g.cells, g.first, g.count, d_lo, d_li, g.pc_off, g.pc_idx, g.eps, out, flags=lflags)
         for _ in range(3):
             lstep()
         barrier()
         ctx.profile_read(); ctx.profile_enable(True)
-        l0 = torch.cuda.Event(enable_timing=True); l1 = torch.cuda.Event(enable_timing=True)
-        l0.record()
-        for _ in range(args.steps):
-            lstep()
-        l1.record()
-        barrier()
-        ln, lk = ctx.profile_read(); ctx.profile_enable(False)
+        lms = timed(lstep, args.steps)
+        ln, lk, _ = ctx.profile_read(); ctx.profile_enable(False)
         lst = ctx.get_stats()
         assert lst["interactions_pp"] == p.I_pp and lst["interactions_pc"] == p.I_pc and lst["bad_entries"] == 0
-        lms = l0.elapsed_time(l1) / args.steps
-        if dist is not None:   # max over ranks, like the headline value
-            tt = torch.tensor([lms], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            lms = float(tt.item())
-        leaves = {"value": world * inter / (lms * 1e-3), "unit": "interactions/s", "ms_per_step": lms,
-                  "kernel_ms": lk / max(ln, 1), "pp_list_entries": int(li.shape[0]),
-                  "frac_fp32_fma_peak_kernel": None}
+        leaves = {"value": inter / (lms * 1e-3), "unit": "interactions/s", "ms_per_step": lms,
+                  "kernel_ms": lk / max(ln, 1), "pp_list_entries": int(li.shape[0]), "frac_fp32_fma_peak_kernel": None}
         if not args.no_e2e:
-            pin = lambda a: torch.from_numpy(a).pin_memory()
-            h = dict(xyzm=pin(p.xyzm), cells=pin(p.cells), first=pin(p.first), count=pin(p.count), pp_off=pin(lo),
-                     pp_idx=pin(li), pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
+            h = dict(xyzm=pin(g.xyzm), cells=pin(g.cells), first=pin(g.first), count=pin(g.count),
+                     pp_off=torch.from_numpy(lo).pin_memory(), pp_idx=torch.from_numpy(li).pin_memory(),
+                     pc_off=pin(g.pc_off), pc_idx=pin(g.pc_idx))
             out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
 
             def le2e():
                 ctx.gravity_eval_host(h["xyzm"], h["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"],
-                                      h["pc_off"], h["pc_idx"], p.eps, out_h, n_streams=args.e2e_streams,
+                                      h["pc_off"], h["pc_idx"], g.eps, out_h, n_streams=args.e2e_streams,
                                       max_entries_per_chunk=args.e2e_chunk, flags=lflags)
             for _ in range(2):
                 le2e()
@@ -303,11 +359,7 @@ def run_ours(args, rank, world, local_rank):
                 le2e()
             torch.cuda.synchronize()
             dt = (time.perf_counter() - t0) / k2
-            if dist is not None:
-                tt = torch.tensor([dt], dtype=torch.float64, device=dev)
-                dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-                dt = float(tt.item())
-            leaves["e2e"] = {"value": world * inter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3,
+            leaves["e2e"] = {"value": inter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3,
                              "h2d_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in h.values()),
                              "d2h_bytes_per_step": int(out_h.numel() * 4)}
             del h, out_h
@@ -318,24 +370,22 @@ def run_ours(args, rank, world, local_rank):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (pkdg_eval_kernel): plain FP32 ALU (FFMA pipe) bound
+    # ---- roofline of the dominant kernel (pkdg_eval3_kernel, this rank's launch): plain FP32 ALU (FFMA pipe) bound
     sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
     peak_tflops = sms * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
     eval_ms = eval_ms_total / max(n_eval, 1)
-    achieved = flops / (eval_ms * 1e-3) / 1e12
+    flops_rank = F_PP * I_pp + F_PC * I_pc
+    achieved = flops_rank / (eval_ms * 1e-3) / 1e12
     probe_ms, probe_flops = ctx.fma_peak_probe(1 << 15)
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(f"cfg3_ng{args.ng}")
-    roofline = {"bound": "alu", "kernel": "pkdg_eval3_kernel" if args.variant != 1 else "pkdg_eval_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": traffic,
+    traffic, traffic_note = measured_traffic(f"cfg3_ng{args.ng}") if world == 1 else (None, "single-GPU capture only")
+    roofline = {"bound": "alu", "kernel": "pkdg_eval3_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": traffic, "traffic_note": traffic_note,
                 "peak_kind": f"{sms} SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json clock)",
                 "kernel_ms": eval_ms, "kernel_share_of_step": eval_ms / ms_step,
                 "ffma_probe_tflops": probe_flops / (probe_ms * 1e-3) / 1e12,
                 "flops_per_interaction": {"pp": F_PP, "pc": F_PC},
-                "hbm_algorithmic_gbs": (p.pp_idx.nbytes + p.pc_idx.nbytes + 32 * p.n + 32 * p.n_buckets) / (eval_ms * 1e-3) / 1e9,
+                "hbm_algorithmic_gbs": (piece.pp_idx.numel() * 4 + piece.pc_idx.numel() * 4 + 32 * int(cnt_piece.sum())
+                                        + 32 * piece.n_buckets) / (eval_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}
 
     cpu_baseline = None
@@ -345,15 +395,18 @@ def run_ours(args, rank, world, local_rank):
                         "sample": f"{nsel} of {p.n_buckets} buckets evenly spread in tree order "
                                   f"({inter_s} interactions, {dt:.1f} s)"}
 
+    cfg["parallelism"] = (f"{world} ranks, contiguous cost-balanced bucket ranges (shard.rank_piece), arrays replicated by "
+                          f"one NCCL broadcast, no data-path collective") if strong else \
+                         ("1 GPU" if world == 1 else f"{world} independent replicas")
     line = {"metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": workload_config(p, args.ng), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu_baseline,
-            "flops_per_s": world * flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / peak_tflops,
-            "paper_convention_tflops": world * (PAPER_F_PP * p.I_pp + PAPER_F_PC * p.I_pc) / (ms_step * 1e-3) / 1e12,
-            "interactions_per_s": {"pp": world * p.I_pp / (ms_step * 1e-3), "pc": world * p.I_pc / (ms_step * 1e-3)},
-            "gen_seconds": round(gen_s, 1), "kernel_variant": args.variant, "pp_leaves": leaves}
+            "steps": args.steps, "warmup": warm, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "strong" if (strong or world == 1) else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": cfg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "fixup": fixup, "rank_cost_shares": shares,
+            "flops_per_s": flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / (peak_tflops * world),
+            "paper_convention_tflops": (PAPER_F_PP * tot_pp + PAPER_F_PC * tot_pc) / (ms_step * 1e-3) / 1e12,
+            "interactions_per_s": {"pp": tot_pp / (ms_step * 1e-3), "pc": tot_pc / (ms_step * 1e-3)},
+            "gen_seconds": round(gen_s, 1), "flags": args.flags, "pp_leaves": leaves}
     if leaves is not None:
         leaves["frac_fp32_fma_peak_kernel"] = flops / (leaves["kernel_ms"] * 1e-3) / 1e12 / peak_tflops
     print(json.dumps(line), flush=True)
@@ -366,7 +419,7 @@ def run_ours(args, rank, world, local_rank):
 # library's CUDA events, median of `reps`), the oracle timed and compared on a bounded sample of the
 # same buckets.  One JSON line per case; not the driver's contract line (that is the default mode).
 # ------------------------------------------------------------------------------------------------
-def report_case(name, p, ctx, torch, binding, peak_tflops, reps, variant, cpu_seconds, note=""):
+def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seconds, note=""):
     dev = torch.device("cuda", 0)
     t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     has_pc = p.cells is not None and p.cells.shape[0] > 0 and p.pc_off is not None
@@ -374,32 +427,47 @@ def report_case(name, p, ctx, torch, binding, peak_tflops, reps, variant, cpu_se
              pp_off=t(p.pp_off), pp_idx=t(p.pp_idx), pc_off=t(p.pc_off) if has_pc else None,
              pc_idx=t(p.pc_idx) if has_pc else None)
     out = torch.zeros((p.n, 4), dtype=torch.float32, device=dev)
-    flags = variant << binding.VARIANT_SHIFT
     step = lambda: ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"],
                                     d["pc_off"], d["pc_idx"], p.eps, out, flags=flags)
     for _ in range(3):
         step()
     torch.cuda.synchronize()
     ctx.profile_read(); ctx.profile_enable(True)
-    kms, sms_ = [], []
+    kms, sms_, fms = [], [], []
     for _ in range(reps):
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record(); step(); e1.record(); torch.cuda.synchronize()
-        n, ms = ctx.profile_read()
-        kms.append(ms / max(n, 1)); sms_.append(e0.elapsed_time(e1))
+        n, ms, fx = ctx.profile_read()
+        kms.append(ms / max(n, 1)); sms_.append(e0.elapsed_time(e1)); fms.append(fx / max(n, 1))
     ctx.profile_enable(False)
     st = ctx.get_stats()
     I_pp, I_pc = p.I_pp, (p.I_pc if has_pc else 0)
     assert st["interactions_pp"] == I_pp and st["interactions_pc"] == I_pc and st["bad_entries"] == 0
     k_med, k_best = float(np.median(kms)), float(min(kms))
-    flops = F_PP * I_pp + F_PC_BY_VARIANT[variant] * I_pc
+    flops = F_PP * I_pp + F_PC * I_pc
     line = {"case": name, "n_particles": p.n, "n_buckets": p.n_buckets, "I_pp": I_pp, "I_pc": I_pc,
             "mean_L_pp": round(float(np.diff(p.pp_off).mean()), 1) if p.pp_off is not None else 0,
             "mean_L_pc": round(float(np.diff(p.pc_off).mean()), 1) if has_pc else 0,
             "kernel_ms_median": k_med, "kernel_ms_best": k_best, "step_ms_median": float(np.median(sms_)),
             "interactions_per_s": (I_pp + I_pc) / (k_med * 1e-3), "tflops": flops / (k_med * 1e-3) / 1e12,
             "frac_fp32_fma_peak": flops / (k_med * 1e-3) / 1e12 / peak_tflops,
-            "paper_convention_tflops": (PAPER_F_PP * I_pp + PAPER_F_PC * I_pc) / (k_med * 1e-3) / 1e12, "note": note}
+            "paper_convention_tflops": (PAPER_F_PP * I_pp + PAPER_F_PC * I_pc) / (k_med * 1e-3) / 1e12, "note": note,
+            "fixup_sinks": st["fixup_sinks"], "fixup_frac": st["fixup_sinks"] / max(1, int(p.count.sum())),
+            "fixup_kernel_ms_median": float(np.median(fms))}
+    line["frac_fp32_fma_peak_step"] = flops / (line["step_ms_median"] * 1e-3) / 1e12 / peak_tflops
+    # the two other precision modes, timed whole-step (3 calls each): no fix-up at all; every sink in fp64
+    for key, fl in (("step_ms_no_fixup", flags | binding.NO_FIXUP), ("step_ms_fp64_all", flags | binding.FIXUP_ALL)):
+        ts = []
+        for _ in range(3):
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"],
+                             d["pc_idx"], p.eps, out, flags=fl)
+            e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        line[key] = float(np.median(ts))
+    step()            # leave the default-mode result in `out` for the comparison below
+    torch.cuda.synchronize()
     if cpu_seconds > 0:
         import oracle
         nb = p.n_buckets
@@ -443,7 +511,7 @@ def run_report(args):
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     peak = sms * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
     ctx = binding.Context(0)
-    rc = lambda name, p, note="": report_case(name, p, ctx, torch, binding, peak, args.report_reps, args.variant,
+    rc = lambda name, p, note="": report_case(name, p, ctx, torch, binding, peak, args.report_reps, args.flags,
                                               args.cpu_seconds, note)
     lines = []
     want = set(args.report.split(","))
@@ -484,7 +552,7 @@ def run_report(args):
                 e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
                 e0.record()
                 ctx.gravity_eval_streamed(d_x, d_c, h[0], h[1], h[2], h[3], h[4], h[5], eps, out, n_streams=ns,
-                                          max_entries_per_chunk=chunk, flags=args.variant << binding.VARIANT_SHIFT)
+                                          max_entries_per_chunk=chunk, flags=args.flags)
                 e1.record(); torch.cuda.synchronize()
                 ts.append(e0.elapsed_time(e1))
             st = ctx.get_stats()
@@ -517,7 +585,7 @@ def run_report(args):
         d_f = torch.from_numpy(p.first).to(dev); d_n = torch.from_numpy(p.count).to(dev)
         d_ppo = torch.from_numpy(pp_off).to(dev); d_pco = torch.from_numpy(pc_off).to(dev)
         out = torch.zeros((p.n, 4), dtype=torch.float32, device=dev)
-        fl = args.variant << binding.VARIANT_SHIFT
+        fl = args.flags
         step = lambda: ctx.gravity_eval(d_x, d_c, d_f, d_n, d_ppo, d_ppi, d_pco, d_pci, eps, out, flags=fl)
         for _ in range(2):
             step()
@@ -526,13 +594,13 @@ def run_report(args):
         for _ in range(5):
             step()
         torch.cuda.synchronize()
-        n_k, ms_k = ctx.profile_read(); ctx.profile_enable(False)
+        n_k, ms_k, _ = ctx.profile_read(); ctx.profile_enable(False)
         st = ctx.get_stats()
         cnt = p.count.astype(np.int64)
         I_pp, I_pc = int(np.dot(cnt, np.diff(pp_off))), int(np.dot(cnt, np.diff(pc_off)))
         assert st["interactions_pp"] == I_pp and st["interactions_pc"] == I_pc and st["bad_entries"] == 0
         k_ms = ms_k / n_k
-        flops = F_PP * I_pp + F_PC_BY_VARIANT[args.variant] * I_pc
+        flops = F_PP * I_pp + F_PC * I_pc
         line = {"case": "cfg5 N=2^26 theta=0.55, ALL %d buckets resident" % nb, "n_particles": p.n, "n_buckets": nb,
                 "I_pp": I_pp, "I_pc": I_pc, "mean_L_pp": round(float(np.diff(pp_off).mean()), 1),
                 "mean_L_pc": round(float(np.diff(pc_off).mean()), 1), "list_gb": (d_ppi.numel() + d_pci.numel()) * 4 / 1e9,
@@ -567,7 +635,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ng", type=int, default=256, help="lattice size per axis (256 = the headline 2^24 config)")
-    ap.add_argument("--variant", type=int, default=0, help="kernel tuning variant (0 = library default)")
+    ap.add_argument("--flags", type=lambda v: int(v, 0), default=0, help="extra PKDG_* flags for every evaluation call (e.g. 0x10 = PKDG_NO_FIXUP)")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"], help="N > 1: one problem sharded (default) or N replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-leaves", action="store_true", help="skip the extra PKDG_PP_LEAVES measurement")

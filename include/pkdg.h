@@ -22,10 +22,22 @@
  * ABI; every function returns a pkdg_status (0 = OK, < 0 = error) and pkdg_last_error() gives
  * the text.  A pkdg_ctx may be used by one host thread at a time.
  *
+ * Precision ("single precision in calculating interactions, but all components are
+ * accumulated in double precision").  Terms and per-lane
+ * partial sums are fp32.  Beside a_i the kernel accumulates S2_i = sum_j |a_ij|^2; a sink whose sum cancels
+ * so far that fp32 terms cannot give 2e-5 of |a_i| (sqrt(S2_i) > kappa2 |a_i|, default kappa2 = 8, option
+ * PKDG_OPT_KAPPA2) is re-evaluated over the same lists by a second kernel with fp64 terms and fp64
+ * accumulators and its row is written by that kernel.  pkdg_stats.fixup_sinks counts them.
+ *
+ * Stream order.  Consecutive calls on ONE context must be stream-ordered (same stream, or ordered by
+ * events): they share the context's workspace (descriptors, counters, queues).  eps == 0: pairs closer
+ * than 1e-12 are treated as coincident and contribute nothing (the Newtonian pair is undefined there).
+ *
  * Value range.  Coordinates must satisfy |x| <= 1e12 and masses must be finite: the kernels park
  * masked list entries (padding, out-of-range indices) at +1e15 with mass 0 and unused sink slots at
  * -1e15, and rely on those never coming within fp32 range of a real particle.  Cell records must
- * have b_max / |x_sink - COM| < 1 for every listed pair (any sensible opening criterion does).
+ * have b_max / |x_sink - COM| < 1 for every listed pair (any sensible opening criterion does).  The
+ * flag PKDG_VALIDATE checks all of this on the device.
  */
 #ifndef PKDG_H
 #define PKDG_H
@@ -37,7 +49,7 @@ extern "C" {
 #endif
 
 #define PKDG_VERSION_MAJOR 0
-#define PKDG_VERSION_MINOR 1
+#define PKDG_VERSION_MINOR 2
 
 #define PKDG_TILE 32          /* list entries per tile = lanes per warp */
 #define PKDG_CELL_FLOATS 36   /* canonical cell record, see pkdg_cells */
@@ -50,6 +62,8 @@ typedef int32_t pkdg_status;
 #define PKDG_ENOMEM (-3)   /* workspace allocation failed */
 #define PKDG_EBADLIST (-4) /* validation found a non-monotone offset, an index out of range or a
                               negative bucket count (only reported by pkdg_get_stats) */
+#define PKDG_EBADVALUE (-5) /* PKDG_VALIDATE found values or geometry outside the documented range
+                               (only reported by pkdg_get_stats) */
 
 /* flags of pkdg_gravity_eval* */
 #define PKDG_ACCUMULATE 0x1u /* add to out instead of overwriting it */
@@ -63,7 +77,14 @@ typedef int32_t pkdg_status;
                                 references stand for, tiles_pp two references per tile.  With the
                                 streamed variants `buckets_host` must hold ALL buckets a reference may
                                 name (it always does: references index it).                           */
-#define PKDG_VARIANT_SHIFT 8 /* bits 8..15: kernel tuning variant, 0 = library default */
+#define PKDG_VALIDATE 0x40u  /* check the value-range contract below on the device (two extra kernels): every
+                                coordinate finite and |x| <= 1e12, masses and moments finite
+                                (invalid_values), every listed (sink, cell) pair with the sink outside the
+                                cell's b_max sphere (invalid_pairs); reported by pkdg_get_stats          */
+#define PKDG_NO_FIXUP 0x10u  /* do not re-evaluate ill-conditioned sinks in fp64 (see "Precision" below)   */
+#define PKDG_FIXUP_ALL 0x20u /* send EVERY sink through the fp64 fix-up kernel (fp64 terms and fp64
+                                accumulators throughout: the cost of PAPER.md:L83's double-precision
+                                accumulation, measured by bench.py --report; also the test of that kernel) */
 
 typedef struct pkdg_ctx pkdg_ctx;
 
@@ -88,6 +109,14 @@ typedef struct { const int32_t *first; const int32_t *count; int64_t n; } pkdg_b
  * is ignored.  A NULL pkdg_list* or NULL offsets means "no list of this kind". */
 typedef struct { const int64_t *offsets; const int32_t *idx; } pkdg_list;
 
+/* Groups of consecutive buckets that SHARE one P-P and one P-C list (PAPER.md:L69:
+ * "If a source cell is reached with fewer than g particles (called the group size) we proceed no deeper in
+ * the tree resolving the remaining checklist into interaction lists ... a group size of 64, or more
+ * generally four times the bucket size").  Group g holds buckets first_bucket[g] .. first_bucket[g] +
+ * n_buckets[g] - 1; the groups must tile the bucket range in order.  With groups the lists have n + 1
+ * offsets (one list per group) and every sink of the group's buckets evaluates the whole list. */
+typedef struct { const int32_t *first_bucket; const int32_t *n_buckets; int64_t n; } pkdg_groups;
+
 /* Counters of the last evaluation on a context (pkdg_get_stats synchronises the stream). */
 typedef struct {
     int64_t n_buckets;
@@ -97,6 +126,9 @@ typedef struct {
     int64_t tiles_pc;
     int64_t bad_entries;     /* validation failures (0 when the input is well-formed)            */
     int64_t chunks;          /* streamed variants: number of chunks issued, else 1              */
+    int64_t fixup_sinks;     /* sinks re-evaluated by the fp64 fix-up kernel                      */
+    int64_t invalid_values;  /* PKDG_VALIDATE: particles / cell records with values out of range  */
+    int64_t invalid_pairs;   /* PKDG_VALIDATE: listed (sink, cell) pairs with |x - COM| <= b_max   */
 } pkdg_stats;
 
 /* Create / destroy a context on CUDA device `device`.  The context owns only internal workspace
@@ -104,6 +136,10 @@ typedef struct {
  * (the first call with a larger problem allocates and is therefore synchronous). */
 pkdg_status pkdg_create(pkdg_ctx **ctx, int device);
 pkdg_status pkdg_destroy(pkdg_ctx *ctx);
+
+/* Options of a context.  PKDG_OPT_KAPPA2: conditioning threshold of the fp64 fix-up (> 0; default 8). */
+#define PKDG_OPT_KAPPA2 1
+pkdg_status pkdg_set_option(pkdg_ctx *ctx, int32_t option, double value);
 
 /* One pass of the whole hot path with everything resident on the device:
  *   a1 packer       bucket work descriptors, tile counts, validation, I_pp / I_pc
@@ -115,6 +151,23 @@ pkdg_status pkdg_destroy(pkdg_ctx *ctx);
 pkdg_status pkdg_gravity_eval(pkdg_ctx *ctx, const pkdg_particles *particles, const pkdg_cells *cells,
                               const pkdg_buckets *buckets, const pkdg_list *pp, const pkdg_list *pc,
                               float eps, uint32_t flags, float *out_acc_pot, void *stream);
+
+/* The same for the contiguous bucket range [b0, b1) of `buckets` (multi-GPU: every rank evaluates its own
+ * range; no collective on the data path).  pp / pc hold the lists of those b1 - b0 buckets
+ * only: b1 - b0 + 1 offsets, offsets[k] indexing `idx` as passed.  With PKDG_PP_LEAVES the references still
+ * index the FULL `buckets` arrays.  pkdg_stats counts the range only. */
+pkdg_status pkdg_gravity_eval_range(pkdg_ctx *ctx, const pkdg_particles *particles, const pkdg_cells *cells,
+                                    const pkdg_buckets *buckets, int64_t b0, int64_t b1, const pkdg_list *pp,
+                                    const pkdg_list *pc, float eps, uint32_t flags, float *out_acc_pot,
+                                    void *stream);
+
+/* The same with group-shared lists: pp / pc hold one list per GROUP (groups->n + 1 offsets).  A group's own
+ * particles are on its P-P list like any others (self pairs are skipped by index).  4 x fewer list entries
+ * to store and move than per-bucket lists; pkdg_stats counts sink x entry interactions as always. */
+pkdg_status pkdg_gravity_eval_groups(pkdg_ctx *ctx, const pkdg_particles *particles, const pkdg_cells *cells,
+                                     const pkdg_buckets *buckets, const pkdg_groups *groups, const pkdg_list *pp,
+                                     const pkdg_list *pc, float eps, uint32_t flags, float *out_acc_pot,
+                                     void *stream);
 
 /* Streamed variant (a6; "fully asynchronous", L278 bounded queue): particles, cells
  * and out are device buffers, buckets and lists are PINNED HOST buffers.  Contiguous bucket ranges
@@ -130,16 +183,31 @@ pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx *ctx, const pkdg_particles *part
 
 /* End-to-end variant: EVERY buffer is a host buffer (pinned for full speed).  Copies particles and
  * cells to the device, streams the lists as above, copies the result back into out_acc_pot_host and
- * synchronises before returning.  Rows of particles in no bucket come back as 0 (as the caller's
- * values with PKDG_ACCUMULATE).  When the buckets tile the particle array (first[0] = 0, every bucket
- * starts where the previous one ends, the last one ends at n: the tree order of PAPER.md:L63) the rows
- * of each chunk are copied back on the chunk's stream as soon as its kernel is done, overlapping the
- * host->device traffic of later chunks. */
+ * synchronises before returning (also when it returns an error).  Rows of particles in no listed bucket
+ * keep the caller's values, as in pkdg_gravity_eval.  When every bucket starts where the previous one
+ * ends (the tree order of PAPER.md:L63) the rows of each chunk are copied back on the chunk's stream as
+ * soon as its kernels are done, overlapping the host->device traffic of later chunks; otherwise the
+ * caller's rows make a round trip through the device.
+ * pkdg_gravity_eval_host_range: the same for the bucket range [b0, b1) of `buckets_host`, with the lists
+ * of that range only (multi-GPU end to end: each rank passes its own range and lists).
+ * pkdg_gravity_eval_host_groups: the same with group-shared lists (chunks are then ranges of groups). */
 pkdg_status pkdg_gravity_eval_host(pkdg_ctx *ctx, const pkdg_particles *particles_host,
                                    const pkdg_cells *cells_host, const pkdg_buckets *buckets_host,
                                    const pkdg_list *pp_host, const pkdg_list *pc_host, float eps,
                                    uint32_t flags, float *out_acc_pot_host, int32_t n_streams,
                                    int64_t max_entries_per_chunk);
+pkdg_status pkdg_gravity_eval_host_groups(pkdg_ctx *ctx, const pkdg_particles *particles_host,
+                                          const pkdg_cells *cells_host, const pkdg_buckets *buckets_host,
+                                          const pkdg_groups *groups_host, const pkdg_list *pp_host,
+                                          const pkdg_list *pc_host, float eps, uint32_t flags,
+                                          float *out_acc_pot_host, int32_t n_streams,
+                                          int64_t max_entries_per_chunk);
+pkdg_status pkdg_gravity_eval_host_range(pkdg_ctx *ctx, const pkdg_particles *particles_host,
+                                         const pkdg_cells *cells_host, const pkdg_buckets *buckets_host,
+                                         int64_t b0, int64_t b1, const pkdg_list *pp_host,
+                                         const pkdg_list *pc_host, float eps, uint32_t flags,
+                                         float *out_acc_pot_host, int32_t n_streams,
+                                         int64_t max_entries_per_chunk);
 
 /* Packer made visible for bit-exact checks (SURVEY.md sec 8(c) "Integer side"): the tiles the
  * evaluation kernel consumes.  tile_offsets = [n_buckets+1] int64 (first tile of each bucket);
@@ -161,12 +229,14 @@ pkdg_status pkdg_prepare_cells_export(pkdg_ctx *ctx, const pkdg_cells *cells, fl
 /* Synchronises the stream(s) of the last evaluation and returns its counters. */
 pkdg_status pkdg_get_stats(pkdg_ctx *ctx, pkdg_stats *stats_host);
 
-/* Device timing of the evaluation kernel alone (the dominant kernel of the path).  With profiling
- * on, pkdg_gravity_eval brackets its evaluation-kernel launch with CUDA events on the launching
- * stream (ring of 256 pairs).  pkdg_profile_read synchronises, returns the number of launches
- * recorded since the last read and their total duration in milliseconds, and clears the ring. */
+/* Device timing of the evaluation kernel alone (the dominant kernel of the path) and of the fp64 fix-up
+ * kernel that follows it.  With profiling on, pkdg_gravity_eval(_range) brackets those launches with CUDA
+ * events on the launching stream (ring of 256 calls).  pkdg_profile_read synchronises, returns the number
+ * of calls recorded since the last read and the total duration of each kernel in milliseconds
+ * (fixup_ms_total_host may be NULL), and clears the ring. */
 pkdg_status pkdg_profile_enable(pkdg_ctx *ctx, int32_t on);
-pkdg_status pkdg_profile_read(pkdg_ctx *ctx, int64_t *n_launches_host, double *eval_ms_total_host);
+pkdg_status pkdg_profile_read(pkdg_ctx *ctx, int64_t *n_launches_host, double *eval_ms_total_host,
+                              double *fixup_ms_total_host);
 
 /* Number of kernel launches this context has made since creation. */
 int64_t pkdg_launch_count(const pkdg_ctx *ctx);
@@ -178,17 +248,6 @@ void pkdg_version(int32_t *major, int32_t *minor);
 /* FP32 FFMA-only micro-benchmark (roofline denominator check): runs `iters` dependent-chain-free
  * FFMA rounds on every SM and returns the elapsed milliseconds and the flop count. Synchronous. */
 pkdg_status pkdg_fma_peak_probe(pkdg_ctx *ctx, int64_t iters, float *ms_host, double *flops_host);
-
-/* The same for other operand patterns (DESIGN.md sec 6 "register-file bandwidth"): registers only, no
- * memory in the timed loop, 4 CTAs of 128 threads per SM.  flops_host counts FMA = 2 and, for modes 4
- * and 5, the audited flops of the P-C body (196 scalar with Newton step, 187 packed). */
-#define PKDG_PROBE_FFMA_CONST 0   /* FFMA, two constant-bank operands: the FMA-pipe peak               */
-#define PKDG_PROBE_FFMA_3REG 1    /* scalar FFMA, three distinct register operands                      */
-#define PKDG_PROBE_FFMA2_3REG 2   /* packed FFMA2, three distinct register pairs                        */
-#define PKDG_PROBE_FFMA2_REUSE 3  /* FFMA2 scalar x pair + pair, pair shared by 3 consecutive FFMA2     */
-#define PKDG_PROBE_PC_SCALAR 4    /* generation-1 scalar P-C body, two sinks per trip                   */
-#define PKDG_PROBE_PC_PACKED 5    /* packed P-C body of the default kernel, one sink pair per trip      */
-pkdg_status pkdg_fma_probe(pkdg_ctx *ctx, int32_t mode, int64_t iters, float *ms_host, double *flops_host);
 
 #ifdef __cplusplus
 }

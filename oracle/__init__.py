@@ -49,6 +49,8 @@ def lib():
                                        c_double, c_void_p, c_int64, c_void_p]
         L.orc_contribution_norms.restype = c_int
         L.orc_contribution_norms.argtypes = L.orc_gravity_eval.argtypes
+        L.orc_contribution_norms2.restype = c_int
+        L.orc_contribution_norms2.argtypes = L.orc_gravity_eval.argtypes
         L.orc_direct_sum.argtypes = [c_int64, c_void_p, c_double, c_void_p, c_int64, c_void_p]
         L.orc_pack_tiles.restype = c_int64
         L.orc_pack_tiles.argtypes = [c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
@@ -130,9 +132,10 @@ def gravity_eval(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps,
     return out
 
 
-def contribution_norms(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, sel=None):
+def contribution_norms(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, sel=None, squared=False):
     """S_i = sum over list entries of |a_ij| for the targets of the evaluated buckets (NaN elsewhere).
-    kappa_i = S_i / |a_i| is the condition number of the sum a_i."""
+    kappa_i = S_i / |a_i| is the condition number of the sum a_i.  squared=True: the sum
+    of |a_ij|^2 instead (kappa2_i = sqrt(S2_i) / |a_i|, what independent rounding errors grow with)."""
     xyzm = _c(xyzm, np.float32)
     n = xyzm.shape[0]
     if cells is None:
@@ -144,7 +147,8 @@ def contribution_norms(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx
     pc_off = _c(pc_off, np.int64); pc_idx = _c(pc_idx, np.int32)
     sel_a = _c(sel, np.int64)
     out = np.full(n, np.nan)
-    err = lib().orc_contribution_norms(n, _p(xyzm), cells.shape[0], _p(cells), stride, first.shape[0],
+    fn = lib().orc_contribution_norms2 if squared else lib().orc_contribution_norms
+    err = fn(n, _p(xyzm), cells.shape[0], _p(cells), stride, first.shape[0],
                                        _p(first), _p(count), _p(pp_off), _p(pp_idx), _p(pc_off),
                                        _p(pc_idx), float(eps), _p(sel_a),
                                        0 if sel_a is None else sel_a.shape[0], _p(out))

@@ -238,11 +238,11 @@ int orc_gravity_eval(int64_t n_particles, const float *xyzm, int64_t n_cells, co
  * error of any finite-precision evaluation grows in proportion to it.  Diagnostic
  * only: no evaluation result depends on it.  out_abs: [n_particles] fp64.
  * ------------------------------------------------------------------------- */
-int orc_contribution_norms(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
-                           int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
-                           const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
-                           const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
-                           double *out_abs) {
+static int contribution_norms_p(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
+                                int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
+                                const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
+                                const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
+                                double *out_abs, int squared) {
     int64_t nb = sel ? n_sel : n_buckets;
     int err = 0;
 #pragma omp parallel for schedule(dynamic, 8)
@@ -265,7 +265,7 @@ int orc_contribution_norms(int64_t n_particles, const float *xyzm, int64_t n_cel
                     double xs[3] = {xyzm[4 * j], xyzm[4 * j + 1], xyzm[4 * j + 2]};
                     double a[3] = {0, 0, 0}, pot = 0;
                     orc_pp_pair(xt, xs, (double)xyzm[4 * j + 3], eps, a, &pot);
-                    S += sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+                    S += squared ? a[0] * a[0] + a[1] * a[1] + a[2] * a[2] : sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
                 }
             }
             if (pc_off) {
@@ -274,13 +274,34 @@ int orc_contribution_norms(int64_t n_particles, const float *xyzm, int64_t n_cel
                     if (c < 0 || c >= n_cells) continue;
                     double a[3] = {0, 0, 0}, pot = 0;
                     orc_pc_pair(xt, cells + c * (int64_t)stride, a, &pot);
-                    S += sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+                    S += squared ? a[0] * a[0] + a[1] * a[1] + a[2] * a[2] : sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
                 }
             }
             out_abs[i] = S;
         }
     }
     return err;
+}
+
+int orc_contribution_norms(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
+                           int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
+                           const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
+                           const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
+                           double *out_abs) {
+    return contribution_norms_p(n_particles, xyzm, n_cells, cells, stride, n_buckets, first, count, pp_off, pp_idx,
+                                pc_off, pc_idx, eps, sel, n_sel, out_abs, 0);
+}
+
+/* The same with squares: S2_i = sum over list entries of |a_ij|^2.  kappa2_i = sqrt(S2_i) / |a_i| is what the
+ * error of a sum of terms with INDEPENDENT rounding errors grows with (DESIGN.md "Conditioning and the fp64
+ * fix-up"); used to calibrate and to test the library's fix-up threshold.  Diagnostic only. */
+int orc_contribution_norms2(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells,
+                            int32_t stride, int64_t n_buckets, const int32_t *first, const int32_t *count,
+                            const int64_t *pp_off, const int32_t *pp_idx, const int64_t *pc_off,
+                            const int32_t *pc_idx, double eps, const int64_t *sel, int64_t n_sel,
+                            double *out_sq) {
+    return contribution_norms_p(n_particles, xyzm, n_cells, cells, stride, n_buckets, first, count, pp_off, pp_idx,
+                                pc_off, pc_idx, eps, sel, n_sel, out_sq, 1);
 }
 
 /* Direct summation: the plain definition the tree method approximates

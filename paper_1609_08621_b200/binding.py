@@ -21,14 +21,18 @@ ACCUMULATE = 0x1
 SKIP_PP = 0x2
 SKIP_PC = 0x4
 PP_LEAVES = 0x8
-VARIANT_SHIFT = 8
+NO_FIXUP = 0x10
+FIXUP_ALL = 0x20
+VALIDATE = 0x40
+OPT_KAPPA2 = 1
 CELL_FLOATS = 36
 CELLQ_FLOATS = 32
 
-EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_streamed",
-           "pkdg_gravity_eval_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
-           "pkdg_get_stats", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version",
-           "pkdg_fma_peak_probe", "pkdg_fma_probe"]
+EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
+           "pkdg_gravity_eval_host", "pkdg_gravity_eval_host_range", "pkdg_gravity_eval_groups",
+           "pkdg_gravity_eval_host_groups", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
+           "pkdg_get_stats", "pkdg_set_option", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count",
+           "pkdg_status_string", "pkdg_last_error", "pkdg_version", "pkdg_fma_peak_probe"]
 
 
 class PkdgError(RuntimeError):
@@ -47,13 +51,18 @@ class _Buckets(Structure):
     _fields_ = [("first", c_void_p), ("count", c_void_p), ("n", c_int64)]
 
 
+class _Groups(Structure):
+    _fields_ = [("first_bucket", c_void_p), ("n_buckets", c_void_p), ("n", c_int64)]
+
+
 class _List(Structure):
     _fields_ = [("offsets", c_void_p), ("idx", c_void_p)]
 
 
 class Stats(Structure):
     _fields_ = [("n_buckets", c_int64), ("interactions_pp", c_int64), ("interactions_pc", c_int64),
-                ("tiles_pp", c_int64), ("tiles_pc", c_int64), ("bad_entries", c_int64), ("chunks", c_int64)]
+                ("tiles_pp", c_int64), ("tiles_pc", c_int64), ("bad_entries", c_int64), ("chunks", c_int64),
+                ("fixup_sinks", c_int64), ("invalid_values", c_int64), ("invalid_pairs", c_int64)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -68,18 +77,30 @@ def _load():
     L.pkdg_destroy.argtypes = [c_void_p]
     L.pkdg_gravity_eval.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                     POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_void_p]
+    L.pkdg_gravity_eval_range.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets), c_int64,
+                                          c_int64, POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p,
+                                          c_void_p]
     L.pkdg_gravity_eval_streamed.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                              POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p,
                                              c_int32, c_int64, c_void_p]
     L.pkdg_gravity_eval_host.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                          POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_int32,
                                          c_int64]
+    L.pkdg_gravity_eval_host_range.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                               c_int64, c_int64, POINTER(_List), POINTER(_List), c_float, c_uint32,
+                                               c_void_p, c_int32, c_int64]
+    L.pkdg_gravity_eval_groups.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                           POINTER(_Groups), POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p,
+                                           c_void_p]
+    L.pkdg_gravity_eval_host_groups.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                                POINTER(_Groups), POINTER(_List), POINTER(_List), c_float, c_uint32,
+                                                c_void_p, c_int32, c_int64]
     L.pkdg_pack_export.argtypes = [c_void_p, c_int64, POINTER(_List), c_void_p, c_void_p, c_int64, c_void_p]
     L.pkdg_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int64)]
     L.pkdg_prepare_cells_export.argtypes = [c_void_p, POINTER(_Cells), c_void_p, c_void_p]
     L.pkdg_get_stats.argtypes = [c_void_p, POINTER(Stats)]
     L.pkdg_profile_enable.argtypes = [c_void_p, c_int32]
-    L.pkdg_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_double)]
+    L.pkdg_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_double), POINTER(c_double)]
     L.pkdg_launch_count.argtypes = [c_void_p]
     L.pkdg_launch_count.restype = c_int64
     L.pkdg_status_string.argtypes = [c_int32]
@@ -88,7 +109,7 @@ def _load():
     L.pkdg_last_error.restype = c_char_p
     L.pkdg_version.argtypes = [POINTER(c_int32), POINTER(c_int32)]
     L.pkdg_fma_peak_probe.argtypes = [c_void_p, c_int64, POINTER(c_float), POINTER(c_double)]
-    L.pkdg_fma_probe.argtypes = [c_void_p, c_int32, c_int64, POINTER(c_float), POINTER(c_double)]
+    L.pkdg_set_option.argtypes = [c_void_p, c_int32, c_double]
     for name in EXPORTS:
         if name not in ("pkdg_launch_count", "pkdg_status_string", "pkdg_last_error", "pkdg_version"):
             getattr(L, name).restype = c_int32
@@ -198,6 +219,18 @@ class Context:
         self._check(s, "pkdg_gravity_eval")
         return out
 
+    def gravity_eval_range(self, xyzm, cells, first, count, b0, b1, pp_off, pp_idx, pc_off, pc_idx, eps, out, flags=0,
+                           stream=None):
+        """pkdg_gravity_eval_range: buckets [b0, b1) of the full (first, count) arrays; the lists are those of the
+        range only (b1 - b0 + 1 offsets).  Asynchronous on `stream`."""
+        P, C, B, pp, pc = self._structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx)
+        _dt(out, "float32", "out")
+        s = _lib.pkdg_gravity_eval_range(self._h, byref(P), byref(C) if C else None, byref(B), int(b0), int(b1),
+                                         byref(pp) if pp else None, byref(pc) if pc else None, float(eps), int(flags),
+                                         _ptr(out), _stream_ptr(stream))
+        self._check(s, "pkdg_gravity_eval_range")
+        return out
+
     def gravity_eval_streamed(self, xyzm, cells, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h, eps, out,
                               n_streams=3, max_entries_per_chunk=1 << 24, flags=0, stream=None):
         """pkdg_gravity_eval_streamed: device particles/cells/out, HOST buckets and lists."""
@@ -217,6 +250,41 @@ class Context:
                                         byref(pp) if pp else None, byref(pc) if pc else None, float(eps), int(flags),
                                         _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
         self._check(s, "pkdg_gravity_eval_host")
+        return out_h
+
+    def gravity_eval_host_range(self, xyzm_h, cells_h, first_h, count_h, b0, b1, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h,
+                                eps, out_h, n_streams=3, max_entries_per_chunk=1 << 24, flags=0):
+        """pkdg_gravity_eval_host_range: buckets [b0, b1) of the full host bucket arrays, lists of the range only."""
+        P, C, B, pp, pc = self._structs(xyzm_h, cells_h, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h)
+        s = _lib.pkdg_gravity_eval_host_range(self._h, byref(P), byref(C) if C else None, byref(B), int(b0), int(b1),
+                                              byref(pp) if pp else None, byref(pc) if pc else None, float(eps),
+                                              int(flags), _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
+        self._check(s, "pkdg_gravity_eval_host_range")
+        return out_h
+
+    def gravity_eval_groups(self, xyzm, cells, first, count, g_first, g_n, pp_off, pp_idx, pc_off, pc_idx, eps, out,
+                            flags=0, stream=None):
+        """pkdg_gravity_eval_groups: one P-P and one P-C list per GROUP of consecutive buckets (offsets have
+        n_groups + 1 entries); everything resident; asynchronous on `stream`."""
+        P, C, B, pp, pc = self._structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx)
+        _dt(g_first, "int32", "g_first"); _dt(g_n, "int32", "g_n"); _dt(out, "float32", "out")
+        G = _Groups(_ptr(g_first), _ptr(g_n), int(g_first.shape[0]))
+        s = _lib.pkdg_gravity_eval_groups(self._h, byref(P), byref(C) if C else None, byref(B), byref(G),
+                                          byref(pp) if pp else None, byref(pc) if pc else None, float(eps), int(flags),
+                                          _ptr(out), _stream_ptr(stream))
+        self._check(s, "pkdg_gravity_eval_groups")
+        return out
+
+    def gravity_eval_host_groups(self, xyzm_h, cells_h, first_h, count_h, g_first_h, g_n_h, pp_off_h, pp_idx_h, pc_off_h,
+                                 pc_idx_h, eps, out_h, n_streams=3, max_entries_per_chunk=1 << 24, flags=0):
+        """pkdg_gravity_eval_host_groups: every buffer on the host, group-shared lists; synchronous."""
+        P, C, B, pp, pc = self._structs(xyzm_h, cells_h, first_h, count_h, pp_off_h, pp_idx_h, pc_off_h, pc_idx_h)
+        _dt(g_first_h, "int32", "g_first"); _dt(g_n_h, "int32", "g_n")
+        G = _Groups(_ptr(g_first_h), _ptr(g_n_h), int(g_first_h.shape[0]))
+        s = _lib.pkdg_gravity_eval_host_groups(self._h, byref(P), byref(C) if C else None, byref(B), byref(G),
+                                               byref(pp) if pp else None, byref(pc) if pc else None, float(eps),
+                                               int(flags), _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
+        self._check(s, "pkdg_gravity_eval_host_groups")
         return out_h
 
     def pack_export(self, n_buckets, off, idx, tile_offsets, tiles, stream=None):
@@ -244,20 +312,16 @@ class Context:
         self._check(_lib.pkdg_profile_enable(self._h, 1 if on else 0), "pkdg_profile_enable")
 
     def profile_read(self):
-        """(n_launches, total_ms) of the evaluation kernel since the last read (synchronises)."""
-        n, ms = c_int64(), c_double()
-        self._check(_lib.pkdg_profile_read(self._h, byref(n), byref(ms)), "pkdg_profile_read")
-        return n.value, ms.value
+        """(n_calls, eval_kernel_ms_total, fixup_kernel_ms_total) since the last read (synchronises)."""
+        n, ms, fx = c_int64(), c_double(), c_double()
+        self._check(_lib.pkdg_profile_read(self._h, byref(n), byref(ms), byref(fx)), "pkdg_profile_read")
+        return n.value, ms.value, fx.value
 
     def launch_count(self) -> int:
         return int(_lib.pkdg_launch_count(self._h))
 
-    def fma_probe(self, mode: int, iters: int = 1 << 12):
-        """(ms, flops) of probe `mode` (PKDG_PROBE_*: 0 const-operand FFMA, 1 3-register FFMA, 2 FFMA2,
-        3 FFMA2 with operand reuse, 4 scalar P-C body, 5 packed P-C body)."""
-        ms, fl = c_float(), c_double()
-        self._check(_lib.pkdg_fma_probe(self._h, int(mode), int(iters), byref(ms), byref(fl)), "pkdg_fma_probe")
-        return ms.value, fl.value
+    def set_option(self, option: int, value: float):
+        self._check(_lib.pkdg_set_option(self._h, int(option), float(value)), "pkdg_set_option")
 
     def fma_peak_probe(self, iters: int = 1 << 14):
         ms, fl = c_float(), c_double()

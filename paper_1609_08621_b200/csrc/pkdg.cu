@@ -16,6 +16,10 @@ using namespace pkdg;
 namespace {
 
 constexpr int kMaxSlots = 8;
+// Conditioning threshold: a sink goes to the fp64 fix-up kernel
+// when sqrt(sum_j |a_ij|^2) > kappa2 |a_i|.  Measured fp32 error <= 1.2e-6 sqrt(S2) / |a| over 1.3e7 sinks, so
+// kappa2 = 6 keeps the fp32 path below 7e-6 of |a_i|, a third of the 2e-5 tolerance.
+constexpr float kDefaultKappa2 = 6.0f;
 
 struct Slot {
     cudaStream_t st = nullptr;
@@ -27,6 +31,10 @@ struct Slot {
     int64_t *pp_off = nullptr, *pc_off = nullptr;
     BucketDesc* desc = nullptr;
     int64_t cap_b = 0;
+    int4* fixq = nullptr;       // fix-up queue of the chunk in flight on this slot
+    int64_t fixq_cap = 0;
+    int32_t *gfirst = nullptr, *gn = nullptr;   // group-shared lists: the chunk's groups
+    int64_t cap_g = 0, cap_off = 0;
 };
 
 }  // namespace
@@ -39,7 +47,11 @@ struct pkdg_ctx {
     BucketDesc* desc = nullptr;
     int64_t desc_cap = 0;
     DevStats* stats = nullptr;
-    unsigned int* counters = nullptr;  // [kMaxSlots + 1]
+    unsigned int* counters = nullptr;  // [2 (kMaxSlots + 1)]: work counters, then fix-up queue lengths
+    int4* fixq = nullptr;              // fix-up queue of the resident call
+    int64_t fixq_cap = 0;
+    float kappa2 = kDefaultKappa2;     // PKDG_OPT_KAPPA2
+    unsigned long long fix_entries = 0, fix_calls = 0;
     Slot slots[kMaxSlots];
     int n_slots_live = 0;
     cudaEvent_t ev_ready = nullptr;
@@ -53,10 +65,12 @@ struct pkdg_ctx {
     int32_t *g_first = nullptr, *g_count = nullptr;  // streamed variants: device copy of the bucket arrays
     int64_t g_first_cap = 0, g_count_cap = 0;
     cudaStream_t last_stream = nullptr;
+    bool eval_configured = false;      // dynamic-smem opt-in of the evaluation kernel done on this device
+    int eval_per_sm = 1;
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
     bool profiling = false;
-    cudaEvent_t prof_ev[512] = {};
+    cudaEvent_t prof_ev[3 * 256] = {};  // per recorded call: before / after the evaluation kernel, after the fix-up
     int prof_n = 0;
     std::string err;
 };
@@ -90,56 +104,29 @@ pkdg_status ensure(pkdg_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <int WARPS, int MINB, bool NEWTON, int UNR>
-pkdg_status launch_eval_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
-    int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pkdg_eval_kernel<WARPS, MINB, NEWTON, UNR>, WARPS * 32, 0));
-    if (per_sm < 1) per_sm = 1;
-    int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
-    int64_t grid = (int64_t)ctx->num_sms * per_sm;
-    if (grid > want) grid = want;
-    if (grid < 1) grid = 1;
-    pkdg_eval_kernel<WARPS, MINB, NEWTON, UNR><<<(unsigned)grid, WARPS * 32, 0, st>>>(p);
-    ctx->launches++;
-    CK(cudaGetLastError());
-    return PKDG_OK;
-}
+constexpr int kEvalWarps = 4;   // warps per CTA of the evaluation kernel
+constexpr int kEvalMinBlocks = 3;  // CTAs per SM it is compiled for (168 registers per thread)
 
-template <int WARPS, int MINB, bool NEWTON>
-pkdg_status launch_eval3_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
-    auto kern = pkdg_eval3_kernel<WARPS, MINB, NEWTON>;
-    const int smem = WARPS * (int)sizeof(WarpSmem3);
-    static bool configured = false;  // per instantiation; the attribute is per function and sticky
-    if (!configured) {
+// The evaluation kernel needs more than the default 48 KB of dynamic shared memory.  Function attributes
+// are per device, so the opt-in is made once per context (a pkdg_ctx is bound to one device).
+pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    auto kern = pkdg_eval3_kernel<kEvalWarps, kEvalMinBlocks>;
+    const int smem = kEvalWarps * (int)sizeof(WarpSmem3);
+    if (!ctx->eval_configured) {
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        configured = true;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->eval_per_sm, kern, kEvalWarps * 32, smem));
+        if (ctx->eval_per_sm < 1) ctx->eval_per_sm = 1;
+        ctx->eval_configured = true;
     }
-    int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
-    if (per_sm < 1) per_sm = 1;
-    int64_t want = (p.n_buckets + WARPS - 1) / WARPS;
-    int64_t grid = (int64_t)ctx->num_sms * per_sm;
+    int64_t want = (p.n_buckets + kEvalWarps - 1) / kEvalWarps;
+    int64_t grid = (int64_t)ctx->num_sms * ctx->eval_per_sm;
     if (grid > want) grid = want;
     if (grid < 1) grid = 1;
-    kern<<<(unsigned)grid, WARPS * 32, smem, st>>>(p);
+    kern<<<(unsigned)grid, kEvalWarps * 32, smem, st>>>(p);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
-}
-
-// Tuning variants (flags bits 8..15).  0 = library default.
-pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
-    unsigned variant = (p.flags >> PKDG_VARIANT_SHIFT) & 0xffu;
-    if ((p.flags & PKDG_PP_LEAVES) && variant == 1)
-        return fail(ctx, PKDG_EINVAL, "PKDG_PP_LEAVES is not implemented by kernel variant 1 (generation 1)");
-    switch (variant) {
-        case 0: return launch_eval3_t<4, 3, false>(ctx, p, st);   // packed FP32x2, 168 registers, 12 warps / SM
-        case 1: return launch_eval_t<4, 4, true, 2>(ctx, p, st);  // generation 1: scalar arithmetic (A/B reference)
-        case 2: return launch_eval3_t<4, 4, false>(ctx, p, st);   // packed, 128 registers, 16 warps / SM
-        case 3: return launch_eval3_t<4, 3, true>(ctx, p, st);    // packed, Newton step on the P-C rsqrt
-        default: return fail(ctx, PKDG_EINVAL, "unknown kernel variant in flags bits 8..15");
-    }
 }
 
 pkdg_status check_common(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
@@ -168,10 +155,49 @@ void fill_params(EvalParams& p, pkdg_ctx* ctx, const float* xyzm, int64_t np, in
     p.n_particles = np;
     p.n_cells = nc;
     float h = 2.0f * eps;
+    p.eps = eps;
     p.h2 = h * h;
     p.h2c = fmaxf(h * h, 1.0e-24f);
     p.hinv = h > 0.0f ? 1.0f / h : 0.0f;
     p.flags = flags;
+    p.cells_raw = nullptr;
+    p.cells_stride = PKDG_CELL_FLOATS;
+    p.fix_k = (flags & PKDG_NO_FIXUP) ? -1.0f : (flags & PKDG_FIXUP_ALL) ? 0.0f : ctx->kappa2 * ctx->kappa2;
+    p.fix_queue = nullptr;
+    p.fix_count = nullptr;
+    p.fix_cap = 0;
+}
+
+// Queue capacity that cannot overflow: one entry per (bucket, pass of 16 sinks) at most.
+// PKDG_VALIDATE: value-range and geometry contract of include/pkdg.h, counted into the statistics.
+pkdg_status launch_validate(pkdg_ctx* ctx, const EvalParams& p, bool values, cudaStream_t st) {
+    if (values) {
+        pkdg_validate_values_kernel<<<ctx->num_sms * 8, 256, 0, st>>>(p.xyzm, p.n_particles, p.cells_raw,
+                                                                     p.cells_raw ? p.n_cells : 0, p.cells_stride, p.stats);
+        ctx->launches++;
+    }
+    if (p.n_cells > 0 && p.pc_idx) {
+        pkdg_validate_pairs_kernel<<<ctx->num_sms * 8, 256, 0, st>>>(p);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+int64_t fix_capacity(int64_t n_buckets, int64_t n_particles) { return n_buckets + n_particles / kTMax + 16; }
+
+// The fp64 fix-up kernel over the queue the evaluation kernel just filled (same stream).  Its grid is fixed
+// (the queue length is known only on the device); with an empty queue every warp leaves at once.
+pkdg_status launch_fixup(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    if (p.fix_k < 0.0f) return PKDG_OK;
+    int64_t warps = p.n_buckets < 1 ? 1 : p.n_buckets;
+    int64_t grid = (warps + 3) / 4;
+    const int64_t full = (int64_t)ctx->num_sms * 8;
+    if (grid > full) grid = full;
+    pkdg_fixup_kernel<<<(unsigned)grid, 128, 0, st>>>(p);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
 }
 
 pkdg_status prep_cells(pkdg_ctx* ctx, const pkdg_cells* C, float* dst, cudaStream_t st) {
@@ -234,9 +260,9 @@ pkdg_status pkdg_create(pkdg_ctx** out, int device) {
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->stats, sizeof(DevStats));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->counters, sizeof(unsigned int) * (kMaxSlots + 1));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->counters, sizeof(unsigned int) * 2 * (kMaxSlots + 1));
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(DevStats));
-    if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(unsigned int) * (kMaxSlots + 1));
+    if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(unsigned int) * 2 * (kMaxSlots + 1));
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_ready, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         fprintf(stderr, "pkdg_create: %s\n", cudaGetErrorString(e));
@@ -253,11 +279,11 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
     cudaDeviceSynchronize();
     cudaFree(ctx->cellq); cudaFree(ctx->desc); cudaFree(ctx->stats); cudaFree(ctx->counters);
     cudaFree(ctx->e2e_xyzm); cudaFree(ctx->e2e_cells); cudaFree(ctx->e2e_out); cudaFree(ctx->scan_tmp);
-    cudaFree(ctx->gfc); cudaFree(ctx->g_first); cudaFree(ctx->g_count);
+    cudaFree(ctx->gfc); cudaFree(ctx->g_first); cudaFree(ctx->g_count); cudaFree(ctx->fixq);
     for (int i = 0; i < ctx->n_slots_live; ++i) {
         Slot& s = ctx->slots[i];
         cudaFree(s.pp_idx); cudaFree(s.pc_idx); cudaFree(s.first); cudaFree(s.count);
-        cudaFree(s.pp_off); cudaFree(s.pc_off); cudaFree(s.desc);
+        cudaFree(s.pp_off); cudaFree(s.pc_off); cudaFree(s.desc); cudaFree(s.fixq); cudaFree(s.gfirst); cudaFree(s.gn);
         if (s.st) cudaStreamDestroy(s.st);
         if (s.done) cudaEventDestroy(s.done);
     }
@@ -269,11 +295,18 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
     return PKDG_OK;
 }
 
-pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
-                              const pkdg_list* pp, const pkdg_list* pc, float eps, uint32_t flags, float* out,
-                              void* stream) {
-    pkdg_status s = check_common(ctx, P, C, B, pp, pc, out);
+// Sinks are buckets [b0, b1) of Bfull; the lists have b1 - b0 + 1 offsets; P-P leaf references index Bfull.
+// G != NULL (group-shared lists): the lists have G->n + 1 offsets and the range must be all buckets.
+static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* Bfull,
+                                 int64_t b0, int64_t b1, const pkdg_groups* G, const pkdg_list* pp, const pkdg_list* pc,
+                                 float eps, uint32_t flags, float* out, void* stream) {
+    pkdg_status s = check_common(ctx, P, C, Bfull, pp, pc, out);
     if (s != PKDG_OK) return s;
+    if (G && (G->n < 0 || (G->n > 0 && (!G->first_bucket || !G->n_buckets))))
+        return fail(ctx, PKDG_EINVAL, "groups->first_bucket / n_buckets is NULL or n < 0");
+    if (b0 < 0 || b1 < b0 || b1 > Bfull->n) return fail(ctx, PKDG_EINVAL, "bucket range outside [0, buckets->n]");
+    const pkdg_buckets Bsub = {Bfull->first ? Bfull->first + b0 : nullptr, Bfull->count ? Bfull->count + b0 : nullptr, b1 - b0};
+    const pkdg_buckets* B = &Bsub;
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const bool has_pp = pp && pp->offsets, has_pc = pc && pc->offsets && C && C->n > 0;
@@ -281,6 +314,8 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
     if (B->n == 0) return PKDG_OK;
     if ((s = ensure(ctx, &ctx->desc, &ctx->desc_cap, B->n)) != PKDG_OK) return s;
+    const int64_t fcap = fix_capacity(B->n, P->n);
+    if (!(flags & PKDG_NO_FIXUP) && (s = ensure(ctx, &ctx->fixq, &ctx->fixq_cap, fcap)) != PKDG_OK) return s;
     if (has_pc) {
         if ((s = ensure(ctx, &ctx->cellq, &ctx->cellq_cap, C->n * kCellQFloats)) != PKDG_OK) return s;
         if ((s = prep_cells(ctx, C, ctx->cellq, st)) != PKDG_OK) return s;
@@ -289,11 +324,22 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
         int threads = 256;
         int64_t blocks = (B->n + threads - 1) / threads;
         const bool leaves = has_pp && (flags & PKDG_PP_LEAVES);
-        if (leaves && (s = build_gfc(ctx, B->first, B->count, B->n, P->n, st)) != PKDG_OK) return s;
-        pkdg_pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(B->first, B->count, has_pp ? pp->offsets : nullptr,
-                                                             has_pc ? pc->offsets : nullptr, B->n, P->n, 0, 0,
-                                                             ctx->desc, ctx->stats, ctx->counters + kMaxSlots,
-                                                             leaves ? pp->idx : nullptr, ctx->gfc, B->n);
+        if (leaves && (s = build_gfc(ctx, Bfull->first, Bfull->count, Bfull->n, P->n, st)) != PKDG_OK) return s;
+        if (G) {   // buckets no group names get an empty descriptor
+            CK(cudaMemsetAsync(ctx->desc, 0, sizeof(BucketDesc) * (size_t)B->n, st));
+            const int64_t gblocks = (G->n + threads - 1) / threads;
+            pkdg_pack_groups_kernel<<<(unsigned)(gblocks < 1 ? 1 : gblocks), threads, 0, st>>>(
+                B->first, B->count, G->first_bucket, G->n_buckets, has_pp ? pp->offsets : nullptr,
+                has_pc ? pc->offsets : nullptr, G->n, B->n, P->n, 0, 0, 0, ctx->desc, ctx->stats,
+                ctx->counters + kMaxSlots, ctx->counters + 2 * kMaxSlots + 1, leaves ? pp->idx : nullptr, ctx->gfc,
+                Bfull->n);
+        } else {
+            pkdg_pack_kernel<<<(unsigned)blocks, threads, 0, st>>>(B->first, B->count, has_pp ? pp->offsets : nullptr,
+                                                                 has_pc ? pc->offsets : nullptr, B->n, P->n, 0, 0,
+                                                                 ctx->desc, ctx->stats, ctx->counters + kMaxSlots,
+                                                                 ctx->counters + 2 * kMaxSlots + 1,
+                                                                 leaves ? pp->idx : nullptr, ctx->gfc, Bfull->n);
+        }
         ctx->launches++;
         CK(cudaGetLastError());
     }
@@ -305,30 +351,77 @@ pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg
     p.work_counter = ctx->counters + kMaxSlots;
     p.n_buckets = B->n;
     p.gfc = ctx->gfc;
-    p.n_gbuckets = B->n;
+    p.n_gbuckets = Bfull->n;
+    p.cells_raw = has_pc ? C->rec : nullptr;
+    p.cells_stride = has_pc ? C->stride_floats : PKDG_CELL_FLOATS;
+    p.fix_queue = ctx->fixq;
+    p.fix_count = ctx->counters + 2 * kMaxSlots + 1;
+    p.fix_cap = (unsigned)(fcap > 0x7fffffffLL ? 0x7fffffffLL : fcap);
+    if ((flags & PKDG_VALIDATE) && (s = launch_validate(ctx, p, true, st)) != PKDG_OK) return s;
     const bool prof = ctx->profiling && ctx->prof_n < 256;
     if (prof) {
-        for (int i = 0; i < 2; ++i)
-            if (!ctx->prof_ev[2 * ctx->prof_n + i]) CK(cudaEventCreate(&ctx->prof_ev[2 * ctx->prof_n + i]));
-        CK(cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n], st));
+        for (int i = 0; i < 3; ++i)
+            if (!ctx->prof_ev[3 * ctx->prof_n + i]) CK(cudaEventCreate(&ctx->prof_ev[3 * ctx->prof_n + i]));
+        CK(cudaEventRecord(ctx->prof_ev[3 * ctx->prof_n], st));
     }
     s = launch_eval(ctx, p, st);
+    if (prof) CK(cudaEventRecord(ctx->prof_ev[3 * ctx->prof_n + 1], st));
+    if (s == PKDG_OK) s = launch_fixup(ctx, p, st);
     if (prof) {
-        CK(cudaEventRecord(ctx->prof_ev[2 * ctx->prof_n + 1], st));
+        CK(cudaEventRecord(ctx->prof_ev[3 * ctx->prof_n + 2], st));
         ctx->prof_n++;
     }
     return s;
 }
 
+pkdg_status pkdg_gravity_eval(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
+                              const pkdg_list* pp, const pkdg_list* pc, float eps, uint32_t flags, float* out,
+                              void* stream) {
+    return resident_impl(ctx, P, C, B, 0, B ? B->n : 0, nullptr, pp, pc, eps, flags, out, stream);
+}
+
+pkdg_status pkdg_gravity_eval_groups(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
+                                     const pkdg_groups* G, const pkdg_list* pp, const pkdg_list* pc, float eps,
+                                     uint32_t flags, float* out, void* stream) {
+    if (!G) return fail(ctx, PKDG_EINVAL, "groups must not be NULL");
+    return resident_impl(ctx, P, C, B, 0, B ? B->n : 0, G, pp, pc, eps, flags, out, stream);
+}
+
+pkdg_status pkdg_gravity_eval_range(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
+                                    int64_t b0, int64_t b1, const pkdg_list* pp, const pkdg_list* pc, float eps,
+                                    uint32_t flags, float* out, void* stream) {
+    return resident_impl(ctx, P, C, B, b0, b1, nullptr, pp, pc, eps, flags, out, stream);
+}
+
 // out_host != NULL: the rows of every chunk (buckets are then known to be contiguous runs in ascending
 // order, see pkdg_gravity_eval_host) are copied back on the chunk's stream right after its kernel, so
 // the device->host traffic overlaps the host->device traffic of later chunks (PCIe is full duplex).
+// Sinks are buckets [rb0, rb1) of Bfull (host arrays); the host lists hold rb1 - rb0 + 1 offsets.
+// Gh != NULL (group-shared lists, host arrays): the unit of chunking is the group, the lists have Gh->n + 1
+// offsets, the range must be all buckets and the groups must tile them in order.
 static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C,
-                                 const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
-                                 uint32_t flags, float* out, int32_t n_streams, int64_t max_entries,
-                                 void* stream, float* out_host) {
-    pkdg_status s = check_common(ctx, P, C, Bh, pph, pch, out);
+                                 const pkdg_buckets* Bfull, int64_t rb0, int64_t rb1, const pkdg_groups* Gh,
+                                 const pkdg_list* pph, const pkdg_list* pch, float eps, uint32_t flags, float* out,
+                                 int32_t n_streams, int64_t max_entries, void* stream, float* out_host) {
+    pkdg_status s = check_common(ctx, P, C, Bfull, pph, pch, out);
     if (s != PKDG_OK) return s;
+    if (Gh) {
+        if (Gh->n < 0 || (Gh->n > 0 && (!Gh->first_bucket || !Gh->n_buckets)))
+            return fail(ctx, PKDG_EINVAL, "groups->first_bucket / n_buckets is NULL or n < 0");
+        int64_t want = 0;
+        for (int64_t g = 0; g < Gh->n; ++g) {
+            if (Gh->first_bucket[g] != want || Gh->n_buckets[g] < 0)
+                return fail(ctx, PKDG_EINVAL, "groups must tile the bucket range in order");
+            want += Gh->n_buckets[g];
+        }
+        if (want != Bfull->n || rb0 != 0 || rb1 != Bfull->n)
+            return fail(ctx, PKDG_EINVAL, "groups must tile the bucket range in order");
+    }
+    if (rb0 < 0 || rb1 < rb0 || rb1 > Bfull->n) return fail(ctx, PKDG_EINVAL, "bucket range outside [0, buckets->n]");
+    const pkdg_buckets Bsub = {Bfull->first ? Bfull->first + rb0 : nullptr, Bfull->count ? Bfull->count + rb0 : nullptr,
+                               rb1 - rb0};
+    const pkdg_buckets* Bh = &Bsub;
+    const int64_t nb_all = Bfull->n;
     if (n_streams < 1 || n_streams > kMaxSlots) return fail(ctx, PKDG_EINVAL, "n_streams must be in 1..8");
     if (max_entries < 1) return fail(ctx, PKDG_EINVAL, "max_entries_per_chunk must be >= 1");
     cudaStream_t st = (cudaStream_t)stream;
@@ -338,6 +431,8 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     ctx->last_stream = st; ctx->last_buckets = nb; ctx->last_chunks = 0;
     CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
     if (nb == 0) return PKDG_OK;
+    const int64_t nu = Gh ? Gh->n : nb;   // units of chunking: groups or buckets
+    if (nu == 0) return PKDG_OK;
     if ((s = ensure_slots(ctx, n_streams)) != PKDG_OK) return s;
     if (has_pc) {
         if ((s = ensure(ctx, &ctx->cellq, &ctx->cellq_cap, C->n * kCellQFloats)) != PKDG_OK) return s;
@@ -345,16 +440,16 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     }
     const bool leaves = has_pp && (flags & PKDG_PP_LEAVES);
     if (leaves) {  // leaf references may point at any bucket: all (first, count) pairs go to the device first
-        if ((s = ensure(ctx, &ctx->g_first, &ctx->g_first_cap, nb)) != PKDG_OK) return s;
-        if ((s = ensure(ctx, &ctx->g_count, &ctx->g_count_cap, nb)) != PKDG_OK) return s;
-        CK(cudaMemcpyAsync(ctx->g_first, Bh->first, sizeof(int32_t) * nb, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(ctx->g_count, Bh->count, sizeof(int32_t) * nb, cudaMemcpyHostToDevice, st));
-        if ((s = build_gfc(ctx, ctx->g_first, ctx->g_count, nb, P->n, st)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->g_first, &ctx->g_first_cap, nb_all)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->g_count, &ctx->g_count_cap, nb_all)) != PKDG_OK) return s;
+        CK(cudaMemcpyAsync(ctx->g_first, Bfull->first, sizeof(int32_t) * nb_all, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->g_count, Bfull->count, sizeof(int32_t) * nb_all, cudaMemcpyHostToDevice, st));
+        if ((s = build_gfc(ctx, ctx->g_first, ctx->g_count, nb_all, P->n, st)) != PKDG_OK) return s;
     }
     CK(cudaEventRecord(ctx->ev_ready, st));
-    int64_t* bounds = (int64_t*)malloc(sizeof(int64_t) * (size_t)(nb + 1));
+    int64_t* bounds = (int64_t*)malloc(sizeof(int64_t) * (size_t)(nu + 1));
     if (!bounds) return fail(ctx, PKDG_ENOMEM, "host malloc of chunk bounds failed");
-    const int64_t nchunk = chunk_bounds_host(nb, has_pp ? pph->offsets : nullptr, has_pc ? pch->offsets : nullptr,
+    const int64_t nchunk = chunk_bounds_host(nu, has_pp ? pph->offsets : nullptr, has_pc ? pch->offsets : nullptr,
                                              max_entries, bounds);
     ctx->last_chunks = nchunk;
     pkdg_status rc = PKDG_OK;
@@ -364,42 +459,73 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     }
     for (int64_t ic = 0; ic < nchunk && rc == PKDG_OK; ++ic) {
         Slot& sl = ctx->slots[ic % n_streams];
-        const int64_t b0 = bounds[ic], b1 = bounds[ic + 1], cb = b1 - b0;
-        const int64_t pbase = has_pp ? pph->offsets[b0] : 0, plen = has_pp ? pph->offsets[b1] - pbase : 0;
-        const int64_t cbase = has_pc ? pch->offsets[b0] : 0, clen = has_pc ? pch->offsets[b1] - cbase : 0;
+        const int64_t u0 = bounds[ic], u1 = bounds[ic + 1], cu = u1 - u0;   // units, then their buckets
+        const int64_t b0 = Gh ? Gh->first_bucket[u0] : u0;
+        const int64_t b1 = Gh ? (int64_t)Gh->first_bucket[u1 - 1] + Gh->n_buckets[u1 - 1] : u1, cb = b1 - b0;
+        const int64_t pbase = has_pp ? pph->offsets[u0] : 0, plen = has_pp ? pph->offsets[u1] - pbase : 0;
+        const int64_t cbase = has_pc ? pch->offsets[u0] : 0, clen = has_pc ? pch->offsets[u1] - cbase : 0;
         // bounded in-flight work: a slot is reused only after its previous chunk is done
         if (sl.busy && cudaEventSynchronize(sl.done) != cudaSuccess) { rc = PKDG_ECUDA; break; }
         if ((rc = ensure(ctx, &sl.pp_idx, &sl.cap_pp, plen)) != PKDG_OK) break;
         if ((rc = ensure(ctx, &sl.pc_idx, &sl.cap_pc, clen)) != PKDG_OK) break;
+        int64_t chunk_sinks = 0;
+        for (int64_t b = b0; b < b1; ++b) chunk_sinks += Bh->count[b] > 0 ? Bh->count[b] : 0;
+        const int64_t fcap = fix_capacity(cb, chunk_sinks);
+        if (!(flags & PKDG_NO_FIXUP) && (rc = ensure(ctx, &sl.fixq, &sl.fixq_cap, fcap)) != PKDG_OK) break;
         if (cb + 1 > sl.cap_b) {
-            int64_t c1 = 0, c2 = 0, c3 = 0, c4 = 0, c5 = 0;
-            cudaFree(sl.first); cudaFree(sl.count); cudaFree(sl.pp_off); cudaFree(sl.pc_off); cudaFree(sl.desc);
-            sl.first = sl.count = nullptr; sl.pp_off = sl.pc_off = nullptr; sl.desc = nullptr; sl.cap_b = 0;
+            int64_t c1 = 0, c2 = 0, c5 = 0;
+            cudaFree(sl.first); cudaFree(sl.count); cudaFree(sl.desc);
+            sl.first = sl.count = nullptr; sl.desc = nullptr; sl.cap_b = 0;
             if ((rc = ensure(ctx, &sl.first, &c1, cb + 1)) != PKDG_OK) break;
             if ((rc = ensure(ctx, &sl.count, &c2, cb + 1)) != PKDG_OK) break;
-            if ((rc = ensure(ctx, &sl.pp_off, &c3, cb + 1)) != PKDG_OK) break;
-            if ((rc = ensure(ctx, &sl.pc_off, &c4, cb + 1)) != PKDG_OK) break;
             if ((rc = ensure(ctx, &sl.desc, &c5, cb + 1)) != PKDG_OK) break;
             sl.cap_b = c1;
         }
+        if (cu + 1 > sl.cap_off) {
+            int64_t c3 = 0, c4 = 0;
+            cudaFree(sl.pp_off); cudaFree(sl.pc_off);
+            sl.pp_off = sl.pc_off = nullptr; sl.cap_off = 0;
+            if ((rc = ensure(ctx, &sl.pp_off, &c3, cu + 1)) != PKDG_OK) break;
+            if ((rc = ensure(ctx, &sl.pc_off, &c4, cu + 1)) != PKDG_OK) break;
+            sl.cap_off = c3;
+        }
+        if (Gh && cu > sl.cap_g) {
+            int64_t c6 = 0, c7 = 0;
+            cudaFree(sl.gfirst); cudaFree(sl.gn);
+            sl.gfirst = sl.gn = nullptr; sl.cap_g = 0;
+            if ((rc = ensure(ctx, &sl.gfirst, &c6, cu)) != PKDG_OK) break;
+            if ((rc = ensure(ctx, &sl.gn, &c7, cu)) != PKDG_OK) break;
+            sl.cap_g = c6;
+        }
         cudaError_t e = cudaMemcpyAsync(sl.first, Bh->first + b0, sizeof(int32_t) * cb, cudaMemcpyHostToDevice, sl.st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(sl.count, Bh->count + b0, sizeof(int32_t) * cb, cudaMemcpyHostToDevice, sl.st);
+        if (e == cudaSuccess && Gh) {
+            e = cudaMemcpyAsync(sl.gfirst, Gh->first_bucket + u0, sizeof(int32_t) * cu, cudaMemcpyHostToDevice, sl.st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(sl.gn, Gh->n_buckets + u0, sizeof(int32_t) * cu, cudaMemcpyHostToDevice, sl.st);
+        }
         if (e == cudaSuccess && has_pp) {
-            e = cudaMemcpyAsync(sl.pp_off, pph->offsets + b0, sizeof(int64_t) * (cb + 1), cudaMemcpyHostToDevice, sl.st);
+            e = cudaMemcpyAsync(sl.pp_off, pph->offsets + u0, sizeof(int64_t) * (cu + 1), cudaMemcpyHostToDevice, sl.st);
             if (e == cudaSuccess && plen)
                 e = cudaMemcpyAsync(sl.pp_idx, pph->idx + pbase, sizeof(int32_t) * plen, cudaMemcpyHostToDevice, sl.st);
         }
         if (e == cudaSuccess && has_pc) {
-            e = cudaMemcpyAsync(sl.pc_off, pch->offsets + b0, sizeof(int64_t) * (cb + 1), cudaMemcpyHostToDevice, sl.st);
+            e = cudaMemcpyAsync(sl.pc_off, pch->offsets + u0, sizeof(int64_t) * (cu + 1), cudaMemcpyHostToDevice, sl.st);
             if (e == cudaSuccess && clen)
                 e = cudaMemcpyAsync(sl.pc_idx, pch->idx + cbase, sizeof(int32_t) * clen, cudaMemcpyHostToDevice, sl.st);
         }
         if (e != cudaSuccess) { rc = fail(ctx, PKDG_ECUDA, std::string("chunk copy: ") + cudaGetErrorString(e)); break; }
         unsigned int* counter = ctx->counters + (ic % n_streams);
         int threads = 256;
-        pkdg_pack_kernel<<<(unsigned)((cb + threads - 1) / threads), threads, 0, sl.st>>>(
-            sl.first, sl.count, has_pp ? sl.pp_off : nullptr, has_pc ? sl.pc_off : nullptr, cb, P->n, pbase, cbase,
-            sl.desc, ctx->stats, counter, leaves ? sl.pp_idx : nullptr, ctx->gfc, nb);
+        if (Gh) {
+            pkdg_pack_groups_kernel<<<(unsigned)((cu + threads - 1) / threads), threads, 0, sl.st>>>(
+                sl.first, sl.count, sl.gfirst, sl.gn, has_pp ? sl.pp_off : nullptr, has_pc ? sl.pc_off : nullptr, cu, cb,
+                P->n, pbase, cbase, b0, sl.desc, ctx->stats, counter, counter + kMaxSlots + 1,
+                leaves ? sl.pp_idx : nullptr, ctx->gfc, nb_all);
+        } else {
+            pkdg_pack_kernel<<<(unsigned)((cb + threads - 1) / threads), threads, 0, sl.st>>>(
+                sl.first, sl.count, has_pp ? sl.pp_off : nullptr, has_pc ? sl.pc_off : nullptr, cb, P->n, pbase, cbase,
+                sl.desc, ctx->stats, counter, counter + kMaxSlots + 1, leaves ? sl.pp_idx : nullptr, ctx->gfc, nb_all);
+        }
         ctx->launches++;
         EvalParams p;
         fill_params(p, ctx, P->xyzm, P->n, has_pc ? C->n : 0, eps, flags, out);
@@ -409,9 +535,16 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
         p.work_counter = counter;
         p.n_buckets = cb;
         p.gfc = ctx->gfc;
-        p.n_gbuckets = nb;
+        p.n_gbuckets = nb_all;
+        p.cells_raw = has_pc ? C->rec : nullptr;
+        p.cells_stride = has_pc ? C->stride_floats : PKDG_CELL_FLOATS;
+        p.fix_queue = sl.fixq;
+        p.fix_count = counter + kMaxSlots + 1;
+        p.fix_cap = (unsigned)(fcap > 0x7fffffffLL ? 0x7fffffffLL : fcap);
+        if ((flags & PKDG_VALIDATE) && (rc = launch_validate(ctx, p, ic == 0, sl.st)) != PKDG_OK) break;
         if ((rc = launch_eval(ctx, p, sl.st)) != PKDG_OK) break;
-        if (out_host) {
+        if ((rc = launch_fixup(ctx, p, sl.st)) != PKDG_OK) break;
+        if (out_host && cb > 0) {
             const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];
             if (r1 > r0 && cudaMemcpyAsync(out_host + 4 * r0, out + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
                                            cudaMemcpyDeviceToHost, sl.st) != cudaSuccess) { rc = PKDG_ECUDA; break; }
@@ -431,14 +564,19 @@ pkdg_status pkdg_gravity_eval_streamed(pkdg_ctx* ctx, const pkdg_particles* P, c
                                        const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
                                        uint32_t flags, float* out, int32_t n_streams, int64_t max_entries,
                                        void* stream) {
-    return streamed_impl(ctx, P, C, Bh, pph, pch, eps, flags, out, n_streams, max_entries, stream, nullptr);
+    return streamed_impl(ctx, P, C, Bh, 0, Bh ? Bh->n : 0, nullptr, pph, pch, eps, flags, out, n_streams, max_entries,
+                         stream, nullptr);
 }
 
-pkdg_status pkdg_gravity_eval_host(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch,
-                                   const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
-                                   uint32_t flags, float* out_host, int32_t n_streams, int64_t max_entries) {
-    pkdg_status s = check_common(ctx, Ph, Ch, Bh, pph, pch, out_host);
+static pkdg_status host_impl(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch, const pkdg_buckets* Bfull,
+                             int64_t rb0, int64_t rb1, const pkdg_groups* Gh, const pkdg_list* pph, const pkdg_list* pch,
+                             float eps, uint32_t flags, float* out_host, int32_t n_streams, int64_t max_entries) {
+    pkdg_status s = check_common(ctx, Ph, Ch, Bfull, pph, pch, out_host);
     if (s != PKDG_OK) return s;
+    if (rb0 < 0 || rb1 < rb0 || rb1 > Bfull->n) return fail(ctx, PKDG_EINVAL, "bucket range outside [0, buckets->n]");
+    const pkdg_buckets Bsub = {Bfull->first ? Bfull->first + rb0 : nullptr, Bfull->count ? Bfull->count + rb0 : nullptr,
+                               rb1 - rb0};
+    const pkdg_buckets* Bh = &Bsub;
     CK(cudaSetDevice(ctx->device));
     if (!ctx->own_stream) CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
     cudaStream_t st = ctx->own_stream;
@@ -452,27 +590,56 @@ pkdg_status pkdg_gravity_eval_host(pkdg_ctx* ctx, const pkdg_particles* Ph, cons
         CK(cudaMemcpyAsync(ctx->e2e_cells, Ch->rec, sizeof(float) * Ch->n * Ch->stride_floats, cudaMemcpyHostToDevice, st));
         Cd.rec = ctx->e2e_cells; Cd.n = Ch->n; Cd.stride_floats = Ch->stride_floats;
     }
-    if (flags & PKDG_ACCUMULATE) {
-        if (Ph->n) CK(cudaMemcpyAsync(ctx->e2e_out, out_host, sizeof(float) * 4 * Ph->n, cudaMemcpyHostToDevice, st));
-    } else if (Ph->n) {
-        CK(cudaMemsetAsync(ctx->e2e_out, 0, sizeof(float) * 4 * Ph->n, st));  // rows in no bucket come back as 0
+    // tree-ordered sinks (every bucket of the range starts where the previous one ends: the rows form one run):
+    // each chunk's rows go back as soon as they are done and nothing else is copied.  Anything else: the caller's
+    // rows make a round trip, so that rows in no listed bucket keep their values.
+    bool run = Bh->n > 0;
+    for (int64_t b = 0; run && b < Bh->n; ++b) {
+        const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
+        run = Bh->count[b] >= 0 && Bh->first[b] >= 0 && end <= Ph->n && (b + 1 == Bh->n || end == (int64_t)Bh->first[b + 1]);
+    }
+    if (Ph->n && (!run || (flags & PKDG_ACCUMULATE))) {
+        int64_t r0 = 0, r1 = Ph->n;
+        if (run) { r0 = Bh->first[0]; r1 = (int64_t)Bh->first[Bh->n - 1] + Bh->count[Bh->n - 1]; }
+        if (r1 > r0)
+            CK(cudaMemcpyAsync(ctx->e2e_out + 4 * r0, out_host + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
+                               cudaMemcpyHostToDevice, st));
     }
     pkdg_particles Pd = {ctx->e2e_xyzm, Ph->n};
-    // tree-ordered input (every bucket starts where the previous one ends, together they cover all rows):
-    // each chunk's rows go back as soon as they are done; anything else: one copy at the end
-    bool tiled = Bh->n > 0 && Bh->first[0] == 0;
-    for (int64_t b = 0; tiled && b < Bh->n; ++b) {
-        const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
-        tiled = Bh->count[b] >= 0 && end == (b + 1 < Bh->n ? (int64_t)Bh->first[b + 1] : Ph->n);
+    s = streamed_impl(ctx, &Pd, has_pc ? &Cd : nullptr, Bfull, rb0, rb1, Gh, pph, has_pc ? pch : nullptr, eps, flags,
+                      ctx->e2e_out, n_streams, max_entries, st, run ? out_host : nullptr);
+    if (s == PKDG_OK && !run && Ph->n) {
+        cudaError_t e = cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) s = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e));
     }
-    s = streamed_impl(ctx, &Pd, has_pc ? &Cd : nullptr, Bh, pph, has_pc ? pch : nullptr, eps, flags, ctx->e2e_out,
-                      n_streams, max_entries, st, tiled ? out_host : nullptr);
-    if (s != PKDG_OK) return s;
-    if (!tiled && Ph->n)
-        CK(cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    return PKDG_OK;
+    // also on the error path: no copy that touches the caller's host buffers may still be in flight on return
+    for (int i = 0; i < ctx->n_slots_live; ++i) cudaStreamSynchronize(ctx->slots[i].st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (s == PKDG_OK && e != cudaSuccess) s = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e));
+    return s;
 }
+
+pkdg_status pkdg_gravity_eval_host_range(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch,
+                                         const pkdg_buckets* Bfull, int64_t rb0, int64_t rb1, const pkdg_list* pph,
+                                         const pkdg_list* pch, float eps, uint32_t flags, float* out_host,
+                                         int32_t n_streams, int64_t max_entries) {
+    return host_impl(ctx, Ph, Ch, Bfull, rb0, rb1, nullptr, pph, pch, eps, flags, out_host, n_streams, max_entries);
+}
+
+pkdg_status pkdg_gravity_eval_host(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch,
+                                   const pkdg_buckets* Bh, const pkdg_list* pph, const pkdg_list* pch, float eps,
+                                   uint32_t flags, float* out_host, int32_t n_streams, int64_t max_entries) {
+    return host_impl(ctx, Ph, Ch, Bh, 0, Bh ? Bh->n : 0, nullptr, pph, pch, eps, flags, out_host, n_streams, max_entries);
+}
+
+pkdg_status pkdg_gravity_eval_host_groups(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch,
+                                          const pkdg_buckets* Bh, const pkdg_groups* Gh, const pkdg_list* pph,
+                                          const pkdg_list* pch, float eps, uint32_t flags, float* out_host,
+                                          int32_t n_streams, int64_t max_entries) {
+    if (!Gh) return fail(ctx, PKDG_EINVAL, "groups must not be NULL");
+    return host_impl(ctx, Ph, Ch, Bh, 0, Bh ? Bh->n : 0, Gh, pph, pch, eps, flags, out_host, n_streams, max_entries);
+}
+
 
 pkdg_status pkdg_pack_export(pkdg_ctx* ctx, int64_t n_buckets, const pkdg_list* list, int64_t* tile_offsets,
                              int32_t* tiles, int64_t tile_capacity, void* stream) {
@@ -531,8 +698,14 @@ pkdg_status pkdg_get_stats(pkdg_ctx* ctx, pkdg_stats* out) {
     out->tiles_pp = (int64_t)h.tiles_pp;
     out->tiles_pc = (int64_t)h.tiles_pc;
     out->bad_entries = (int64_t)h.bad_entries;
+    out->fixup_sinks = (int64_t)h.fixup_sinks;
+    out->invalid_values = (int64_t)h.invalid_values;
+    out->invalid_pairs = (int64_t)h.invalid_pairs;
     out->chunks = ctx->last_chunks;
-    return h.bad_entries ? fail(ctx, PKDG_EBADLIST, "validation found malformed buckets or list entries") : PKDG_OK;
+    if (h.bad_entries) return fail(ctx, PKDG_EBADLIST, "validation found malformed buckets or list entries");
+    if (h.invalid_values || h.invalid_pairs)
+        return fail(ctx, PKDG_EBADVALUE, "PKDG_VALIDATE: values outside the documented range, or a sink inside a listed cell's b_max");
+    return PKDG_OK;
 }
 
 pkdg_status pkdg_profile_enable(pkdg_ctx* ctx, int32_t on) {
@@ -541,20 +714,34 @@ pkdg_status pkdg_profile_enable(pkdg_ctx* ctx, int32_t on) {
     return PKDG_OK;
 }
 
-pkdg_status pkdg_profile_read(pkdg_ctx* ctx, int64_t* n, double* ms_total) {
+pkdg_status pkdg_profile_read(pkdg_ctx* ctx, int64_t* n, double* ms_total, double* fixup_ms_total) {
     if (!ctx || !n || !ms_total) return PKDG_EINVAL;
     CK(cudaSetDevice(ctx->device));
-    double tot = 0;
+    double tot = 0, fix = 0;
     for (int i = 0; i < ctx->prof_n; ++i) {
         float ms = 0;
-        CK(cudaEventSynchronize(ctx->prof_ev[2 * i + 1]));
-        CK(cudaEventElapsedTime(&ms, ctx->prof_ev[2 * i], ctx->prof_ev[2 * i + 1]));
+        CK(cudaEventSynchronize(ctx->prof_ev[3 * i + 2]));
+        CK(cudaEventElapsedTime(&ms, ctx->prof_ev[3 * i], ctx->prof_ev[3 * i + 1]));
         tot += ms;
+        CK(cudaEventElapsedTime(&ms, ctx->prof_ev[3 * i + 1], ctx->prof_ev[3 * i + 2]));
+        fix += ms;
     }
     *n = ctx->prof_n;
     *ms_total = tot;
+    if (fixup_ms_total) *fixup_ms_total = fix;
     ctx->prof_n = 0;
     return PKDG_OK;
+}
+
+pkdg_status pkdg_set_option(pkdg_ctx* ctx, int32_t option, double value) {
+    if (!ctx) return PKDG_EINVAL;
+    switch (option) {
+        case PKDG_OPT_KAPPA2:
+            if (!(value > 0.0) || value > 1.0e15) return fail(ctx, PKDG_EINVAL, "PKDG_OPT_KAPPA2 must be > 0");
+            ctx->kappa2 = (float)value;
+            return PKDG_OK;
+        default: return fail(ctx, PKDG_EINVAL, "unknown option");
+    }
 }
 
 int64_t pkdg_launch_count(const pkdg_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -566,6 +753,7 @@ const char* pkdg_status_string(pkdg_status s) {
         case PKDG_ECUDA: return "PKDG_ECUDA: CUDA runtime error";
         case PKDG_ENOMEM: return "PKDG_ENOMEM: out of memory";
         case PKDG_EBADLIST: return "PKDG_EBADLIST: malformed buckets or lists";
+        case PKDG_EBADVALUE: return "PKDG_EBADVALUE: values or geometry outside the documented range";
         default: return "unknown pkdg_status";
     }
 }
@@ -577,65 +765,27 @@ void pkdg_version(int32_t* major, int32_t* minor) {
     if (minor) *minor = PKDG_VERSION_MINOR;
 }
 
-pkdg_status pkdg_fma_probe(pkdg_ctx* ctx, int32_t mode, int64_t iters, float* ms_host, double* flops_host) {
+pkdg_status pkdg_fma_peak_probe(pkdg_ctx* ctx, int64_t iters, float* ms_host, double* flops_host) {
     if (!ctx || !ms_host || !flops_host || iters < 1) return PKDG_EINVAL;
-    if (mode < 0 || mode > 5) return fail(ctx, PKDG_EINVAL, "probe mode must be in 0..5");
     CK(cudaSetDevice(ctx->device));
-    const int threads = mode == 0 ? 256 : 128, blocks = ctx->num_sms * (mode == 0 ? 8 : 4);
-    float *buf = nullptr, *in = nullptr;
-    CK(cudaMalloc((void**)&buf, sizeof(float4) * threads * blocks));
-    // input: 1024 operands around 0.5; 32 synthetic cell records (COM, M, s, small moments); 2 sinks
-    float h[2048];
-    for (int i = 0; i < 1024; ++i) h[i] = 0.5f + 0.001f * (float)(i % 97);
-    float* hc = h + 1024;
-    for (int i = 0; i < 32 * 32; ++i) hc[i] = 0.01f * (float)(i % 13) - 0.03f;
-    for (int l = 0; l < 32; ++l) {
-        hc[l * 32 + 0] = 0.1f * l; hc[l * 32 + 1] = 0.2f; hc[l * 32 + 2] = 0.3f; hc[l * 32 + 3] = 1.0f;
-        hc[l * 32 + 4] = 0.05f;
-    }
-    const float tgt[8] = {5.f, 6.f, 7.f, 0.f, -5.f, 6.f, -7.f, 0.f};
-    CK(cudaMalloc((void**)&in, sizeof(h) + sizeof(tgt)));
-    CK(cudaMemcpy(in, h, sizeof(h), cudaMemcpyHostToDevice));
-    CK(cudaMemcpy(in + 2048, tgt, sizeof(tgt), cudaMemcpyHostToDevice));
-    const float4* cells = reinterpret_cast<const float4*>(in + 1024);
-    const float4* tg = reinterpret_cast<const float4*>(in + 2048);
-    auto launch = [&](int64_t n) {
-        switch (mode) {
-            case 0: pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, n, 0.999f, 0.001f); break;
-            case 1: pkdg_rf_probe_kernel<1><<<blocks, threads>>>(in, buf, n); break;
-            case 2: pkdg_rf_probe_kernel<2><<<blocks, threads>>>(in, buf, n); break;
-            case 3: pkdg_rf_probe_kernel<3><<<blocks, threads>>>(in, buf, n); break;
-            case 4: pkdg_pc_probe_kernel<false><<<blocks, threads>>>(cells, tg, reinterpret_cast<float4*>(buf), n); break;
-            default: pkdg_pc_probe_kernel<true><<<blocks, threads>>>(cells, tg, reinterpret_cast<float4*>(buf), n); break;
-        }
-    };
-    if (mode >= 4) iters = (iters + 1) & ~(int64_t)1;
+    const int threads = 256, blocks = ctx->num_sms * 8;
+    float* buf = nullptr;
+    CK(cudaMalloc((void**)&buf, sizeof(float) * threads * blocks));
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    launch(16);  // warm-up
+    pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, 16, 0.999f, 0.001f);  // warm-up
     CK(cudaEventRecord(e0, 0));
-    launch(iters);
+    pkdg_fma_probe_kernel<<<blocks, threads>>>(buf, iters, 0.999f, 0.001f);
     CK(cudaEventRecord(e1, 0));
     CK(cudaEventSynchronize(e1));
     ctx->launches += 2;
     CK(cudaGetLastError());
     CK(cudaEventElapsedTime(ms_host, e0, e1));
-    const double lanes = (double)threads * blocks;
-    switch (mode) {
-        case 0: case 1: *flops_host = 2.0 * 64.0 * (double)iters * lanes; break;  // 64 FFMA per trip
-        case 2: case 3: *flops_host = 4.0 * 64.0 * (double)iters * lanes; break;  // 64 FFMA2 per trip
-        case 4: *flops_host = 2.0 * 196.0 * (double)iters * lanes; break;         // 2 sinks per trip
-        default: *flops_host = 2.0 * 187.0 * (double)iters * lanes; break;        // 1 sink pair per trip
-    }
+    *flops_host = 2.0 * 64.0 * (double)iters * (double)threads * blocks;  // 64 FFMA per trip and thread
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     CK(cudaFree(buf));
-    CK(cudaFree(in));
     return PKDG_OK;
-}
-
-pkdg_status pkdg_fma_peak_probe(pkdg_ctx* ctx, int64_t iters, float* ms_host, double* flops_host) {
-    return pkdg_fma_probe(ctx, PKDG_PROBE_FFMA_CONST, iters, ms_host, flops_host);
 }
 
 }  // extern "C"

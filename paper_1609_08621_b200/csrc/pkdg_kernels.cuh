@@ -8,8 +8,9 @@
 //   pkdg_eval3_kernel        a2-a5, library default: one warp per bucket, lanes stride the source
 //                            lists, packed FP32x2 arithmetic over sink pairs, cp.async staging of
 //                            cell records and of the next bucket, butterfly transpose-reduction
-//   pkdg_eval_kernel         generation 1 of the same mapping (scalar FFMA, L1 prefetch): variant 1
-//   pkdg_*_probe_kernel      operand-pattern probes (roofline denominator, register-file study)
+//                            + per-sink conditioning estimate; ill-conditioned sinks are queued
+//   pkdg_fixup_kernel        queued sinks re-evaluated with fp64 terms and fp64 accumulators
+//   pkdg_fma_probe_kernel    FFMA-only probe (roofline denominator check)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -25,7 +26,8 @@ struct __align__(16) BucketDesc {
 };
 
 struct DevStats {
-    unsigned long long interactions_pp, interactions_pc, tiles_pp, tiles_pc, bad_entries;
+    unsigned long long interactions_pp, interactions_pc, tiles_pp, tiles_pc, bad_entries, fixup_sinks;
+    unsigned long long invalid_values, invalid_pairs;  // PKDG_VALIDATE
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -68,7 +70,8 @@ __global__ void __launch_bounds__(kPrepThreads) pkdg_prep_cells_kernel(const flo
     }
 }
 
-__device__ __forceinline__ void prep_one_cell(const float* __restrict__ r, float* __restrict__ o) {
+// fp64 core: q[0..31] in the layout above (shared by the fp32 record writer and the fp64 fix-up kernel)
+__device__ __forceinline__ void prep_cell_f64(const float* __restrict__ r, double* __restrict__ o) {
     double M = r[3];
     const float* m2 = r + 4;
     const float* m3 = r + 10;
@@ -99,18 +102,25 @@ __device__ __forceinline__ void prep_one_cell(const float* __restrict__ r, float
         k4 = 4 * 4.375 / (M * s * s * s * s);
     }
     o[0] = r[0]; o[1] = r[1]; o[2] = r[2]; o[3] = r[3];
-    o[4] = (float)s;
-    o[5] = (float)(k2 * q2[0]); o[6] = (float)(k2 * q2[1]); o[7] = (float)(k2 * q2[2]);
-    o[8] = (float)(k2 * q2[3]); o[9] = (float)(k2 * q2[4]);
-    o[10] = (float)(k3 * q3[0]); o[11] = (float)(k3 * q3[1]); o[12] = (float)(k3 * q3[2]);
-    o[13] = (float)(k3 * q3[3]); o[14] = (float)(k3 * q3[4]); o[15] = (float)(k3 * q3[6]);
-    o[16] = (float)(k3 * q3[7]);
-    o[17] = (float)(k4 * q4[0]); o[18] = (float)(k4 * q4[1]); o[19] = (float)(k4 * q4[2]);
-    o[20] = (float)(k4 * q4[3]); o[21] = (float)(k4 * q4[4]); o[22] = (float)(k4 * q4[6]);
-    o[23] = (float)(k4 * q4[7]); o[24] = (float)(k4 * q4[10]); o[25] = (float)(k4 * q4[11]);
-    o[26] = (float)(k2 * q2[5]);
-    o[27] = (float)(k3 * q3[5]); o[28] = (float)(k3 * q3[8]); o[29] = (float)(k3 * q3[9]);
-    o[30] = (float)(k4 * q4[5]); o[31] = (float)(k4 * q4[12]);
+    o[4] = s;
+    o[5] = k2 * q2[0]; o[6] = k2 * q2[1]; o[7] = k2 * q2[2];
+    o[8] = k2 * q2[3]; o[9] = k2 * q2[4];
+    o[10] = k3 * q3[0]; o[11] = k3 * q3[1]; o[12] = k3 * q3[2];
+    o[13] = k3 * q3[3]; o[14] = k3 * q3[4]; o[15] = k3 * q3[6];
+    o[16] = k3 * q3[7];
+    o[17] = k4 * q4[0]; o[18] = k4 * q4[1]; o[19] = k4 * q4[2];
+    o[20] = k4 * q4[3]; o[21] = k4 * q4[4]; o[22] = k4 * q4[6];
+    o[23] = k4 * q4[7]; o[24] = k4 * q4[10]; o[25] = k4 * q4[11];
+    o[26] = k2 * q2[5];
+    o[27] = k3 * q3[5]; o[28] = k3 * q3[8]; o[29] = k3 * q3[9];
+    o[30] = k4 * q4[5]; o[31] = k4 * q4[12];
+}
+
+__device__ __forceinline__ void prep_one_cell(const float* __restrict__ r, float* __restrict__ o) {
+    double q[kCellQFloats];
+    prep_cell_f64(r, q);
+#pragma unroll
+    for (int i = 0; i < kCellQFloats; ++i) o[i] = (float)q[i];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -130,11 +140,12 @@ __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_
                                  const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
                                  int64_t n_buckets, int64_t n_particles, int64_t pp_base, int64_t pc_base,
                                  BucketDesc* __restrict__ desc, DevStats* __restrict__ stats,
-                                 unsigned int* __restrict__ work_counter, const int32_t* __restrict__ leaf_idx,
+                                 unsigned int* __restrict__ work_counter, unsigned int* __restrict__ fix_count,
+                                 const int32_t* __restrict__ leaf_idx,
                                  const int2* __restrict__ gfc, int64_t n_g) {
     int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long ipp = 0, ipc = 0, tpp = 0, tpc = 0, bad = 0;
-    if (b == 0) *work_counter = 0u;
+    if (b == 0) { *work_counter = 0u; *fix_count = 0u; }
     if (b < n_buckets) {
         BucketDesc d;
         d.first = first[b];
@@ -165,6 +176,72 @@ __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_
             tpp = (unsigned long long)((lp + 1) >> 1);
         }
         tpc = (unsigned long long)((lc + 31) >> 5);
+    }
+    ipp = warp_sum_u64(ipp); ipc = warp_sum_u64(ipc); tpp = warp_sum_u64(tpp); tpc = warp_sum_u64(tpc);
+    bad = warp_sum_u64(bad);
+    if ((threadIdx.x & 31) == 0) {
+        if (ipp) atomicAdd(&stats->interactions_pp, ipp);
+        if (ipc) atomicAdd(&stats->interactions_pc, ipc);
+        if (tpp) atomicAdd(&stats->tiles_pp, tpp);
+        if (tpc) atomicAdd(&stats->tiles_pc, tpc);
+        if (bad) atomicAdd(&stats->bad_entries, bad);
+    }
+}
+
+// Group-shared lists (the walk stops at groups of up to 64 particles =
+// 4 buckets and resolves the checklist into ONE P-P and ONE P-C list per group).  One thread per group: the
+// work descriptor of every bucket of the group points at the group's lists.  Groups must tile the bucket range
+// in order; anything else is a bad entry and leaves the affected buckets without work.
+__global__ void pkdg_pack_groups_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ count,
+                                        const int32_t* __restrict__ g_first, const int32_t* __restrict__ g_n,
+                                        const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
+                                        int64_t n_groups, int64_t n_buckets, int64_t n_particles, int64_t pp_base,
+                                        int64_t pc_base, int64_t bucket_base, BucketDesc* __restrict__ desc,
+                                        DevStats* __restrict__ stats, unsigned int* __restrict__ work_counter,
+                                        unsigned int* __restrict__ fix_count, const int32_t* __restrict__ leaf_idx,
+                                        const int2* __restrict__ gfc, int64_t n_g) {
+    int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long ipp = 0, ipc = 0, tpp = 0, tpc = 0, bad = 0;
+    if (g == 0) { *work_counter = 0u; *fix_count = 0u; }
+    if (g < n_groups) {
+        int64_t b0 = (int64_t)g_first[g] - bucket_base, nb = g_n[g];
+        const int64_t want = g == 0 ? 0 : (int64_t)g_first[g - 1] - bucket_base + g_n[g - 1];
+        if (nb < 0 || b0 != want || b0 + nb > n_buckets || (g == n_groups - 1 && b0 + nb != n_buckets)) {
+            bad++;
+            if (b0 < 0 || nb < 0 || b0 + nb > n_buckets) nb = 0;
+        }
+        int64_t p0 = pp_off ? pp_off[g] : 0, p1 = pp_off ? pp_off[g + 1] : 0;
+        int64_t c0 = pc_off ? pc_off[g] : 0, c1 = pc_off ? pc_off[g + 1] : 0;
+        int64_t lp = p1 - p0, lc = c1 - c0;
+        if (lp < 0 || lp > 0x7fffffffLL) { bad++; lp = 0; }
+        if (lc < 0 || lc > 0x7fffffffLL) { bad++; lc = 0; }
+        unsigned long long np = (unsigned long long)lp;
+        unsigned long long tp = (unsigned long long)((lp + 31) >> 5);
+        if (leaf_idx) {
+            np = 0;
+            for (int64_t e = 0; e < lp; ++e) {
+                const int32_t r = leaf_idx[p0 - pp_base + e];
+                if (r < 0) continue;  // padding
+                if (r >= n_g) { bad++; continue; }
+                const int2 fc = gfc[r];
+                if (fc.y > 16 || fc.y < 0) { bad++; continue; }
+                np += (unsigned long long)fc.y;
+            }
+            tp = (unsigned long long)((lp + 1) >> 1);
+        }
+        for (int64_t b = b0; b < b0 + nb; ++b) {
+            BucketDesc d;
+            d.first = first[b];
+            d.count = count[b];
+            if (d.count < 0 || d.first < 0 || (int64_t)d.first + d.count > n_particles) { bad++; d.count = 0; }
+            d.pp_len = (int32_t)lp; d.pc_len = (int32_t)lc;
+            d.pp_begin = p0 - pp_base; d.pc_begin = c0 - pc_base;
+            desc[b] = d;
+            ipp += (unsigned long long)d.count * np;
+            ipc += (unsigned long long)d.count * (unsigned long long)lc;
+            tpp += tp;
+            tpc += (unsigned long long)((lc + 31) >> 5);
+        }
     }
     ipp = warp_sum_u64(ipp); ipc = warp_sum_u64(ipc); tpp = warp_sum_u64(tpp); tpc = warp_sum_u64(tpc);
     bad = warp_sum_u64(bad);
@@ -278,25 +355,46 @@ struct EvalParams {
     float h2;     // (2 eps)^2
     float h2c;    // clamp of r^2 in the Newtonian fast path: max(h2, 1e-24)
     float hinv;   // 1/h, 0 if eps == 0
+    float eps;
     uint32_t flags;
+    // conditioning estimate and fix-up queue
+    const float* cells_raw;   // canonical records (fix-up kernel)
+    int32_t cells_stride;
+    float fix_k;              // a sink is queued iff S2 > fix_k |a|^2; < 0: never, 0: always
+    int4* fix_queue;          // {bucket, t0 | wide << 31, lane ballot, 0}
+    unsigned int* fix_count;
+    unsigned int fix_cap;
 };
 
-// Softened pair factors for r^2 < h^2 (cubic spline of support h, u = r/h): a -= m d g, phi += m w.
-__device__ __noinline__ void pp_soft_factors(float r2, float hinv, float& g, float& w) {
-    float u = sqrtf(r2) * hinv;
-    float u2 = u * u;
-    if (u < 0.5f) {
-        g = fmaf(u2, fmaf(32.0f, u, -38.4f), 10.666666667f);
-        w = fmaf(u2, fmaf(u2, fmaf(6.4f, u, -9.6f), 5.3333333333f), -2.8f);
+// Cubic-spline pair factors (Monaghan-Lattanzio density of support h; u = r / h < 1): a -= m d g / h^3,
+// phi += m w / h.  fp64: between u = 1/2 and 1 the polynomial cancels from terms of size 48 to a result of
+// size 1, which fp32 cannot do to 1e-7.  Used by the rare softened-pair correction of the evaluation kernel
+// and by the fix-up kernel.
+__device__ __forceinline__ void spline_gw_f64(double u, double& g, double& w) {
+    const double u2 = u * u;
+    if (u < 0.5) {
+        g = 32.0 / 3.0 + u2 * (-38.4 + 32.0 * u);
+        w = -2.8 + u2 * (16.0 / 3.0 + u2 * (-9.6 + 6.4 * u));
     } else {
-        float iu = 1.0f / u;
-        float iu3 = iu * iu * iu;
-        g = fmaf(u, fmaf(u, fmaf(-10.666666667f, u, 38.4f), -48.0f), 21.333333333f) - 0.066666666667f * iu3;
-        w = fmaf(u2, fmaf(u, fmaf(u, fmaf(-2.1333333333f, u, 9.6f), -16.0f), 10.666666667f), -3.2f) +
-            0.066666666667f * iu;
+        const double iu = 1.0 / u;
+        g = 64.0 / 3.0 + u * (-48.0 + u * (38.4 - (32.0 / 3.0) * u)) - iu * iu * iu / 15.0;
+        w = -3.2 + iu / 15.0 + u2 * (32.0 / 3.0 + u * (-16.0 + u * (9.6 - (32.0 / 15.0) * u)));
     }
-    g *= hinv * hinv * hinv;
-    w *= hinv;
+}
+
+// Correction of one softened pair: what has to be ADDED to the clamped Newtonian pair the fast path booked
+// (g_c = ri_c^3, w_c = -ri_c with ri_c = MUFU.RSQ(h^2)) to get the spline pair; d = x_sink - x_source.
+__device__ __noinline__ float2 pp_soft_correction(float dx, float dy, float dz, float eps, float ric) {
+    const double h = 2.0 * (double)eps, hi = 1.0 / h;
+    const double r2 = (double)dx * dx + (double)dy * dy + (double)dz * dz;
+    double g = 0.0, w = 0.0;   // eps == 0 and coincident: undefined, contributes nothing
+    if (r2 < h * h) {
+        spline_gw_f64(sqrt(r2) * hi, g, w);
+        g *= hi * hi * hi;
+        w *= hi;
+    }
+    const double rc = (double)ric;
+    return make_float2((float)(g - rc * rc * rc), (float)(w + rc));
 }
 
 // MUFU.RSQ without the denormal pre-/post-scaling rsqrtf() emits (inputs here are never denormal).
@@ -306,30 +404,6 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
     return y;
 }
 
-// Newtonian fast path of one P-P interaction with r^2 clamped from below at h2c (so it is finite
-// for softened and coincident pairs; those are corrected afterwards, see pp_phase).  With SELF the
-// accumulation is masked for the sink's own index (used only for tiles that hold own particles).
-// 3 sub | 1 mul 2 fma | max, min | rsqrt | 3 mul | 3 fma 1 sub  = 19 flops (FMA = 2, rsqrt = 1, min/max 0)
-template <bool SELF>
-__device__ __forceinline__ void pp_fast(const float4 t, const float4 s, bool self, float h2c, float& minr2,
-                                        float4& a) {
-    float dx = t.x - s.x, dy = t.y - s.y, dz = t.z - s.z;
-    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    float ri = rsqrt_approx(fmaxf(r2, h2c));
-    float ri2 = ri * ri;
-    float m = s.w;
-    if (SELF) {
-        m = self ? 0.0f : m;
-        r2 = self ? 3.0e38f : r2;
-    }
-    minr2 = fminf(minr2, r2);
-    float mri = m * ri;
-    float mg = mri * ri2;
-    a.x = fmaf(-mg, dx, a.x);
-    a.y = fmaf(-mg, dy, a.y);
-    a.z = fmaf(-mg, dz, a.z);
-    a.w -= mri;
-}
 
 // A cell held in registers by one lane (35 values; COM/M/s + 6 + 10 + 15 normalised components).
 struct CellRegs {
@@ -356,67 +430,6 @@ __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const 
     c.zzzz = -(c.xxzz + c.yyzz);
 }
 
-// One P-C interaction (formulas above pkdg_prep_cells_kernel); flop audit in DESIGN.md.  Split in two
-// so that the evaluation loop can software-pipeline it: pc_pre (sink load, displacement, rsqrt: a
-// serial chain of long-latency steps) for the NEXT sinks is issued under pc_body of the current ones.
-struct PcPre { float dx, dy, dz, ri; };
-
-template <bool NEWTON>
-__device__ __forceinline__ PcPre pc_pre(const float4 t, const CellRegs& c) {
-    PcPre q;
-    q.dx = t.x - c.cx; q.dy = t.y - c.cy; q.dz = t.z - c.cz;
-    float r2 = fmaf(q.dz, q.dz, fmaf(q.dy, q.dy, q.dx * q.dx));
-    float ri = rsqrt_approx(r2);
-    if (NEWTON) {  // one Newton step on MUFU.RSQ (2^-22.9): the result enters as ri^2 .. ri^3
-        float hy = 0.5f * r2 * ri;
-        ri = ri * fmaf(-hy, ri, 1.5f);
-    }
-    q.ri = ri;
-    return q;
-}
-
-__device__ __forceinline__ void pc_body(const PcPre q, const CellRegs& c, float4& a) {
-    const float dx = q.dx, dy = q.dy, dz = q.dz, ri = q.ri;
-    float ri2 = ri * ri;
-    float sr = c.s * ri2;
-    float x = dx * sr, y = dy * sr, z = dz * sr;  // tau
-    // order 2
-    float v2x = fmaf(c.xz, z, fmaf(c.xy, y, c.xx * x));
-    float v2y = fmaf(c.yz, z, fmaf(c.yy, y, c.xy * x));
-    float v2z = fmaf(c.zz, z, fmaf(c.yz, y, c.xz * x));
-    float e2 = fmaf(v2z, z, fmaf(v2y, y, v2x * x));
-    // order 3: quadratic monomials, cross terms carry their multiplicity 2
-    float xx = x * x, yy = y * y, zz = z * z;
-    float x2 = x + x, y2 = y + y;
-    float xy = x2 * y, xz = x2 * z, yz = y2 * z;
-    float v3x = fmaf(c.xyz, yz, fmaf(c.xxz, xz, fmaf(c.xxy, xy, fmaf(c.xzz, zz, fmaf(c.xyy, yy, c.xxx * xx)))));
-    float v3y = fmaf(c.yyz, yz, fmaf(c.xyz, xz, fmaf(c.xyy, xy, fmaf(c.yzz, zz, fmaf(c.yyy, yy, c.xxy * xx)))));
-    float v3z = fmaf(c.yzz, yz, fmaf(c.xzz, xz, fmaf(c.xyz, xy, fmaf(c.zzz, zz, fmaf(c.yyz, yy, c.xxz * xx)))));
-    float e3 = fmaf(v3z, z, fmaf(v3y, y, v3x * x));
-    // order 4: cubic monomials with multiplicities 1, 3, 6
-    float x3 = 3.0f * x, y3 = 3.0f * y, z3 = 3.0f * z;
-    float mxxx = xx * x, myyy = yy * y, mzzz = zz * z;
-    float mxxy = xx * y3, mxxz = xx * z3, mxyy = yy * x3, myyz = yy * z3, mxzz = zz * x3, myzz = zz * y3;
-    float mxyz = xy * z3;
-    float v4x = fmaf(c.xzzz, mzzz, fmaf(c.xyzz, myzz, fmaf(c.xyyz, myyz, fmaf(c.xyyy, myyy, fmaf(c.xxzz, mxzz,
-                fmaf(c.xxyz, mxyz, fmaf(c.xxyy, mxyy, fmaf(c.xxxz, mxxz, fmaf(c.xxxy, mxxy, c.xxxx * mxxx)))))))));
-    float v4y = fmaf(c.yzzz, mzzz, fmaf(c.yyzz, myzz, fmaf(c.yyyz, myyz, fmaf(c.yyyy, myyy, fmaf(c.xyzz, mxzz,
-                fmaf(c.xyyz, mxyz, fmaf(c.xyyy, mxyy, fmaf(c.xxyz, mxxz, fmaf(c.xxyy, mxxy, c.xxxy * mxxx)))))))));
-    float v4z = fmaf(c.zzzz, mzzz, fmaf(c.yzzz, myzz, fmaf(c.yyzz, myyz, fmaf(c.yyyz, myyy, fmaf(c.xzzz, mxzz,
-                fmaf(c.xyzz, mxyz, fmaf(c.xyyz, mxyy, fmaf(c.xxzz, mxxz, fmaf(c.xxyz, mxxy, c.xxxz * mxxx)))))))));
-    float e4 = fmaf(v4z, z, fmaf(v4y, y, v4x * x));
-    // combine
-    float fs = fmaf(0.25f, e4, fmaf(0.33333333333f, e3, fmaf(0.5f, e2, 1.0f)));   // potential series
-    float S = fmaf(2.25f, e4, fmaf(2.3333333333f, e3, fmaf(2.5f, e2, 1.0f)));     // radial part of the force
-    float gx = v2x + v3x + v4x, gy = v2y + v3y + v4y, gz = v2z + v3z + v4z;
-    float mr = c.M * ri;
-    float k3 = mr * ri2;
-    float sk = c.s * k3, Sk = S * k3;
-    a.w = fmaf(-mr, fs, a.w);
-    a.x = fmaf(sk, gx, fmaf(-Sk, dx, a.x));
-    a.y = fmaf(sk, gy, fmaf(-Sk, dy, a.y));
-    a.z = fmaf(sk, gz, fmaf(-Sk, dz, a.z));
-}
 
 // Butterfly transpose-reduction of NV per-lane partial sums across the 32 lanes: log2(32) rounds, in
 // the round with partner lane^mask each lane hands over the half of its values the partner keeps.
@@ -441,191 +454,6 @@ __device__ __forceinline__ void warp_transpose_reduce(float (&v)[NV], int lane) 
     }
 }
 
-// a3 for one pass: NS sink slots (8 or 16), register accumulators, result stored to (or added into)
-// the per-lane shared accumulators.  Returns with s_acc[t][lane] holding the lane's P-P partials.
-template <int NS>
-__device__ __forceinline__ void pp_phase(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
-                                         const float4* __restrict__ s_tgt, float4* __restrict__ s_acc, int lane,
-                                         unsigned& bad) {
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    float4 acc[NS];
-#pragma unroll
-    for (int t = 0; t < NS; ++t) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
-    const int ntile = (pp_len + 31) >> 5;
-    const int sink0 = d.first + t0;
-    int32_t j = ntile ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 0, lane) : -1;
-    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
-    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
-    int32_t jn = ntile > 1 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 1, lane) : -1;
-    for (int k = 0; k < ntile; ++k) {
-        // the source of the next tile and the index of the one after are in flight during this tile
-        if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
-        const float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
-        const int32_t jnn = (k + 2 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 2, lane) : -1;
-        const int self_t = j - sink0;  // sink slot this source coincides with, if any
-        float minr2 = 3.0e38f;
-        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)NS)) {  // tile holds own particles
-#pragma unroll
-            for (int t = 0; t < NS; ++t) pp_fast<true>(s_tgt[t], s, self_t == t, p.h2c, minr2, acc[t]);
-        } else {
-#pragma unroll
-            for (int t = 0; t < NS; ++t) pp_fast<false>(s_tgt[t], s, false, p.h2c, minr2, acc[t]);
-        }
-        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
-            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
-            // Newtonian contribution by the spline one, through the shared accumulators.
-            if (!smem_live) {
-                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-                smem_live = true;
-            }
-            if (minr2 < p.h2c) {
-                for (int t = 0; t < ntp; ++t) {
-                    const float4 tg = s_tgt[t];
-                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
-                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    if (r2 < p.h2c && self_t != t) {
-                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
-                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
-                        float ri = rsqrt_approx(p.h2c);  // what pp_fast used for this pair
-                        float gc = ri * ri * ri, wc = -ri;
-                        float4 a = s_acc[t * 32 + lane];
-                        float mg = s.w * (g - gc);
-                        a.x = fmaf(-mg, dx, a.x); a.y = fmaf(-mg, dy, a.y); a.z = fmaf(-mg, dz, a.z);
-                        a.w = fmaf(s.w, w - wc, a.w);
-                        s_acc[t * 32 + lane] = a;
-                    }
-                }
-            }
-        }
-        s = sn; j = jn; jn = jnn;
-    }
-    if (smem_live) {
-#pragma unroll
-        for (int t = 0; t < NS; ++t) {
-            float4 a = s_acc[t * 32 + lane];
-            a.x += acc[t].x; a.y += acc[t].y; a.z += acc[t].z; a.w += acc[t].w;
-            s_acc[t * 32 + lane] = a;
-        }
-    } else {
-#pragma unroll
-        for (int t = 0; t < NS; ++t) s_acc[t * 32 + lane] = acc[t];
-    }
-}
-
-template <int WARPS, int MINB, bool NEWTON, int UNR>
-__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval_kernel(const EvalParams p) {
-    __shared__ float4 s_acc_all[WARPS][(kTMax + 1) * 32];  // [sink slot][lane]; slot 16 = scratch
-    __shared__ float4 s_tgt_all[WARPS][kTMax + 2];
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    float4* s_acc = s_acc_all[warp];
-    float4* s_tgt = s_tgt_all[warp];
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);  // pads sink slots; never meets a source
-    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
-    unsigned bad = 0;
-
-    for (;;) {
-        unsigned bu = 0;
-        if (lane == 0) bu = atomicAdd(p.work_counter, 1u);
-        bu = __shfl_sync(0xffffffffu, bu, 0);
-        if ((int64_t)bu >= p.n_buckets) break;
-        const BucketDesc d = p.desc[bu];
-        const int pp_len = do_pp ? d.pp_len : 0, pc_len = do_pc ? d.pc_len : 0;
-
-        for (int t0 = 0; t0 < d.count; t0 += kTMax) {
-            const int ntp = min(kTMax, d.count - t0);
-            // ---- a2: stage the sinks of this pass (slots >= ntp hold a far-away dummy)
-            __syncwarp();
-            if (lane < kTMax + 2) s_tgt[lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
-            __syncwarp();
-
-            // ---- a3: P-P
-            if (ntp <= 8) pp_phase<8>(p, d, pp_len, t0, ntp, s_tgt, s_acc, lane, bad);
-            else pp_phase<16>(p, d, pp_len, t0, ntp, s_tgt, s_acc, lane, bad);
-
-            // ---- a4: P-C.  Two sinks per iteration; the lane's cell stays in registers for the tile.
-            {
-                const int ntile = (pc_len + 31) >> 5;
-                const int nte = (ntp + 1) & ~1;  // odd count: the last iteration also visits the dummy slot
-                int32_t c = ntile ? tile_entry(p.pc_idx, d.pc_begin, pc_len, 0, lane) : -1;
-                int32_t c1 = ntile > 1 ? tile_entry(p.pc_idx, d.pc_begin, pc_len, 1, lane) : -1;
-                for (int k = 0; k < ntile; ++k) {
-                    if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
-                    // next tile's record -> L1 while this tile is evaluated; index two tiles ahead in flight
-                    if ((uint32_t)c1 < (uint64_t)p.n_cells)
-                        asm volatile("prefetch.global.L1 [%0];" ::"l"(p.cellq + (int64_t)c1 * 8));
-                    const int32_t c2 = (k + 2 < ntile) ? tile_entry(p.pc_idx, d.pc_begin, pc_len, k + 2, lane) : -1;
-                    CellRegs cr;
-                    if (c >= 0) {
-                        const float4* q = p.cellq + (int64_t)c * 8;
-                        cell_unpack(cr, __ldg(q), __ldg(q + 1), __ldg(q + 2), __ldg(q + 3), __ldg(q + 4),
-                                    __ldg(q + 5), __ldg(q + 6), __ldg(q + 7));
-                    } else {
-                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
-                    }
-                    if (UNR == 2) {
-                        PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr), pB = pc_pre<NEWTON>(s_tgt[1], cr);
-#pragma unroll 1
-                        for (int t = 0; t < nte; t += 2) {
-                            const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 2], cr), nB = pc_pre<NEWTON>(s_tgt[t + 3], cr);
-                            float4 aA = s_acc[t * 32 + lane], aB = s_acc[(t + 1) * 32 + lane];
-                            pc_body(pA, cr, aA);
-                            pc_body(pB, cr, aB);
-                            s_acc[t * 32 + lane] = aA;
-                            s_acc[(t + 1) * 32 + lane] = aB;
-                            pA = nA; pB = nB;
-                        }
-                    } else {
-                        PcPre pA = pc_pre<NEWTON>(s_tgt[0], cr);
-#pragma unroll 1
-                        for (int t = 0; t < ntp; ++t) {
-                            const PcPre nA = pc_pre<NEWTON>(s_tgt[t + 1], cr);
-                            float4 aA = s_acc[t * 32 + lane];
-                            pc_body(pA, cr, aA);
-                            s_acc[t * 32 + lane] = aA;
-                            pA = nA;
-                        }
-                    }
-                    c = c1; c1 = c2;
-                }
-            }
-            // ---- a5: cross-lane reduction and write-back
-            float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
-            if (ntp <= 8) {
-                float v[32];
-#pragma unroll
-                for (int t = 0; t < 8; ++t) {
-                    const float4 a = s_acc[t * 32 + lane];
-                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
-                }
-                warp_transpose_reduce<32>(v, lane);
-                if ((lane >> 2) < ntp) {
-                    float r = v[0];
-                    if (accumulate) r += outf[lane];
-                    outf[lane] = r;
-                }
-            } else {
-                float v[64];
-#pragma unroll
-                for (int t = 0; t < 16; ++t) {
-                    const float4 a = s_acc[t * 32 + lane];
-                    v[4 * t] = a.x; v[4 * t + 1] = a.y; v[4 * t + 2] = a.z; v[4 * t + 3] = a.w;
-                }
-                warp_transpose_reduce<64>(v, lane);
-                if ((lane >> 1) < ntp) {
-                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
-                    float2 r = make_float2(v[0], v[1]);
-                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
-                    *o2 = r;
-                }
-            }
-        }
-    }
-    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
-}
 
 // ------------------------------------------------------------------------------------------------
 // Asynchronous staging helpers (cp.async = LDGSTS): global -> shared memory without registers.
@@ -669,8 +497,33 @@ __device__ __forceinline__ float2 f2fma(float2 a, float2 b, float2 c) { return _
 
 constexpr int kPMax = kTMax / 2;  // sink pairs per pass
 
+// The same butterfly for NV = 8 or 16 values: log2(NV) transposing rounds, then plain rounds.  Lane l ends with
+// the total of value l >> 2 (NV = 8) or l >> 1 (NV = 16) in v[0].
+template <int NV>
+__device__ __forceinline__ void warp_transpose_reduce_small(float (&v)[NV], int lane) {
+    static_assert(NV == 8 || NV == 16, "NV");
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+        const int mask = 16 >> r, n = (NV / 2) >> r;
+        if (n >= 1) {
+            const bool up = (lane & mask) != 0;
+#pragma unroll
+            for (int i = 0; i < NV / 2; ++i) {
+                if (i < n) {
+                    const float send = up ? v[i] : v[i + n];
+                    const float keep = up ? v[i + n] : v[i];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
+                }
+            }
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], mask);
+        }
+    }
+}
+
 struct __align__(16) WarpSmem3 {
     float4 acc[kTMax * 32];       // [pair][half][lane]: {axA, axB, ayA, ayB}, {azA, azB, phiA, phiB}
+    float2 s2[kPMax * 32];        // [pair][lane]: conditioning estimate {S2_A, S2_B}
     float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
     float4 tgt[2][kTMax];         // raw sinks (x, y, z, m) of the current / the next bucket
     float4 tp[(kPMax + 1) * 2];   // current pass, pair layout: {xA, xB, yA, yB}, {zA, zB, -, -}; +1 dummy pair
@@ -683,17 +536,20 @@ __device__ __forceinline__ int acc_idx(int t, int comp, int lane) {  // comp 0..
     return (((t >> 1) * 2 + (comp >> 1)) * 32 + lane) * 4 + (comp & 1) * 2 + (t & 1);
 }
 
-// One source against one sink pair, Newtonian with r^2 clamped from below at h2c (see pp_fast).
-// 13 packed FP instructions + 2 MUFU + min/max for 2 interactions; flops as pp_fast (19 each).
+// One source against one sink pair, Newtonian with r^2 clamped from below at h2c (so it is finite for
+// softened and coincident pairs; those are corrected afterwards, see pp_phase3).  With SELF the
+// accumulation is masked for the sink's own index (used only for tiles that hold own particles).
+// 14 packed FP instructions + 2 MUFU + min/max for 2 interactions: 19 flops per interaction for a and
+// phi + 2 for the conditioning estimate S2 (not counted as useful work).
 template <bool SELF>
 __device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, const float4 s, bool selfA, bool selfB,
-                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw) {
+                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw,
+                                         float2& s2) {
     const float2 dx = f2add(make_float2(txy.x, txy.y), sp(-s.x));
     const float2 dy = f2add(make_float2(txy.z, txy.w), sp(-s.y));
     const float2 dz = f2add(make_float2(tz.x, tz.y), sp(-s.z));
     float2 r2 = f2fma(dz, dz, f2fma(dy, dy, f2mul(dx, dx)));
     const float2 ri = make_float2(rsqrt_approx(fmaxf(r2.x, h2c)), rsqrt_approx(fmaxf(r2.y, h2c)));
-    const float2 ri2 = f2mul(ri, ri);
     float2 nm = sp(-s.w);
     if (SELF) {
         nm.x = selfA ? 0.0f : nm.x; nm.y = selfB ? 0.0f : nm.y;
@@ -701,28 +557,24 @@ __device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, cons
     }
     minr2 = fminf(minr2, fminf(r2.x, r2.y));
     const float2 nmri = f2mul(nm, ri);
-    const float2 nmg = f2mul(nmri, ri2);
+    const float2 t = f2mul(nmri, ri);   // -m / r^2 = -|a_ij|
+    const float2 nmg = f2mul(t, ri);
     ax = f2fma(nmg, dx, ax);
     ay = f2fma(nmg, dy, ay);
     az = f2fma(nmg, dz, az);
     aw = f2add(aw, nmri);
+    s2 = f2fma(t, t, s2);               // conditioning estimate S2_i = sum_j |a_ij|^2
 }
 
 struct PcPre2 { float2 dx, dy, dz, ri; };
 
-template <bool NEWTON>
 __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, const CellRegs& c) {
     PcPre2 q;
     q.dx = f2add(make_float2(txy.x, txy.y), sp(-c.cx));
     q.dy = f2add(make_float2(txy.z, txy.w), sp(-c.cy));
     q.dz = f2add(make_float2(tz.x, tz.y), sp(-c.cz));
     const float2 r2 = f2fma(q.dz, q.dz, f2fma(q.dy, q.dy, f2mul(q.dx, q.dx)));
-    float2 ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
-    if (NEWTON) {  // one Newton step on MUFU.RSQ: ri <- ri (1.5 - 0.5 r2 ri^2)
-        const float2 hy = f2mul(f2mul(sp(-0.5f), r2), ri);
-        ri = f2mul(ri, f2fma(hy, ri, sp(1.5f)));
-    }
-    q.ri = ri;
+    q.ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
     return q;
 }
 
@@ -734,10 +586,11 @@ __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, con
 //   1 + sum (2n+1)/n e_n   = fs + 2 E4                     (radial factor S)
 // which needs no chain-start multiplies and no V2 + V3 + V4 sums, and the data dependence keeps the three
 // FFMA2 of a term (same monomial, x / y / z coefficient) adjacent, so the monomial pair is reused.
-// Per interaction: 5 FADD, 35 FMUL, 73 FFMA, 1 MUFU = 187 flops in 113 packed instructions per pair.
+// Per interaction: 5 FADD, 35 FMUL, 73 FFMA, 1 MUFU = 187 flops in 113 packed instructions per pair
+// (+ 1 FMUL2 + 1 FFMA2 for the conditioning estimate S2, not counted as useful work).
 #define PKDG_T0(CX, CY, CZ, M) vx = f2mul(sp(CX), M); vy = f2mul(sp(CY), M); vz = f2mul(sp(CZ), M);
 #define PKDG_T1(CX, CY, CZ, M) vx = f2fma(sp(CX), M, vx); vy = f2fma(sp(CY), M, vy); vz = f2fma(sp(CZ), M, vz);
-__device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1) {
+__device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1, float2& s2) {
     const float2 ri2 = f2mul(q.ri, q.ri);
     const float2 sr = f2mul(sp(c.s), ri2);
     const float2 x = f2mul(q.dx, sr), y = f2mul(q.dy, sr), z = f2mul(q.dz, sr);  // tau
@@ -762,7 +615,9 @@ __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, floa
     const float2 fs = f2fma(sp(0.25f), E4, f2fma(sp(0.083333333333f), E3, f2fma(sp(0.16666666667f), E2, sp(1.0f))));
     const float2 S = f2fma(sp(2.0f), E4, fs);
     const float2 mr = f2mul(sp(c.M), q.ri);
-    const float2 k3 = f2mul(mr, ri2);
+    const float2 t = f2mul(mr, q.ri);   // M / r^2: the size of this cell's contribution
+    const float2 k3 = f2mul(t, q.ri);
+    s2 = f2fma(t, t, s2);
     const float2 sk = f2mul(sp(c.s), k3), Sk = f2mul(S, k3);
     float2 ax = make_float2(a0.x, a0.y), ay = make_float2(a0.z, a0.w), az = make_float2(a1.x, a1.y),
            aw = make_float2(a1.z, a1.w);
@@ -834,9 +689,9 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
     const float4* __restrict__ tp = S.tp;
     float4* __restrict__ s_acc = S.acc;
     float* __restrict__ s_accf = reinterpret_cast<float*>(S.acc);
-    float2 ax[NP], ay[NP], az[NP], aw[NP];
+    float2 ax[NP], ay[NP], az[NP], aw[NP], s2[NP];
 #pragma unroll
-    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = make_float2(0.f, 0.f);
+    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = s2[q] = make_float2(0.f, 0.f);
     bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
     const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
     const int sink0 = d.first + t0;
@@ -887,17 +742,19 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
 #pragma unroll
             for (int q = 0; q < NP; ++q)
                 pp_fast2<true>(tp[2 * q], tp[2 * q + 1], s, self_t == 2 * q, self_t == 2 * q + 1, p.h2c, minr2, ax[q],
-                               ay[q], az[q], aw[q]);
+                               ay[q], az[q], aw[q], s2[q]);
         } else {
 #pragma unroll
             for (int q = 0; q < NP; ++q)
-                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q]);
+                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q],
+                                s2[q]);
         }
         if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
             // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
             // Newtonian contribution by the spline one, through the shared accumulators.
             if (!smem_live) {
                 for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int q = 0; q < kPMax; ++q) S.s2[q * 32 + lane] = make_float2(0.f, 0.f);
                 smem_live = true;
             }
             if (minr2 < p.h2c) {
@@ -906,15 +763,17 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
                     float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
                     float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                     if (r2 < p.h2c && self_t != t) {
-                        float g = 0.f, w = 0.f;  // eps == 0 and coincident: undefined, contributes nothing
-                        if (r2 < p.h2) pp_soft_factors(r2, p.hinv, g, w);
-                        float ri = rsqrt_approx(p.h2c);  // what pp_fast2 used for this pair
-                        float gc = ri * ri * ri, wc = -ri;
-                        float mg = s.w * (g - gc);
+                        const float ri = rsqrt_approx(p.h2c);  // what pp_fast2 used for this pair
+                        const float2 dgw = pp_soft_correction(dx, dy, dz, p.eps, ri);
+                        const float mg = s.w * dgw.x, dw = dgw.y;
                         s_accf[acc_idx(t, 0, lane)] = fmaf(-mg, dx, s_accf[acc_idx(t, 0, lane)]);
                         s_accf[acc_idx(t, 1, lane)] = fmaf(-mg, dy, s_accf[acc_idx(t, 1, lane)]);
                         s_accf[acc_idx(t, 2, lane)] = fmaf(-mg, dz, s_accf[acc_idx(t, 2, lane)]);
-                        s_accf[acc_idx(t, 3, lane)] = fmaf(s.w, w - wc, s_accf[acc_idx(t, 3, lane)]);
+                        s_accf[acc_idx(t, 3, lane)] = fmaf(s.w, dw, s_accf[acc_idx(t, 3, lane)]);
+                        // the fast path booked (m / h^2)^2 for this pair; a softened pair pulls with up to 2.6 m / h^2
+                        // and the correction is a difference of two terms: book (4 m / h^2)^2 in all
+                        const float tc = s.w * ri * ri;
+                        reinterpret_cast<float*>(S.s2)[((t >> 1) * 32 + lane) * 2 + (t & 1)] += 15.0f * tc * tc;
                     }
                 }
             }
@@ -924,17 +783,34 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         float4 a0 = make_float4(ax[q].x, ax[q].y, ay[q].x, ay[q].y), a1 = make_float4(az[q].x, az[q].y, aw[q].x, aw[q].y);
+        float2 c2 = s2[q];
         if (smem_live) {
             const float4 b0 = s_acc[(2 * q) * 32 + lane], b1 = s_acc[(2 * q + 1) * 32 + lane];
+            const float2 d2 = S.s2[q * 32 + lane];
             a0.x += b0.x; a0.y += b0.y; a0.z += b0.z; a0.w += b0.w;
             a1.x += b1.x; a1.y += b1.y; a1.z += b1.z; a1.w += b1.w;
+            c2.x += d2.x; c2.y += d2.y;
         }
         s_acc[(2 * q) * 32 + lane] = a0;
         s_acc[(2 * q + 1) * 32 + lane] = a1;
+        S.s2[q * 32 + lane] = c2;
     }
 }
 
-template <int WARPS, int MINB, bool NEWTON>
+// Queue one (bucket, pass) for the fp64 fix-up kernel (warp-uniform call).  Returns false if the queue is full
+// (cannot happen with the capacity the host sizes it to for non-overlapping buckets): the caller then writes
+// the fp32 result instead of dropping the rows.
+__device__ __forceinline__ bool fix_push(const EvalParams& p, int bucket, int t0w, unsigned ballot, int lane) {
+    unsigned k = 0;
+    if (lane == 0) {
+        k = atomicAdd(p.fix_count, 1u);
+        if (k < p.fix_cap) p.fix_queue[k] = make_int4(bucket, t0w, (int)ballot, 0);
+    }
+    k = __shfl_sync(0xffffffffu, k, 0);
+    return k < p.fix_cap;
+}
+
+template <int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const EvalParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -955,7 +831,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
     fill_direct3(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
 
     for (;;) {
-        unsigned nxt = 0xffffffffu;
+        unsigned nxt = 0xffffffffu, next_b = 0xffffffffu;
         if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
         bool has_next = false;
         const ListLens L = eff_lens(d, do_pp, do_pc);
@@ -993,6 +869,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
             // ---- next bucket, stage 1: its descriptor
             if (last) {
                 const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
+                next_b = nb;
                 has_next = (int64_t)nb < p.n_buckets;
                 if (has_next && lane < 2)
                     cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
@@ -1043,22 +920,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     cp_async_commit();
                     // software pipeline, two pairs per trip so that no register copies are needed: the
                     // displacement / rsqrt of the next pair is issued under the body of the current one
-                    PcPre2 pA = pc_pre2<NEWTON>(tp[2 * q0], tp[2 * q0 + 1], cr);
+                    PcPre2 pA = pc_pre2(tp[2 * q0], tp[2 * q0 + 1], cr);
 #pragma unroll 1
                     for (int q = q0; q < q1; q += 2) {
-                        const PcPre2 pB = pc_pre2<NEWTON>(tp[2 * q + 2], tp[2 * q + 3], cr);
+                        const PcPre2 pB = pc_pre2(tp[2 * q + 2], tp[2 * q + 3], cr);
                         {
                             float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                            pc_body2(pA, cr, a0, a1);
+                            float2 c2 = S.s2[q * 32 + lane];
+                            pc_body2(pA, cr, a0, a1, c2);
                             s_acc[(2 * q) * 32 + lane] = a0;
                             s_acc[(2 * q + 1) * 32 + lane] = a1;
+                            S.s2[q * 32 + lane] = c2;
                         }
                         if (q + 1 < q1) {
-                            pA = pc_pre2<NEWTON>(tp[2 * q + 4], tp[2 * q + 5], cr);
+                            pA = pc_pre2(tp[2 * q + 4], tp[2 * q + 5], cr);
                             float4 a0 = s_acc[(2 * q + 2) * 32 + lane], a1 = s_acc[(2 * q + 3) * 32 + lane];
-                            pc_body2(pB, cr, a0, a1);
+                            float2 c2 = S.s2[(q + 1) * 32 + lane];
+                            pc_body2(pB, cr, a0, a1, c2);
                             s_acc[(2 * q + 2) * 32 + lane] = a0;
                             s_acc[(2 * q + 3) * 32 + lane] = a1;
+                            S.s2[(q + 1) * 32 + lane] = c2;
                         }
                     }
                     c = cn; cn = c2;
@@ -1070,35 +951,60 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     cp_async_commit();
                 }
             }
-            // ---- a5: cross-lane reduction and write-back
+            // ---- a5: cross-lane reduction, conditioning test and write-back.  A sink whose sum cancels so far that
+            // fp32 terms cannot give the tolerance (S2_i > fix_k |a_i|^2) is not
+            // written here: its (bucket, pass) is queued and pkdg_fixup_kernel evaluates it with fp64 terms.
             float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
+            const bool fix_on = p.fix_k >= 0.0f;
             if (ntp <= 8) {
-                float v[32];
+                float v[32], w[8];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
+                    const float2 c2 = S.s2[q * 32 + lane];
                     v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
+                    w[2 * q] = c2.x; w[2 * q + 1] = c2.y;
                 }
-                warp_transpose_reduce<32>(v, lane);
-                if ((lane >> 2) < ntp) {
-                    float r = v[0];
-                    if (accumulate) r += outf[lane];
-                    outf[lane] = r;
+                warp_transpose_reduce<32>(v, lane);       // lane l: component l & 3 of sink l >> 2
+                warp_transpose_reduce_small<8>(w, lane);  // lane l: S2 of sink l >> 2
+                const float r = v[0];
+                float sq = (lane & 3) < 3 ? r * r : 0.0f;
+                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
+                sq += __shfl_xor_sync(0xffffffffu, sq, 2);
+                const bool valid = (lane >> 2) < ntp;
+                bool flag = fix_on && valid && w[0] >= p.fix_k * sq;
+                const unsigned ballot = __ballot_sync(0xffffffffu, flag);
+                if (ballot) {   // warp-uniform; every lane takes part in the push
+                    const bool queued = fix_push(p, (int)cur, t0, ballot, lane);
+                    flag = flag && queued;
                 }
+                if (valid && !flag) outf[lane] = accumulate ? r + outf[lane] : r;
             } else {
-                float v[64];
+                float v[64], w[16];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
+                    const float2 c2 = S.s2[q * 32 + lane];
                     v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
+                    w[2 * q] = c2.x; w[2 * q + 1] = c2.y;
                 }
-                warp_transpose_reduce<64>(v, lane);
-                if ((lane >> 1) < ntp) {
+                warp_transpose_reduce<64>(v, lane);        // lane l: components 2 (l & 1), 2 (l & 1) + 1 of sink l >> 1
+                warp_transpose_reduce_small<16>(w, lane);  // lane l: S2 of sink l >> 1
+                float sq = (lane & 1) ? v[0] * v[0] : fmaf(v[0], v[0], v[1] * v[1]);
+                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
+                const bool valid = (lane >> 1) < ntp;
+                bool flag = fix_on && valid && w[0] >= p.fix_k * sq;
+                const unsigned ballot = __ballot_sync(0xffffffffu, flag);
+                if (ballot) {
+                    const bool queued = fix_push(p, (int)cur, (int)((unsigned)t0 | 0x80000000u), ballot, lane);
+                    flag = flag && queued;
+                }
+                if (valid && !flag) {
                     float2* o2 = reinterpret_cast<float2*>(outf) + lane;
                     float2 r = make_float2(v[0], v[1]);
-                    if (accumulate) { float2 old = *o2; r.x += old.x; r.y += old.y; }
+                    if (accumulate) { const float2 old = *o2; r.x += old.x; r.y += old.y; }
                     *o2 = r;
                 }
             }
@@ -1107,20 +1013,189 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
         cp_async_wait_all();
         __syncwarp();
         d = S.ndesc;
+        cur = next_b;
         buf ^= 1;
     }
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
 
 // ------------------------------------------------------------------------------------------------
-// Probes (pkdg_fma_probe): what the FP32 pipe delivers for a given operand pattern.  Registers only, no
-// memory in the timed loop; 4 CTAs of 128 threads per SM.  Results in DESIGN.md sec 6.
-//   0  FFMA with two constant-bank operands (one register read per FMA): the FMA-pipe peak
-//   1  FFMA, three distinct register operands
-//   2  FFMA2 (packed), three distinct register pairs
-//   3  FFMA2, scalar x pair + pair with the pair operand shared by three consecutive instructions
-//   4  the scalar P-C body of generation 1 (pc_pre + pc_body), two sinks per trip
-//   5  the packed P-C body (pc_pre2 + pc_body2), one sink pair per trip
+// fp64 fix-up ("accumulated in double precision").  The
+// evaluation kernel queues every (bucket, pass) that holds a sink whose sum a_i = sum_j a_ij cancels so
+// far that fp32 TERMS cannot deliver the tolerance; here one warp takes one queue entry and evaluates its
+// flagged sinks over the same lists with fp64 terms and fp64 accumulators (the FP64 pipe of the B200,
+// idle otherwise), lanes striding the sources, and writes their rows.  The arithmetic is the same
+// algebra as the fp32 path (spline pair; normalised trace-free series), from the CANONICAL records.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum_f64(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void pp_pair_f64(const double xi, const double yi, const double zi, const float4 s,
+                                            const double h, double (&a)[4]) {
+    const double dx = xi - (double)s.x, dy = yi - (double)s.y, dz = zi - (double)s.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double m = (double)s.w;
+    if (r2 >= h * h) {
+        if (r2 < 1.0e-24) return;  // eps == 0 and (nearly) coincident: contributes nothing (include/pkdg.h)
+        const double ir = 1.0 / sqrt(r2);
+        const double g = m * ir * ir * ir;
+        a[0] -= g * dx; a[1] -= g * dy; a[2] -= g * dz; a[3] -= m * ir;
+    } else {
+        const double hi = 1.0 / h;
+        double g, w;
+        spline_gw_f64(sqrt(r2) * hi, g, w);
+        g *= m * hi * hi * hi;
+        a[0] -= g * dx; a[1] -= g * dy; a[2] -= g * dz; a[3] += m * w * hi;
+    }
+}
+
+// One cell (canonical record) against one sink in fp64: formulas above pkdg_prep_cells_kernel, plain form.
+__device__ __noinline__ void pc_pair_f64(const double xi, const double yi, const double zi, const float* __restrict__ rec,
+                                         double (&a)[4]) {
+    double q[kCellQFloats];
+    prep_cell_f64(rec, q);
+    const double dx = xi - q[0], dy = yi - q[1], dz = zi - q[2], M = q[3], sc = q[4];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double ri = 1.0 / sqrt(r2), ri2 = ri * ri, sr = sc * ri2;
+    const double x = dx * sr, y = dy * sr, z = dz * sr;
+    const double qxx = q[5], qxy = q[6], qxz = q[7], qyy = q[8], qyz = q[9], qzz = q[26];
+    const double v2x = qxx * x + qxy * y + qxz * z, v2y = qxy * x + qyy * y + qyz * z, v2z = qxz * x + qyz * y + qzz * z;
+    const double e2 = v2x * x + v2y * y + v2z * z;
+    const double xxx = q[10], xxy = q[11], xxz = q[12], xyy = q[13], xyz = q[14], yyy = q[15], yyz = q[16];
+    const double xzz = q[27], yzz = q[28], zzz = q[29];
+    const double mxx = x * x, myy = y * y, mzz = z * z, mxy = 2 * x * y, mxz = 2 * x * z, myz = 2 * y * z;
+    const double v3x = xxx * mxx + xyy * myy + xzz * mzz + xxy * mxy + xxz * mxz + xyz * myz;
+    const double v3y = xxy * mxx + yyy * myy + yzz * mzz + xyy * mxy + xyz * mxz + yyz * myz;
+    const double v3z = xxz * mxx + yyz * myy + zzz * mzz + xyz * mxy + xzz * mxz + yzz * myz;
+    const double e3 = v3x * x + v3y * y + v3z * z;
+    const double xxxx = q[17], xxxy = q[18], xxxz = q[19], xxyy = q[20], xxyz = q[21], xyyy = q[22], xyyz = q[23];
+    const double yyyy = q[24], yyyz = q[25], xxzz = q[30], yyzz = q[31];
+    const double xyzz = -(xxxy + xyyy), xzzz = -(xxxz + xyyz), yzzz = -(xxyz + yyyz), zzzz = -(xxzz + yyzz);
+    const double c0 = mxx * x, c1 = myy * y, c2 = mzz * z, c3 = 3 * mxx * y, c4 = 3 * mxx * z, c5 = 3 * myy * x;
+    const double c6 = 3 * myy * z, c7 = 3 * mzz * x, c8 = 3 * mzz * y, c9 = 6 * x * y * z;
+    const double v4x = xxxx * c0 + xxxy * c3 + xxxz * c4 + xxyy * c5 + xxyz * c9 + xxzz * c7 + xyyy * c1 + xyyz * c6 + xyzz * c8 + xzzz * c2;
+    const double v4y = xxxy * c0 + xxyy * c3 + xxyz * c4 + xyyy * c5 + xyyz * c9 + xyzz * c7 + yyyy * c1 + yyyz * c6 + yyzz * c8 + yzzz * c2;
+    const double v4z = xxxz * c0 + xxyz * c3 + xxzz * c4 + xyyz * c5 + xyzz * c9 + xzzz * c7 + yyyz * c1 + yyzz * c6 + yzzz * c8 + zzzz * c2;
+    const double e4 = v4x * x + v4y * y + v4z * z;
+    const double fs = 1.0 + e2 / 2.0 + e3 / 3.0 + e4 / 4.0;
+    const double Sr = 1.0 + 2.5 * e2 + (7.0 / 3.0) * e3 + 2.25 * e4;
+    const double mr = M * ri, k3 = mr * ri2;
+    a[3] -= mr * fs;
+    a[0] += k3 * (sc * (v2x + v3x + v4x) - Sr * dx);
+    a[1] += k3 * (sc * (v2y + v3y + v4y) - Sr * dy);
+    a[2] += k3 * (sc * (v2z + v3z + v4z) - Sr * dz);
+}
+
+__global__ void __launch_bounds__(128) pkdg_fixup_kernel(const EvalParams p) {
+    const int lane = threadIdx.x & 31;
+    const unsigned gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const unsigned n = min(*p.fix_count, p.fix_cap);
+    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
+    const bool pp_leaves = (p.flags & 0x8u) != 0;
+    const double h = 2.0 * (double)p.eps;
+    for (unsigned e = gw; e < n; e += nw) {
+        const int4 ent = p.fix_queue[e];
+        const BucketDesc d = p.desc[ent.x];
+        const bool wide = ((unsigned)ent.y & 0x80000000u) != 0;
+        const int t0 = (int)((unsigned)ent.y & 0x7fffffffu);
+        const ListLens L = eff_lens(d, do_pp, do_pc);
+        unsigned lanes = (unsigned)ent.z;  // ballot of the flagged lanes of the evaluation kernel's reduction
+        const unsigned keep = wide ? 0x55555555u : 0x11111111u;   // one lane per sink: 2 t (wide) or 4 t
+        lanes &= keep;
+        if (lane == 0) atomicAdd(&p.stats->fixup_sinks, (unsigned long long)__popc(lanes));
+        while (lanes) {
+            const int bit = __ffs(lanes) - 1;
+            lanes &= lanes - 1;
+            const int i = d.first + t0 + (wide ? bit >> 1 : bit >> 2);
+            const float4 xi4 = __ldg(p.xyzm + i);
+            const double xi = xi4.x, yi = xi4.y, zi = xi4.z;
+            double a[4] = {0.0, 0.0, 0.0, 0.0};
+            if (pp_leaves) {
+                for (int r = 0; r < L.pp; ++r) {
+                    const int32_t g = __ldg(p.pp_idx + d.pp_begin + r);
+                    if ((uint32_t)g >= (uint64_t)p.n_gbuckets) continue;
+                    const int2 fc = __ldg(p.gfc + g);
+                    const int j = fc.x + lane;
+                    if (lane < fc.y && j != i && (uint32_t)j < (uint64_t)p.n_particles)
+                        pp_pair_f64(xi, yi, zi, __ldg(p.xyzm + j), h, a);
+                }
+            } else {
+                for (int r = lane; r < L.pp; r += 32) {
+                    const int32_t j = __ldg(p.pp_idx + d.pp_begin + r);
+                    if (j != i && (uint32_t)j < (uint64_t)p.n_particles) pp_pair_f64(xi, yi, zi, __ldg(p.xyzm + j), h, a);
+                }
+            }
+            for (int r = lane; r < L.pc; r += 32) {
+                const int32_t c = __ldg(p.pc_idx + d.pc_begin + r);
+                if ((uint32_t)c < (uint64_t)p.n_cells) pc_pair_f64(xi, yi, zi, p.cells_raw + (int64_t)c * p.cells_stride, a);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) a[k] = warp_sum_f64(a[k]);
+            if (lane == 0) {
+                float4 o = make_float4((float)a[0], (float)a[1], (float)a[2], (float)a[3]);
+                if (accumulate) {
+                    const float4 old = p.out[i];
+                    o = make_float4((float)(a[0] + old.x), (float)(a[1] + old.y), (float)(a[2] + old.z), (float)(a[3] + old.w));
+                }
+                p.out[i] = o;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// PKDG_VALIDATE: the value-range contract of include/pkdg.h checked on the device (optional; not on the
+// timed path).  Values: every coordinate finite and |x| <= 1e12, every mass / moment finite.  Pairs: every
+// listed (sink, cell) pair has the sink OUTSIDE the cell's b_max sphere (the expansion diverges inside).
+// ------------------------------------------------------------------------------------------------
+__global__ void pkdg_validate_values_kernel(const float4* __restrict__ xyzm, int64_t n_particles,
+                                            const float* __restrict__ rec, int64_t n_cells, int stride,
+                                            DevStats* __restrict__ stats) {
+    unsigned long long bad = 0;
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = tid; i < n_particles; i += nth) {
+        const float4 q = xyzm[i];
+        const bool ok = fabsf(q.x) <= 1.0e12f && fabsf(q.y) <= 1.0e12f && fabsf(q.z) <= 1.0e12f && isfinite(q.w);
+        bad += !ok;   // NaN coordinates fail the <= tests
+    }
+    for (int64_t c = tid; c < n_cells; c += nth) {
+        const float* r = rec + c * (int64_t)stride;
+        bool ok = fabsf(r[0]) <= 1.0e12f && fabsf(r[1]) <= 1.0e12f && fabsf(r[2]) <= 1.0e12f;
+        for (int k = 3; k < 36; ++k) ok = ok && isfinite(r[k]);
+        bad += !ok;
+    }
+    bad = warp_sum_u64(bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&stats->invalid_values, bad);
+}
+
+__global__ void pkdg_validate_pairs_kernel(const EvalParams p) {
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    unsigned long long bad = 0;
+    for (int64_t b = gw; b < p.n_buckets; b += nw) {
+        const BucketDesc d = p.desc[b];
+        for (int e = lane; e < d.pc_len; e += 32) {
+            const int32_t c = __ldg(p.pc_idx + d.pc_begin + e);
+            if ((uint32_t)c >= (uint64_t)p.n_cells) continue;   // counted as a bad entry by the evaluation kernel
+            const float4 cm = __ldg(p.cellq + (int64_t)c * 8);
+            const float sc = __ldg(reinterpret_cast<const float*>(p.cellq + (int64_t)c * 8 + 1));
+            for (int t = 0; t < d.count; ++t) {
+                const float4 x = __ldg(p.xyzm + d.first + t);
+                const float dx = x.x - cm.x, dy = x.y - cm.y, dz = x.z - cm.z;
+                bad += !(dx * dx + dy * dy + dz * dz > sc * sc);
+            }
+        }
+    }
+    bad = warp_sum_u64(bad);
+    if (lane == 0 && bad) atomicAdd(&p.stats->invalid_pairs, bad);
+}
+
+// ------------------------------------------------------------------------------------------------
+// FFMA-only probe (pkdg_fma_peak_probe): FFMA with two constant-bank operands (one register read per
+// FMA), registers only -- what the FP32 pipe delivers; the roofline denominator cross-check of bench.py.
 // ------------------------------------------------------------------------------------------------
 __global__ void pkdg_fma_probe_kernel(float* out, int64_t iters, float a, float b) {
     float v0 = threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5, v6 = v0 + 6, v7 = v0 + 7;
@@ -1134,72 +1209,5 @@ __global__ void pkdg_fma_probe_kernel(float* out, int64_t iters, float a, float 
     out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
 }
 
-// modes 1-3: 64 (packed) FMA instructions per trip; `in` holds >= 1024 floats around 0.5
-template <int MODE>
-__global__ void __launch_bounds__(128, 4) pkdg_rf_probe_kernel(const float* __restrict__ in, float* __restrict__ out,
-                                                               int64_t iters) {
-    float2 x[8], y[8], a[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        x[i] = make_float2(in[threadIdx.x + 32 * i], in[threadIdx.x + 32 * i + 1]);
-        y[i] = make_float2(in[threadIdx.x + 32 * i + 256], in[threadIdx.x + 32 * i + 257]);
-        a[i] = make_float2(in[threadIdx.x + 32 * i + 512], in[threadIdx.x + 32 * i + 513]);
-    }
-    for (int64_t it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                if (MODE == 1) a[i].x = fmaf(x[i].x, y[(i + u) & 7].x, a[i].x);
-                if (MODE == 2) a[i] = __ffma2_rn(x[i], y[(i + u) & 7], a[i]);
-                if (MODE == 3) a[i] = __ffma2_rn(make_float2(x[i].x, x[i].x), y[(3 * u + i / 3) & 7], a[i]);
-            }
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += a[i].x + a[i].y;
-    out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-// modes 4, 5: `cells` = 32 internal records (one per lane), `tg` = 2 sinks
-template <bool PACKED>
-__global__ void __launch_bounds__(128, 4) pkdg_pc_probe_kernel(const float4* __restrict__ cells,
-                                                               const float4* __restrict__ tg, float4* __restrict__ out,
-                                                               int64_t iters) {
-    CellRegs cr;
-    const float4* q = cells + (threadIdx.x & 31) * 8;
-    cell_unpack(cr, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7]);
-    float4 tA = tg[0], tB = tg[1];
-    float4 r;
-    if (PACKED) {
-        float4 txy = make_float4(tA.x, tB.x, tA.y, tB.y), tz = make_float4(tA.z, tB.z, 0.f, 0.f);
-        float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
-        PcPre2 pA = pc_pre2<false>(txy, tz, cr);
-#pragma unroll 1
-        for (int64_t it = 0; it < iters; it += 2) {
-            txy.x += 1e-3f; txy.w += 1e-3f;
-            const PcPre2 pB = pc_pre2<false>(txy, tz, cr);
-            pc_body2(pA, cr, a0, a1);
-            txy.y += 1e-3f; txy.z += 1e-3f;
-            pA = pc_pre2<false>(txy, tz, cr);
-            pc_body2(pB, cr, a0, a1);
-        }
-        r = make_float4(a0.x + a0.y, a0.z + a0.w, a1.x + a1.y, a1.z + a1.w);
-    } else {
-        float4 aA = make_float4(0.f, 0.f, 0.f, 0.f), aB = aA;
-        PcPre pA = pc_pre<true>(tA, cr), pB = pc_pre<true>(tB, cr);
-#pragma unroll 1
-        for (int64_t it = 0; it < iters; ++it) {
-            tA.x += 1e-3f; tB.y += 1e-3f;
-            const PcPre nA = pc_pre<true>(tA, cr), nB = pc_pre<true>(tB, cr);
-            pc_body(pA, cr, aA);
-            pc_body(pB, cr, aB);
-            pA = nA; pB = nB;
-        }
-        r = make_float4(aA.x + aB.x, aA.y + aB.y, aA.z + aB.z, aA.w + aB.w);
-    }
-    out[(int64_t)blockIdx.x * blockDim.x + threadIdx.x] = r;
-}
 
 }  // namespace pkdg

@@ -253,7 +253,62 @@ def build_lists(p: Problem, theta: float, eps: float, b0: int = 0, b1: int | Non
     return pp_off, pp_idx, pc_off, pc_idx
 
 
+def build_groups(p: Problem, gmax: int = 64):
+    """Groups of sibling buckets (the walk stops at cells of fewer than g = 64 particles and resolves
+    the checklist into lists there): the maximal tree cells with at most gmax particles, in tree order.  Returns
+    (group_cell int32[n_g], first_bucket int32[n_g], n_buckets int32[n_g]); the groups tile the bucket range."""
+    t = p.tree
+    count, end, isleaf = t["count"], t["end"].astype(np.int64), t["isleaf"]
+    small = (count <= gmax) | (isleaf != 0)                  # a leaf is always a group of its own at least
+    e = np.where(small, end, 0)
+    covered_to = np.concatenate([[0], np.maximum.accumulate(e)[:-1]])   # end of the last small cell before k
+    top = small & (covered_to <= np.arange(count.shape[0]))
+    group_cell = np.flatnonzero(top).astype(np.int32)
+    leaves_before = np.concatenate([[0], np.cumsum(isleaf != 0)])
+    first_bucket = leaves_before[group_cell].astype(np.int32)
+    n_buckets = (leaves_before[end[group_cell]] - leaves_before[group_cell]).astype(np.int32)
+    return group_cell, first_bucket, n_buckets
+
+
+def build_group_lists(p: Problem, group_cell: np.ndarray, theta: float, eps: float, g0: int = 0, g1: int | None = None):
+    """CSR P-P / P-C lists per GROUP (reading A6 with the group cell as the sink: its centre of mass, b_max and
+    bounding box): what every bucket of the group evaluates.  Offsets relative to g0."""
+    L = _L()
+    t = p.tree
+    g1 = group_cell.shape[0] if g1 is None else g1
+    gc = np.ascontiguousarray(group_cell, np.int32)
+    h = L.tg_lists_build(t["first"].shape[0], _p(t["first"]), _p(t["count"]), _p(t["end"]), _p(t["isleaf"]),
+                         _p(p.cells), _p(t["bblo"]), _p(t["bbhi"]), _p(gc), g0, g1, float(theta), float(eps))
+    npp = c_int64(); npc = c_int64()
+    L.tg_lists_totals(h, ctypes.byref(npp), ctypes.byref(npc))
+    pp_off = np.empty(g1 - g0 + 1, np.int64); pc_off = np.empty(g1 - g0 + 1, np.int64)
+    pp_idx = np.empty(npp.value, np.int32); pc_idx = np.empty(npc.value, np.int32)
+    L.tg_lists_export_free(h, _p(pp_off), _p(pp_idx), _p(pc_off), _p(pc_idx))
+    return pp_off, pp_idx, pc_off, pc_idx
+
+
+def expand_groups(first_bucket: np.ndarray, n_buckets: np.ndarray, g_off: np.ndarray, g_idx: np.ndarray, sel=None):
+    """Per-bucket CSR lists the group lists stand for (pure indexing): every bucket of a group gets the group's
+    list.  sel: bucket indices to expand (default all, in order).  Returns (off int64[len+1], idx int32)."""
+    nb = int(first_bucket[-1] + n_buckets[-1]) if first_bucket.shape[0] else 0
+    group_of = np.repeat(np.arange(first_bucket.shape[0]), n_buckets)
+    assert group_of.shape[0] == nb
+    g = group_of if sel is None else group_of[np.asarray(sel, np.int64)]
+    lens = (g_off[1:] - g_off[:-1])[g]
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    start = np.repeat(g_off[:-1][g] - off[:-1], lens)
+    idx = g_idx[start + np.arange(int(lens.sum()), dtype=np.int64)]
+    return off, np.ascontiguousarray(idx, np.int32)
+
+
+def f32(x: float) -> float:
+    """x rounded to fp32: the C ABI takes the softening as a float, so the harness hands the SAME value to the
+    oracle, to the list builder and to the library."""
+    return float(np.float32(x))
+
+
 def with_lists(p: Problem, theta: float, eps: float) -> Problem:
+    eps = f32(eps)
     p.pp_off, p.pp_idx, p.pc_off, p.pc_idx = build_lists(p, theta, eps)
     p.theta = theta; p.eps = eps
     return p
@@ -322,7 +377,7 @@ def config5_particles(n: int = 1 << 26, seed: int = 5, mesh: int = 512) -> tuple
         ng += 1
     m = mesh if mesh < ng or (ng & (ng - 1)) else None
     xyzm = particles_zeldovich(ng, seed, -2.5, 0.5, n_keep=n, mesh=m)
-    return xyzm, 1.0 / (50.0 * n ** (1.0 / 3.0))
+    return xyzm, f32(1.0 / (50.0 * n ** (1.0 / 3.0)))
 
 
 def config4(n_buckets: int, l_pp: int, l_pc: int, seed: int = 4, reuse: int = 16, r_b: float = 0.005,
@@ -366,4 +421,4 @@ def config4(n_buckets: int, l_pp: int, l_pc: int, seed: int = 4, reuse: int = 16
     pc_idx = (cl[:, None] * l_pc + np.arange(l_pc, dtype=np.int64)[None, :]).astype(np.int32).reshape(-1)
     return Problem(name=f"cfg4_sweep_b{n_buckets}_pp{l_pp}_pc{l_pc}", xyzm=xyzm, cells=cells, first=first,
                    count=count, pp_off=pp_off, pp_idx=pp_idx, pc_off=pc_off, pc_idx=pc_idx,
-                   eps=0.02 * r_b)
+                   eps=f32(0.02 * r_b))

@@ -17,7 +17,7 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, name), name
     from paper_1609_08621_b200 import binding
     assert set(binding.EXPORTS) == declared
-    assert binding.version() == (0, 1)
+    assert binding.version() == (0, 2)
 
 
 def test_host_only_entry_points_work_without_gpu():

@@ -1,7 +1,14 @@
 """-m gpu: parity at BASELINE.json's full sizes, in the launch configuration bench.py times (resident
-pkdg_gravity_eval, default kernel variant), on SAMPLED buckets the oracle can compute one by one, plus
-properties that hold at any size and bit-exact integer counters.  (DESIGN.md sec 7 for the recipes.)
+pkdg_gravity_eval, default flags).  The bar is north_star's AS WRITTEN on every config: per-particle
+|a_gpu - a_or| / |a_or| <= 2e-5 and |phi_gpu - phi_or| / |phi_or| <= 2e-5, max over all compared particles.
+
+Coverage: config 2 and config 3 compare EVERY particle with the oracle; config 4 compares >= 10^6 sinks per
+shape (5.2e5 for the two shapes with 2048 cells per list, whose clouds need 4 GB per 2^15 buckets on the
+host); config 5 evaluates all 6.6 M buckets resident and compares 2^16 + 2^11 aimed buckets (longest lists,
+densest buckets) with the conditioning of every compared sum printed.  Integer counters are bit-exact.
 """
+import time
+
 import numpy as np
 import pytest
 
@@ -14,7 +21,7 @@ TOL = 2e-5
 def torch():
     import torch
     if not torch.cuda.is_available():
-        pytest.skip("no CUDA device")
+        pytest.fail("-m gpu tests need a CUDA device")
     return torch
 
 
@@ -26,26 +33,15 @@ def ctx(torch):
     c.close()
 
 
-def _sample(p, n_even, n_long, seed=0):
-    """Evenly spread buckets plus the longest-list ones plus a few random ones."""
-    nb = p.n_buckets
-    ltot = np.diff(p.pp_off) + np.diff(p.pc_off)
-    rng = np.random.default_rng(seed)
-    sel = np.concatenate([np.linspace(0, nb - 1, n_even).astype(np.int64), np.argsort(ltot)[-n_long:],
-                          np.argsort(np.diff(p.pp_off))[-n_long:], rng.integers(0, nb, n_even // 4)])
-    return np.unique(sel)
+def _rows_of(first, count, sel):
+    f = first[sel].astype(np.int64); c = count[sel].astype(np.int64)
+    return np.repeat(f - np.concatenate([[0], np.cumsum(c)[:-1]]), c) + np.arange(int(c.sum()))
 
 
-KAPPA0 = 80.0   # DESIGN.md sec 8: fp32 evaluation error <= 2.5e-7 kappa, so 2e-5 is attainable up to kappa = 80
-
-
-def _check_sampled(ctx, torch, p, sel, flags=0, conditioned=False):
-    """conditioned=False: the north_star bound as written, max over sampled particles <= 2e-5.
-    conditioned=True (config 4 only, whose isotropic source shells put sinks in force nulls): the bound
-    is 2e-5 max(1, kappa_i / KAPPA0) with kappa_i = sum_j |a_ij| / |a_i| from the oracle, and at most
-    one sampled particle in 10^4 may exceed the plain 2e-5."""
+def _check(ctx, torch, p, sel=None, flags=0, label=None):
+    """Resident call vs the oracle on buckets `sel` (None = every bucket); the bound as written."""
     import oracle
-    from gpu_util import bucket_rows, rel_errors, run_resident
+    from gpu_util import rel_errors, run_resident
     out = run_resident(ctx, p, torch, flags=flags)
     st = ctx.get_stats()
     assert st["interactions_pp"] == oracle.interactions(p.count, p.pp_off) == p.I_pp      # bit-exact integers
@@ -53,45 +49,33 @@ def _check_sampled(ctx, torch, p, sel, flags=0, conditioned=False):
     assert st["tiles_pp"] == int(((np.diff(p.pp_off) + 31) // 32).sum())
     assert st["tiles_pc"] == int(((np.diff(p.pc_off) + 31) // 32).sum())
     assert st["bad_entries"] == 0 and st["n_buckets"] == p.n_buckets
+    t0 = time.perf_counter()
     ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
-    rows = bucket_rows(p, sel)
+    dt = time.perf_counter() - t0
+    rows = _rows_of(p.first, p.count, np.arange(p.n_buckets) if sel is None else sel)
     ea, ep = rel_errors(out, ref, rows)
-    if conditioned:
-        S = oracle.contribution_norms(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps,
-                                      sel=sel)
-        kappa = S[rows] / np.linalg.norm(ref[rows, :3], axis=1)
-        bound = TOL * np.maximum(1.0, kappa / KAPPA0)
-        w = int(np.argmax(ea / bound))
-        assert (ea <= bound).all(), (p.name, ea[w], kappa[w])
-        assert (ea > TOL).sum() <= max(1, len(ea) // 10000), (p.name, int((ea > TOL).sum()), len(ea))
-        assert ep.max() <= TOL, (p.name, ep.max())
-    else:
-        assert ea.max() <= TOL and ep.max() <= TOL, (p.name, ea.max(), ep.max())
-    return out, ea, ep
+    print(f"\n[{label or p.name}] compared {len(rows)} particles of {int(p.count.sum())} ({dt:.1f} s of oracle): "
+          f"acc max {ea.max():.2e} rms {np.sqrt(np.mean(ea ** 2)):.2e} | pot max {ep.max():.2e} rms "
+          f"{np.sqrt(np.mean(ep ** 2)):.2e} | fp64 fix-up: {st['fixup_sinks']} sinks ({st['fixup_sinks'] / max(1, int(p.count.sum())):.2e})")
+    assert ea.max() <= TOL and ep.max() <= TOL, (p.name, float(ea.max()), float(ep.max()), int((ea > TOL).sum()))
+    return out, ref, rows
 
 
 def _check_properties(p, out):
-    """Hold at any size: every row of a listed bucket is finite; the potential is negative; the net
-    force sum_i m_i a_i is far below sum_i m_i |a_i| (exact for P-P pairs, O(theta^5) for P-C)."""
+    """Every row of a listed bucket is finite and its potential negative; buckets cover every particle."""
     covered = np.zeros(p.n, bool)
-    covered[np.repeat(p.first.astype(np.int64) - np.concatenate([[0], np.cumsum(p.count.astype(np.int64))[:-1]]),
-                      p.count) + np.arange(int(p.count.sum()))] = True
+    covered[_rows_of(p.first, p.count, np.arange(p.n_buckets))] = True
     assert covered.all()
     assert np.isfinite(out).all()
     assert (out[:, 3] < 0).all()
-    m = p.xyzm[:, 3].astype(np.float64)
-    a = out[:, :3].astype(np.float64)
-    net = np.linalg.norm((m[:, None] * a).sum(axis=0))
-    tot = (m * np.linalg.norm(a, axis=1)).sum()
-    assert net <= 2e-3 * tot, (net, tot)
 
 
-def test_config2_full(ctx, torch):
-    """configs[1]: N = 2^20, 32 Plummer spheres + background, binary tree, theta = 0.7."""
+def test_config2_every_particle(ctx, torch):
+    """configs[1]: N = 2^20, 32 Plummer spheres + background, binary tree, theta = 0.7 -- all particles."""
     from paper_1609_08621_b200 import inputs
     p = inputs.config2()
     assert p.n == 1 << 20
-    out, ea, ep = _check_sampled(ctx, torch, p, _sample(p, 6000, 64))
+    out, _, _ = _check(ctx, torch, p)
     _check_properties(p, out)
 
 
@@ -101,82 +85,170 @@ def cfg3():
     return inputs.config3(256)
 
 
-def test_config3_headline_full(ctx, torch, cfg3):
-    """configs[2], the configuration bench.py times: N = 2^24 Zel'dovich lattice, theta = 0.7."""
+@pytest.fixture(scope="module")
+def cfg3_resident(ctx, torch, cfg3):
+    from gpu_util import run_resident
+    return run_resident(ctx, cfg3, torch)
+
+
+def test_config3_headline_every_particle(ctx, torch, cfg3):
+    """configs[2], the configuration bench.py times: N = 2^24 Zel'dovich lattice, theta = 0.7.  EVERY one of
+    the 16.8 M particles is compared with the oracle (about two minutes of host time)."""
     p = cfg3
     assert p.n == 1 << 24
-    out, ea, ep = _check_sampled(ctx, torch, p, _sample(p, 4096, 64))
+    out, _, _ = _check(ctx, torch, p)
     _check_properties(p, out)
 
 
-def test_config3_headline_pp_leaves(ctx, torch, cfg3):
-    """The headline configuration with its P-P lists as bucket references (PKDG_PP_LEAVES)."""
+def test_config3_headline_pp_leaves(ctx, torch, cfg3, cfg3_resident):
+    """The headline configuration with its P-P lists as bucket references (PKDG_PP_LEAVES): same sums in another
+    order, so it is compared with the (oracle-checked) particle-list result at a tolerance far below 2e-5, and
+    with the oracle on sampled buckets."""
     import copy
+    import oracle
     from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors, run_resident
     p = cfg3
     q = copy.copy(p)
     q.pp_off, q.pp_idx = inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
     assert q.pp_idx.shape[0] * 8 < p.pp_idx.shape[0]
-    import oracle
-    from gpu_util import bucket_rows, rel_errors, run_resident
     out = run_resident(ctx, q, torch, flags=binding.PP_LEAVES)
     st = ctx.get_stats()
     assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
-    sel = _sample(p, 2048, 32, seed=1)
+    sel = np.unique(np.concatenate([np.linspace(0, p.n_buckets - 1, 8192).astype(np.int64),
+                                    np.argsort(np.diff(p.pp_off))[-64:]]))
     ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
-    ea, ep = rel_errors(out, ref, bucket_rows(p, sel))
+    ea, ep = rel_errors(out, ref, _rows_of(p.first, p.count, sel))
     assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())
+    eb, epb = rel_errors(out, cfg3_resident.astype(np.float64))
+    assert eb.max() <= TOL and epb.max() <= 2e-6, (eb.max(), epb.max())
     _check_properties(p, out)
 
 
-def test_config3_sharded_equals_unsharded(ctx, torch, cfg3):
-    """Multi-GPU path emulated as consecutive calls on one GPU (no kernel waits on another): the two
-    ranks' pieces, evaluated separately, give the same bits as one call."""
+def test_config3_variants_bit_equal_to_resident(ctx, torch, cfg3, cfg3_resident):
+    """Stand-in for racecheck (compute-sanitizer is closed on this pool) at 1.06 M buckets: the streamed call
+    (3 chunkings), the all-host call and the two-shard evaluation give the SAME BITS as one resident call.  A
+    shared-memory race, a stale cp.async slot or a fix-up queue mix-up would break the equality."""
     from paper_1609_08621_b200 import shard
     from gpu_util import to_dev
     p = cfg3
+    whole = cfg3_resident
     d = to_dev(p, torch)
-    whole = torch.zeros((p.n, 4), dtype=torch.float32, device="cuda:0")
-    ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"], d["pc_idx"],
-                     p.eps, whole)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h = dict(first=pin(p.first), count=pin(p.count), pp_off=pin(p.pp_off), pp_idx=pin(p.pp_idx),
+             pc_off=pin(p.pc_off), pc_idx=pin(p.pc_idx))
+    for n_streams, max_entries in ((1, 1 << 26), (4, 1 << 23), (3, 1 << 20)):
+        out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda:0")
+        ctx.gravity_eval_streamed(d["xyzm"], d["cells"], h["first"], h["count"], h["pp_off"], h["pp_idx"],
+                                  h["pc_off"], h["pc_idx"], p.eps, out, n_streams=n_streams,
+                                  max_entries_per_chunk=max_entries)
+        torch.cuda.synchronize()
+        st = ctx.get_stats()
+        assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
+        assert np.array_equal(out.cpu().numpy(), whole), (n_streams, max_entries)
+        del out
+    out_h = torch.full((p.n, 4), float("nan"), dtype=torch.float32).pin_memory()
+    ctx.gravity_eval_host(torch.from_numpy(p.xyzm).pin_memory(), torch.from_numpy(p.cells).pin_memory(), h["first"],
+                          h["count"], h["pp_off"], h["pp_idx"], h["pc_off"], h["pc_idx"], p.eps, out_h, n_streams=4,
+                          max_entries_per_chunk=1 << 23)
+    assert np.array_equal(out_h.numpy(), whole)
+    # two shards, evaluated one after the other on this GPU (no kernel waits on another rank)
     parts = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda:0")
-    bounds = shard.shard_bounds(shard.bucket_cost(p.count, p.pp_off, p.pc_off), 2)
     tot_pp = tot_pc = 0
     for r in range(2):
-        b0, b1 = int(bounds[r]), int(bounds[r + 1])
-        first, count, ppo, ppi, pco, pci = shard.slice_problem(p.first, p.count, p.pp_off, p.pp_idx, p.pc_off,
-                                                               p.pc_idx, b0, b1)
+        piece = shard.rank_piece(p, r, 2)
         t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
-        ctx.gravity_eval(d["xyzm"], d["cells"], t(first), t(count), t(ppo), t(ppi), t(pco), t(pci), p.eps, parts)
+        ctx.gravity_eval(d["xyzm"], d["cells"], t(piece.first), t(piece.count), t(piece.pp_off), t(piece.pp_idx),
+                         t(piece.pc_off), t(piece.pc_idx), p.eps, parts)
         st = ctx.get_stats()
         tot_pp += st["interactions_pp"]; tot_pc += st["interactions_pc"]
     torch.cuda.synchronize()
     assert tot_pp == p.I_pp and tot_pc == p.I_pc
-    assert torch.equal(whole, parts)
+    assert np.array_equal(parts.cpu().numpy(), whole)
 
 
-@pytest.mark.parametrize("nb,lpp,lpc", [(65536, 32, 0), (65536, 4096, 0), (65536, 0, 32), (65536, 128, 128),
-                                        (16384, 512, 512), (8192, 0, 2048), (4096, 2048, 2048), (65536, 100, 70)])
+# (buckets, L_pp, L_pc): every BASELINE.json length, the extremes at >= 10^6 sinks
+CFG4_SHAPES = [(65536, 32, 0), (65536, 128, 0), (65536, 4096, 0), (65536, 0, 32), (65536, 0, 128), (65536, 32, 32),
+               (65536, 128, 128), (65536, 100, 70), (65536, 512, 512), (32768, 0, 2048), (32768, 2048, 2048)]
+
+
+@pytest.mark.parametrize("nb,lpp,lpc", CFG4_SHAPES)
 def test_config4_sweep_full(ctx, torch, nb, lpp, lpc):
-    """configs[3]: 65,536 buckets of 16 sinks; the extreme list lengths.  (The shapes with >= 512 cells
-    per list use fewer buckets: building their 64-particle clouds on the host needs 15 GB and 30 s at
-    65,536 buckets, which does not belong in a test suite.)"""
+    """configs[3]: buckets of 16 sinks inside isotropic source shells.  Net forces nearly cancel there (Newton's
+    shell theorem), so these are the worst-conditioned sums of the whole suite: the bound is asserted AS WRITTEN
+    on every sink; the conditioning-triggered fp64 fix-up is what makes it hold."""
     from paper_1609_08621_b200 import inputs
     p = inputs.config4(nb, lpp, lpc)
-    n_s = int(min(nb, max(96, 4.0e7 / (16 * (lpp / 20.0 + lpc + 1)))))     # ~2 s of oracle time per shape
-    sel = np.unique(np.concatenate([np.linspace(0, nb - 1, n_s).astype(np.int64), [0, 1, nb - 1]]))
-    _check_sampled(ctx, torch, p, sel, conditioned=True)
+    _check(ctx, torch, p, label=f"cfg4 {nb} buckets L_pp={lpp} L_pc={lpc}")
+
+
+def test_config5_all_buckets_resident(ctx, torch):
+    """configs[4]: N = 2^26, theta = 0.55 -- ALL 6.6 M buckets evaluated resident (lists built range by range on
+    the host and assembled on the device, 15 GB), 2^16 evenly spread + the 1024 longest-list + the 1024 densest
+    (most softened) buckets compared with the oracle; kappa of every compared sum reported."""
+    import oracle
+    from paper_1609_08621_b200 import inputs
+    from gpu_util import rel_errors
+    xyzm, eps = inputs.config5_particles()
+    assert xyzm.shape[0] == 1 << 26
+    p = inputs.build_tree(xyzm, "binary", 16, name="cfg5")
+    del xyzm
+    nb = p.n_buckets
+    dev = "cuda:0"
+    step_b = 1 << 20
+    pp_offs, pc_offs, pp_parts, pc_parts = [np.zeros(1, np.int64)], [np.zeros(1, np.int64)], [], []
+    for b0 in range(0, nb, step_b):
+        po, pi, co, ci = inputs.build_lists(p, 0.55, eps, b0, min(nb, b0 + step_b))
+        pp_offs.append(po[1:] + pp_offs[-1][-1]); pc_offs.append(co[1:] + pc_offs[-1][-1])
+        pp_parts.append(torch.from_numpy(pi).to(dev)); pc_parts.append(torch.from_numpy(ci).to(dev))
+    pp_off = np.concatenate(pp_offs); pc_off = np.concatenate(pc_offs)
+    d_ppi = torch.cat(pp_parts); del pp_parts
+    d_pci = torch.cat(pc_parts); del pc_parts
+    t = lambda a: torch.from_numpy(a).to(dev)
+    out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device=dev)
+    ctx.gravity_eval(t(p.xyzm), t(p.cells), t(p.first), t(p.count), t(pp_off), d_ppi, t(pc_off), d_pci, eps, out)
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    cnt = p.count.astype(np.int64)
+    assert st["interactions_pp"] == int(np.dot(cnt, np.diff(pp_off)))
+    assert st["interactions_pc"] == int(np.dot(cnt, np.diff(pc_off)))
+    assert st["bad_entries"] == 0 and st["n_buckets"] == nb
+    bmax = p.cells[p.tree["leaf_cell"], 35]
+    sel = np.unique(np.concatenate([np.linspace(0, nb - 1, 1 << 16).astype(np.int64),
+                                    np.argsort(np.diff(pp_off) + np.diff(pc_off))[-1024:],
+                                    np.argsort(np.where(p.count >= 8, bmax, np.inf))[:1024]]))
+    # the oracle needs host lists: rebuild them for the compared buckets (same generator, same result)
+    runs = np.split(sel, np.flatnonzero(np.diff(sel) != 1) + 1)
+    o_ppo, o_pco, o_ppi, o_pci = [np.zeros(1, np.int64)], [np.zeros(1, np.int64)], [], []
+    for r in runs:
+        po, pi, co, ci = inputs.build_lists(p, 0.55, eps, int(r[0]), int(r[-1]) + 1)
+        o_ppo.append(po[1:] + o_ppo[-1][-1]); o_pco.append(co[1:] + o_pco[-1][-1]); o_ppi.append(pi); o_pci.append(ci)
+    s_ppo = np.concatenate(o_ppo); s_pco = np.concatenate(o_pco)
+    s_ppi = np.concatenate(o_ppi); s_pci = np.concatenate(o_pci)
+    assert np.array_equal(np.diff(s_ppo), np.diff(pp_off)[sel]) and np.array_equal(np.diff(s_pco), np.diff(pc_off)[sel])
+    first = np.ascontiguousarray(p.first[sel]); count = np.ascontiguousarray(p.count[sel])
+    args = (p.xyzm, p.cells, first, count, s_ppo, s_ppi, s_pco, s_pci, eps)
+    ref = oracle.gravity_eval(*args)
+    S = oracle.contribution_norms(*args)
+    rows = _rows_of(first, count, np.arange(len(sel)))
+    got = out[torch.from_numpy(rows).to(dev)].cpu().numpy()
+    ea, ep = rel_errors(got, ref[rows])
+    kappa = S[rows] / np.linalg.norm(ref[rows, :3], axis=1)
+    print(f"\n[cfg5 all {nb} buckets resident] compared {len(rows)} particles in {len(sel)} buckets: acc max {ea.max():.2e} "
+          f"rms {np.sqrt(np.mean(ea ** 2)):.2e} | pot max {ep.max():.2e} | kappa max {kappa.max():.0f} median "
+          f"{np.median(kappa):.1f} | fp64 fix-up: {st['fixup_sinks']} of {p.n} sinks")
+    assert ea.max() <= TOL and ep.max() <= TOL, (float(ea.max()), float(ep.max()))
+    o = out.cpu().numpy()
+    assert np.isfinite(o).all() and (o[:, 3] < 0).all()
 
 
 def test_config5_streamed_range(ctx, torch):
-    """configs[4]: N = 2^26 particles, theta = 0.55; lists are built chunk by chunk on the host and
-    streamed (a6).  A contiguous range of 2^19 buckets is evaluated through the streamed call on 3
-    streams; sampled buckets are compared with the oracle; chunk accounting is bit-exact."""
+    """configs[4] through the streamed call (a6): a contiguous range of 2^19 buckets, lists in pinned host memory,
+    3 streams; sampled buckets against the oracle; chunk accounting bit-exact; rows outside the range untouched."""
     import oracle
-    from paper_1609_08621_b200 import binding, inputs
-    from gpu_util import bucket_rows, rel_errors
+    from paper_1609_08621_b200 import inputs
+    from gpu_util import rel_errors
     xyzm, eps = inputs.config5_particles()
-    assert xyzm.shape[0] == 1 << 26
     p = inputs.build_tree(xyzm, "binary", 16, name="cfg5")
     del xyzm
     nb_all = p.n_buckets
@@ -199,10 +271,10 @@ def test_config5_streamed_range(ctx, torch):
     assert st["interactions_pc"] == int(np.dot(cnt, np.diff(pc_off)))
     assert st["chunks"] == len(oracle.chunk_bounds(pp_off, pc_off, max_entries)) - 1 and st["chunks"] > 3
     assert st["bad_entries"] == 0
-    sel = np.unique(np.concatenate([np.linspace(0, b1 - b0 - 1, 2048).astype(np.int64),
-                                    np.argsort(np.diff(pp_off) + np.diff(pc_off))[-32:]]))
+    sel = np.unique(np.concatenate([np.linspace(0, b1 - b0 - 1, 4096).astype(np.int64),
+                                    np.argsort(np.diff(pp_off) + np.diff(pc_off))[-64:]]))
     ref = oracle.gravity_eval(p.xyzm, p.cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, sel=sel)
-    rows = np.concatenate([np.arange(first[b], first[b] + count[b]) for b in sel]).astype(np.int64)
+    rows = _rows_of(first, count, sel)
     got = out[torch.from_numpy(rows).to(dev)].cpu().numpy()
     ea, ep = rel_errors(got, ref[rows])
     assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max())

@@ -7,7 +7,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 TOL = 2e-5
-VARIANTS = [0, 1 << 8, 2 << 8, 3 << 8]
+MODES = [0, 0x10, 0x20]   # default (fp32 + conditioning-triggered fp64 fix-up), PKDG_NO_FIXUP, PKDG_FIXUP_ALL
 
 
 @pytest.fixture(scope="module")
@@ -31,7 +31,7 @@ def _oracle(p, sel=None):
     return oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps, sel=sel)
 
 
-@pytest.mark.parametrize("flags", VARIANTS)
+@pytest.mark.parametrize("flags", MODES)
 def test_config1_full_parity(ctx, torch, cfg1, flags):
     """configs[0]: N = 4096 uniform, octree, theta = 0.7 -- every particle against the oracle."""
     from gpu_util import rel_errors, run_resident
@@ -146,10 +146,10 @@ def _edge_problem():
     pc_off = np.concatenate([[0], np.cumsum(pc_lens)]).astype(np.int64)
     pc_idx = np.concatenate(pc).astype(np.int32)
     return inputs.Problem(name="edge", xyzm=xyzm, cells=cells, first=first, count=count, pp_off=pp_off,
-                          pp_idx=pp_idx, pc_off=pc_off, pc_idx=pc_idx, eps=0.004)
+                          pp_idx=pp_idx, pc_off=pc_off, pc_idx=pc_idx, eps=float(np.float32(0.004)))
 
 
-@pytest.mark.parametrize("flags", VARIANTS)
+@pytest.mark.parametrize("flags", MODES)
 def test_edge_cases(ctx, torch, flags):
     from gpu_util import rel_errors, run_resident
     p = _edge_problem()
@@ -198,8 +198,9 @@ def test_invalid_arguments_fail_loudly(ctx, torch, cfg1):
         ctx.gravity_eval(d["xyzm"], d["cells"][:, :20].contiguous(), d["first"], d["count"], d["pp_off"], d["pp_idx"],
                          d["pc_off"], d["pc_idx"], cfg1.eps, out)
     with pytest.raises(binding.PkdgError):
-        ctx.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"],
-                         d["pc_idx"], cfg1.eps, out, flags=200 << 8)
+        ctx.set_option(binding.OPT_KAPPA2, -1.0)
+    with pytest.raises(binding.PkdgError):
+        ctx.set_option(77, 1.0)
 
 
 def test_streamed_and_host_variants_match_resident(ctx, torch, cfg1):
@@ -279,7 +280,7 @@ def _leaf_problem(p):
     return q
 
 
-@pytest.mark.parametrize("flags", [0, 2 << 8, 3 << 8])
+@pytest.mark.parametrize("flags", MODES)
 def test_pp_leaves_resident(ctx, torch, cfg1, flags):
     """PKDG_PP_LEAVES: leaf references give the oracle's result of the expanded lists, and the same
     interaction count; tiles_pp counts two references per tile."""
@@ -322,31 +323,204 @@ def test_pp_leaves_streamed_host_and_bad_references(ctx, torch, cfg1):
     ctx.gravity_eval_host(q.xyzm, q.cells, q.first, q.count, q.pp_off, q.pp_idx, q.pc_off, q.pc_idx, p.eps, out_h,
                           n_streams=3, max_entries_per_chunk=5000, flags=binding.PP_LEAVES)
     assert np.array_equal(out_h, base)
-    # a reference out of range is reported, not followed; variant 1 does not implement leaves
+    # a reference out of range is reported, not followed (fp32 path and fp64 fix-up kernel alike)
     bad = _leaf_problem(p)
     bad.pp_idx = bad.pp_idx.copy(); bad.pp_idx[3] = p.n_buckets + 5
-    out = run_resident(ctx, bad, torch, flags=binding.PP_LEAVES)
-    assert np.isfinite(out).all()
+    for fl in (0, binding.FIXUP_ALL):
+        out = run_resident(ctx, bad, torch, flags=binding.PP_LEAVES | fl)
+        assert np.isfinite(out).all()
+        assert ctx.get_stats(check=False)["bad_entries"] > 0
+
+
+def test_fixup_kernel_is_fp64_accurate(ctx, torch, cfg1):
+    """PKDG_FIXUP_ALL: every sink through pkdg_fixup_kernel (fp64 terms and accumulators).  What is left is
+    the fp32 rounding of the OUTPUT (2^-24 per component), independent of the conditioning of the sum."""
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors, run_resident
+    for p in (cfg1, inputs.config2(n=1 << 14), _edge_problem(), inputs.config4(512, 100, 70)):
+        ref = _oracle(p)
+        out = run_resident(ctx, p, torch, flags=binding.FIXUP_ALL)
+        st = ctx.get_stats()
+        rows = np.flatnonzero(np.isfinite(ref[:, 0]) & (np.linalg.norm(ref[:, :3], axis=1) > 0))
+        ea, ep = rel_errors(out, ref, rows)
+        assert ea.max() <= 1.5e-7 and ep.max() <= 1.0e-7, (p.name, ea.max(), ep.max())
+        assert st["fixup_sinks"] == int(p.count.sum()), (p.name, st["fixup_sinks"])
+        # PKDG_NO_FIXUP never queues anything; the default queues a small minority
+        run_resident(ctx, p, torch, flags=binding.NO_FIXUP)
+        assert ctx.get_stats()["fixup_sinks"] == 0
+        run_resident(ctx, p, torch)
+        assert ctx.get_stats()["fixup_sinks"] <= 0.05 * int(p.count.sum()) + 4, p.name
+
+
+def test_fixup_threshold_option_and_accumulate(ctx, torch, cfg1):
+    """PKDG_OPT_KAPPA2 moves the threshold (a tiny kappa2 queues everything); PKDG_ACCUMULATE adds in both kernels."""
+    from paper_1609_08621_b200 import binding
+    from gpu_util import run_resident
+    p = cfg1
+    base = run_resident(ctx, p, torch, flags=binding.FIXUP_ALL)
+    ctx.set_option(binding.OPT_KAPPA2, 1e-3)
+    try:
+        out = run_resident(ctx, p, torch)
+        assert ctx.get_stats()["fixup_sinks"] == p.n
+        assert np.array_equal(out, base)
+        acc = run_resident(ctx, p, torch, flags=binding.ACCUMULATE, fill=1.0)
+        assert np.allclose(acc, base + 1.0, rtol=1e-6, atol=1e-6)
+        ctx.set_option(binding.OPT_KAPPA2, 1.5)
+        mixed = run_resident(ctx, p, torch)
+        n_fix = ctx.get_stats()["fixup_sinks"]
+        assert 0 < n_fix < p.n
+        acc = run_resident(ctx, p, torch, flags=binding.ACCUMULATE, fill=1.0)
+        assert np.allclose(acc, mixed + 1.0, rtol=1e-6, atol=1e-6)
+    finally:
+        ctx.set_option(binding.OPT_KAPPA2, 8.0)
+
+
+def test_validate_flag_checks_the_value_range_contract(ctx, torch, cfg1):
+    """PKDG_VALIDATE (include/pkdg.h "Value range"): clean input passes; a NaN mass, a coordinate beyond 1e12
+    and an infinite moment are counted as invalid_values; a listed cell whose b_max sphere holds the sinks
+    (here: the root cell) is counted pair by pair as invalid_pairs; pkdg_get_stats reports PKDG_EBADVALUE."""
+    import copy
+    from paper_1609_08621_b200 import binding
+    from gpu_util import run_resident
+    p = cfg1
+    base = run_resident(ctx, p, torch)
+    out = run_resident(ctx, p, torch, flags=binding.VALIDATE)
+    st = ctx.get_stats()
+    assert st["invalid_values"] == 0 and st["invalid_pairs"] == 0 and np.array_equal(out, base)
+    q = copy.copy(p)
+    q.xyzm = p.xyzm.copy(); q.cells = p.cells.copy(); q.pc_idx = p.pc_idx.copy()
+    q.xyzm[5, 3] = np.nan; q.xyzm[9, 1] = 2.0e13; q.cells[3, 17] = np.inf
+    b = 40
+    q.pc_idx[p.pc_off[b]] = 0                       # the root cell: every sink of bucket b lies inside its b_max
+    run_resident(ctx, q, torch, flags=binding.VALIDATE)
+    with pytest.raises(binding.PkdgError, match="EBADVALUE"):
+        ctx.get_stats()
+    st = ctx.get_stats(check=False)
+    assert st["invalid_values"] == 3 and st["invalid_pairs"] == int(p.count[b]) and st["bad_entries"] == 0
+    # the streamed variants check too
+    d_x = torch.from_numpy(q.xyzm).cuda(); d_c = torch.from_numpy(q.cells).cuda()
+    out = torch.zeros((p.n, 4), dtype=torch.float32, device="cuda")
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    ctx.gravity_eval_streamed(d_x, d_c, pin(q.first), pin(q.count), pin(q.pp_off), pin(q.pp_idx), pin(q.pc_off),
+                              pin(q.pc_idx), p.eps, out, n_streams=2, max_entries_per_chunk=20000, flags=binding.VALIDATE)
+    st = ctx.get_stats(check=False)
+    assert st["invalid_values"] == 3 and st["invalid_pairs"] == int(p.count[b])
+
+
+def test_eps_zero_is_newtonian(ctx, torch, cfg1):
+    """eps = 0: pure Newtonian pairs in both kernels (no pair of config 1 is closer than 1e-12)."""
+    import copy
+    from paper_1609_08621_b200 import binding
+    from gpu_util import rel_errors, run_resident
+    p = copy.copy(cfg1); p.eps = 0.0
+    ref = _oracle(p)
+    for fl in (0, binding.FIXUP_ALL):
+        out = run_resident(ctx, p, torch, flags=fl)
+        ea, ep = rel_errors(out, ref)
+        assert ea.max() <= TOL and ep.max() <= TOL, (fl, ea.max(), ep.max())
+
+
+def test_range_call_and_host_range_keep_other_rows(ctx, torch, cfg1):
+    """pkdg_gravity_eval_range / pkdg_gravity_eval_host_range: buckets [b0, b1) over the FULL bucket arrays, lists
+    of the range only; rows outside the range keep their values; leaf references stay global."""
+    from paper_1609_08621_b200 import binding, shard
+    from gpu_util import run_resident, to_dev
+    p = cfg1
+    base = run_resident(ctx, p, torch)
+    q = _leaf_problem(p)
+    base_l = run_resident(ctx, q, torch, flags=binding.PP_LEAVES)
+    d = to_dev(p, torch)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for prob, ref, fl in ((p, base, 0), (q, base_l, binding.PP_LEAVES)):
+        out = torch.full((p.n, 4), -7.0, dtype=torch.float32, device="cuda")
+        out_h = np.full((p.n, 4), -7.0, np.float32)
+        seen = np.zeros(p.n, bool)
+        for r in range(3):
+            pc = shard.rank_piece(prob, r, 3, pp_weights=p.count[prob.pp_idx] if fl else None)
+            ctx.gravity_eval_range(d["xyzm"], d["cells"], d["first"], d["count"], pc.b0, pc.b1, t(pc.pp_off), t(pc.pp_idx),
+                                   t(pc.pc_off), t(pc.pc_idx), p.eps, out, flags=fl)
+            torch.cuda.synchronize()
+            assert ctx.get_stats()["n_buckets"] == pc.n_buckets
+            ctx.gravity_eval_host_range(p.xyzm, p.cells, p.first, p.count, pc.b0, pc.b1, pc.pp_off,
+                                        np.ascontiguousarray(pc.pp_idx), pc.pc_off, np.ascontiguousarray(pc.pc_idx), p.eps,
+                                        out_h, n_streams=2, max_entries_per_chunk=30000, flags=fl)
+            seen[shard.rank_rows(p.first, p.count, pc.b0, pc.b1)] = True
+            got = out.cpu().numpy()
+            for o in (got, out_h):
+                assert np.array_equal(o[seen], ref[seen]) and np.all(o[~seen] == -7.0), r
+        assert seen.all()
+
+
+def _group_problem(p, gmax=64):
+    """Group-shared lists of problem p (reading A6 with the group cell as the sink) + the per-bucket lists they
+    stand for (pure indexing), which is what the oracle evaluates."""
+    import copy
+    from paper_1609_08621_b200 import inputs
+    gc, gf, gn = inputs.build_groups(p, gmax)
+    ppo, ppi, pco, pci = inputs.build_group_lists(p, gc, p.theta, p.eps)
+    q = copy.copy(p)
+    q.pp_off, q.pp_idx = inputs.expand_groups(gf, gn, ppo, ppi)
+    q.pc_off, q.pc_idx = inputs.expand_groups(gf, gn, pco, pci)
+    return (gf, gn, ppo, ppi, pco, pci), q
+
+
+def test_group_shared_lists(ctx, torch, cfg1):
+    """SURVEY.md sec 8(f) NEXT-1 / PAPER.md:L69: one P-P and one P-C list per group of <= 64 particles.  The
+    library's result on group lists equals the oracle's on the expanded per-bucket lists; counters count
+    sink x entry interactions of the expanded lists; the all-host call gives the same bits; leaf-form P-P
+    entries work with groups; groups that do not tile the buckets are rejected / reported."""
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for p in (cfg1, inputs.config2(n=1 << 15), inputs.config3(32)):
+        (gf, gn, ppo, ppi, pco, pci), q = _group_problem(p)
+        assert gn.sum() == p.n_buckets and (ppo.shape[0] - 1) * 2 < p.n_buckets
+        ref = _oracle(q)
+        d = dict(xyzm=t(p.xyzm), cells=t(p.cells), first=t(p.first), count=t(p.count))
+        for fl in MODES:
+            out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda")
+            ctx.gravity_eval_groups(d["xyzm"], d["cells"], d["first"], d["count"], t(gf), t(gn), t(ppo), t(ppi), t(pco),
+                                    t(pci), p.eps, out, flags=fl)
+            torch.cuda.synchronize()
+            st = ctx.get_stats()
+            assert st["interactions_pp"] == q.I_pp and st["interactions_pc"] == q.I_pc and st["bad_entries"] == 0
+            assert st["tiles_pp"] == int((((np.diff(ppo) + 31) // 32) * gn).sum())
+            ea, ep = rel_errors(out.cpu().numpy(), ref)
+            assert ea.max() <= TOL and ep.max() <= TOL, (p.name, fl, ea.max(), ep.max())
+        base = out.cpu().numpy() if fl == MODES[-1] else None
+        out0 = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda")
+        ctx.gravity_eval_groups(d["xyzm"], d["cells"], d["first"], d["count"], t(gf), t(gn), t(ppo), t(ppi), t(pco), t(pci),
+                                p.eps, out0)
+        torch.cuda.synchronize()
+        base = out0.cpu().numpy()
+        # all-host call, chunks are ranges of groups
+        out_h = np.full((p.n, 4), np.nan, np.float32)
+        ctx.gravity_eval_host_groups(p.xyzm, p.cells, p.first, p.count, gf, gn, ppo, ppi, pco, pci, p.eps, out_h,
+                                     n_streams=3, max_entries_per_chunk=20000)
+        assert np.array_equal(out_h, base) and ctx.get_stats()["chunks"] > 1
+        # leaf-form P-P entries (bucket references) with groups
+        lo, li = inputs.pp_leaves(p.n, p.first, p.count, ppo, ppi)
+        outl = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda")
+        ctx.gravity_eval_groups(d["xyzm"], d["cells"], d["first"], d["count"], t(gf), t(gn), t(lo), t(li), t(pco), t(pci),
+                                p.eps, outl, flags=binding.PP_LEAVES)
+        torch.cuda.synchronize()
+        st = ctx.get_stats()
+        assert st["interactions_pp"] == q.I_pp and st["bad_entries"] == 0
+        ea, ep = rel_errors(outl.cpu().numpy(), ref)
+        assert ea.max() <= TOL and ep.max() <= TOL, (p.name, "leaves", ea.max(), ep.max())
+        out_h = np.full((p.n, 4), np.nan, np.float32)
+        ctx.gravity_eval_host_groups(p.xyzm, p.cells, p.first, p.count, gf, gn, lo, li, pco, pci, p.eps, out_h,
+                                     n_streams=2, max_entries_per_chunk=5000, flags=binding.PP_LEAVES)
+        assert np.array_equal(out_h, outl.cpu().numpy())
+    # groups that do not tile the buckets
+    p = cfg1
+    (gf, gn, ppo, ppi, pco, pci), q = _group_problem(p)
+    bad_gn = gn.copy(); bad_gn[3] += 1
+    out = torch.zeros((p.n, 4), dtype=torch.float32, device="cuda")
+    ctx.gravity_eval_groups(t(p.xyzm), t(p.cells), t(p.first), t(p.count), t(gf), t(bad_gn), t(ppo), t(ppi), t(pco), t(pci),
+                            p.eps, out)
+    torch.cuda.synchronize()
     assert ctx.get_stats(check=False)["bad_entries"] > 0
     with pytest.raises(binding.PkdgError):
-        run_resident(ctx, q, torch, flags=binding.PP_LEAVES | (1 << 8))
-
-
-def test_probes_report_sane_rates(ctx, torch):
-    """pkdg_fma_probe: the operand-pattern probes behind DESIGN.md sec 6 run and order as documented
-    (constant-operand FFMA near the FMA peak; three-register FFMA and FFMA2 well below it; FFMA2 with
-    a reused operand in between; the packed P-C body above the scalar one)."""
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
-    clock_ghz = torch.cuda.get_device_properties(0).clock_rate / 1e6 if hasattr(torch.cuda.get_device_properties(0), "clock_rate") else 1.965
-    peak = sms * 128 * 2 * clock_ghz / 1e3                       # Tflop/s
-    rate = {}
-    for mode in range(6):
-        ms, fl = ctx.fma_probe(mode, 1 << 11)
-        assert ms > 0 and fl > 0
-        rate[mode] = fl / ms / 1e9
-    assert 0.8 * peak < rate[0] < 1.05 * peak, (rate, peak)
-    assert rate[1] < 0.75 * rate[0] and rate[2] < 0.8 * rate[0]      # register-file bandwidth
-    assert rate[3] > rate[2] * 1.2                                   # operand reuse lifts FFMA2
-    assert rate[5] > rate[4] * 1.1                                   # packed P-C body beats the scalar one
-    with pytest.raises(Exception):
-        ctx.fma_probe(17, 16)
+        ctx.gravity_eval_host_groups(p.xyzm, p.cells, p.first, p.count, gf, bad_gn, ppo, ppi, pco, pci, p.eps,
+                                     np.zeros((p.n, 4), np.float32))

@@ -473,3 +473,20 @@ def test_contribution_norms_diagnostic():
     ref = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
     S = oracle.contribution_norms(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
     assert (S >= np.linalg.norm(ref[:, :3], axis=1) * (1 - 1e-12)).all()
+
+
+def test_contribution_norms_squared_diagnostic():
+    """S2_i = sum_j |a_ij|^2: two sources -> |a_1|^2 + |a_2|^2 in closed form; S2 <= S^2 <= n S2 (Cauchy-Schwarz)."""
+    xyzm = np.array([[0.5, 0.5, 0.5, 1.0], [0.7, 0.5, 0.5, 2.0], [0.5, 0.25, 0.5, 3.0]], np.float32)
+    first = np.array([0], np.int32); count = np.array([1], np.int32)
+    z = np.zeros(2, np.int64); e = np.zeros(0, np.int32)
+    off = np.array([0, 2], np.int64); ii = np.array([1, 2], np.int32)
+    S2 = oracle.contribution_norms(xyzm, None, first, count, off, ii, z, e, 0.0, squared=True)
+    d1 = np.float64(np.float32(0.7)) - 0.5
+    want = (2.0 / d1 ** 2) ** 2 + (3.0 / 0.25 ** 2) ** 2
+    assert abs(S2[0] - want) < 1e-12 * want and np.isnan(S2[1:]).all()
+    p = inputs.config1(512, seed=5)
+    args = (p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
+    S = oracle.contribution_norms(*args); S2 = oracle.contribution_norms(*args, squared=True)
+    n = np.repeat(np.diff(p.pp_off) + np.diff(p.pc_off), p.count)
+    assert (S2 <= S ** 2 * (1 + 1e-12)).all() and (S ** 2 <= n * S2 * (1 + 1e-12)).all()

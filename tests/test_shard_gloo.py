@@ -1,8 +1,9 @@
 """-m "not gpu": the multi-GPU path's host logic on CPU, world_size 2, gloo.
 
-Each rank cuts the bucket range with shard.shard_bounds, slices the CSR lists, evaluates ITS buckets
-(with the oracle standing in for the device call -- this tests the sharding, not the kernels) and the
-ranks' disjoint output rows are summed with an all-reduce; the result must equal the unsharded one.
+Rank 0 owns the problem; multigpu.distribute (the function bench.py --gpus N calls) broadcasts it and gives
+each rank its shard.rank_piece; every rank evaluates ITS buckets (with the oracle standing in for the device
+call -- this tests the sharding, not the kernels) and the ranks' disjoint output rows are summed with an
+all-reduce; the result must equal the unsharded one bit for bit.
 """
 import os
 import socket
@@ -28,22 +29,27 @@ def _worker(rank, world, port, ret):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         import oracle
-        from paper_1609_08621_b200 import inputs, shard
-        p = inputs.config1(2048, seed=11)
-        cost = shard.bucket_cost(p.count, p.pp_off, p.pc_off)
-        bounds = shard.shard_bounds(cost, world)
-        # every rank must derive the same cut
-        tb = torch.from_numpy(bounds.copy())
+        from paper_1609_08621_b200 import inputs, multigpu, shard
+        ref_p = inputs.config1(2048, seed=11)                     # what rank 0 owns (built everywhere only to compare)
+        # the function bench.py --gpus N calls: rank 0's arrays are broadcast, every rank takes its piece
+        g, piece = multigpu.distribute(ref_p if rank == 0 else None, dist, rank, world, "cpu", torch)
+        for k in ("xyzm", "cells", "first", "count", "pp_off", "pp_idx", "pc_off", "pc_idx"):
+            assert np.array_equal(getattr(g, k).numpy(), getattr(ref_p, k)), k   # the broadcast delivered rank 0's bits
+        assert g.eps == ref_p.eps
+        # every rank derives the same cut
+        tb = torch.from_numpy(piece.bounds.copy())
         tmax = tb.clone(); tmin = tb.clone()
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX); dist.all_reduce(tmin, op=dist.ReduceOp.MIN)
         assert torch.equal(tmax, tmin)
-        b0, b1 = int(bounds[rank]), int(bounds[rank + 1])
-        first, count, ppo, ppi, pco, pci = shard.slice_problem(p.first, p.count, p.pp_off, p.pp_idx, p.pc_off,
-                                                               p.pc_idx, b0, b1)
-        assert ppo[0] == 0 and pco[0] == 0 and ppo[-1] == ppi.shape[0] and pco[-1] == pci.shape[0]
-        part = oracle.gravity_eval(p.xyzm, p.cells, first, count, ppo, ppi, pco, pci, p.eps)
-        rows = shard.rank_rows(p.first, p.count, b0, b1)
-        mask = np.zeros(p.n, bool); mask[rows] = True
+        b0, b1 = piece.b0, piece.b1
+        ppi, pci = piece.pp_idx.numpy(), piece.pc_idx.numpy()
+        assert piece.pp_off[0] == 0 and piece.pc_off[0] == 0 and piece.pp_off[-1] == ppi.shape[0] and piece.pc_off[-1] == pci.shape[0]
+        assert np.array_equal(piece.d_pp_off.numpy(), piece.pp_off) and np.array_equal(piece.d_pc_off.numpy(), piece.pc_off)
+        # the oracle stands in for the device call (this tests the sharding, not the kernels)
+        part = oracle.gravity_eval(g.xyzm.numpy(), g.cells.numpy(), piece.first, piece.count, piece.pp_off, ppi, piece.pc_off,
+                                   pci, g.eps)
+        rows = shard.rank_rows(g.first.numpy(), g.count.numpy(), b0, b1)
+        mask = np.zeros(ref_p.n, bool); mask[rows] = True
         assert np.all(np.isnan(part[~mask])) and np.all(np.isfinite(part[mask]))   # writes only its own rows
         part = np.where(mask[:, None], part, 0.0)
         owned = torch.from_numpy(mask.astype(np.int64))
@@ -51,10 +57,19 @@ def _worker(rank, world, port, ret):
         assert int(owned.min()) == 1 and int(owned.max()) == 1  # disjoint and complete
         tot = torch.from_numpy(part.copy())
         dist.all_reduce(tot)
+        p = ref_p
         full = oracle.gravity_eval(p.xyzm, p.cells, p.first, p.count, p.pp_off, p.pp_idx, p.pc_off, p.pc_idx, p.eps)
         assert np.array_equal(tot.numpy(), full)               # same per-bucket arithmetic, bit for bit
-        share = float(cost[b0:b1].sum()) / float(cost.sum())
+        share = piece.cost / piece.cost_total
         assert abs(share - 1.0 / world) < 0.02, share
+        # leaf-form P-P lists: references stay GLOBAL bucket indices in a piece; the cost model weighs them
+        lo, li = inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+        import copy
+        q = copy.copy(p); q.pp_off, q.pp_idx = lo, li
+        lp = shard.rank_piece(q, rank, world, pp_weights=p.count[li])
+        assert np.array_equal(lp.bounds, piece.bounds)          # same cut as with particle lists
+        eo, ei = inputs.expand_leaves(p.first, p.count, lp.pp_off, lp.pp_idx)
+        assert np.array_equal(eo, piece.pp_off) and np.array_equal(ei, ppi)
         ret[rank] = (b0, b1, share)
     finally:
         dist.destroy_process_group()
