@@ -365,6 +365,119 @@ def run_ours(args, rank, world, local_rank):
             del h, out_h
         del d_lo, d_li
 
+    # ---- group-shared lists (g = 64) with leaf-form P-P entries: extra key, N = 1
+    groups = None
+    if not args.no_groups and world == 1:
+        from paper_1609_08621_b200 import inputs as _inputs
+        t0 = time.perf_counter()
+        gc_, gf, gn = _inputs.build_groups(p, 64)
+        gppo, gppi, gpco, gpci = _inputs.build_group_lists(p, gc_, p.theta, p.eps)
+        glo, gli = _inputs.pp_leaves(p.n, p.first, p.count, gppo, gppi)
+        g_gen = time.perf_counter() - t0
+        gI_pp = int(np.dot(np.add.reduceat(p.count.astype(np.int64), gf), np.diff(gppo)))
+        gI_pc = int(np.dot(np.add.reduceat(p.count.astype(np.int64), gf), np.diff(gpco)))
+        gflags = flags | binding.PP_LEAVES
+        T = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        dg = dict(gf=T(gf), gn=T(gn), lo=T(glo), li=T(gli), co=T(gpco), ci=T(gpci))
+
+        def gstep():
+            ctx.gravity_eval_groups(g.xyzm, g.cells, g.first, g.count, dg["gf"], dg["gn"], dg["lo"], dg["li"], dg["co"],
+                                    dg["ci"], g.eps, out, flags=gflags)
+        for _ in range(3):
+            gstep()
+        barrier()
+        ctx.profile_read(); ctx.profile_enable(True)
+        gms = timed(gstep, args.steps)
+        gn_, gk, gfx = ctx.profile_read(); ctx.profile_enable(False)
+        gst = ctx.get_stats()
+        assert gst["interactions_pp"] == gI_pp and gst["interactions_pc"] == gI_pc and gst["bad_entries"] == 0
+        ginter = gI_pp + gI_pc
+        groups = {"n_groups": int(gf.shape[0]), "mean_buckets_per_group": float(gn.mean()),
+                  "mean_L_pp_particles": gI_pp / p.n, "mean_L_pc": gI_pc / p.n, "I_pp": gI_pp, "I_pc": gI_pc,
+                  "list_entries": int(gli.shape[0] + gpci.shape[0]),
+                  "list_entries_per_bucket_lists": int(p.pp_idx.shape[0] + p.pc_idx.shape[0]),
+                  "value": ginter / (gms * 1e-3), "unit": "interactions/s", "ms_per_step": gms, "kernel_ms": gk / max(gn_, 1),
+                  "fixup_sinks": gst["fixup_sinks"], "host_list_build_s": round(g_gen, 1),
+                  "frac_fp32_fma_peak_kernel": None,
+                  "note": "one P-P (bucket references) and one P-C list per group of <= 64 particles; every sink of the group "
+                          "evaluates the whole list, so there are more interactions per sink than with per-bucket lists"}
+        if not args.no_e2e:
+            P_ = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+            h = dict(xyzm=pin(g.xyzm), cells=pin(g.cells), first=pin(g.first), count=pin(g.count), gf=P_(gf), gn=P_(gn),
+                     lo=P_(glo), li=P_(gli), co=P_(gpco), ci=P_(gpci))
+            out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+
+            def ge2e():
+                ctx.gravity_eval_host_groups(h["xyzm"], h["cells"], h["first"], h["count"], h["gf"], h["gn"], h["lo"], h["li"],
+                                             h["co"], h["ci"], g.eps, out_h, n_streams=args.e2e_streams,
+                                             max_entries_per_chunk=max(1, args.e2e_chunk // 8), flags=gflags)
+            for _ in range(2):
+                ge2e()
+            barrier()
+            k2 = max(2, min(args.steps, 5))
+            t0 = time.perf_counter()
+            for _ in range(k2):
+                ge2e()
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) / k2
+            groups["e2e"] = {"value": ginter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3,
+                             "sinks_per_s": p.n / dt,
+                             "h2d_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in h.values()),
+                             "d2h_bytes_per_step": int(out_h.numel() * 4)}
+            del h, out_h
+        del dg
+
+    # ---- list construction on the device: walk time, and the end-to-end time it gives when
+    #      particles, cells and the tree (not the lists) cross PCIe.  Extra key, N = 1.
+    devlists = None
+    if not args.no_device_lists and world == 1:
+        tr = p.tree
+        T = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        tree_h = {k: torch.from_numpy(np.ascontiguousarray(tr[k])).pin_memory() for k in ("first", "count", "end", "isleaf", "bblo", "bbhi")}
+        sink_h = torch.from_numpy(np.ascontiguousarray(tr["leaf_cell"].astype(np.int32))).pin_memory()
+        xy_h, ce_h = pin(g.xyzm), pin(g.cells)
+        fb_h, cb_h = pin(g.first), pin(g.count)
+        out_h = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+        nb_ = p.n_buckets
+        d_ppo = torch.empty(nb_ + 1, dtype=torch.int64, device=dev); d_pco = torch.empty(nb_ + 1, dtype=torch.int64, device=dev)
+        d_ppi = torch.empty(p.pp_idx.shape[0], dtype=torch.int32, device=dev)
+        d_pci = torch.empty(p.pc_idx.shape[0], dtype=torch.int32, device=dev)
+        tree_d = {k: v.to(dev) for k, v in tree_h.items()}
+        sink_d = sink_h.to(dev)
+
+        def walk():
+            npp, npc = ctx.build_lists_count(tree_d, g.cells, sink_d, p.theta, p.eps, d_ppo, d_pco)
+            assert npp == p.pp_idx.shape[0] and npc == p.pc_idx.shape[0]
+            ctx.build_lists_fill(tree_d, g.cells, sink_d, p.theta, p.eps, d_ppo, d_pco, d_ppi, d_pci)
+        for _ in range(2):
+            walk()
+        walk_ms = timed(walk, max(3, args.steps // 2))
+        same = bool(torch.equal(d_ppi, g.pp_idx) and torch.equal(d_pci, g.pc_idx) and torch.equal(d_ppo, g.pp_off))
+
+        def dl_e2e():
+            x = xy_h.to(dev, non_blocking=True); c = ce_h.to(dev, non_blocking=True)
+            td = {k: v.to(dev, non_blocking=True) for k, v in tree_h.items()}
+            sk = sink_h.to(dev, non_blocking=True); fb = fb_h.to(dev, non_blocking=True); cb = cb_h.to(dev, non_blocking=True)
+            ctx.build_lists_count(td, c, sk, p.theta, p.eps, d_ppo, d_pco)
+            ctx.build_lists_fill(td, c, sk, p.theta, p.eps, d_ppo, d_pco, d_ppi, d_pci)
+            ctx.gravity_eval(x, c, fb, cb, d_ppo, d_ppi, d_pco, d_pci, g.eps, out, flags=flags)
+            out_h.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        for _ in range(2):
+            dl_e2e()
+        k2 = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            dl_e2e()
+        dt = (time.perf_counter() - t0) / k2
+        h2d = sum(int(v.numel() * v.element_size()) for v in list(tree_h.values()) + [sink_h, xy_h, ce_h, fb_h, cb_h])
+        devlists = {"walk_ms": walk_ms, "bit_identical_to_host_generator": same,
+                    "list_entries": int(p.pp_idx.shape[0] + p.pc_idx.shape[0]),
+                    "e2e": {"value": inter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3, "h2d_bytes_per_step": h2d,
+                            "d2h_bytes_per_step": int(out_h.numel() * 4),
+                            "api": "H2D of particles, cells, tree; pkdg_build_lists_count + _fill; pkdg_gravity_eval; D2H"}}
+        del tree_d, sink_d, d_ppo, d_pco, d_ppi, d_pci, out_h
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -406,7 +519,10 @@ def run_ours(args, rank, world, local_rank):
             "flops_per_s": flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / (peak_tflops * world),
             "paper_convention_tflops": (PAPER_F_PP * tot_pp + PAPER_F_PC * tot_pc) / (ms_step * 1e-3) / 1e12,
             "interactions_per_s": {"pp": tot_pp / (ms_step * 1e-3), "pc": tot_pc / (ms_step * 1e-3)},
-            "gen_seconds": round(gen_s, 1), "flags": args.flags, "pp_leaves": leaves}
+            "gen_seconds": round(gen_s, 1), "flags": args.flags, "pp_leaves": leaves, "group_lists": groups,
+            "device_lists": devlists}
+    if groups is not None:
+        groups["frac_fp32_fma_peak_kernel"] = (F_PP * groups["I_pp"] + F_PC * groups["I_pc"]) / (groups["kernel_ms"] * 1e-3) / 1e12 / peak_tflops
     if leaves is not None:
         leaves["frac_fp32_fma_peak_kernel"] = flops / (leaves["kernel_ms"] * 1e-3) / 1e12 / peak_tflops
     print(json.dumps(line), flush=True)
@@ -640,6 +756,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-leaves", action="store_true", help="skip the extra PKDG_PP_LEAVES measurement")
+    ap.add_argument("--no-groups", action="store_true", help="skip the extra group-shared-lists measurement")
+    ap.add_argument("--no-device-lists", action="store_true", help="skip the extra device list-construction measurement")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-chunk", type=int, default=1 << 23)

@@ -209,6 +209,36 @@ pkdg_status pkdg_gravity_eval_host_range(pkdg_ctx *ctx, const pkdg_particles *pa
                                          float *out_acc_pot_host, int32_t n_streams,
                                          int64_t max_entries_per_chunk);
 
+/* List construction on the device.  The tree as the walk needs it, all arrays on
+ * the device, cells in depth-first pre-order ("hierarchically sorted"): cell k's subtree is
+ * cells [k, end[k]), its first child is k + 1; first / count = its particle run; isleaf != 0 marks a bucket;
+ * bblo / bbhi = [n_cells][3] bounding boxes of the fp32 coordinates; the centre of mass and
+ * b_max come from the canonical cell records.  leaf_rank (may be NULL) = [n_cells], bucket index of a leaf. */
+typedef struct {
+    const int32_t *first, *count, *end, *isleaf;
+    const float *bblo, *bbhi;
+    const int32_t *leaf_rank;
+    int64_t n_cells;
+} pkdg_tree;
+
+/* The tree walk that resolves a sink cell's checklist into its P-P and P-C list (the
+ * acceptance test is DESIGN.md reading A6: cell k is a P-C source for sink B iff k != B, it holds >= 2
+ * particles, |COM_B - COM_k| > b_max,B + b_max,k / theta and the bounding boxes are >= 2 eps apart; a leaf
+ * that fails joins the P-P list whole; any other cell is opened).  sink_cell[n_sinks] names the sink cells:
+ * the leaf cells for per-bucket lists, the group cells for group-shared lists.  Two calls, because the caller
+ * owns the index arrays: _count writes the CSR offsets (n_sinks + 1 each, device) and returns the two totals
+ * in totals_host[2] (synchronises; NULL = stay asynchronous); _fill writes the entries, in walk order.  With
+ * PKDG_PP_LEAVES a P-P entry is the bucket index of the leaf instead of its particles.  Decisions are taken in
+ * fp64 with IEEE operations and no contraction: offsets and indices are bit-identical to a host walk. */
+pkdg_status pkdg_build_lists_count(pkdg_ctx *ctx, const pkdg_tree *tree, const pkdg_cells *cells,
+                                   const int32_t *sink_cell, int64_t n_sinks, double theta, double eps,
+                                   uint32_t flags, int64_t *pp_offsets, int64_t *pc_offsets,
+                                   int64_t *totals_host, void *stream);
+pkdg_status pkdg_build_lists_fill(pkdg_ctx *ctx, const pkdg_tree *tree, const pkdg_cells *cells,
+                                  const int32_t *sink_cell, int64_t n_sinks, double theta, double eps,
+                                  uint32_t flags, const int64_t *pp_offsets, const int64_t *pc_offsets,
+                                  int32_t *pp_idx, int32_t *pc_idx, void *stream);
+
 /* Packer made visible for bit-exact checks (SURVEY.md sec 8(c) "Integer side"): the tiles the
  * evaluation kernel consumes.  tile_offsets = [n_buckets+1] int64 (first tile of each bucket);
  * tiles = [tile_capacity][32] int32, list order, last tile of a bucket padded with PKDG_PAD.

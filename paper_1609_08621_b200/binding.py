@@ -30,7 +30,7 @@ CELLQ_FLOATS = 32
 
 EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_gravity_eval_host_range", "pkdg_gravity_eval_groups",
-           "pkdg_gravity_eval_host_groups", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
+           "pkdg_gravity_eval_host_groups", "pkdg_build_lists_count", "pkdg_build_lists_fill", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
            "pkdg_get_stats", "pkdg_set_option", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count",
            "pkdg_status_string", "pkdg_last_error", "pkdg_version", "pkdg_fma_peak_probe"]
 
@@ -53,6 +53,11 @@ class _Buckets(Structure):
 
 class _Groups(Structure):
     _fields_ = [("first_bucket", c_void_p), ("n_buckets", c_void_p), ("n", c_int64)]
+
+
+class _Tree(Structure):
+    _fields_ = [("first", c_void_p), ("count", c_void_p), ("end", c_void_p), ("isleaf", c_void_p), ("bblo", c_void_p),
+                ("bbhi", c_void_p), ("leaf_rank", c_void_p), ("n_cells", c_int64)]
 
 
 class _List(Structure):
@@ -95,6 +100,10 @@ def _load():
     L.pkdg_gravity_eval_host_groups.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                                 POINTER(_Groups), POINTER(_List), POINTER(_List), c_float, c_uint32,
                                                 c_void_p, c_int32, c_int64]
+    L.pkdg_build_lists_count.argtypes = [c_void_p, POINTER(_Tree), POINTER(_Cells), c_void_p, c_int64, c_double, c_double,
+                                         c_uint32, c_void_p, c_void_p, c_void_p, c_void_p]
+    L.pkdg_build_lists_fill.argtypes = [c_void_p, POINTER(_Tree), POINTER(_Cells), c_void_p, c_int64, c_double, c_double,
+                                        c_uint32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     L.pkdg_pack_export.argtypes = [c_void_p, c_int64, POINTER(_List), c_void_p, c_void_p, c_int64, c_void_p]
     L.pkdg_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int64)]
     L.pkdg_prepare_cells_export.argtypes = [c_void_p, POINTER(_Cells), c_void_p, c_void_p]
@@ -286,6 +295,38 @@ class Context:
                                                int(flags), _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
         self._check(s, "pkdg_gravity_eval_host_groups")
         return out_h
+
+    @staticmethod
+    def _tree(tree, cells):
+        """tree: dict of device tensors first, count, end, isleaf (int32), bblo, bbhi (float32 [n,3]) and
+        optionally leaf_rank (int32)."""
+        for k in ("first", "count", "end", "isleaf"):
+            _dt(tree[k], "int32", k)
+        _dt(tree["bblo"], "float32", "bblo"); _dt(tree["bbhi"], "float32", "bbhi"); _dt(cells, "float32", "cells")
+        T = _Tree(_ptr(tree["first"]), _ptr(tree["count"]), _ptr(tree["end"]), _ptr(tree["isleaf"]), _ptr(tree["bblo"]),
+                  _ptr(tree["bbhi"]), _ptr(tree.get("leaf_rank")), int(tree["first"].shape[0]))
+        C = _Cells(_ptr(cells), int(cells.shape[0]), int(cells.shape[1]))
+        return T, C
+
+    def build_lists_count(self, tree, cells, sink_cell, theta, eps, pp_off, pc_off, flags=0, stream=None, sync=True):
+        """pkdg_build_lists_count: CSR offsets (device int64 [n_sinks + 1] each); returns (n_pp, n_pc) if sync."""
+        T, C = self._tree(tree, cells)
+        _dt(sink_cell, "int32", "sink_cell"); _dt(pp_off, "int64", "pp_off"); _dt(pc_off, "int64", "pc_off")
+        tot = (c_int64 * 2)()
+        s = _lib.pkdg_build_lists_count(self._h, byref(T), byref(C), _ptr(sink_cell), int(sink_cell.shape[0]),
+                                        float(theta), float(eps), int(flags), _ptr(pp_off), _ptr(pc_off),
+                                        ctypes.cast(tot, c_void_p) if sync else None, _stream_ptr(stream))
+        self._check(s, "pkdg_build_lists_count")
+        return (int(tot[0]), int(tot[1])) if sync else None
+
+    def build_lists_fill(self, tree, cells, sink_cell, theta, eps, pp_off, pc_off, pp_idx, pc_idx, flags=0, stream=None):
+        """pkdg_build_lists_fill: the entries, in walk order, at the offsets build_lists_count wrote."""
+        T, C = self._tree(tree, cells)
+        _dt(pp_idx, "int32", "pp_idx"); _dt(pc_idx, "int32", "pc_idx")
+        s = _lib.pkdg_build_lists_fill(self._h, byref(T), byref(C), _ptr(sink_cell), int(sink_cell.shape[0]),
+                                       float(theta), float(eps), int(flags), _ptr(pp_off), _ptr(pc_off), _ptr(pp_idx),
+                                       _ptr(pc_idx), _stream_ptr(stream))
+        self._check(s, "pkdg_build_lists_fill")
 
     def pack_export(self, n_buckets, off, idx, tile_offsets, tiles, stream=None):
         """pkdg_pack_export: tile_offsets[n_buckets+1] int64 and tiles[cap,32] int32 (device)."""

@@ -190,11 +190,10 @@ int64_t fix_capacity(int64_t n_buckets, int64_t n_particles) { return n_buckets 
 // (the queue length is known only on the device); with an empty queue every warp leaves at once.
 pkdg_status launch_fixup(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     if (p.fix_k < 0.0f) return PKDG_OK;
-    int64_t warps = p.n_buckets < 1 ? 1 : p.n_buckets;
-    int64_t grid = (warps + 3) / 4;
-    const int64_t full = (int64_t)ctx->num_sms * 8;
+    int64_t grid = p.n_buckets < 1 ? 1 : p.n_buckets;   // one CTA per queue entry, persistent beyond 16 per SM
+    const int64_t full = (int64_t)ctx->num_sms * 16;
     if (grid > full) grid = full;
-    pkdg_fixup_kernel<<<(unsigned)grid, 128, 0, st>>>(p);
+    pkdg_fixup_kernel<<<(unsigned)grid, kFixThreads, 0, st>>>(p);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -667,6 +666,84 @@ pkdg_status pkdg_pack_export(pkdg_ctx* ctx, int64_t n_buckets, const pkdg_list* 
                                                             tile_capacity);
         ctx->launches++;
     }
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+// Exclusive scan of v[0 .. n) in place, total at v[n] (device).
+static pkdg_status device_scan(pkdg_ctx* ctx, int64_t* v, int64_t n, cudaStream_t st) {
+    const int64_t per = (int64_t)kScanBlock * kScanItems;
+    const int64_t nblk = n > 0 ? (n + per - 1) / per : 1;
+    pkdg_status s = ensure(ctx, &ctx->scan_tmp, &ctx->scan_cap, nblk + 1);
+    if (s != PKDG_OK) return s;
+    pkdg_scan_blocks_kernel<<<(unsigned)nblk, kScanBlock, 0, st>>>(v, n, ctx->scan_tmp);
+    pkdg_scan_kernel<<<1, 1024, 0, st>>>(ctx->scan_tmp, nblk);
+    pkdg_scan_add_kernel<<<(unsigned)((n + 1 + 255) / 256), 256, 0, st>>>(v, n, ctx->scan_tmp, nblk);
+    ctx->launches += 3;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+static pkdg_status check_tree(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_cells* C, const int32_t* sink_cell,
+                              int64_t n_sinks, double theta) {
+    if (!ctx) return PKDG_EINVAL;
+    if (!T || !C || !T->first || !T->count || !T->end || !T->isleaf || !T->bblo || !T->bbhi || !C->rec)
+        return fail(ctx, PKDG_EINVAL, "tree arrays and cell records must not be NULL");
+    if (T->n_cells < 0 || T->n_cells != C->n || C->stride_floats < PKDG_CELL_FLOATS || T->n_cells > 0x7fffffffLL)
+        return fail(ctx, PKDG_EINVAL, "tree->n_cells must equal cells->n; stride_floats >= 36");
+    if (n_sinks < 0 || (n_sinks > 0 && !sink_cell)) return fail(ctx, PKDG_EINVAL, "sink_cell is NULL or n_sinks < 0");
+    if (!(theta > 0.0)) return fail(ctx, PKDG_EINVAL, "theta must be > 0");
+    return PKDG_OK;
+}
+
+static TreeView tree_view(const pkdg_tree* T, const pkdg_cells* C, bool leaves) {
+    TreeView v;
+    v.first = T->first; v.count = T->count; v.end = T->end; v.isleaf = T->isleaf;
+    v.bblo = T->bblo; v.bbhi = T->bbhi; v.rec = C->rec; v.stride = C->stride_floats; v.n_cells = T->n_cells;
+    v.leaf_rank = leaves ? T->leaf_rank : nullptr;
+    return v;
+}
+
+pkdg_status pkdg_build_lists_count(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_cells* C, const int32_t* sink_cell,
+                                   int64_t n_sinks, double theta, double eps, uint32_t flags, int64_t* pp_off,
+                                   int64_t* pc_off, int64_t* totals_host, void* stream) {
+    pkdg_status s = check_tree(ctx, T, C, sink_cell, n_sinks, theta);
+    if (s != PKDG_OK) return s;
+    if (!pp_off || !pc_off) return fail(ctx, PKDG_EINVAL, "pp_offsets / pc_offsets must not be NULL");
+    if ((flags & PKDG_PP_LEAVES) && !T->leaf_rank) return fail(ctx, PKDG_EINVAL, "PKDG_PP_LEAVES needs tree->leaf_rank");
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
+    if (n_sinks > 0) {
+        pkdg_walk_kernel<false><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(v, sink_cell, n_sinks, theta, eps, pp_off,
+                                                                                   pc_off, nullptr, nullptr, nullptr, nullptr);
+        ctx->launches++;
+        CK(cudaGetLastError());
+    }
+    if ((s = device_scan(ctx, pp_off, n_sinks, st)) != PKDG_OK) return s;
+    if ((s = device_scan(ctx, pc_off, n_sinks, st)) != PKDG_OK) return s;
+    if (totals_host) {   // the caller allocates the index arrays from these: synchronous
+        CK(cudaMemcpyAsync(totals_host, pp_off + n_sinks, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(totals_host + 1, pc_off + n_sinks, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return PKDG_OK;
+}
+
+pkdg_status pkdg_build_lists_fill(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_cells* C, const int32_t* sink_cell,
+                                  int64_t n_sinks, double theta, double eps, uint32_t flags, const int64_t* pp_off,
+                                  const int64_t* pc_off, int32_t* pp_idx, int32_t* pc_idx, void* stream) {
+    pkdg_status s = check_tree(ctx, T, C, sink_cell, n_sinks, theta);
+    if (s != PKDG_OK) return s;
+    if (!pp_off || !pc_off) return fail(ctx, PKDG_EINVAL, "pp_offsets / pc_offsets must not be NULL");
+    if ((flags & PKDG_PP_LEAVES) && !T->leaf_rank) return fail(ctx, PKDG_EINVAL, "PKDG_PP_LEAVES needs tree->leaf_rank");
+    if (n_sinks == 0) return PKDG_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
+    pkdg_walk_kernel<true><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(v, sink_cell, n_sinks, theta, eps, nullptr,
+                                                                              nullptr, pp_off, pc_off, pp_idx, pc_idx);
+    ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
 }

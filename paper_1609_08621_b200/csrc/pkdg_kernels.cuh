@@ -497,38 +497,14 @@ __device__ __forceinline__ float2 f2fma(float2 a, float2 b, float2 c) { return _
 
 constexpr int kPMax = kTMax / 2;  // sink pairs per pass
 
-// The same butterfly for NV = 8 or 16 values: log2(NV) transposing rounds, then plain rounds.  Lane l ends with
-// the total of value l >> 2 (NV = 8) or l >> 1 (NV = 16) in v[0].
-template <int NV>
-__device__ __forceinline__ void warp_transpose_reduce_small(float (&v)[NV], int lane) {
-    static_assert(NV == 8 || NV == 16, "NV");
-#pragma unroll
-    for (int r = 0; r < 5; ++r) {
-        const int mask = 16 >> r, n = (NV / 2) >> r;
-        if (n >= 1) {
-            const bool up = (lane & mask) != 0;
-#pragma unroll
-            for (int i = 0; i < NV / 2; ++i) {
-                if (i < n) {
-                    const float send = up ? v[i] : v[i + n];
-                    const float keep = up ? v[i + n] : v[i];
-                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
-                }
-            }
-        } else {
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], mask);
-        }
-    }
-}
-
 struct __align__(16) WarpSmem3 {
     float4 acc[kTMax * 32];       // [pair][half][lane]: {axA, axB, ayA, ayB}, {azA, azB, phiA, phiB}
-    float2 s2[kPMax * 32];        // [pair][lane]: conditioning estimate {S2_A, S2_B}
     float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
     float4 tgt[2][kTMax];         // raw sinks (x, y, z, m) of the current / the next bucket
     float4 tp[(kPMax + 1) * 2];   // current pass, pair layout: {xA, xB, yA, yB}, {zA, zB, -, -}; +1 dummy pair
     int32_t nidx[4][32];          // tiles 0, 1 of the P-P list and tiles 0, 1 of the P-C list
     BucketDesc ndesc;             // descriptor of the next bucket
+    unsigned int bucket[2];       // index of the current / the next bucket (fix-up queue entries name it)
 };
 
 // per-lane partial sums of sink t in the pair layout, as scalars (correction path, reduction)
@@ -539,17 +515,17 @@ __device__ __forceinline__ int acc_idx(int t, int comp, int lane) {  // comp 0..
 // One source against one sink pair, Newtonian with r^2 clamped from below at h2c (so it is finite for
 // softened and coincident pairs; those are corrected afterwards, see pp_phase3).  With SELF the
 // accumulation is masked for the sink's own index (used only for tiles that hold own particles).
-// 14 packed FP instructions + 2 MUFU + min/max for 2 interactions: 19 flops per interaction for a and
-// phi + 2 for the conditioning estimate S2 (not counted as useful work).
+// 13 packed FP instructions + 2 MUFU + min/max for 2 interactions; 19 flops per interaction.  minr2 (the
+// smallest r^2 between this lane's source and any sink of the pass) also feeds the conditioning bound.
 template <bool SELF>
 __device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, const float4 s, bool selfA, bool selfB,
-                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw,
-                                         float2& s2) {
+                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw) {
     const float2 dx = f2add(make_float2(txy.x, txy.y), sp(-s.x));
     const float2 dy = f2add(make_float2(txy.z, txy.w), sp(-s.y));
     const float2 dz = f2add(make_float2(tz.x, tz.y), sp(-s.z));
     float2 r2 = f2fma(dz, dz, f2fma(dy, dy, f2mul(dx, dx)));
     const float2 ri = make_float2(rsqrt_approx(fmaxf(r2.x, h2c)), rsqrt_approx(fmaxf(r2.y, h2c)));
+    const float2 ri2 = f2mul(ri, ri);
     float2 nm = sp(-s.w);
     if (SELF) {
         nm.x = selfA ? 0.0f : nm.x; nm.y = selfB ? 0.0f : nm.y;
@@ -557,24 +533,23 @@ __device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, cons
     }
     minr2 = fminf(minr2, fminf(r2.x, r2.y));
     const float2 nmri = f2mul(nm, ri);
-    const float2 t = f2mul(nmri, ri);   // -m / r^2 = -|a_ij|
-    const float2 nmg = f2mul(t, ri);
+    const float2 nmg = f2mul(nmri, ri2);
     ax = f2fma(nmg, dx, ax);
     ay = f2fma(nmg, dy, ay);
     az = f2fma(nmg, dz, az);
     aw = f2add(aw, nmri);
-    s2 = f2fma(t, t, s2);               // conditioning estimate S2_i = sum_j |a_ij|^2
 }
 
 struct PcPre2 { float2 dx, dy, dz, ri; };
 
-__device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, const CellRegs& c) {
+__device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, const CellRegs& c, float& minr2) {
     PcPre2 q;
     q.dx = f2add(make_float2(txy.x, txy.y), sp(-c.cx));
     q.dy = f2add(make_float2(txy.z, txy.w), sp(-c.cy));
     q.dz = f2add(make_float2(tz.x, tz.y), sp(-c.cz));
     const float2 r2 = f2fma(q.dz, q.dz, f2fma(q.dy, q.dy, f2mul(q.dx, q.dx)));
     q.ri = make_float2(rsqrt_approx(r2.x), rsqrt_approx(r2.y));
+    minr2 = fminf(minr2, fminf(r2.x, r2.y));   // conditioning bound (min/max run on the ALU pipe, not the FMA pipe)
     return q;
 }
 
@@ -586,11 +561,10 @@ __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, con
 //   1 + sum (2n+1)/n e_n   = fs + 2 E4                     (radial factor S)
 // which needs no chain-start multiplies and no V2 + V3 + V4 sums, and the data dependence keeps the three
 // FFMA2 of a term (same monomial, x / y / z coefficient) adjacent, so the monomial pair is reused.
-// Per interaction: 5 FADD, 35 FMUL, 73 FFMA, 1 MUFU = 187 flops in 113 packed instructions per pair
-// (+ 1 FMUL2 + 1 FFMA2 for the conditioning estimate S2, not counted as useful work).
+// Per interaction: 5 FADD, 35 FMUL, 73 FFMA, 1 MUFU = 187 flops in 113 packed instructions per pair.
 #define PKDG_T0(CX, CY, CZ, M) vx = f2mul(sp(CX), M); vy = f2mul(sp(CY), M); vz = f2mul(sp(CZ), M);
 #define PKDG_T1(CX, CY, CZ, M) vx = f2fma(sp(CX), M, vx); vy = f2fma(sp(CY), M, vy); vz = f2fma(sp(CZ), M, vz);
-__device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1, float2& s2) {
+__device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1) {
     const float2 ri2 = f2mul(q.ri, q.ri);
     const float2 sr = f2mul(sp(c.s), ri2);
     const float2 x = f2mul(q.dx, sr), y = f2mul(q.dy, sr), z = f2mul(q.dz, sr);  // tau
@@ -615,9 +589,7 @@ __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, floa
     const float2 fs = f2fma(sp(0.25f), E4, f2fma(sp(0.083333333333f), E3, f2fma(sp(0.16666666667f), E2, sp(1.0f))));
     const float2 S = f2fma(sp(2.0f), E4, fs);
     const float2 mr = f2mul(sp(c.M), q.ri);
-    const float2 t = f2mul(mr, q.ri);   // M / r^2: the size of this cell's contribution
-    const float2 k3 = f2mul(t, q.ri);
-    s2 = f2fma(t, t, s2);
+    const float2 k3 = f2mul(mr, ri2);
     const float2 sk = f2mul(sp(c.s), k3), Sk = f2mul(S, k3);
     float2 ax = make_float2(a0.x, a0.y), ay = make_float2(a0.z, a0.w), az = make_float2(a1.x, a1.y),
            aw = make_float2(a1.z, a1.w);
@@ -684,14 +656,18 @@ __device__ __forceinline__ void make_pairs(WarpSmem3& S, int buf, int lane) {
 // at most 16), so the source gather is two contiguous runs and the list is 16 times shorter.
 template <int NP, bool LEAF>
 __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
-                                          const float4* __restrict__ s_tgt, WarpSmem3& S, int lane, unsigned& bad) {
+                                          const float4* __restrict__ s_tgt, WarpSmem3& S, int lane, unsigned& bad,
+                                          float& s2_bound) {
     const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
     const float4* __restrict__ tp = S.tp;
     float4* __restrict__ s_acc = S.acc;
     float* __restrict__ s_accf = reinterpret_cast<float*>(S.acc);
-    float2 ax[NP], ay[NP], az[NP], aw[NP], s2[NP];
+    float2 ax[NP], ay[NP], az[NP], aw[NP];
 #pragma unroll
-    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = s2[q] = make_float2(0.f, 0.f);
+    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = make_float2(0.f, 0.f);
+    // Conditioning of the P-P part: S2_i = sum_j |a_ij|^2 = sum_j m_j^2 / r_ij^4 <= sum_j m_j^2 / (min_i' r_i'j)^4, one
+    // bound for all sinks of the pass, from the minimum distance the tile loop tracks anyway.
+    float bsum = 0.0f;
     bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
     const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
     const int sink0 = d.first + t0;
@@ -742,19 +718,22 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
 #pragma unroll
             for (int q = 0; q < NP; ++q)
                 pp_fast2<true>(tp[2 * q], tp[2 * q + 1], s, self_t == 2 * q, self_t == 2 * q + 1, p.h2c, minr2, ax[q],
-                               ay[q], az[q], aw[q], s2[q]);
+                               ay[q], az[q], aw[q]);
         } else {
 #pragma unroll
             for (int q = 0; q < NP; ++q)
-                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q],
-                                s2[q]);
+                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q]);
+        }
+        {   // this lane's source pulls on no sink of the pass with more than m / max(min r^2, h^2)
+            const float ir = rsqrt_approx(fmaxf(minr2, p.h2c));
+            const float tb = s.w * ir * ir;
+            bsum = fmaf(tb, tb, bsum);
         }
         if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
             // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
             // Newtonian contribution by the spline one, through the shared accumulators.
             if (!smem_live) {
                 for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-                for (int q = 0; q < kPMax; ++q) S.s2[q * 32 + lane] = make_float2(0.f, 0.f);
                 smem_live = true;
             }
             if (minr2 < p.h2c) {
@@ -770,10 +749,10 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
                         s_accf[acc_idx(t, 1, lane)] = fmaf(-mg, dy, s_accf[acc_idx(t, 1, lane)]);
                         s_accf[acc_idx(t, 2, lane)] = fmaf(-mg, dz, s_accf[acc_idx(t, 2, lane)]);
                         s_accf[acc_idx(t, 3, lane)] = fmaf(s.w, dw, s_accf[acc_idx(t, 3, lane)]);
-                        // the fast path booked (m / h^2)^2 for this pair; a softened pair pulls with up to 2.6 m / h^2
-                        // and the correction is a difference of two terms: book (4 m / h^2)^2 in all
+                        // the bound above booked (m / h^2)^2 for this source; a softened pair pulls with up to
+                        // 2.6 m / h^2 and the correction is a difference of two terms: book (4 m / h^2)^2 in all
                         const float tc = s.w * ri * ri;
-                        reinterpret_cast<float*>(S.s2)[((t >> 1) * 32 + lane) * 2 + (t & 1)] += 15.0f * tc * tc;
+                        bsum = fmaf(15.0f * tc, tc, bsum);
                     }
                 }
             }
@@ -783,18 +762,15 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         float4 a0 = make_float4(ax[q].x, ax[q].y, ay[q].x, ay[q].y), a1 = make_float4(az[q].x, az[q].y, aw[q].x, aw[q].y);
-        float2 c2 = s2[q];
         if (smem_live) {
             const float4 b0 = s_acc[(2 * q) * 32 + lane], b1 = s_acc[(2 * q + 1) * 32 + lane];
-            const float2 d2 = S.s2[q * 32 + lane];
             a0.x += b0.x; a0.y += b0.y; a0.z += b0.z; a0.w += b0.w;
             a1.x += b1.x; a1.y += b1.y; a1.z += b1.z; a1.w += b1.w;
-            c2.x += d2.x; c2.y += d2.y;
         }
         s_acc[(2 * q) * 32 + lane] = a0;
         s_acc[(2 * q + 1) * 32 + lane] = a1;
-        S.s2[q * 32 + lane] = c2;
     }
+    s2_bound = bsum;
 }
 
 // Queue one (bucket, pass) for the fp64 fix-up kernel (warp-uniform call).  Returns false if the queue is full
@@ -826,12 +802,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
     if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
     cur = __shfl_sync(0xffffffffu, cur, 0);
     if ((int64_t)cur >= p.n_buckets) return;
+    if (lane == 0) S.bucket[0] = cur;
     BucketDesc d = p.desc[cur];
     int buf = 0;
     fill_direct3(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
 
     for (;;) {
-        unsigned nxt = 0xffffffffu, next_b = 0xffffffffu;
+        unsigned nxt = 0xffffffffu;
         if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
         bool has_next = false;
         const ListLens L = eff_lens(d, do_pp, do_pc);
@@ -858,18 +835,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
 
             // ---- a2: pair layout of the sinks;  a3: P-P
             make_pairs(S, buf, lane);
+            float s2_b = 0.0f;   // per-lane part of the conditioning bound of this pass (P-P, then P-C)
             if (pp_leaves) {
-                if (ntp <= 8) pp_phase3<4, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
-                else pp_phase3<8, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+                if (ntp <= 8) pp_phase3<4, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
+                else pp_phase3<8, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
             } else {
-                if (ntp <= 8) pp_phase3<4, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
-                else pp_phase3<8, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad);
+                if (ntp <= 8) pp_phase3<4, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
+                else pp_phase3<8, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
             }
 
             // ---- next bucket, stage 1: its descriptor
             if (last) {
                 const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
-                next_b = nb;
+                if (lane == 0) S.bucket[1] = nb;
                 has_next = (int64_t)nb < p.n_buckets;
                 if (has_next && lane < 2)
                     cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
@@ -920,27 +898,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     cp_async_commit();
                     // software pipeline, two pairs per trip so that no register copies are needed: the
                     // displacement / rsqrt of the next pair is issued under the body of the current one
-                    PcPre2 pA = pc_pre2(tp[2 * q0], tp[2 * q0 + 1], cr);
+                    float pc_minr2 = 3.0e38f;
+                    PcPre2 pA = pc_pre2(tp[2 * q0], tp[2 * q0 + 1], cr, pc_minr2);
 #pragma unroll 1
                     for (int q = q0; q < q1; q += 2) {
-                        const PcPre2 pB = pc_pre2(tp[2 * q + 2], tp[2 * q + 3], cr);
+                        const PcPre2 pB = pc_pre2(tp[2 * q + 2], tp[2 * q + 3], cr, pc_minr2);
                         {
                             float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                            float2 c2 = S.s2[q * 32 + lane];
-                            pc_body2(pA, cr, a0, a1, c2);
+                            pc_body2(pA, cr, a0, a1);
                             s_acc[(2 * q) * 32 + lane] = a0;
                             s_acc[(2 * q + 1) * 32 + lane] = a1;
-                            S.s2[q * 32 + lane] = c2;
                         }
                         if (q + 1 < q1) {
-                            pA = pc_pre2(tp[2 * q + 4], tp[2 * q + 5], cr);
+                            pA = pc_pre2(tp[2 * q + 4], tp[2 * q + 5], cr, pc_minr2);
                             float4 a0 = s_acc[(2 * q + 2) * 32 + lane], a1 = s_acc[(2 * q + 3) * 32 + lane];
-                            float2 c2 = S.s2[(q + 1) * 32 + lane];
-                            pc_body2(pB, cr, a0, a1, c2);
+                            pc_body2(pB, cr, a0, a1);
                             s_acc[(2 * q + 2) * 32 + lane] = a0;
                             s_acc[(2 * q + 3) * 32 + lane] = a1;
-                            S.s2[(q + 1) * 32 + lane] = c2;
                         }
+                    }
+                    {   // this lane's cell pulls on none of the sinks it was evaluated for with more than M / min r^2
+                        const float ir = rsqrt_approx(pc_minr2);
+                        const float tb = cr.M * ir * ir;
+                        s2_b = fmaf(tb, tb, s2_b);
                     }
                     c = cn; cn = c2;
                 }
@@ -956,49 +936,45 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
             // written here: its (bucket, pass) is queued and pkdg_fixup_kernel evaluates it with fp64 terms.
             float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
             const bool fix_on = p.fix_k >= 0.0f;
+#pragma unroll
+            for (int o = 16; o; o >>= 1) s2_b += __shfl_xor_sync(0xffffffffu, s2_b, o);
             if (ntp <= 8) {
-                float v[32], w[8];
+                float v[32];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                    const float2 c2 = S.s2[q * 32 + lane];
                     v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
-                    w[2 * q] = c2.x; w[2 * q + 1] = c2.y;
                 }
                 warp_transpose_reduce<32>(v, lane);       // lane l: component l & 3 of sink l >> 2
-                warp_transpose_reduce_small<8>(w, lane);  // lane l: S2 of sink l >> 2
                 const float r = v[0];
                 float sq = (lane & 3) < 3 ? r * r : 0.0f;
                 sq += __shfl_xor_sync(0xffffffffu, sq, 1);
                 sq += __shfl_xor_sync(0xffffffffu, sq, 2);
                 const bool valid = (lane >> 2) < ntp;
-                bool flag = fix_on && valid && w[0] >= p.fix_k * sq;
+                bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
                 const unsigned ballot = __ballot_sync(0xffffffffu, flag);
                 if (ballot) {   // warp-uniform; every lane takes part in the push
-                    const bool queued = fix_push(p, (int)cur, t0, ballot, lane);
+                    const bool queued = fix_push(p, (int)S.bucket[0], t0, ballot, lane);
                     flag = flag && queued;
                 }
                 if (valid && !flag) outf[lane] = accumulate ? r + outf[lane] : r;
             } else {
-                float v[64], w[16];
+                float v[64];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                    const float2 c2 = S.s2[q * 32 + lane];
                     v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
-                    w[2 * q] = c2.x; w[2 * q + 1] = c2.y;
                 }
                 warp_transpose_reduce<64>(v, lane);        // lane l: components 2 (l & 1), 2 (l & 1) + 1 of sink l >> 1
-                warp_transpose_reduce_small<16>(w, lane);  // lane l: S2 of sink l >> 1
                 float sq = (lane & 1) ? v[0] * v[0] : fmaf(v[0], v[0], v[1] * v[1]);
                 sq += __shfl_xor_sync(0xffffffffu, sq, 1);
                 const bool valid = (lane >> 1) < ntp;
-                bool flag = fix_on && valid && w[0] >= p.fix_k * sq;
+                bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
                 const unsigned ballot = __ballot_sync(0xffffffffu, flag);
                 if (ballot) {
-                    const bool queued = fix_push(p, (int)cur, (int)((unsigned)t0 | 0x80000000u), ballot, lane);
+                    const bool queued = fix_push(p, (int)S.bucket[0], (int)((unsigned)t0 | 0x80000000u), ballot, lane);
                     flag = flag && queued;
                 }
                 if (valid && !flag) {
@@ -1013,7 +989,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
         cp_async_wait_all();
         __syncwarp();
         d = S.ndesc;
-        cur = next_b;
+        if (lane == 0) S.bucket[0] = S.bucket[1];
         buf ^= 1;
     }
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
@@ -1040,7 +1016,7 @@ __device__ __forceinline__ void pp_pair_f64(const double xi, const double yi, co
     const double m = (double)s.w;
     if (r2 >= h * h) {
         if (r2 < 1.0e-24) return;  // eps == 0 and (nearly) coincident: contributes nothing (include/pkdg.h)
-        const double ir = 1.0 / sqrt(r2);
+        const double ir = rsqrt(r2);
         const double g = m * ir * ir * ir;
         a[0] -= g * dx; a[1] -= g * dy; a[2] -= g * dz; a[3] -= m * ir;
     } else {
@@ -1059,7 +1035,7 @@ __device__ __noinline__ void pc_pair_f64(const double xi, const double yi, const
     prep_cell_f64(rec, q);
     const double dx = xi - q[0], dy = yi - q[1], dz = zi - q[2], M = q[3], sc = q[4];
     const double r2 = dx * dx + dy * dy + dz * dz;
-    const double ri = 1.0 / sqrt(r2), ri2 = ri * ri, sr = sc * ri2;
+    const double ri = rsqrt(r2), ri2 = ri * ri, sr = sc * ri2;
     const double x = dx * sr, y = dy * sr, z = dz * sr;
     const double qxx = q[5], qxy = q[6], qxz = q[7], qyy = q[8], qyz = q[9], qzz = q[26];
     const double v2x = qxx * x + qxy * y + qxz * z, v2y = qxy * x + qyy * y + qyz * z, v2z = qxz * x + qyz * y + qzz * z;
@@ -1089,14 +1065,17 @@ __device__ __noinline__ void pc_pair_f64(const double xi, const double yi, const
     a[2] += k3 * (sc * (v2z + v3z + v4z) - Sr * dz);
 }
 
-__global__ void __launch_bounds__(128) pkdg_fixup_kernel(const EvalParams p) {
-    const int lane = threadIdx.x & 31;
-    const unsigned gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+// One CTA of kFixThreads threads per queue entry; its flagged sinks one after the other, all threads striding
+// the lists of the bucket (a flagged sink is rare, its lists may be thousands of entries long).
+constexpr int kFixThreads = 128;
+__global__ void __launch_bounds__(kFixThreads) pkdg_fixup_kernel(const EvalParams p) {
+    __shared__ double s_red[4][kFixThreads / 32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const unsigned n = min(*p.fix_count, p.fix_cap);
     const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
     const bool pp_leaves = (p.flags & 0x8u) != 0;
     const double h = 2.0 * (double)p.eps;
-    for (unsigned e = gw; e < n; e += nw) {
+    for (unsigned e = blockIdx.x; e < n; e += gridDim.x) {
         const int4 ent = p.fix_queue[e];
         const BucketDesc d = p.desc[ent.x];
         const bool wide = ((unsigned)ent.y & 0x80000000u) != 0;
@@ -1105,7 +1084,7 @@ __global__ void __launch_bounds__(128) pkdg_fixup_kernel(const EvalParams p) {
         unsigned lanes = (unsigned)ent.z;  // ballot of the flagged lanes of the evaluation kernel's reduction
         const unsigned keep = wide ? 0x55555555u : 0x11111111u;   // one lane per sink: 2 t (wide) or 4 t
         lanes &= keep;
-        if (lane == 0) atomicAdd(&p.stats->fixup_sinks, (unsigned long long)__popc(lanes));
+        if (tid == 0) atomicAdd(&p.stats->fixup_sinks, (unsigned long long)__popc(lanes));
         while (lanes) {
             const int bit = __ffs(lanes) - 1;
             lanes &= lanes - 1;
@@ -1113,37 +1092,158 @@ __global__ void __launch_bounds__(128) pkdg_fixup_kernel(const EvalParams p) {
             const float4 xi4 = __ldg(p.xyzm + i);
             const double xi = xi4.x, yi = xi4.y, zi = xi4.z;
             double a[4] = {0.0, 0.0, 0.0, 0.0};
-            if (pp_leaves) {
-                for (int r = 0; r < L.pp; ++r) {
+            if (pp_leaves) {   // a reference stands for <= 16 particles: 8 references per sweep of the CTA
+                const int sub = tid >> 4, slot = tid & 15;
+                for (int r = sub; r < L.pp; r += kFixThreads / 16) {
                     const int32_t g = __ldg(p.pp_idx + d.pp_begin + r);
                     if ((uint32_t)g >= (uint64_t)p.n_gbuckets) continue;
                     const int2 fc = __ldg(p.gfc + g);
-                    const int j = fc.x + lane;
-                    if (lane < fc.y && j != i && (uint32_t)j < (uint64_t)p.n_particles)
+                    const int j = fc.x + slot;
+                    if (slot < fc.y && j != i && (uint32_t)j < (uint64_t)p.n_particles)
                         pp_pair_f64(xi, yi, zi, __ldg(p.xyzm + j), h, a);
                 }
             } else {
-                for (int r = lane; r < L.pp; r += 32) {
+                for (int r = tid; r < L.pp; r += kFixThreads) {
                     const int32_t j = __ldg(p.pp_idx + d.pp_begin + r);
                     if (j != i && (uint32_t)j < (uint64_t)p.n_particles) pp_pair_f64(xi, yi, zi, __ldg(p.xyzm + j), h, a);
                 }
             }
-            for (int r = lane; r < L.pc; r += 32) {
+            for (int r = tid; r < L.pc; r += kFixThreads) {
                 const int32_t c = __ldg(p.pc_idx + d.pc_begin + r);
                 if ((uint32_t)c < (uint64_t)p.n_cells) pc_pair_f64(xi, yi, zi, p.cells_raw + (int64_t)c * p.cells_stride, a);
             }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) a[k] = warp_sum_f64(a[k]);
-            if (lane == 0) {
-                float4 o = make_float4((float)a[0], (float)a[1], (float)a[2], (float)a[3]);
+            for (int k = 0; k < 4; ++k) {
+                a[k] = warp_sum_f64(a[k]);
+                if (lane == 0) s_red[k][wid] = a[k];
+            }
+            __syncthreads();
+            if (tid == 0) {
+                double r[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) r[k] = (s_red[k][0] + s_red[k][1]) + (s_red[k][2] + s_red[k][3]);
                 if (accumulate) {
                     const float4 old = p.out[i];
-                    o = make_float4((float)(a[0] + old.x), (float)(a[1] + old.y), (float)(a[2] + old.z), (float)(a[3] + old.w));
+                    r[0] += old.x; r[1] += old.y; r[2] += old.z; r[3] += old.w;
                 }
-                p.out[i] = o;
+                p.out[i] = make_float4((float)r[0], (float)r[1], (float)r[2], (float)r[3]);
             }
+            __syncthreads();
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// List construction on the device (PAPER.md:L65 checklist walk, L69 opening radius
+// RO = b_max / theta and the 2-softenings gap, Table 3 "Opening criteria").  One thread per sink cell (a
+// bucket, or a group cell for group-shared lists) walks the tree in depth-first pre-order through the
+// skip list `end` (cell k's subtree is [k, end[k])): for source cell k and sink B (reading A6)
+//   P-C   iff  k != B, count[k] >= 2, |COM_B - COM_k| > b_max,B + b_max,k / theta, gap(bbox_B, bbox_k) >= 2 eps
+//   else  a leaf joins the P-P list whole (its particle indices, or ONE bucket reference with leaf_rank != NULL)
+//   else  the cell is opened (k + 1 is its first child).
+// Neighbouring threads are neighbouring sinks and take nearly the same path.  The arithmetic is fp64 with
+// explicit round-to-nearest operations and no fused multiply-add, so that every accept / open decision --
+// hence every offset and every index -- equals the host generator's (gcc, x86-64 SSE2) bit for bit.
+// FILL = false counts the entries of each list, FILL = true writes them at the given offsets.
+// ------------------------------------------------------------------------------------------------
+struct TreeView {
+    const int32_t* first; const int32_t* count; const int32_t* end; const int32_t* isleaf;
+    const float* bblo; const float* bbhi;   // [n_cells][3]
+    const float* rec; int32_t stride;       // canonical cell records: COM at [0..2], b_max at [35]
+    int64_t n_cells;
+    const int32_t* leaf_rank;               // NULL, or [n_cells]: bucket index of a leaf cell (PKDG_PP_LEAVES output)
+};
+
+template <bool FILL>
+__global__ void pkdg_walk_kernel(const TreeView T, const int32_t* __restrict__ sink_cell, int64_t n_sinks, double theta,
+                                 double eps, int64_t* __restrict__ pp_len, int64_t* __restrict__ pc_len,
+                                 const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
+                                 int32_t* __restrict__ pp_idx, int32_t* __restrict__ pc_idx) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_sinks) return;
+    const int64_t cb = sink_cell[s];
+    const float* rb = T.rec + cb * (int64_t)T.stride;
+    const double bx = rb[0], by = rb[1], bz = rb[2], bmaxB = rb[35];
+    const double lob0 = T.bblo[3 * cb], lob1 = T.bblo[3 * cb + 1], lob2 = T.bblo[3 * cb + 2];
+    const double hib0 = T.bbhi[3 * cb], hib1 = T.bbhi[3 * cb + 1], hib2 = T.bbhi[3 * cb + 2];
+    const double gap_min2 = __dmul_rn(__dmul_rn(4.0, eps), eps);
+    int64_t npp = 0, npc = 0;
+    int64_t wpp = FILL ? pp_off[s] : 0, wpc = FILL ? pc_off[s] : 0;
+    int64_t k = 0;
+    while (k < T.n_cells) {
+        bool accept = false;
+        const int32_t cnt = __ldg(T.count + k);
+        if (k != cb && cnt >= 2) {
+            const float* rk = T.rec + k * (int64_t)T.stride;
+            const double dx = __dsub_rn(bx, (double)__ldg(rk)), dy = __dsub_rn(by, (double)__ldg(rk + 1)),
+                         dz = __dsub_rn(bz, (double)__ldg(rk + 2));
+            const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+            if (d > __dadd_rn(bmaxB, __ddiv_rn((double)__ldg(rk + 35), theta))) {
+                const double lok0 = __ldg(T.bblo + 3 * k), lok1 = __ldg(T.bblo + 3 * k + 1), lok2 = __ldg(T.bblo + 3 * k + 2);
+                const double hik0 = __ldg(T.bbhi + 3 * k), hik1 = __ldg(T.bbhi + 3 * k + 1), hik2 = __ldg(T.bbhi + 3 * k + 2);
+                double g0 = 0.0, g1 = 0.0, g2 = 0.0, t;
+                t = __dsub_rn(lok0, hib0); if (t > g0) g0 = t;
+                t = __dsub_rn(lob0, hik0); if (t > g0) g0 = t;
+                t = __dsub_rn(lok1, hib1); if (t > g1) g1 = t;
+                t = __dsub_rn(lob1, hik1); if (t > g1) g1 = t;
+                t = __dsub_rn(lok2, hib2); if (t > g2) g2 = t;
+                t = __dsub_rn(lob2, hik2); if (t > g2) g2 = t;
+                const double gg = __dadd_rn(__dadd_rn(__dmul_rn(g0, g0), __dmul_rn(g1, g1)), __dmul_rn(g2, g2));
+                accept = gg >= gap_min2;
+            }
+        }
+        if (accept) {
+            if (FILL) pc_idx[wpc++] = (int32_t)k;
+            ++npc;
+            k = __ldg(T.end + k);
+        } else if (__ldg(T.isleaf + k)) {
+            if (T.leaf_rank) {
+                if (FILL) pp_idx[wpp++] = __ldg(T.leaf_rank + k);
+                ++npp;
+            } else {
+                if (FILL) {
+                    const int32_t f = __ldg(T.first + k);
+                    for (int32_t j = 0; j < cnt; ++j) pp_idx[wpp++] = f + j;
+                }
+                npp += cnt;
+            }
+            k = __ldg(T.end + k);
+        } else {
+            k = k + 1;
+        }
+    }
+    if (!FILL) { pp_len[s] = npp; pc_len[s] = npc; }
+}
+
+// Exclusive scan of n int64 values in three launches (block scans, scan of the block totals, add): v[i] ->
+// sum_{j<i} v[j], total at v[n].  kScanBlock * kScanItems values per block; the middle launch is one block.
+constexpr int kScanBlock = 256, kScanItems = 8;
+__global__ void __launch_bounds__(kScanBlock) pkdg_scan_blocks_kernel(int64_t* __restrict__ v, int64_t n,
+                                                                       int64_t* __restrict__ block_tot) {
+    __shared__ int64_t s_warp[kScanBlock / 32];
+    const int64_t base = ((int64_t)blockIdx.x * kScanBlock + threadIdx.x) * kScanItems;
+    int64_t x[kScanItems], run = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) { x[i] = base + i < n ? v[base + i] : 0; run += x[i]; }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int64_t inc = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int64_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    int64_t wpre = 0;
+    for (int w = 0; w < wid; ++w) wpre += s_warp[w];
+    int64_t pre = wpre + inc - run;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) { if (base + i < n) v[base + i] = pre; pre += x[i]; }
+    if (threadIdx.x == kScanBlock - 1) block_tot[blockIdx.x] = wpre + inc;
+}
+
+__global__ void pkdg_scan_add_kernel(int64_t* __restrict__ v, int64_t n, const int64_t* __restrict__ block_pre,
+                                     int64_t n_blocks) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) v[i] += block_pre[i / (kScanBlock * kScanItems)];
+    else if (i == n) v[n] = block_pre[n_blocks];
 }
 
 // ------------------------------------------------------------------------------------------------
