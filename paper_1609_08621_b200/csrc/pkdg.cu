@@ -67,6 +67,7 @@ struct pkdg_ctx {
     cudaStream_t last_stream = nullptr;
     bool eval_configured = false;      // dynamic-smem opt-in of the evaluation kernel done on this device
     int eval_per_sm = 1;
+    int evalg_per_sm[2] = {0, 0};      // the same for the two instantiations of the group kernel (0 = not yet)
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
     bool profiling = false;
@@ -129,6 +130,35 @@ pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     return PKDG_OK;
 }
 
+constexpr int kGroupWarps = 4;      // warps per CTA of the group kernel (one group per warp)
+constexpr int kGroupMinBlocks = 4;  // 128 registers per thread: 16 warps per SM
+
+template <bool LEAF>
+pkdg_status launch_eval_groups_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    auto kern = pkdg_evalg_kernel<kGroupWarps, kGroupMinBlocks, LEAF>;
+    const int smem = kGroupWarps * (int)sizeof(WarpSmemG);
+    int& per_sm = ctx->evalg_per_sm[LEAF ? 1 : 0];
+    if (per_sm == 0) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kGroupWarps * 32, smem));
+        if (per_sm < 1) per_sm = 1;
+    }
+    int64_t want = (p.n_groups + kGroupWarps - 1) / kGroupWarps;
+    int64_t grid = (int64_t)ctx->num_sms * per_sm;
+    if (grid > want) grid = want;
+    if (grid < 1) grid = 1;
+    kern<<<(unsigned)grid, kGroupWarps * 32, smem, st>>>(p);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+// Group-shared lists: one warp per group, one lane per sink pair (pkdg_evalg_kernel).
+pkdg_status launch_eval_groups(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    return (p.flags & PKDG_PP_LEAVES) ? launch_eval_groups_t<true>(ctx, p, st) : launch_eval_groups_t<false>(ctx, p, st);
+}
+
 pkdg_status check_common(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
                          const pkdg_list* pp, const pkdg_list* pc, const float* out) {
     if (!ctx) return PKDG_EINVAL;
@@ -166,6 +196,10 @@ void fill_params(EvalParams& p, pkdg_ctx* ctx, const float* xyzm, int64_t np, in
     p.fix_queue = nullptr;
     p.fix_count = nullptr;
     p.fix_cap = 0;
+    p.g_first = nullptr;
+    p.g_n = nullptr;
+    p.n_groups = 0;
+    p.g_base = 0;
 }
 
 // Queue capacity that cannot overflow: one entry per (bucket, pass of 16 sinks) at most.
@@ -313,7 +347,8 @@ static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
     if (B->n == 0) return PKDG_OK;
     if ((s = ensure(ctx, &ctx->desc, &ctx->desc_cap, B->n)) != PKDG_OK) return s;
-    const int64_t fcap = fix_capacity(B->n, P->n);
+    // the group kernel queues one entry per flagged SINK, the bucket kernel one per (bucket, pass)
+    const int64_t fcap = G ? P->n + B->n + 16 : fix_capacity(B->n, P->n);
     if (!(flags & PKDG_NO_FIXUP) && (s = ensure(ctx, &ctx->fixq, &ctx->fixq_cap, fcap)) != PKDG_OK) return s;
     if (has_pc) {
         if ((s = ensure(ctx, &ctx->cellq, &ctx->cellq_cap, C->n * kCellQFloats)) != PKDG_OK) return s;
@@ -356,6 +391,7 @@ static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     p.fix_queue = ctx->fixq;
     p.fix_count = ctx->counters + 2 * kMaxSlots + 1;
     p.fix_cap = (unsigned)(fcap > 0x7fffffffLL ? 0x7fffffffLL : fcap);
+    if (G) { p.g_first = G->first_bucket; p.g_n = G->n_buckets; p.n_groups = G->n; p.g_base = 0; }
     if ((flags & PKDG_VALIDATE) && (s = launch_validate(ctx, p, true, st)) != PKDG_OK) return s;
     const bool prof = ctx->profiling && ctx->prof_n < 256;
     if (prof) {
@@ -363,7 +399,7 @@ static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
             if (!ctx->prof_ev[3 * ctx->prof_n + i]) CK(cudaEventCreate(&ctx->prof_ev[3 * ctx->prof_n + i]));
         CK(cudaEventRecord(ctx->prof_ev[3 * ctx->prof_n], st));
     }
-    s = launch_eval(ctx, p, st);
+    s = G ? launch_eval_groups(ctx, p, st) : launch_eval(ctx, p, st);
     if (prof) CK(cudaEventRecord(ctx->prof_ev[3 * ctx->prof_n + 1], st));
     if (s == PKDG_OK) s = launch_fixup(ctx, p, st);
     if (prof) {
@@ -469,7 +505,7 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
         if ((rc = ensure(ctx, &sl.pc_idx, &sl.cap_pc, clen)) != PKDG_OK) break;
         int64_t chunk_sinks = 0;
         for (int64_t b = b0; b < b1; ++b) chunk_sinks += Bh->count[b] > 0 ? Bh->count[b] : 0;
-        const int64_t fcap = fix_capacity(cb, chunk_sinks);
+        const int64_t fcap = Gh ? chunk_sinks + cb + 16 : fix_capacity(cb, chunk_sinks);
         if (!(flags & PKDG_NO_FIXUP) && (rc = ensure(ctx, &sl.fixq, &sl.fixq_cap, fcap)) != PKDG_OK) break;
         if (cb + 1 > sl.cap_b) {
             int64_t c1 = 0, c2 = 0, c5 = 0;
@@ -540,8 +576,9 @@ static pkdg_status streamed_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
         p.fix_queue = sl.fixq;
         p.fix_count = counter + kMaxSlots + 1;
         p.fix_cap = (unsigned)(fcap > 0x7fffffffLL ? 0x7fffffffLL : fcap);
+        if (Gh) { p.g_first = sl.gfirst; p.g_n = sl.gn; p.n_groups = cu; p.g_base = b0; }
         if ((flags & PKDG_VALIDATE) && (rc = launch_validate(ctx, p, ic == 0, sl.st)) != PKDG_OK) break;
-        if ((rc = launch_eval(ctx, p, sl.st)) != PKDG_OK) break;
+        if ((rc = Gh ? launch_eval_groups(ctx, p, sl.st) : launch_eval(ctx, p, sl.st)) != PKDG_OK) break;
         if ((rc = launch_fixup(ctx, p, sl.st)) != PKDG_OK) break;
         if (out_host && cb > 0) {
             const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];

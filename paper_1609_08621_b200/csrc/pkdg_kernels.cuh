@@ -14,6 +14,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace pkdg {
 
@@ -364,6 +365,11 @@ struct EvalParams {
     int4* fix_queue;          // {bucket, t0 | wide << 31, lane ballot, 0}
     unsigned int* fix_count;
     unsigned int fix_cap;
+    // group-shared lists (pkdg_evalg_kernel): group g = buckets g_first[g] - g_base .. + g_n[g] of `desc`
+    const int32_t* g_first;
+    const int32_t* g_n;
+    int64_t n_groups;
+    int64_t g_base;
 };
 
 // Cubic-spline pair factors (Monaghan-Lattanzio density of support h; u = r / h < 1): a -= m d g / h^3,
@@ -506,6 +512,18 @@ struct __align__(16) WarpSmem3 {
     BucketDesc ndesc;             // descriptor of the next bucket
     unsigned int bucket[2];       // index of the current / the next bucket (fix-up queue entries name it)
 };
+
+// The lane's cell record c (>= 0: valid) starts its way into the lane's staging slots (cp.async, 8 x 16 bytes).
+// (One cp.async.bulk of 128 bytes per lane with mbarrier completion was measured instead: 12 % SLOWER at N = 2^24 --
+// 32 single-lane bulk copies per tile serialise in the copy engine's issue path.)
+__device__ __forceinline__ void stage_cell(WarpSmem3& S, const EvalParams& p, int32_t c, int lane) {
+    if (c >= 0) {
+        const float4* q = p.cellq + (int64_t)c * 8;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
+    }
+}
+__device__ __forceinline__ float4 staged(const WarpSmem3& S, int src, int i) { return S.stage[i * 32 + src]; }
 
 // per-lane partial sums of sink t in the pair layout, as scalars (correction path, reduction)
 __device__ __forceinline__ int acc_idx(int t, int comp, int lane) {  // comp 0..3 = ax ay az phi
@@ -680,8 +698,9 @@ __device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc&
         return r < 64 ? S.nidx[r >> 5][r & 31] : __ldg(p.pp_idx + d.pp_begin + r);
     };
     auto leaf_fc = [&](int32_t g) -> int2 {
-        if ((uint32_t)g >= (uint64_t)p.n_gbuckets) { bad += (g >= 0 && slot == 0); return make_int2(0, 0); }
-        return __ldg(p.gfc + g);
+        if ((uint32_t)g >= (uint64_t)p.n_gbuckets) return make_int2(0, 0);   // counted as a bad entry by the packer
+        const int2 fc = __ldg(p.gfc + g);
+        return fc.y > 16 ? make_int2(0, 0) : fc;
     };
     auto leaf_j = [&](int2 fc) -> int32_t { return slot < fc.y ? fc.x + slot : -1; };
     int32_t j, jn, jnn = -1, gB = -1;
@@ -797,7 +816,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
     const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
     const bool pp_leaves = (p.flags & 0x8u) != 0;
     unsigned bad = 0;
-
     unsigned cur = 0;
     if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
     cur = __shfl_sync(0xffffffffu, cur, 0);
@@ -826,11 +844,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
             int32_t c = pc_ntile > 0 ? S.nidx[2][lane] : -1;
             int32_t cn = pc_ntile > 1 ? S.nidx[3][lane] : -1;
             if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
-            if (c >= 0) {
-                const float4* q = p.cellq + (int64_t)c * 8;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
-            }
+            stage_cell(S, p, c, lane);
             cp_async_commit();
 
             // ---- a2: pair layout of the sinks;  a3: P-P
@@ -859,17 +873,20 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
             {
                 const int npair = (ntp + 1) >> 1;  // odd count: the last pair's second half is a dummy sink
                 const float4* tp = S.tp;
-                for (int k = 0; k < pc_ntile; ++k) {
-                    const int32_t c2 = (k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
+                // One tile.  LAST_TILE is a compile-time tag: only the last tile of a list can be partly filled, so only
+                // its copy of the code carries the sharing-out logic and the hand-over to the next bucket.
+                auto do_tile = [&](const int k, auto last_tag) {
+                    constexpr bool LAST_TILE = decltype(last_tag)::value;
+                    const int32_t c2 = (!LAST_TILE && k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
                     cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
                     // A last tile that is at most half (a quarter) full is shared out: 2 (4) groups of lanes take
                     // the same cells and each group a half (a quarter) of the sink pairs, so the tile costs a
                     // half (a quarter) of a full one.  Per-lane partial sums stay in the lane's own column.
-                    const int valid = min(32, L.pc - 32 * k);              // warp-uniform
-                    const int rep = (valid <= 8 && npair >= 4) ? 4 : (valid <= 16 && npair >= 2) ? 2 : 1;
+                    const int valid = LAST_TILE ? min(32, L.pc - 32 * k) : 32;   // warp-uniform
+                    const int rep = !LAST_TILE ? 1 : (valid <= 8 && npair >= 4) ? 4 : (valid <= 16 && npair >= 2) ? 2 : 1;
                     int src = lane, q0 = 0, q1 = npair;
                     int32_t cs = c;
-                    if (rep > 1) {
+                    if (LAST_TILE && rep > 1) {
                         const int width = 32 / rep, chunk = (npair + rep - 1) / rep;
                         src = lane & (width - 1);
                         q0 = min(npair, (lane / width) * chunk);
@@ -879,19 +896,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     }
                     CellRegs cr;
                     if (cs >= 0) {
-                        cell_unpack(cr, S.stage[src], S.stage[32 + src], S.stage[64 + src], S.stage[96 + src],
-                                    S.stage[128 + src], S.stage[160 + src], S.stage[192 + src], S.stage[224 + src]);
+                        cell_unpack(cr, staged(S, src, 0), staged(S, src, 1), staged(S, src, 2), staged(S, src, 3),
+                                    staged(S, src, 4), staged(S, src, 5), staged(S, src, 6), staged(S, src, 7));
                     } else {
                         const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
                         cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
                     }
-                    if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
-                    if (cn >= 0) {  // next tile's record; the slot was read into registers just above
-                        const float4* q = p.cellq + (int64_t)cn * 8;
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
-                    }
-                    if (last && k == pc_ntile - 1 && has_next) {  // next bucket, stage 2
+                    if (!LAST_TILE) {
+                        if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
+                        stage_cell(S, p, cn, lane);  // next tile's record; the slot was read into registers just above
+                    } else if (last && has_next) {   // next bucket, stage 2
                         __syncwarp();
                         stage_next_bucket3(S, p, buf ^ 1, do_pp, do_pc, lane);
                     }
@@ -923,7 +937,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                         s2_b = fmaf(tb, tb, s2_b);
                     }
                     c = cn; cn = c2;
-                }
+                };
+                for (int k = 0; k + 1 < pc_ntile; ++k) do_tile(k, std::false_type{});
+                if (pc_ntile > 0) do_tile(pc_ntile - 1, std::true_type{});
                 if (last && pc_ntile == 0 && has_next) {
                     cp_async_wait_all();
                     __syncwarp();
@@ -991,6 +1007,275 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
         d = S.ndesc;
         if (lane == 0) S.bucket[0] = S.bucket[1];
         buf ^= 1;
+    }
+    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Group kernel (ONE P-P and ONE P-C list per group of up to 64 particles
+// = 4 buckets).  With a list shared by 64 sinks the mapping turns round: one warp per group, one lane per SINK
+// PAIR (the two halves of every packed value are the lane's two sinks, as before), and the SOURCES are
+// warp-uniform: tiles of 32 source particles / 32 cell records stream through shared memory (cp.async, double
+// buffered, coalesced: 8 lanes per 128-byte record) and every lane reads them by broadcast.  Consequences:
+//   - sinks and accumulators live in registers for the whole list: no per-lane partial sums in shared memory,
+//     no cross-lane reduction, no per-tile staging of 35 coefficients per lane;
+//   - a list need not be a multiple of 32: cells are visited one by one, nothing is padded;
+//   - index gather, bounds checks and staging are paid once per 64 sinks instead of once per 16;
+//   - the conditioning estimate is the exact per-sink S2_i = sum_j |a_ij|^2 (one packed FMA per source);
+//   - a softened pair is corrected in place (the lane owns its sinks).
+// Arithmetic per interaction is that of pp_fast2 / pc_body2.
+// ------------------------------------------------------------------------------------------------
+constexpr int kGSinks = 64;   // sinks per pass of a group (2 per lane)
+
+struct __align__(16) WarpSmemG {
+    float4 cell[2][32 * 8];   // P-C tile: 32 internal cell records, double buffered
+    float4 src[2][32];        // P-P tile: 32 source particles (x, y, z, m); padding = far away with mass 0
+    int32_t sidx[2][32];      // their particle indices (self test by index), -1 = padding
+    int32_t cidx[2][32];      // cell indices of the P-C tile being staged
+    int32_t sink[kGSinks];    // particle index of sink slot t of the pass, -1 = none
+    int32_t sbkt[kGSinks];    // its bucket (index into desc) and slot in that bucket: names it in the fix-up queue
+    int32_t sslot[kGSinks];
+};
+
+// One source against the lane's sink pair; as pp_fast2 plus the exact conditioning estimate.
+template <bool SELF>
+__device__ __forceinline__ void pp_pair_g(const float2 X, const float2 Y, const float2 Z, const float4 s, bool selfA,
+                                          bool selfB, float h2c, float& minr2, float2& ax, float2& ay, float2& az,
+                                          float2& aw, float2& s2) {
+    const float2 dx = f2add(X, sp(-s.x)), dy = f2add(Y, sp(-s.y)), dz = f2add(Z, sp(-s.z));
+    float2 r2 = f2fma(dz, dz, f2fma(dy, dy, f2mul(dx, dx)));
+    const float2 ri = make_float2(rsqrt_approx(fmaxf(r2.x, h2c)), rsqrt_approx(fmaxf(r2.y, h2c)));
+    float2 nm = sp(-s.w);
+    if (SELF) {
+        nm.x = selfA ? 0.0f : nm.x; nm.y = selfB ? 0.0f : nm.y;
+        r2.x = selfA ? 3.0e38f : r2.x; r2.y = selfB ? 3.0e38f : r2.y;
+    }
+    minr2 = fminf(minr2, fminf(r2.x, r2.y));
+    const float2 nmri = f2mul(nm, ri);
+    const float2 t = f2mul(nmri, ri);   // -m / r^2 = -|a_ij|
+    const float2 nmg = f2mul(t, ri);
+    ax = f2fma(nmg, dx, ax);
+    ay = f2fma(nmg, dy, ay);
+    az = f2fma(nmg, dz, az);
+    aw = f2add(aw, nmri);
+    s2 = f2fma(t, t, s2);
+}
+
+// Softened-pair correction for one sink (scalar): replaces the clamped Newtonian pair booked by pp_pair_g.
+__device__ __forceinline__ void pp_soft_fix_g(float x, float y, float z, const float4 s, const EvalParams& p, float& ax,
+                                              float& ay, float& az, float& aw, float& s2) {
+    const float dx = x - s.x, dy = y - s.y, dz = z - s.z;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (r2 < p.h2c) {
+        const float ri = rsqrt_approx(p.h2c);
+        const float2 dgw = pp_soft_correction(dx, dy, dz, p.eps, ri);
+        const float mg = s.w * dgw.x;
+        ax = fmaf(-mg, dx, ax); ay = fmaf(-mg, dy, ay); az = fmaf(-mg, dz, az);
+        aw = fmaf(s.w, dgw.y, aw);
+        const float tc = s.w * ri * ri;   // booked (m / h^2)^2; a softened pair pulls with up to 2.6 m / h^2
+        s2 = fmaf(15.0f * tc, tc, s2);
+    }
+}
+
+// One cell against the lane's sink pair, accumulators in registers (pc_pre2 + pc_body2 + conditioning).
+__device__ __forceinline__ void pc_pair_g(const float2 X, const float2 Y, const float2 Z, const CellRegs& c, float2& ax,
+                                          float2& ay, float2& az, float2& aw, float2& s2) {
+    float dummy = 3.0e38f;
+    const PcPre2 q = pc_pre2(make_float4(X.x, X.y, Y.x, Y.y), make_float4(Z.x, Z.y, 0.f, 0.f), c, dummy);
+    float4 a0 = make_float4(ax.x, ax.y, ay.x, ay.y), a1 = make_float4(az.x, az.y, aw.x, aw.y);
+    pc_body2(q, c, a0, a1);
+    ax = make_float2(a0.x, a0.y); ay = make_float2(a0.z, a0.w); az = make_float2(a1.x, a1.y); aw = make_float2(a1.z, a1.w);
+    const float2 t = f2mul(f2mul(sp(c.M), q.ri), q.ri);   // M / r^2: the size of this cell's contribution
+    s2 = f2fma(t, t, s2);
+}
+
+template <int WARPS, int MINB, bool LEAF>
+__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const EvalParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    WarpSmemG& S = reinterpret_cast<WarpSmemG*>(smem_raw)[threadIdx.x >> 5];
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
+    const bool fix_on = p.fix_k >= 0.0f;
+    unsigned bad = 0;
+
+    for (;;) {
+        unsigned gu = 0;
+        if (lane == 0) gu = atomicAdd(p.work_counter, 1u);
+        gu = __shfl_sync(0xffffffffu, gu, 0);
+        if ((int64_t)gu >= p.n_groups) break;
+        const int64_t gb0 = (int64_t)__ldg(p.g_first + gu) - p.g_base;
+        const int gn = __ldg(p.g_n + gu);
+        if (gn <= 0 || gb0 < 0 || gb0 + gn > p.n_buckets) continue;   // counted as a bad entry by the packer
+        const BucketDesc d0 = p.desc[gb0];                              // every bucket of the group names the group's lists
+        const int pp_len = do_pp ? d0.pp_len : 0, pc_len = do_pc ? d0.pc_len : 0;
+        int nt = 0;
+        for (int b = 0; b < gn; ++b) nt += p.desc[gb0 + b].count;
+
+        for (int pass0 = 0; pass0 < nt; pass0 += kGSinks) {
+            // ---- a2: the pass's sinks -> registers (lane l owns sink slots 2l and 2l + 1)
+            __syncwarp();
+            S.sink[lane] = -1; S.sink[lane + 32] = -1;
+            __syncwarp();
+            int off = 0, lo = 0x7fffffff, hi = -1;   // [lo, hi): particle index range of the pass's sinks (self test per tile)
+            for (int b = 0; b < gn; ++b) {
+                const BucketDesc db = p.desc[gb0 + b];
+                for (int t = lane; t < db.count; t += 32) {
+                    const int pos = off + t - pass0;
+                    if (pos >= 0 && pos < kGSinks) {
+                        S.sink[pos] = db.first + t; S.sbkt[pos] = (int32_t)(gb0 + b); S.sslot[pos] = t;
+                    }
+                }
+                const int t_lo = max(0, pass0 - off), t_hi = min(db.count, pass0 + kGSinks - off);
+                if (t_hi > t_lo) { lo = min(lo, db.first + t_lo); hi = max(hi, db.first + t_hi); }
+                off += db.count;
+            }
+            __syncwarp();
+            const int iA = S.sink[2 * lane], iB = S.sink[2 * lane + 1];
+            const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+            const float4 tA = iA >= 0 ? __ldg(p.xyzm + iA) : dummy_tgt, tB = iB >= 0 ? __ldg(p.xyzm + iB) : dummy_tgt;
+            const float2 X = make_float2(tA.x, tB.x), Y = make_float2(tA.y, tB.y), Z = make_float2(tA.z, tB.z);
+            float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, aw = ax, s2 = ax;
+
+            // ---- a3: P-P.  Tile k (32 sources) is computed from buffer k & 1 while tile k + 1 lands in the other.
+            {
+                const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
+                const int half = lane >> 4, slot = lane & 15;
+                auto ref_of = [&](int k) -> int32_t {           // LEAF: bucket reference of this half-warp in tile k
+                    const int r = 2 * k + half;
+                    return r < pp_len ? __ldg(p.pp_idx + d0.pp_begin + r) : -1;
+                };
+                auto fc_of = [&](int32_t g) -> int2 {
+                    if ((uint32_t)g >= (uint64_t)p.n_gbuckets) return make_int2(0, 0);   // counted as a bad entry by the packer
+                    const int2 fc = __ldg(p.gfc + g);
+                    return fc.y > 16 ? make_int2(0, 0) : fc;      // counted as a bad entry by the packer
+                };
+                auto idx_of = [&](int k) -> int32_t { return tile_entry(p.pp_idx, d0.pp_begin, pp_len, k, lane); };
+                auto issue = [&](int32_t j, int buf) {           // the lane's source of a tile starts its way to shared memory
+                    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+                    S.sidx[buf][lane] = j;
+                    if (j >= 0) cp_async16(&S.src[buf][lane], p.xyzm + j);
+                    else S.src[buf][lane] = far4;
+                    cp_async_commit();
+                };
+                int32_t jn = -1, gnn = -1;   // non-LEAF: index of the tile after next;  LEAF: reference of the tile after next
+                int2 fcn = make_int2(0, 0);  // LEAF: (first, count) of the next tile's reference
+                if (LEAF) {
+                    if (ntile > 0) { const int2 fc = fc_of(ref_of(0)); issue(slot < fc.y ? fc.x + slot : -1, 0); }
+                    fcn = ntile > 1 ? fc_of(ref_of(1)) : make_int2(0, 0);
+                    gnn = ntile > 2 ? ref_of(2) : -1;
+                } else {
+                    if (ntile > 0) issue(idx_of(0), 0);
+                    jn = ntile > 1 ? idx_of(1) : -1;
+                }
+                for (int k = 0; k < ntile; ++k) {
+                    const int buf = k & 1;
+                    cp_async_wait_all();
+                    __syncwarp();   // tile k is visible to the warp; everybody is done with the other buffer
+                    if (k + 1 < ntile) {
+                        if (LEAF) {
+                            issue(slot < fcn.y ? fcn.x + slot : -1, buf ^ 1);
+                            fcn = (k + 2 < ntile) ? fc_of(gnn) : make_int2(0, 0);
+                            gnn = (k + 3 < ntile) ? ref_of(k + 3) : -1;
+                        } else {
+                            issue(jn, buf ^ 1);
+                            jn = (k + 2 < ntile) ? idx_of(k + 2) : -1;
+                        }
+                    }
+                    const int32_t jl = S.sidx[buf][lane];
+                    const bool own = __any_sync(0xffffffffu, jl >= lo && jl < hi);   // tile may hold sinks of this pass
+                    float minr2 = 3.0e38f;
+                    if (own) {
+#pragma unroll 4
+                        for (int j = 0; j < 32; ++j) {
+                            const int32_t sj = S.sidx[buf][j];
+                            pp_pair_g<true>(X, Y, Z, S.src[buf][j], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                        }
+                    } else {
+#pragma unroll 8
+                        for (int j = 0; j < 32; ++j)
+                            pp_pair_g<false>(X, Y, Z, S.src[buf][j], false, false, p.h2c, minr2, ax, ay, az, aw, s2);
+                    }
+                    if (minr2 < p.h2c) {   // rare: a pair of this lane inside the softening (or coincident): the lane owns its sinks
+                        for (int j = 0; j < 32; ++j) {
+                            const float4 s = S.src[buf][j];
+                            const int32_t sj = S.sidx[buf][j];
+                            if (sj < 0) continue;
+                            if (sj != iA) pp_soft_fix_g(X.x, Y.x, Z.x, s, p, ax.x, ay.x, az.x, aw.x, s2.x);
+                            if (sj != iB) pp_soft_fix_g(X.y, Y.y, Z.y, s, p, ax.y, ay.y, az.y, aw.y, s2.y);
+                        }
+                    }
+                }
+            }
+
+            // ---- a4: P-C.  Tile k = 32 cell records, copied by the whole warp (8 lanes per record) into buffer k & 1.
+            {
+                const int ntile = (pc_len + 31) >> 5;
+                auto cidx_of = [&](int k) -> int32_t { return tile_entry(p.pc_idx, d0.pc_begin, pc_len, k, lane); };
+                auto issue = [&](int32_t c, int buf) {
+                    if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
+                    S.cidx[buf][lane] = c;
+                    __syncwarp();
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int e = i * 32 + lane, rec = e >> 3, part = e & 7;
+                        const int32_t ci = S.cidx[buf][rec];
+                        if (ci >= 0) cp_async16(&S.cell[buf][e], p.cellq + (int64_t)ci * 8 + part);
+                        else S.cell[buf][e] = part == 0 ? far4 : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                    cp_async_commit();
+                };
+                __syncwarp();
+                if (ntile > 0) issue(cidx_of(0), 0);
+                int32_t cn = ntile > 1 ? cidx_of(1) : -1;
+                for (int k = 0; k < ntile; ++k) {
+                    const int buf = k & 1;
+                    cp_async_wait_all();
+                    __syncwarp();
+                    if (k + 1 < ntile) {
+                        issue(cn, buf ^ 1);
+                        cn = (k + 2 < ntile) ? cidx_of(k + 2) : -1;
+                    }
+                    const int ncell = min(32, pc_len - 32 * k);
+                    const float4* rec = S.cell[buf];
+#pragma unroll 1
+                    for (int c = 0; c < ncell; ++c) {
+                        CellRegs cr;
+                        cell_unpack(cr, rec[8 * c], rec[8 * c + 1], rec[8 * c + 2], rec[8 * c + 3], rec[8 * c + 4],
+                                    rec[8 * c + 5], rec[8 * c + 6], rec[8 * c + 7]);
+                        pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
+                    }
+                }
+            }
+
+            // ---- a5: no reduction -- the lane holds its sinks' totals.  Conditioning test, queue, write-back.
+            {
+                const float a2A = fmaf(az.x, az.x, fmaf(ay.x, ay.x, ax.x * ax.x)), a2B = fmaf(az.y, az.y, fmaf(ay.y, ay.y, ax.y * ax.y));
+                bool flagA = fix_on && iA >= 0 && s2.x >= p.fix_k * a2A, flagB = fix_on && iB >= 0 && s2.y >= p.fix_k * a2B;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const bool flag = h ? flagB : flagA;
+                    if (flag) {   // one queue entry per flagged sink, in the evaluation kernel's format (wide pass: lane 2 t)
+                        const int t = S.sslot[2 * lane + h];
+                        const unsigned k = atomicAdd(p.fix_count, 1u);
+                        if (k < p.fix_cap)
+                            p.fix_queue[k] = make_int4(S.sbkt[2 * lane + h], (int)((unsigned)(t & ~15) | 0x80000000u),
+                                                       (int)(1u << (2 * (t & 15))), 0);
+                        else if (h) flagB = false; else flagA = false;   // queue full (cannot happen): keep the fp32 row
+                    }
+                }
+                if (iA >= 0 && !flagA) {
+                    float4 r = make_float4(ax.x, ay.x, az.x, aw.x);
+                    if (accumulate) { const float4 o = p.out[iA]; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }
+                    p.out[iA] = r;
+                }
+                if (iB >= 0 && !flagB) {
+                    float4 r = make_float4(ax.y, ay.y, az.y, aw.y);
+                    if (accumulate) { const float4 o = p.out[iB]; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }
+                    p.out[iB] = r;
+                }
+            }
+        }
     }
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
