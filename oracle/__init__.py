@@ -51,6 +51,12 @@ def lib():
         L.orc_contribution_norms.argtypes = L.orc_gravity_eval.argtypes
         L.orc_contribution_norms2.restype = c_int
         L.orc_contribution_norms2.argtypes = L.orc_gravity_eval.argtypes
+        L.orc_cc_accumulate.argtypes = [c_void_p, c_void_p, c_void_p]
+        L.orc_cp_accumulate.argtypes = [c_void_p, c_void_p, c_double, c_void_p]
+        L.orc_local_eval.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.orc_fmm_eval.restype = c_int
+        L.orc_fmm_eval.argtypes = [c_int64, c_void_p, c_int64, c_void_p, c_int32, c_int64, c_void_p, c_void_p, c_void_p,
+                                   c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
         L.orc_direct_sum.argtypes = [c_int64, c_void_p, c_double, c_void_p, c_int64, c_void_p]
         L.orc_pack_tiles.restype = c_int64
         L.orc_pack_tiles.argtypes = [c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
@@ -155,6 +161,56 @@ def contribution_norms(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx
     if err:
         raise ValueError("oracle: bucket index out of range")
     return out
+
+
+NLOC = 56  # local-expansion coefficients, |n| <= 5
+
+
+def local_index():
+    """Multi-indices (a, b, c) of the 56 local coefficients in storage order."""
+    return [(a, b, n - a - b) for n in range(6) for a in range(n, -1, -1) for b in range(n - a, -1, -1)]
+
+
+def cc_accumulate(zB, rec, L=None):
+    """L (56 fp64, created if None) += local expansion about zB of one source cell (canonical 36-float record)."""
+    zB = _c(zB, np.float64); rec = _c(rec, np.float32)
+    L = np.zeros(NLOC) if L is None else L
+    lib().orc_cc_accumulate(_p(zB), _p(rec), _p(L))
+    return L
+
+
+def cp_accumulate(zB, xs, ms, L=None):
+    """L += local expansion about zB of one source particle."""
+    zB = _c(zB, np.float64); xs = _c(xs, np.float64)
+    L = np.zeros(NLOC) if L is None else L
+    lib().orc_cp_accumulate(_p(zB), _p(xs), float(ms), _p(L))
+    return L
+
+
+def local_eval(zB, L, xt):
+    """(acc[3], pot) of the local expansion L about zB at xt."""
+    zB = _c(zB, np.float64); L = _c(L, np.float64); xt = _c(xt, np.float64)
+    acc = np.zeros(3); pot = np.zeros(1)
+    lib().orc_local_eval(_p(zB), _p(L), _p(xt), _p(acc), _p(pot))
+    return acc, float(pot[0])
+
+
+def fmm_eval(xyzm, cells, first, count, zB, cc_off, cc_idx, cp_off, cp_idx, out=None, want_L=False):
+    """The C-C / C-P part of the path: per bucket, local expansion about zB[b] from its C-C and C-P lists,
+    evaluated at the bucket's particles and ADDED to out[n,4] (zeros if None).  Returns out (and L[n_b,56])."""
+    xyzm = _c(xyzm, np.float32); n = xyzm.shape[0]
+    cells = _c(np.zeros((0, 36), np.float32) if cells is None else cells, np.float32)
+    first = _c(first, np.int32); count = _c(count, np.int32); zB = _c(zB, np.float32)
+    cc_off = _c(cc_off, np.int64); cc_idx = _c(cc_idx, np.int32); cp_off = _c(cp_off, np.int64); cp_idx = _c(cp_idx, np.int32)
+    out = np.zeros((n, 4)) if out is None else out
+    assert out.dtype == np.float64 and out.flags["C_CONTIGUOUS"]
+    Lout = np.zeros((first.shape[0], NLOC)) if want_L else None
+    err = lib().orc_fmm_eval(n, _p(xyzm), cells.shape[0], _p(cells), cells.shape[1] if cells.ndim == 2 else 36,
+                             first.shape[0], _p(first), _p(count), _p(zB), _p(cc_off), _p(cc_idx), _p(cp_off), _p(cp_idx),
+                             _p(out), _p(Lout))
+    if err:
+        raise ValueError("oracle: index out of range in buckets or lists")
+    return (out, Lout) if want_L else out
 
 
 def direct_sum(xyzm, eps, targets=None):

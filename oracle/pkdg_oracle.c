@@ -327,6 +327,163 @@ void orc_direct_sum(int64_t n_particles, const float *xyzm, double eps, const in
 }
 
 /* ---------------------------------------------------------------------------
+ * Cell-cell and cell-particle interactions and the local expansion
+ * ("FMM also considers cell-cell (CC)
+ * interactions by approximating the potential landscape within a given cell (the
+ * sink cell) that is induced by a sufficiently distant multipole (the source
+ * cell)"; L69 fn 2 "Cell-particle interactions ... are the expansions of the
+ * potential within the sink cell induced by a single source particle"; L71 "The
+ * local expansion of the potential about the sink's center of mass is actually
+ * done to 5th order ... accumulating the CC and CP interactions").
+ *
+ * The paper prints no formula (readings A20-A22).  With the notation of
+ * orc_pc_pair -- t_k(r) = d^k(1/|r|)/k!, raw moments M_m of the source cell about
+ * its centre z_C -- the source's potential at x is
+ *     phi(x) = - sum_m (-1)^|m| M_m t_m(x - z_C).
+ * Expanding about the sink's centre z_B (x = z_B + s, R = z_B - z_C):
+ *     t_m(R + s) = sum_n binom(n + m, m) t_{n+m}(R) s^n      (Taylor's theorem),
+ * so phi(z_B + s) = sum_n L_n s^n with
+ *     L_n = - sum_m (-1)^|m| M_m binom(n + m, m) t_{n+m}(R),
+ * binom(n + m, m) = prod_i (n_i + m_i)! / (n_i! m_i!).  Truncation (A20): the local
+ * expansion holds |n| <= 5 and a term is kept iff |n| + |m| <= 5 (total order 5:
+ * exactly the derivatives of 1/r up to 5th order that the P-C kernel uses too);
+ * |m| in {0, 2, 3, 4}, the dipole about the centre of mass is dropped (A9).
+ * A source PARTICLE (x_j, m_j) is the case z_C = x_j, M_0 = m_j, no higher moment:
+ *     L_n += - m_j t_n(z_B - x_j),  |n| <= 5.
+ * Unsoftened, like P-C (A4): the list builder accepts C-C / C-P only for boxes at
+ * least two softenings apart.
+ *
+ * Local coefficients are stored in the order of the moments: for n = 0..5,
+ * a = n..0, b = n-a..0, c = n-a-b: 56 doubles.
+ * ------------------------------------------------------------------------- */
+#define ORC_NLOC 56
+
+static double binom1(int n, int m) { /* binom(n + m, m), small arguments */
+    double r = 1.0;
+    for (int i = 1; i <= m; ++i) r = r * (double)(n + i) / (double)i;
+    return r;
+}
+
+/* L += contribution of one source cell (canonical record) to the local expansion about zB. */
+void orc_cc_accumulate(const double zB[3], const float *rec, double *L) {
+    double R[3] = {zB[0] - (double)rec[0], zB[1] - (double)rec[1], zB[2] - (double)rec[2]};
+    double t[ORC_TDIM * ORC_TDIM * ORC_TDIM];
+    orc_taylor_coeffs(R, 5, t);
+    int li = 0;
+    for (int n = 0; n <= 5; ++n)
+        for (int na = n; na >= 0; --na)
+            for (int nb = n - na; nb >= 0; --nb) {
+                int nc = n - na - nb;
+                double sum = 0.0;
+                int pos = 3; /* rec[3] is M_000 */
+                for (int m = 0; m <= 4; ++m) {
+                    if (m == 1) continue;
+                    double sign = (m % 2 == 0) ? 1.0 : -1.0;
+                    for (int ma = m; ma >= 0; --ma)
+                        for (int mb = m - ma; mb >= 0; --mb) {
+                            int mc = m - ma - mb;
+                            double M = (double)rec[pos++];
+                            if (n + m > 5) continue;
+                            sum += sign * M * binom1(na, ma) * binom1(nb, mb) * binom1(nc, mc) *
+                                   t[TIDX(na + ma, nb + mb, nc + mc)];
+                        }
+                }
+                L[li++] -= sum;
+            }
+}
+
+/* L += contribution of one source particle (xs, ms) to the local expansion about zB. */
+void orc_cp_accumulate(const double zB[3], const double xs[3], double ms, double *L) {
+    double R[3] = {zB[0] - xs[0], zB[1] - xs[1], zB[2] - xs[2]};
+    double t[ORC_TDIM * ORC_TDIM * ORC_TDIM];
+    orc_taylor_coeffs(R, 5, t);
+    int li = 0;
+    for (int n = 0; n <= 5; ++n)
+        for (int na = n; na >= 0; --na)
+            for (int nb = n - na; nb >= 0; --nb) L[li++] -= ms * t[TIDX(na, nb, n - na - nb)];
+}
+
+/* Evaluate the local expansion at xt: pot += sum_n L_n s^n, acc_l -= sum_n L_n n_l s^(n - e_l), s = xt - zB
+ * (the acceleration is minus the exact gradient of the polynomial). */
+void orc_local_eval(const double zB[3], const double *L, const double xt[3], double acc[3], double *pot) {
+    double s[3] = {xt[0] - zB[0], xt[1] - zB[1], xt[2] - zB[2]};
+    double pw[3][7];
+    for (int d = 0; d < 3; ++d) {
+        pw[d][0] = 1.0;
+        for (int e = 1; e < 7; ++e) pw[d][e] = pw[d][e - 1] * s[d];
+    }
+    int li = 0;
+    for (int n = 0; n <= 5; ++n)
+        for (int a = n; a >= 0; --a)
+            for (int b = n - a; b >= 0; --b) {
+                int c = n - a - b;
+                double Ln = L[li++];
+                *pot += Ln * pw[0][a] * pw[1][b] * pw[2][c];
+                if (a >= 1) acc[0] -= Ln * a * pw[0][a - 1] * pw[1][b] * pw[2][c];
+                if (b >= 1) acc[1] -= Ln * b * pw[0][a] * pw[1][b - 1] * pw[2][c];
+                if (c >= 1) acc[2] -= Ln * c * pw[0][a] * pw[1][b] * pw[2][c - 1];
+            }
+}
+
+/* The FMM part of the path for a set of sink buckets: for bucket b, the local expansion about the
+ * bucket's centre zB[b] (fp32, widened) accumulates its C-C list (cell indices) and its C-P list
+ * (particle indices), and is evaluated at every particle of the bucket.  out: [n_particles][4] fp64,
+ * ADDED to (the caller sums it with the P-P / P-C part); Lout (may be NULL): [n_buckets][56]. */
+int orc_fmm_eval(int64_t n_particles, const float *xyzm, int64_t n_cells, const float *cells, int32_t stride,
+                 int64_t n_buckets, const int32_t *first, const int32_t *count, const float *zB,
+                 const int64_t *cc_off, const int32_t *cc_idx, const int64_t *cp_off, const int32_t *cp_idx,
+                 double *out, double *Lout) {
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t b = 0; b < n_buckets; ++b) {
+        double z[3] = {zB[3 * b], zB[3 * b + 1], zB[3 * b + 2]};
+        double L[ORC_NLOC];
+        for (int i = 0; i < ORC_NLOC; ++i) L[i] = 0.0;
+        if (cc_off)
+            for (int64_t e = cc_off[b]; e < cc_off[b + 1]; ++e) {
+                int64_t c = cc_idx[e];
+                if (c < 0) continue;
+                if (c >= n_cells) {
+#pragma omp atomic write
+                    err = 1;
+                    continue;
+                }
+                orc_cc_accumulate(z, cells + c * (int64_t)stride, L);
+            }
+        if (cp_off)
+            for (int64_t e = cp_off[b]; e < cp_off[b + 1]; ++e) {
+                int64_t j = cp_idx[e];
+                if (j < 0) continue;
+                if (j >= n_particles) {
+#pragma omp atomic write
+                    err = 1;
+                    continue;
+                }
+                double xs[3] = {xyzm[4 * j], xyzm[4 * j + 1], xyzm[4 * j + 2]};
+                orc_cp_accumulate(z, xs, (double)xyzm[4 * j + 3], L);
+            }
+        if (Lout)
+            for (int i = 0; i < ORC_NLOC; ++i) Lout[b * ORC_NLOC + i] = L[i];
+        for (int32_t ti = 0; ti < count[b]; ++ti) {
+            int64_t i = (int64_t)first[b] + ti;
+            if (i < 0 || i >= n_particles) {
+#pragma omp atomic write
+                err = 1;
+                continue;
+            }
+            double xt[3] = {xyzm[4 * i], xyzm[4 * i + 1], xyzm[4 * i + 2]};
+            double acc[3] = {0, 0, 0}, pot = 0;
+            orc_local_eval(z, L, xt, acc, &pot);
+            out[4 * i + 0] += acc[0];
+            out[4 * i + 1] += acc[1];
+            out[4 * i + 2] += acc[2];
+            out[4 * i + 3] += pot;
+        }
+    }
+    return err;
+}
+
+/* ---------------------------------------------------------------------------
  * Integer side (SURVEY.md sec 8(c) "Integer side"; PAPER.md:L168, L188 fn 11:
  * lists are cut at warp multiples -- "655 elements ... 640 ... and 15").
  * Written spec of the packer: per bucket, tiles of 32 entries in list order,

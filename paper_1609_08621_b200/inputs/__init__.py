@@ -56,6 +56,10 @@ def _L():
         L.tg_pp_to_leaves.restype = c_int64
         L.tg_pp_to_leaves.argtypes = [c_int64, c_int64, c_void_p, c_void_p, c_int64, c_void_p, c_void_p, c_void_p,
                                       c_void_p]
+        L.tg_fmm_build.restype = c_void_p
+        L.tg_fmm_build.argtypes = [c_int64] + [c_void_p] * 9 + [c_int64, c_int64, c_double, c_double]
+        L.tg_fmm_totals.argtypes = [c_void_p, c_void_p]
+        L.tg_fmm_export_free.argtypes = [c_void_p, c_void_p, c_void_p]
         L.tg_num_threads.restype = c_int
         _lib = L
     return _lib
@@ -305,6 +309,29 @@ def f32(x: float) -> float:
     """x rounded to fp32: the C ABI takes the softening as a float, so the harness hands the SAME value to the
     oracle, to the list builder and to the library."""
     return float(np.float32(x))
+
+
+def build_fmm_lists(p: Problem, theta: float, eps: float, b0: int = 0, b1: int | None = None):
+    """FMM-style lists per bucket: a dict of four CSR lists
+    'pp', 'pc' (particle-particle / particle-cell, evaluated per sink), 'cp', 'cc' (cell-particle / cell-cell:
+    they feed the bucket's local expansion), each (off int64[n+1], idx int32), plus 'centre' float32[n,3], the
+    bucket centres of mass the local expansions are taken about."""
+    L = _L()
+    t = p.tree
+    b1 = p.n_buckets if b1 is None else b1
+    eps = f32(eps)
+    h = L.tg_fmm_build(t["first"].shape[0], _p(t["first"]), _p(t["count"]), _p(t["end"]), _p(t["isleaf"]), _p(p.cells),
+                       _p(t["bblo"]), _p(t["bbhi"]), _p(t["leaf_cell"]), _p(p.xyzm), b0, b1, float(theta), float(eps))
+    tot = np.zeros(4, np.int64)
+    L.tg_fmm_totals(h, _p(tot))
+    offs = [np.empty(b1 - b0 + 1, np.int64) for _ in range(4)]
+    idxs = [np.empty(int(tot[q]), np.int32) for q in range(4)]
+    op = (c_void_p * 4)(*[a.ctypes.data for a in offs]); ip = (c_void_p * 4)(*[a.ctypes.data for a in idxs])
+    L.tg_fmm_export_free(h, op, ip)
+    out = {k: (offs[q], idxs[q]) for q, k in enumerate(("pp", "pc", "cp", "cc"))}
+    out["centre"] = np.ascontiguousarray(p.cells[t["leaf_cell"][b0:b1], :3])
+    out["theta"] = theta; out["eps"] = eps
+    return out
 
 
 def with_lists(p: Problem, theta: float, eps: float) -> Problem:
