@@ -129,6 +129,8 @@ typedef struct {
     int64_t fixup_sinks;     /* sinks re-evaluated by the fp64 fix-up kernel                      */
     int64_t invalid_values;  /* PKDG_VALIDATE: particles / cell records with values out of range  */
     int64_t invalid_pairs;   /* PKDG_VALIDATE: listed (sink, cell) pairs with |x - COM| <= b_max   */
+    int64_t interactions_cc; /* pkdg_gravity_eval_fmm: entries of the C-C lists (one per bucket x cell)  */
+    int64_t interactions_cp; /* pkdg_gravity_eval_fmm: entries of the C-P lists (one per bucket x particle) */
 } pkdg_stats;
 
 /* Create / destroy a context on CUDA device `device`.  The context owns only internal workspace
@@ -168,6 +170,24 @@ pkdg_status pkdg_gravity_eval_groups(pkdg_ctx *ctx, const pkdg_particles *partic
                                      const pkdg_buckets *buckets, const pkdg_groups *groups, const pkdg_list *pp,
                                      const pkdg_list *pc, float eps, uint32_t flags, float *out_acc_pot,
                                      void *stream);
+
+/* The FMM form of the path (PAPER.md:L57 cell-cell interactions, L69 fn 2 cell-particle
+ * interactions, L71 "The local expansion of the potential about the sink's center of mass is actually done to
+ * 5th order ... accumulating the CC and CP interactions"; readings A20-A22).  Every bucket b has four
+ * lists: pp and pc as in pkdg_gravity_eval, plus cc (indices of source CELLS) and cp (indices of source
+ * PARTICLES) that act on the bucket as a whole through its local expansion about centres[b] ([n_buckets][3]
+ * fp32, device; the bucket's centre of mass in the paper):
+ *     L_n = - sum_m (-1)^|m| M_m binom(n+m, m) t_{n+m}(centres[b] - COM_c),  |n| <= 5,  |n| + |m| <= 5,
+ *           |m| in {0, 2, 3, 4}  (a source particle is a cell with only M_0 = m_j at x_j),
+ *     phi_i += sum_n L_n s^n,   a_i -= grad of that polynomial,   s = x_i - centres[b],
+ * t_k = d^k(1/|r|)/k! as above; unsoftened.  The result is the SUM of the four lists' contributions.  Any of the
+ * four lists may be NULL.  A C-C or C-P source must lie outside the sphere of the bucket's sinks about
+ * centres[b] (the expansion diverges inside; any acceptance criterion of the kind of PAPER.md:L69 ensures it).
+ * PKDG_PP_LEAVES is not supported here.  pkdg_stats: interactions_cc / interactions_cp count list entries. */
+pkdg_status pkdg_gravity_eval_fmm(pkdg_ctx *ctx, const pkdg_particles *particles, const pkdg_cells *cells,
+                                  const pkdg_buckets *buckets, const float *centres, const pkdg_list *pp,
+                                  const pkdg_list *pc, const pkdg_list *cp, const pkdg_list *cc, float eps,
+                                  uint32_t flags, float *out_acc_pot, void *stream);
 
 /* Streamed variant (a6; "fully asynchronous", L278 bounded queue): particles, cells
  * and out are device buffers, buckets and lists are PINNED HOST buffers.  Contiguous bucket ranges

@@ -30,7 +30,7 @@ CELLQ_FLOATS = 32
 
 EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_gravity_eval_host_range", "pkdg_gravity_eval_groups",
-           "pkdg_gravity_eval_host_groups", "pkdg_build_lists_count", "pkdg_build_lists_fill", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
+           "pkdg_gravity_eval_host_groups", "pkdg_gravity_eval_fmm", "pkdg_build_lists_count", "pkdg_build_lists_fill", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
            "pkdg_get_stats", "pkdg_set_option", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count",
            "pkdg_status_string", "pkdg_last_error", "pkdg_version", "pkdg_fma_peak_probe"]
 
@@ -67,7 +67,8 @@ class _List(Structure):
 class Stats(Structure):
     _fields_ = [("n_buckets", c_int64), ("interactions_pp", c_int64), ("interactions_pc", c_int64),
                 ("tiles_pp", c_int64), ("tiles_pc", c_int64), ("bad_entries", c_int64), ("chunks", c_int64),
-                ("fixup_sinks", c_int64), ("invalid_values", c_int64), ("invalid_pairs", c_int64)]
+                ("fixup_sinks", c_int64), ("invalid_values", c_int64), ("invalid_pairs", c_int64),
+                ("interactions_cc", c_int64), ("interactions_cp", c_int64)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -100,6 +101,9 @@ def _load():
     L.pkdg_gravity_eval_host_groups.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                                 POINTER(_Groups), POINTER(_List), POINTER(_List), c_float, c_uint32,
                                                 c_void_p, c_int32, c_int64]
+    L.pkdg_gravity_eval_fmm.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets), c_void_p,
+                                        POINTER(_List), POINTER(_List), POINTER(_List), POINTER(_List), c_float, c_uint32,
+                                        c_void_p, c_void_p]
     L.pkdg_build_lists_count.argtypes = [c_void_p, POINTER(_Tree), POINTER(_Cells), c_void_p, c_int64, c_double, c_double,
                                          c_uint32, c_void_p, c_void_p, c_void_p, c_void_p]
     L.pkdg_build_lists_fill.argtypes = [c_void_p, POINTER(_Tree), POINTER(_Cells), c_void_p, c_int64, c_double, c_double,
@@ -295,6 +299,21 @@ class Context:
                                                int(flags), _ptr(out_h), int(n_streams), int(max_entries_per_chunk))
         self._check(s, "pkdg_gravity_eval_host_groups")
         return out_h
+
+    def gravity_eval_fmm(self, xyzm, cells, first, count, centres, pp_off, pp_idx, pc_off, pc_idx, cp_off, cp_idx,
+                         cc_off, cc_idx, eps, out, flags=0, stream=None):
+        """pkdg_gravity_eval_fmm: four lists per bucket (P-P, P-C per sink; C-P, C-C through the bucket's local
+        expansion about centres[b]); everything resident; asynchronous on `stream`."""
+        P, C, B, pp, pc = self._structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx)
+        _dt(centres, "float32", "centres"); _dt(cp_off, "int64", "cp_off"); _dt(cp_idx, "int32", "cp_idx")
+        _dt(cc_off, "int64", "cc_off"); _dt(cc_idx, "int32", "cc_idx"); _dt(out, "float32", "out")
+        cp = _List(_ptr(cp_off), _ptr(cp_idx)) if cp_off is not None else None
+        cc = _List(_ptr(cc_off), _ptr(cc_idx)) if cc_off is not None else None
+        s = _lib.pkdg_gravity_eval_fmm(self._h, byref(P), byref(C) if C else None, byref(B), _ptr(centres),
+                                       byref(pp) if pp else None, byref(pc) if pc else None, byref(cp) if cp else None,
+                                       byref(cc) if cc else None, float(eps), int(flags), _ptr(out), _stream_ptr(stream))
+        self._check(s, "pkdg_gravity_eval_fmm")
+        return out
 
     @staticmethod
     def _tree(tree, cells):

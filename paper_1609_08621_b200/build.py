@@ -12,7 +12,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = os.path.join(HERE, "csrc", "pkdg.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "pkdg_kernels.cuh"), os.path.join(ROOT, "include", "pkdg.h")]
+DEPS = [SRC, os.path.join(HERE, "csrc", "pkdg_kernels.cuh"), os.path.join(HERE, "csrc", "pkdg_fmm.cuh"),
+        os.path.join(HERE, "csrc", "pkdg_fmm_gen.cuh"), os.path.join(ROOT, "include", "pkdg.h")]
 LIB = os.path.join(HERE, "libpkdg.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

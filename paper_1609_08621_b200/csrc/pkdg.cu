@@ -10,6 +10,7 @@
 #include <string>
 
 #include "pkdg_kernels.cuh"
+#include "pkdg_fmm.cuh"
 
 using namespace pkdg;
 
@@ -47,7 +48,7 @@ struct pkdg_ctx {
     BucketDesc* desc = nullptr;
     int64_t desc_cap = 0;
     DevStats* stats = nullptr;
-    unsigned int* counters = nullptr;  // [2 (kMaxSlots + 1)]: work counters, then fix-up queue lengths
+    unsigned int* counters = nullptr;  // [2 (kMaxSlots + 1) + 1]: work counters, fix-up queue lengths, C-C / C-P kernel
     int4* fixq = nullptr;              // fix-up queue of the resident call
     int64_t fixq_cap = 0;
     float kappa2 = kDefaultKappa2;     // PKDG_OPT_KAPPA2
@@ -293,9 +294,9 @@ pkdg_status pkdg_create(pkdg_ctx** out, int device) {
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->stats, sizeof(DevStats));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->counters, sizeof(unsigned int) * 2 * (kMaxSlots + 1));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->counters, sizeof(unsigned int) * (2 * (kMaxSlots + 1) + 1));
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(DevStats));
-    if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(unsigned int) * 2 * (kMaxSlots + 1));
+    if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(unsigned int) * (2 * (kMaxSlots + 1) + 1));
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_ready, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         fprintf(stderr, "pkdg_create: %s\n", cudaGetErrorString(e));
@@ -332,7 +333,7 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
 // G != NULL (group-shared lists): the lists have G->n + 1 offsets and the range must be all buckets.
 static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* Bfull,
                                  int64_t b0, int64_t b1, const pkdg_groups* G, const pkdg_list* pp, const pkdg_list* pc,
-                                 float eps, uint32_t flags, float* out, void* stream) {
+                                 float eps, uint32_t flags, float* out, void* stream, bool reset_stats = true) {
     pkdg_status s = check_common(ctx, P, C, Bfull, pp, pc, out);
     if (s != PKDG_OK) return s;
     if (G && (G->n < 0 || (G->n > 0 && (!G->first_bucket || !G->n_buckets))))
@@ -344,7 +345,7 @@ static pkdg_status resident_impl(pkdg_ctx* ctx, const pkdg_particles* P, const p
     CK(cudaSetDevice(ctx->device));
     const bool has_pp = pp && pp->offsets, has_pc = pc && pc->offsets && C && C->n > 0;
     ctx->last_stream = st; ctx->last_chunks = 1; ctx->last_buckets = B->n;
-    CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
+    if (reset_stats) CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
     if (B->n == 0) return PKDG_OK;
     if ((s = ensure(ctx, &ctx->desc, &ctx->desc_cap, B->n)) != PKDG_OK) return s;
     // the group kernel queues one entry per flagged SINK, the bucket kernel one per (bucket, pass)
@@ -426,6 +427,54 @@ pkdg_status pkdg_gravity_eval_range(pkdg_ctx* ctx, const pkdg_particles* P, cons
                                     int64_t b0, int64_t b1, const pkdg_list* pp, const pkdg_list* pc, float eps,
                                     uint32_t flags, float* out, void* stream) {
     return resident_impl(ctx, P, C, B, b0, b1, nullptr, pp, pc, eps, flags, out, stream);
+}
+
+// The FMM form of the path: the local expansion of every bucket from its C-C and C-P lists, evaluated at the
+// bucket's particles (pkdg_fmm_kernel), then the P-P and P-C lists on top (PKDG_ACCUMULATE, so that the
+// conditioning test of the evaluation kernel sees the total acceleration).
+pkdg_status pkdg_gravity_eval_fmm(pkdg_ctx* ctx, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
+                                  const float* centres, const pkdg_list* pp, const pkdg_list* pc, const pkdg_list* cp,
+                                  const pkdg_list* cc, float eps, uint32_t flags, float* out, void* stream) {
+    pkdg_status s = check_common(ctx, P, C, B, pp, pc, out);
+    if (s != PKDG_OK) return s;
+    const bool has_cc = cc && cc->offsets, has_cp = cp && cp->offsets;
+    const bool has_near = (pp && pp->offsets) || (pc && pc->offsets);
+    if (has_cc) {
+        if (!C || C->n < 0 || C->n > 0x7fffffffLL || (C->n > 0 && !C->rec) || C->stride_floats < PKDG_CELL_FLOATS)
+            return fail(ctx, PKDG_EINVAL, "C-C list given without valid cells");
+        if (!cc->idx && C->n > 0) return fail(ctx, PKDG_EINVAL, "cc->idx is NULL");
+    }
+    if (has_cp && !cp->idx && P->n > 0) return fail(ctx, PKDG_EINVAL, "cp->idx is NULL");
+    if ((has_cc || has_cp) && B->n > 0 && !centres) return fail(ctx, PKDG_EINVAL, "centres must not be NULL with a C-C or C-P list");
+    if (flags & PKDG_PP_LEAVES) return fail(ctx, PKDG_EINVAL, "PKDG_PP_LEAVES is not supported by pkdg_gravity_eval_fmm");
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    ctx->last_stream = st; ctx->last_chunks = 1; ctx->last_buckets = B->n;
+    CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
+    if (B->n == 0) return PKDG_OK;
+    if (!has_cc && !has_cp) return resident_impl(ctx, P, C, B, 0, B->n, nullptr, pp, pc, eps, flags, out, stream, false);
+    FmmParams f;
+    f.xyzm = reinterpret_cast<const float4*>(P->xyzm);
+    f.rec = has_cc ? C->rec : nullptr;
+    f.stride = has_cc ? C->stride_floats : PKDG_CELL_FLOATS;
+    f.rec_vec4 = has_cc && aligned16(C->rec) && (C->stride_floats % 4 == 0);
+    f.n_particles = P->n; f.n_cells = has_cc ? C->n : 0; f.n_buckets = B->n;
+    f.first = B->first; f.count = B->count; f.centre = centres;
+    f.cc_off = has_cc ? cc->offsets : nullptr; f.cc_idx = has_cc ? cc->idx : nullptr;
+    f.cp_off = has_cp ? cp->offsets : nullptr; f.cp_idx = has_cp ? cp->idx : nullptr;
+    f.out = reinterpret_cast<float4*>(out);
+    f.stats = ctx->stats;
+    f.work_counter = ctx->counters + 2 * (kMaxSlots + 1);
+    f.flags = flags;
+    CK(cudaMemsetAsync(f.work_counter, 0, sizeof(unsigned int), st));
+    int64_t grid = (int64_t)ctx->num_sms * 2;
+    const int64_t want = (B->n + kFmmWarps - 1) / kFmmWarps;
+    if (grid > want) grid = want;
+    pkdg_fmm_kernel<<<(unsigned)grid, kFmmWarps * 32, 0, st>>>(f);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    if (!has_near) return PKDG_OK;
+    return resident_impl(ctx, P, C, B, 0, B->n, nullptr, pp, pc, eps, flags | PKDG_ACCUMULATE, out, stream, false);
 }
 
 // out_host != NULL: the rows of every chunk (buckets are then known to be contiguous runs in ascending
@@ -815,6 +864,8 @@ pkdg_status pkdg_get_stats(pkdg_ctx* ctx, pkdg_stats* out) {
     out->fixup_sinks = (int64_t)h.fixup_sinks;
     out->invalid_values = (int64_t)h.invalid_values;
     out->invalid_pairs = (int64_t)h.invalid_pairs;
+    out->interactions_cc = (int64_t)h.interactions_cc;
+    out->interactions_cp = (int64_t)h.interactions_cp;
     out->chunks = ctx->last_chunks;
     if (h.bad_entries) return fail(ctx, PKDG_EBADLIST, "validation found malformed buckets or list entries");
     if (h.invalid_values || h.invalid_pairs)

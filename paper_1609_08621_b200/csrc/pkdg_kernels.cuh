@@ -29,6 +29,7 @@ struct __align__(16) BucketDesc {
 struct DevStats {
     unsigned long long interactions_pp, interactions_pc, tiles_pp, tiles_pc, bad_entries, fixup_sinks;
     unsigned long long invalid_values, invalid_pairs;  // PKDG_VALIDATE
+    unsigned long long interactions_cc, interactions_cp;  // pkdg_gravity_eval_fmm: entries of the C-C / C-P lists
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -963,18 +964,20 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
                 }
                 warp_transpose_reduce<32>(v, lane);       // lane l: component l & 3 of sink l >> 2
-                const float r = v[0];
+                const bool valid = (lane >> 2) < ntp;
+                // with PKDG_ACCUMULATE the row already holds a part of the sum (the local expansion of
+                // pkdg_gravity_eval_fmm): the conditioning test is against the TOTAL acceleration
+                const float r = (accumulate && valid) ? v[0] + outf[lane] : v[0];
                 float sq = (lane & 3) < 3 ? r * r : 0.0f;
                 sq += __shfl_xor_sync(0xffffffffu, sq, 1);
                 sq += __shfl_xor_sync(0xffffffffu, sq, 2);
-                const bool valid = (lane >> 2) < ntp;
                 bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
                 const unsigned ballot = __ballot_sync(0xffffffffu, flag);
                 if (ballot) {   // warp-uniform; every lane takes part in the push
                     const bool queued = fix_push(p, (int)S.bucket[0], t0, ballot, lane);
                     flag = flag && queued;
                 }
-                if (valid && !flag) outf[lane] = accumulate ? r + outf[lane] : r;
+                if (valid && !flag) outf[lane] = r;
             } else {
                 float v[64];
 #pragma unroll
@@ -984,21 +987,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const Eval
                     v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
                 }
                 warp_transpose_reduce<64>(v, lane);        // lane l: components 2 (l & 1), 2 (l & 1) + 1 of sink l >> 1
-                float sq = (lane & 1) ? v[0] * v[0] : fmaf(v[0], v[0], v[1] * v[1]);
-                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
                 const bool valid = (lane >> 1) < ntp;
+                float2* o2 = reinterpret_cast<float2*>(outf) + lane;
+                float2 r = make_float2(v[0], v[1]);
+                if (accumulate && valid) { const float2 old = *o2; r.x += old.x; r.y += old.y; }
+                float sq = (lane & 1) ? r.x * r.x : fmaf(r.x, r.x, r.y * r.y);
+                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
                 bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
                 const unsigned ballot = __ballot_sync(0xffffffffu, flag);
                 if (ballot) {
                     const bool queued = fix_push(p, (int)S.bucket[0], (int)((unsigned)t0 | 0x80000000u), ballot, lane);
                     flag = flag && queued;
                 }
-                if (valid && !flag) {
-                    float2* o2 = reinterpret_cast<float2*>(outf) + lane;
-                    float2 r = make_float2(v[0], v[1]);
-                    if (accumulate) { const float2 old = *o2; r.x += old.x; r.y += old.y; }
-                    *o2 = r;
-                }
+                if (valid && !flag) *o2 = r;
             }
         }
         if (!has_next) break;
@@ -1250,7 +1251,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
 
             // ---- a5: no reduction -- the lane holds its sinks' totals.  Conditioning test, queue, write-back.
             {
-                const float a2A = fmaf(az.x, az.x, fmaf(ay.x, ay.x, ax.x * ax.x)), a2B = fmaf(az.y, az.y, fmaf(ay.y, ay.y, ax.y * ax.y));
+                float4 rA = make_float4(ax.x, ay.x, az.x, aw.x), rB = make_float4(ax.y, ay.y, az.y, aw.y);
+                if (accumulate) {   // the conditioning test is against the total the row will hold
+                    if (iA >= 0) { const float4 o = p.out[iA]; rA.x += o.x; rA.y += o.y; rA.z += o.z; rA.w += o.w; }
+                    if (iB >= 0) { const float4 o = p.out[iB]; rB.x += o.x; rB.y += o.y; rB.z += o.z; rB.w += o.w; }
+                }
+                const float a2A = fmaf(rA.z, rA.z, fmaf(rA.y, rA.y, rA.x * rA.x)), a2B = fmaf(rB.z, rB.z, fmaf(rB.y, rB.y, rB.x * rB.x));
                 bool flagA = fix_on && iA >= 0 && s2.x >= p.fix_k * a2A, flagB = fix_on && iB >= 0 && s2.y >= p.fix_k * a2B;
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
@@ -1264,16 +1270,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
                         else if (h) flagB = false; else flagA = false;   // queue full (cannot happen): keep the fp32 row
                     }
                 }
-                if (iA >= 0 && !flagA) {
-                    float4 r = make_float4(ax.x, ay.x, az.x, aw.x);
-                    if (accumulate) { const float4 o = p.out[iA]; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }
-                    p.out[iA] = r;
-                }
-                if (iB >= 0 && !flagB) {
-                    float4 r = make_float4(ax.y, ay.y, az.y, aw.y);
-                    if (accumulate) { const float4 o = p.out[iB]; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }
-                    p.out[iB] = r;
-                }
+                if (iA >= 0 && !flagA) p.out[iA] = rA;
+                if (iB >= 0 && !flagB) p.out[iB] = rB;
             }
         }
     }

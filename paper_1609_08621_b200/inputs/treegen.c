@@ -289,75 +289,87 @@ void tg_lists_export_free(tg_lists *L, int64_t *pp_off, int32_t *pp_idx, int64_t
  * Every particle is covered exactly once per bucket by the union of the four lists.
  * ---------------------------------------------------------------------------------------- */
 typedef struct {
-    int64_t b0, b1;
-    ivec v[4];            /* 0 = P-P, 1 = P-C, 2 = C-P, 3 = C-C (serial build: harness sizes only) */
-    int64_t *len[4];
+    int64_t b0, b1, nblk, blk;
+    ivec *v[4];           /* per block: 0 = P-P, 1 = P-C, 2 = C-P, 3 = C-C */
+    int64_t *len[4];      /* per bucket (b - b0) */
 } tg_fmm;
 
 tg_fmm *tg_fmm_build(int64_t ncell, const int32_t *first, const int32_t *count, const int32_t *end,
                      const int32_t *isleaf, const float *rec, const float *bblo, const float *bbhi,
                      const int32_t *leaf_cell, const float *xyzm, int64_t b0, int64_t b1, double theta, double eps) {
     tg_fmm *F = calloc(1, sizeof(tg_fmm));
-    F->b0 = b0; F->b1 = b1;
-    for (int q = 0; q < 4; ++q) F->len[q] = calloc(b1 - b0 + 1, sizeof(int64_t));
+    F->b0 = b0; F->b1 = b1; F->blk = 512;
+    F->nblk = (b1 - b0 + F->blk - 1) / F->blk;
+    for (int q = 0; q < 4; ++q) {
+        F->v[q] = calloc(F->nblk ? F->nblk : 1, sizeof(ivec));
+        F->len[q] = calloc(b1 - b0 + 1, sizeof(int64_t));
+    }
     double gap_min2 = 4.0 * eps * eps;
-    for (int64_t b = b0; b < b1; ++b) {
-        int64_t cb = leaf_cell[b];
-        const float *rb = rec + REC * cb;
-        double bx = rb[0], by = rb[1], bz = rb[2], bmaxB = rb[35];
-        const float *lob = bblo + 3 * cb, *hib = bbhi + 3 * cb;
-        int64_t n0[4];
-        for (int q = 0; q < 4; ++q) n0[q] = F->v[q].n;
-        int64_t k = 0;
-        while (k < ncell) {
-            int kind = 0; /* 0 none, 1 P-C, 3 C-C */
-            if (k != cb && count[k] >= 2) {
-                const float *rk = rec + REC * k;
-                double dx = bx - rk[0], dy = by - rk[1], dz = bz - rk[2];
-                double d = sqrt(dx * dx + dy * dy + dz * dz);
-                const float *lok = bblo + 3 * k, *hik = bbhi + 3 * k;
-                double g2 = 0;
-                for (int a = 0; a < 3; ++a) {
-                    double g = 0;
-                    if ((double)lok[a] - hib[a] > g) g = (double)lok[a] - hib[a];
-                    if ((double)lob[a] - hik[a] > g) g = (double)lob[a] - hik[a];
-                    g2 += g * g;
-                }
-                if (g2 >= gap_min2) {
-                    if (d > 1.5 * bmaxB / theta + (double)rk[35] / theta) kind = 3;
-                    else if (d > bmaxB + (double)rk[35] / theta) kind = 1;
-                }
-            }
-            if (kind) { push(&F->v[kind], (int32_t)k); k = end[k]; }
-            else if (isleaf[k]) {
-                for (int32_t t = 0; t < count[k]; ++t) {
-                    int32_t j = first[k] + t;
-                    int cp = 0;
-                    if (k != cb) {
-                        const float *xj = xyzm + 4 * (int64_t)j;
-                        double dx = bx - xj[0], dy = by - xj[1], dz = bz - xj[2];
-                        double d = sqrt(dx * dx + dy * dy + dz * dz);
-                        double g2 = 0;
-                        for (int a = 0; a < 3; ++a) {
-                            double g = 0;
-                            if ((double)xj[a] - hib[a] > g) g = (double)xj[a] - hib[a];
-                            if ((double)lob[a] - xj[a] > g) g = (double)lob[a] - xj[a];
-                            g2 += g * g;
-                        }
-                        cp = d > 1.5 * bmaxB / theta && g2 >= gap_min2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t ib = 0; ib < F->nblk; ++ib) {
+        ivec *v[4] = {&F->v[0][ib], &F->v[1][ib], &F->v[2][ib], &F->v[3][ib]};
+        int64_t e1 = b0 + (ib + 1) * F->blk; if (e1 > b1) e1 = b1;
+        for (int64_t b = b0 + ib * F->blk; b < e1; ++b) {
+            int64_t cb = leaf_cell[b];
+            const float *rb = rec + REC * cb;
+            double bx = rb[0], by = rb[1], bz = rb[2], bmaxB = rb[35];
+            const float *lob = bblo + 3 * cb, *hib = bbhi + 3 * cb;
+            int64_t n0[4];
+            for (int q = 0; q < 4; ++q) n0[q] = v[q]->n;
+            int64_t k = 0;
+            while (k < ncell) {
+                int kind = 0; /* 0 none, 1 P-C, 3 C-C */
+                if (k != cb && count[k] >= 2) {
+                    const float *rk = rec + REC * k;
+                    double dx = bx - rk[0], dy = by - rk[1], dz = bz - rk[2];
+                    double d = sqrt(dx * dx + dy * dy + dz * dz);
+                    const float *lok = bblo + 3 * k, *hik = bbhi + 3 * k;
+                    double g2 = 0;
+                    for (int a = 0; a < 3; ++a) {
+                        double g = 0;
+                        if ((double)lok[a] - hib[a] > g) g = (double)lok[a] - hib[a];
+                        if ((double)lob[a] - hik[a] > g) g = (double)lob[a] - hik[a];
+                        g2 += g * g;
                     }
-                    push(&F->v[cp ? 2 : 0], j);
+                    if (g2 >= gap_min2) {
+                        if (d > 1.5 * bmaxB / theta + (double)rk[35] / theta) kind = 3;
+                        else if (d > bmaxB + (double)rk[35] / theta) kind = 1;
+                    }
                 }
-                k = end[k];
-            } else k = k + 1;
+                if (kind) { push(v[kind], (int32_t)k); k = end[k]; }
+                else if (isleaf[k]) {
+                    for (int32_t t = 0; t < count[k]; ++t) {
+                        int32_t j = first[k] + t;
+                        int cp = 0;
+                        if (k != cb) {
+                            const float *xj = xyzm + 4 * (int64_t)j;
+                            double dx = bx - xj[0], dy = by - xj[1], dz = bz - xj[2];
+                            double d = sqrt(dx * dx + dy * dy + dz * dz);
+                            double g2 = 0;
+                            for (int a = 0; a < 3; ++a) {
+                                double g = 0;
+                                if ((double)xj[a] - hib[a] > g) g = (double)xj[a] - hib[a];
+                                if ((double)lob[a] - xj[a] > g) g = (double)lob[a] - xj[a];
+                                g2 += g * g;
+                            }
+                            cp = d > 1.5 * bmaxB / theta && g2 >= gap_min2;
+                        }
+                        push(v[cp ? 2 : 0], j);
+                    }
+                    k = end[k];
+                } else k = k + 1;
+            }
+            for (int q = 0; q < 4; ++q) F->len[q][b - b0] = v[q]->n - n0[q];
         }
-        for (int q = 0; q < 4; ++q) F->len[q][b - b0] = F->v[q].n - n0[q];
     }
     return F;
 }
 
 void tg_fmm_totals(const tg_fmm *F, int64_t *tot) {
-    for (int q = 0; q < 4; ++q) tot[q] = F->v[q].n;
+    for (int q = 0; q < 4; ++q) {
+        tot[q] = 0;
+        for (int64_t i = 0; i < F->nblk; ++i) tot[q] += F->v[q][i].n;
+    }
 }
 
 /* off: 4 arrays of b1-b0+1 int64; idx: 4 arrays sized by tg_fmm_totals.  Frees F. */
@@ -366,8 +378,12 @@ void tg_fmm_export_free(tg_fmm *F, int64_t **off, int32_t **idx) {
     for (int q = 0; q < 4; ++q) {
         off[q][0] = 0;
         for (int64_t b = 0; b < nb; ++b) off[q][b + 1] = off[q][b] + F->len[q][b];
-        if (F->v[q].n) memcpy(idx[q], F->v[q].v, sizeof(int32_t) * F->v[q].n);
-        free(F->v[q].v); free(F->len[q]);
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int64_t ib = 0; ib < F->nblk; ++ib) {
+            if (F->v[q][ib].n) memcpy(idx[q] + off[q][ib * F->blk], F->v[q][ib].v, sizeof(int32_t) * F->v[q][ib].n);
+            free(F->v[q][ib].v);
+        }
+        free(F->v[q]); free(F->len[q]);
     }
     free(F);
 }
