@@ -34,6 +34,9 @@ sys.path.insert(0, ROOT)
 F_PP = 19
 F_PC = 187
 PAPER_F_PP, PAPER_F_PC = 53, 215
+# C-C / C-P path (pkdg_fmm.cuh, formulas as executed): per C-C entry, per C-P entry, per sink evaluated, per bucket
+F_CC, F_CP, F_LOC_SINK, F_LOC_BUCKET = 1091, 468, 488, 1848
+PAPER_F_CC, PAPER_F_CP = 479, 213       # PAPER.md Table 3 (L216-217), context only
 SM_COUNT_NOMINAL, FP32_LANES_PER_SM = 148, 128
 
 
@@ -478,6 +481,47 @@ def run_ours(args, rank, world, local_rank):
                             "api": "H2D of particles, cells, tree; pkdg_build_lists_count + _fill; pkdg_gravity_eval; D2H"}}
         del tree_d, sink_d, d_ppo, d_pco, d_ppi, d_pci, out_h
 
+    # ---- FMM form of the path: four lists per bucket, C-C / C-P through the 5th-order local
+    #      expansion.  Extra key, N = 1: the whole call and the local-expansion kernel alone.
+    fmm = None
+    if not args.no_fmm and world == 1:
+        from paper_1609_08621_b200 import inputs as _inputs
+        t0 = time.perf_counter()
+        F = _inputs.build_fmm_lists(p, p.theta, p.eps)
+        f_gen = time.perf_counter() - t0
+        T = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        df = {k: (T(F[k][0]), T(F[k][1])) for k in ("pp", "pc", "cp", "cc")}
+        d_centre = T(F["centre"])
+        cnt_all = p.count.astype(np.int64)
+        fI_pp = int(np.dot(cnt_all, np.diff(F["pp"][0]))); fI_pc = int(np.dot(cnt_all, np.diff(F["pc"][0])))
+        n_cc, n_cp = int(F["cc"][1].shape[0]), int(F["cp"][1].shape[0])
+
+        def fstep(near=True):
+            n_ = df if near else {"pp": (None, None), "pc": (None, None)}
+            ctx.gravity_eval_fmm(g.xyzm, g.cells, g.first, g.count, d_centre, n_["pp"][0], n_["pp"][1], n_["pc"][0],
+                                 n_["pc"][1], df["cp"][0], df["cp"][1], df["cc"][0], df["cc"][1], g.eps, out, flags=flags)
+        for _ in range(3):
+            fstep()
+        fms = timed(fstep, args.steps)
+        fst = ctx.get_stats()
+        assert fst["interactions_cc"] == n_cc and fst["interactions_cp"] == n_cp and fst["bad_entries"] == 0
+        assert fst["interactions_pp"] == fI_pp and fst["interactions_pc"] == fI_pc
+        for _ in range(2):
+            fstep(False)
+        lms = timed(lambda: fstep(False), args.steps)
+        fl_loc = F_CC * n_cc + F_CP * n_cp + F_LOC_SINK * p.n + F_LOC_BUCKET * p.n_buckets
+        fmm = {"lists_per_bucket": {k: F[k][1].shape[0] / p.n_buckets for k in ("pp", "pc", "cp", "cc")},
+               "I_pp": fI_pp, "I_pc": fI_pc, "I_cc": n_cc, "I_cp": n_cp, "ms_per_step": fms,
+               "sinks_per_s": p.n / (fms * 1e-3), "local_expansion_kernel_ms": lms,
+               "flops_as_executed": {"cc": F_CC, "cp": F_CP, "per_sink_evaluation": F_LOC_SINK, "per_bucket_reduction": F_LOC_BUCKET},
+               "local_expansion_tflops": fl_loc / (lms * 1e-3) / 1e12, "frac_fp32_fma_peak_local_kernel": None,
+               "paper_convention_tflops_local": (PAPER_F_CC * n_cc + PAPER_F_CP * n_cp) / (lms * 1e-3) / 1e12,
+               "fixup_sinks": fst["fixup_sinks"], "host_list_build_s": round(f_gen, 1),
+               "speedup_vs_per_sink_lists": ms_step / fms,
+               "note": "same tree, same theta: C-C where |COM_B - COM_k| > 1.5 RO_B + RO_k (PAPER.md:L69), else the per-sink "
+                       "criterion; every bucket keeps its own local expansion (no hierarchical sink side)"}
+        del df, d_centre
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -520,7 +564,9 @@ def run_ours(args, rank, world, local_rank):
             "paper_convention_tflops": (PAPER_F_PP * tot_pp + PAPER_F_PC * tot_pc) / (ms_step * 1e-3) / 1e12,
             "interactions_per_s": {"pp": tot_pp / (ms_step * 1e-3), "pc": tot_pc / (ms_step * 1e-3)},
             "gen_seconds": round(gen_s, 1), "flags": args.flags, "pp_leaves": leaves, "group_lists": groups,
-            "device_lists": devlists}
+            "device_lists": devlists, "fmm": fmm}
+    if fmm is not None:
+        fmm["frac_fp32_fma_peak_local_kernel"] = fmm["local_expansion_tflops"] / peak_tflops
     if groups is not None:
         groups["frac_fp32_fma_peak_kernel"] = (F_PP * groups["I_pp"] + F_PC * groups["I_pc"]) / (groups["kernel_ms"] * 1e-3) / 1e12 / peak_tflops
     if leaves is not None:
@@ -757,6 +803,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-leaves", action="store_true", help="skip the extra PKDG_PP_LEAVES measurement")
     ap.add_argument("--no-groups", action="store_true", help="skip the extra group-shared-lists measurement")
+    ap.add_argument("--no-fmm", action="store_true", help="skip the extra four-list (C-C / C-P local expansion) measurement")
     ap.add_argument("--no-device-lists", action="store_true", help="skip the extra device list-construction measurement")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=4)

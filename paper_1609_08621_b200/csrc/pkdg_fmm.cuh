@@ -19,8 +19,10 @@
 // shift are generated straight-line code (pkdg_fmm_gen.cuh, written by gen_fmm.py from the definition of D_k by
 // exact differentiation -- not from a recurrence).  The 32 lane partials of each coefficient are summed through
 // shared memory in a fixed order, then lanes = sinks evaluate the polynomial and its gradient.
-// Flops as executed per C-C interaction: 52 (monomials) + 196 (derivatives: 140 terms, 56 scalings) + 64 (moments)
-// + 672 (shift) + ~25 (geometry) = 1009; per C-P interaction 52 + 196 + 112 + ~25 = 385; per sink 52 + 2 x 221.
+// Flops as executed (add / mul = 1, FMA = 2, rsqrt = 1): per C-C entry 23 (geometry, Newton step) + 52 (monomials)
+// + 280 (derivative polynomials: 140 terms, 56 scalings) + 64 (moments) + 672 (shift: 336 FMA) = 1091; per C-P entry
+// 23 + 52 + 280 + 113 = 468; per sink 6 + 52 + 112 + 315 + 3 = 488; per bucket 1848 (reduction).  The paper's
+// audit of its own CPU code gives 472 + rsqrt / 206 + rsqrt (Table 3).
 #pragma once
 #include "pkdg_fmm_gen.cuh"
 
