@@ -68,6 +68,8 @@ struct pkdg_ctx {
     cudaStream_t last_stream = nullptr;
     bool eval_configured = false;      // dynamic-smem opt-in of the evaluation kernel done on this device
     int eval_per_sm = 1;
+    int evalb_per_sm[2] = {0, 0};
+    int bucket_gen = 4;                // TEMPORARY A/B switch (env PKDG_BUCKET_GEN)
     int evalg_per_sm[2] = {0, 0};      // the same for the two instantiations of the group kernel (0 = not yet)
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
@@ -111,7 +113,10 @@ constexpr int kEvalMinBlocks = 3;  // CTAs per SM it is compiled for (168 regist
 
 // The evaluation kernel needs more than the default 48 KB of dynamic shared memory.  Function attributes
 // are per device, so the opt-in is made once per context (a pkdg_ctx is bound to one device).
+template <bool LEAF> pkdg_status launch_evalb_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st);
 pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    if (ctx->bucket_gen == 4)
+        return (p.flags & PKDG_PP_LEAVES) ? launch_evalb_t<true>(ctx, p, st) : launch_evalb_t<false>(ctx, p, st);
     auto kern = pkdg_eval3_kernel<kEvalWarps, kEvalMinBlocks>;
     const int smem = kEvalWarps * (int)sizeof(WarpSmem3);
     if (!ctx->eval_configured) {
@@ -126,6 +131,33 @@ pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
     if (grid > want) grid = want;
     if (grid < 1) grid = 1;
     kern<<<(unsigned)grid, kEvalWarps * 32, smem, st>>>(p);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
+constexpr int kBucketWarps = 4;      // generation-4 bucket kernel: one bucket per warp
+#ifndef PKDG_B_MINB
+#define PKDG_B_MINB 5
+#endif
+constexpr int kBucketMinBlocks = PKDG_B_MINB;  // 96 registers per thread: 20 warps per SM
+
+template <bool LEAF>
+pkdg_status launch_evalb_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    auto kern = pkdg_evalb_kernel<kBucketWarps, kBucketMinBlocks, LEAF>;
+    const int smem = kBucketWarps * (int)sizeof(WarpSmemB);
+    int& per_sm = ctx->evalb_per_sm[LEAF ? 1 : 0];
+    if (per_sm == 0) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kBucketWarps * 32, smem));
+        if (per_sm < 1) per_sm = 1;
+    }
+    int64_t want = (p.n_buckets + kBucketWarps - 1) / kBucketWarps;
+    int64_t grid = (int64_t)ctx->num_sms * per_sm;
+    if (grid > want) grid = want;
+    if (grid < 1) grid = 1;
+    kern<<<(unsigned)grid, kBucketWarps * 32, smem, st>>>(p);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -291,6 +323,7 @@ pkdg_status pkdg_create(pkdg_ctx** out, int device) {
     pkdg_ctx* ctx = new (std::nothrow) pkdg_ctx();
     if (!ctx) return PKDG_ENOMEM;
     ctx->device = device;
+    if (const char* g = getenv("PKDG_BUCKET_GEN")) ctx->bucket_gen = atoi(g);
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->stats, sizeof(DevStats));

@@ -474,6 +474,8 @@ __device__ __forceinline__ void cp_async4(void* dst, const void* src) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_pending() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 struct ListLens { int pp, pc; };
 __device__ __forceinline__ ListLens eff_lens(const BucketDesc& d, bool do_pp, bool do_pc) {
@@ -1273,6 +1275,252 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
                 if (iA >= 0 && !flagA) p.out[iA] = rA;
                 if (iB >= 0 && !flagB) p.out[iB] = rB;
             }
+        }
+    }
+    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Bucket kernel, generation 4 (a2-a5 for per-bucket lists).  The group kernel's idea -- a lane OWNS a sink pair,
+// sinks and accumulators stay in registers, sources stream through shared memory -- applied to ONE bucket per
+// warp: a bucket has at most 8 sink pairs per pass, so the 32 lanes are (source slot, sink pair) =
+// (lane >> LG, lane & (2^LG - 1)) with 2^LG = 8 or 4 pairs and NS = 4 or 8 source slots.  A tile of 32 source
+// particles / 32 cell records is staged by the whole warp (cp.async, double buffered, coalesced) and lane
+// (slot, pair) evaluates sources slot, slot + NS, ... of the tile against its pair.  Compared with generation 3
+// (a lane holds a source, per-lane partial sums of all 16 sinks in shared memory):
+//   - a list is padded to a multiple of NS (4 or 8) instead of 32: P-C lists fill 99 % of their slots, not 89 %;
+//   - no accumulator traffic through shared memory, and the cross-lane reduction is 2 (3) xor-shuffle rounds of 10
+//     values instead of a 64-value butterfly;
+//   - the conditioning estimate is the exact per-sink S2_i = sum_j |a_ij|^2, a softened pair is corrected in place;
+//   - 112 registers: 16 warps per SM hide the load chain at the start of a bucket, no hand-built hand-over.
+// ------------------------------------------------------------------------------------------------
+#ifndef PKDG_B_UNROLL
+#define PKDG_B_UNROLL 1
+#endif
+constexpr int kBUnroll = PKDG_B_UNROLL;
+
+constexpr int kBRing = 4;         // P-P source tiles in shared memory: one in use, kBRing - 1 in flight
+struct __align__(16) WarpSmemB {
+    float4 cell[2][8 * 32];       // [float4 of the record][cell of the tile]: writes by lane = cell and reads by
+                                  // slot = cell mod NS are both conflict-free
+    float4 src[kBRing][32];
+    int32_t sidx[kBRing][32];
+};
+
+// One pass (<= 16 sinks = <= 2^LG pairs) of one bucket.
+template <int LG, bool LEAF>
+__device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, const BucketDesc& d, const int bucket,
+                                            const int t0, const int ntp, const int pp_len, const int pc_len,
+                                            const int lane, unsigned& bad) {
+    constexpr int NPP = 1 << LG, NS = 32 >> LG;
+    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
+    const bool accumulate = (p.flags & 0x1u) != 0, fix_on = p.fix_k >= 0.0f;
+    const int pair = lane & (NPP - 1), slot = lane >> LG;
+    const int lo = d.first + t0, hi = lo + ntp;   // particle index range of the pass's sinks (self test per tile)
+    const int iA = 2 * pair < ntp ? lo + 2 * pair : -1, iB = 2 * pair + 1 < ntp ? lo + 2 * pair + 1 : -1;
+    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
+    const float4 tA = iA >= 0 ? __ldg(p.xyzm + iA) : dummy_tgt, tB = iB >= 0 ? __ldg(p.xyzm + iB) : dummy_tgt;
+    const float2 X = make_float2(tA.x, tB.x), Y = make_float2(tA.y, tB.y), Z = make_float2(tA.z, tB.z);
+    float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, aw = ax, s2 = ax;
+
+    // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
+    const int pc_ntile = (pc_len + 31) >> 5;
+    auto cidx_of = [&](int k) -> int32_t { return tile_entry(p.pc_idx, d.pc_begin, pc_len, k, lane); };
+    auto issue_cell = [&](int32_t c, int buf) {
+        if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
+        float4* dst = &S.cell[buf][lane];
+        if (c >= 0) {
+            const float4* q = p.cellq + (int64_t)c * 8;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) cp_async16(dst + 32 * i, q + i);
+        } else {   // padding: a cell of mass 0 far away
+            dst[0] = far4;
+#pragma unroll
+            for (int i = 1; i < 8; ++i) dst[32 * i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        cp_async_commit();
+    };
+    __syncwarp();   // the previous pass / bucket is done with every buffer
+    int32_t cn = -1;
+    if (pc_ntile > 0) {
+        issue_cell(cidx_of(0), 0);
+        cn = pc_ntile > 1 ? cidx_of(1) : -1;
+    }
+
+    // ---- a3: P-P.  Tile k (32 sources) is computed from ring buffer k % kBRing while tiles k + 1 .. k + kBRing - 1 are
+    //      in flight (a tile is only ~130 instructions per lane: one tile of prefetch does not cover a global load).
+    {
+        constexpr int PD = kBRing - 1;
+        const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
+        const int half = lane >> 4, hslot = lane & 15;
+        auto ref_of = [&](int k) -> int32_t {           // LEAF: bucket reference of this half-warp in tile k
+            const int r = 2 * k + half;
+            return r < pp_len ? __ldg(p.pp_idx + d.pp_begin + r) : -1;
+        };
+        auto fc_of = [&](int32_t g) -> int2 {
+            if ((uint32_t)g >= (uint64_t)p.n_gbuckets) return make_int2(0, 0);   // counted as a bad entry by the packer
+            const int2 fc = __ldg(p.gfc + g);
+            return fc.y > 16 ? make_int2(0, 0) : fc;
+        };
+        auto idx_of = [&](int k) -> int32_t { return tile_entry(p.pp_idx, d.pp_begin, pp_len, k, lane); };
+        auto issue = [&](int32_t j, int buf) {           // the lane's source of a tile starts its way to shared memory
+            if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+            S.sidx[buf][lane] = j;
+            if (j >= 0) cp_async16(&S.src[buf][lane], p.xyzm + j);
+            else S.src[buf][lane] = far4;
+            cp_async_commit();
+        };
+        int32_t jn = -1, gnn = -1;
+        int2 fcn = make_int2(0, 0);
+        // tiles 0 .. PD - 1 start now (one commit group per tile, empty if the list is shorter: the group count stays uniform)
+        if (LEAF) {
+            int32_t g0[PD + 2];
+#pragma unroll
+            for (int t = 0; t < PD + 2; ++t) g0[t] = t < ntile ? ref_of(t) : -1;
+            int2 fc0[PD + 1];
+#pragma unroll
+            for (int t = 0; t < PD + 1; ++t) fc0[t] = t < ntile ? fc_of(g0[t]) : make_int2(0, 0);
+#pragma unroll
+            for (int t = 0; t < PD; ++t) {
+                if (t < ntile) issue(hslot < fc0[t].y ? fc0[t].x + hslot : -1, t);
+                else cp_async_commit();
+            }
+            fcn = fc0[PD]; gnn = g0[PD + 1];
+        } else {
+            int32_t j0[PD + 1];
+#pragma unroll
+            for (int t = 0; t < PD + 1; ++t) j0[t] = t < ntile ? idx_of(t) : -1;
+#pragma unroll
+            for (int t = 0; t < PD; ++t) {
+                if (t < ntile) issue(j0[t], t);
+                else cp_async_commit();
+            }
+            jn = j0[PD];
+        }
+        for (int k = 0; k < ntile; ++k) {
+            const int buf = k & (kBRing - 1);
+            cp_async_wait_pending<PD - 1>();
+            __syncwarp();   // tile k is visible to the warp; everybody is done with tile k - 1, whose buffer tile k + PD takes
+            if (k + PD < ntile) {
+                if (LEAF) {
+                    issue(hslot < fcn.y ? fcn.x + hslot : -1, (k + PD) & (kBRing - 1));
+                    fcn = (k + PD + 1 < ntile) ? fc_of(gnn) : make_int2(0, 0);
+                    gnn = (k + PD + 2 < ntile) ? ref_of(k + PD + 2) : -1;
+                } else {
+                    issue(jn, (k + PD) & (kBRing - 1));
+                    jn = (k + PD + 1 < ntile) ? idx_of(k + PD + 1) : -1;
+                }
+            } else {
+                cp_async_commit();
+            }
+            // sources of this tile the lane visits: slot, slot + NS, ...; a short last tile ends early (warp-uniform)
+            const int nsrc = LEAF ? 32 : min(32, pp_len - 32 * k);
+            const int ntrip = (nsrc + NS - 1) >> (5 - LG);
+            const int32_t jl = S.sidx[buf][lane];
+            const bool own = __any_sync(0xffffffffu, jl >= lo && jl < hi);   // tile holds sinks of this pass
+            const float4* src = S.src[buf] + slot;
+            const int32_t* sid = S.sidx[buf] + slot;
+            float minr2 = 3.0e38f;
+            if (ntrip < 32 / NS || own) {   // a short last tile, or a tile with own particles: self test by index
+                if (ntrip == 32 / NS) {
+#pragma unroll
+                    for (int it = 0; it < 32 / NS; ++it) {
+                        const int32_t sj = sid[it * NS];
+                        pp_pair_g<true>(X, Y, Z, src[it * NS], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                    }
+                } else {
+#pragma unroll 2
+                    for (int it = 0; it < ntrip; ++it) {
+                        const int32_t sj = sid[it * NS];
+                        pp_pair_g<true>(X, Y, Z, src[it * NS], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                    }
+                }
+            } else {   // the common tile: straight-line code over its 32 / NS sources, no guards, so that they interleave
+#pragma unroll
+                for (int it = 0; it < 32 / NS; ++it)
+                    pp_pair_g<false>(X, Y, Z, src[it * NS], false, false, p.h2c, minr2, ax, ay, az, aw, s2);
+            }
+            if (minr2 < p.h2c) {   // rare: a pair of this lane inside the softening (or coincident): the lane owns its sinks
+                for (int it = 0; it < ntrip; ++it) {
+                    const float4 s = src[it * NS];
+                    const int32_t sj = sid[it * NS];
+                    if (sj < 0) continue;
+                    if (sj != iA) pp_soft_fix_g(X.x, Y.x, Z.x, s, p, ax.x, ay.x, az.x, aw.x, s2.x);
+                    if (sj != iB) pp_soft_fix_g(X.y, Y.y, Z.y, s, p, ax.y, ay.y, az.y, aw.y, s2.y);
+                }
+            }
+        }
+    }
+
+    // ---- a4: P-C.  Tile k = 32 cell records, one per lane (8 x cp.async of 16 bytes), in buffer k & 1; tile 0 was
+    //      issued before the P-P phase.
+    {
+        for (int k = 0; k < pc_ntile; ++k) {
+            const int buf = k & 1;
+            cp_async_wait_all();
+            __syncwarp();
+            if (k + 1 < pc_ntile) {
+                issue_cell(cn, buf ^ 1);
+                cn = (k + 2 < pc_ntile) ? cidx_of(k + 2) : -1;
+            }
+            const int ncell = min(32, pc_len - 32 * k);
+            const int ntrip = (ncell + NS - 1) >> (5 - LG);
+            const float4* rec = S.cell[buf] + slot;
+#pragma unroll kBUnroll
+            for (int it = 0; it < ntrip; ++it) {
+                const float4* r = rec + it * NS;
+                CellRegs cr;
+                cell_unpack(cr, r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]);
+                pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
+            }
+        }
+    }
+
+    // ---- a5: the NS source slots of every sink pair are summed by xor-shuffles; lanes of slot 0 test and write
+#pragma unroll
+    for (int o = 16; o >= NPP; o >>= 1) {
+        ax.x += __shfl_xor_sync(0xffffffffu, ax.x, o); ax.y += __shfl_xor_sync(0xffffffffu, ax.y, o);
+        ay.x += __shfl_xor_sync(0xffffffffu, ay.x, o); ay.y += __shfl_xor_sync(0xffffffffu, ay.y, o);
+        az.x += __shfl_xor_sync(0xffffffffu, az.x, o); az.y += __shfl_xor_sync(0xffffffffu, az.y, o);
+        aw.x += __shfl_xor_sync(0xffffffffu, aw.x, o); aw.y += __shfl_xor_sync(0xffffffffu, aw.y, o);
+        s2.x += __shfl_xor_sync(0xffffffffu, s2.x, o); s2.y += __shfl_xor_sync(0xffffffffu, s2.y, o);
+    }
+    float4 rA = make_float4(ax.x, ay.x, az.x, aw.x), rB = make_float4(ax.y, ay.y, az.y, aw.y);
+    const bool wA = slot == 0 && iA >= 0, wB = slot == 0 && iB >= 0;
+    if (accumulate) {   // the conditioning test is against the total the row will hold
+        if (wA) { const float4 o = p.out[iA]; rA.x += o.x; rA.y += o.y; rA.z += o.z; rA.w += o.w; }
+        if (wB) { const float4 o = p.out[iB]; rB.x += o.x; rB.y += o.y; rB.z += o.z; rB.w += o.w; }
+    }
+    const float a2A = fmaf(rA.z, rA.z, fmaf(rA.y, rA.y, rA.x * rA.x)), a2B = fmaf(rB.z, rB.z, fmaf(rB.y, rB.y, rB.x * rB.x));
+    bool flagA = fix_on && wA && s2.x >= p.fix_k * a2A, flagB = fix_on && wB && s2.y >= p.fix_k * a2B;
+    // one queue entry per (bucket, pass) in the fix-up kernel's format: sink t of the pass is bit 2 t
+    const unsigned mask = __reduce_or_sync(0xffffffffu, ((unsigned)flagA << (4 * pair)) | ((unsigned)flagB << (4 * pair + 2)));
+    if (mask) {
+        const bool queued = fix_push(p, bucket, (int)((unsigned)t0 | 0x80000000u), mask, lane);
+        flagA = flagA && queued; flagB = flagB && queued;   // queue full (cannot happen): keep the fp32 rows
+    }
+    if (wA && !flagA) p.out[iA] = rA;
+    if (wB && !flagB) p.out[iB] = rB;
+}
+
+template <int WARPS, int MINB, bool LEAF>
+__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalb_kernel(const EvalParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    WarpSmemB& S = reinterpret_cast<WarpSmemB*>(smem_raw)[threadIdx.x >> 5];
+    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u);
+    unsigned bad = 0;
+    for (;;) {
+        unsigned bu = 0;
+        if (lane == 0) bu = atomicAdd(p.work_counter, 1u);
+        bu = __shfl_sync(0xffffffffu, bu, 0);
+        if ((int64_t)bu >= p.n_buckets) break;
+        const BucketDesc d = p.desc[bu];
+        const int pp_len = do_pp ? d.pp_len : 0, pc_len = do_pc ? d.pc_len : 0;
+        for (int t0 = 0; t0 < d.count; t0 += kTMax) {
+            const int ntp = min(kTMax, d.count - t0);
+            if (ntp > 8) bucket_pass<3, LEAF>(p, S, d, (int)bu, t0, ntp, pp_len, pc_len, lane, bad);
+            else bucket_pass<2, LEAF>(p, S, d, (int)bu, t0, ntp, pp_len, pc_len, lane, bad);
         }
     }
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
