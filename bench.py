@@ -527,7 +527,7 @@ def run_ours(args, rank, world, local_rank):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (pkdg_eval3_kernel, this rank's launch): plain FP32 ALU (FFMA pipe) bound
+    # ---- roofline of the dominant kernel (pkdg_evalb_kernel, this rank's launch): plain FP32 ALU (FFMA pipe) bound
     sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
     peak_tflops = sms * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
     eval_ms = eval_ms_total / max(n_eval, 1)
@@ -535,7 +535,7 @@ def run_ours(args, rank, world, local_rank):
     achieved = flops_rank / (eval_ms * 1e-3) / 1e12
     probe_ms, probe_flops = ctx.fma_peak_probe(1 << 15)
     traffic, traffic_note = measured_traffic(f"cfg3_ng{args.ng}") if world == 1 else (None, "single-GPU capture only")
-    roofline = {"bound": "alu", "kernel": "pkdg_eval3_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "pkdg_evalb_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic, "traffic_note": traffic_note,
                 "peak_kind": f"{sms} SMs x 128 FP32 lanes x 2 x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json clock)",
                 "kernel_ms": eval_ms, "kernel_share_of_step": eval_ms / ms_step,

@@ -66,11 +66,10 @@ struct pkdg_ctx {
     int32_t *g_first = nullptr, *g_count = nullptr;  // streamed variants: device copy of the bucket arrays
     int64_t g_first_cap = 0, g_count_cap = 0;
     cudaStream_t last_stream = nullptr;
-    bool eval_configured = false;      // dynamic-smem opt-in of the evaluation kernel done on this device
-    int eval_per_sm = 1;
+    // CTAs per SM of the two instantiations (particle lists / PKDG_PP_LEAVES) of the bucket and of the group kernel;
+    // 0 = the dynamic shared-memory opt-in has not been made on this context's device yet
     int evalb_per_sm[2] = {0, 0};
-    int bucket_gen = 4;                // TEMPORARY A/B switch (env PKDG_BUCKET_GEN)
-    int evalg_per_sm[2] = {0, 0};      // the same for the two instantiations of the group kernel (0 = not yet)
+    int evalg_per_sm[2] = {0, 0};
     int64_t launches = 0;
     int64_t last_chunks = 1, last_buckets = 0;
     bool profiling = false;
@@ -108,35 +107,9 @@ pkdg_status ensure(pkdg_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-constexpr int kEvalWarps = 4;   // warps per CTA of the evaluation kernel
-constexpr int kEvalMinBlocks = 3;  // CTAs per SM it is compiled for (168 registers per thread)
-
-// The evaluation kernel needs more than the default 48 KB of dynamic shared memory.  Function attributes
-// are per device, so the opt-in is made once per context (a pkdg_ctx is bound to one device).
-template <bool LEAF> pkdg_status launch_evalb_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st);
-pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
-    if (ctx->bucket_gen == 4)
-        return (p.flags & PKDG_PP_LEAVES) ? launch_evalb_t<true>(ctx, p, st) : launch_evalb_t<false>(ctx, p, st);
-    auto kern = pkdg_eval3_kernel<kEvalWarps, kEvalMinBlocks>;
-    const int smem = kEvalWarps * (int)sizeof(WarpSmem3);
-    if (!ctx->eval_configured) {
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->eval_per_sm, kern, kEvalWarps * 32, smem));
-        if (ctx->eval_per_sm < 1) ctx->eval_per_sm = 1;
-        ctx->eval_configured = true;
-    }
-    int64_t want = (p.n_buckets + kEvalWarps - 1) / kEvalWarps;
-    int64_t grid = (int64_t)ctx->num_sms * ctx->eval_per_sm;
-    if (grid > want) grid = want;
-    if (grid < 1) grid = 1;
-    kern<<<(unsigned)grid, kEvalWarps * 32, smem, st>>>(p);
-    ctx->launches++;
-    CK(cudaGetLastError());
-    return PKDG_OK;
-}
-
-constexpr int kBucketWarps = 4;      // generation-4 bucket kernel: one bucket per warp
+// The evaluation kernels need more than the default 48 KB of dynamic shared memory.  Function attributes are per
+// device, so the opt-in is made once per context (a pkdg_ctx is bound to one device).
+constexpr int kBucketWarps = 4;      // bucket kernel: one bucket per warp
 #ifndef PKDG_B_MINB
 #define PKDG_B_MINB 5
 #endif
@@ -161,6 +134,10 @@ pkdg_status launch_evalb_t(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) 
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
+}
+
+pkdg_status launch_eval(pkdg_ctx* ctx, const EvalParams& p, cudaStream_t st) {
+    return (p.flags & PKDG_PP_LEAVES) ? launch_evalb_t<true>(ctx, p, st) : launch_evalb_t<false>(ctx, p, st);
 }
 
 constexpr int kGroupWarps = 4;      // warps per CTA of the group kernel (one group per warp)
@@ -323,7 +300,6 @@ pkdg_status pkdg_create(pkdg_ctx** out, int device) {
     pkdg_ctx* ctx = new (std::nothrow) pkdg_ctx();
     if (!ctx) return PKDG_ENOMEM;
     ctx->device = device;
-    if (const char* g = getenv("PKDG_BUCKET_GEN")) ctx->bucket_gen = atoi(g);
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->stats, sizeof(DevStats));

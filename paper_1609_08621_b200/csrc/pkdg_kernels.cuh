@@ -438,30 +438,6 @@ __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const 
 }
 
 
-// Butterfly transpose-reduction of NV per-lane partial sums across the 32 lanes: log2(32) rounds, in
-// the round with partner lane^mask each lane hands over the half of its values the partner keeps.
-// NV = 64: lane l ends with the totals of values 2l, 2l+1 in v[0], v[1];  NV = 32: value l in v[0].
-// NV - NV/32 shuffles instead of 5 NV.
-template <int NV>
-__device__ __forceinline__ void warp_transpose_reduce(float (&v)[NV], int lane) {
-    static_assert(NV == 32 || NV == 64, "NV");
-    int n = NV / 2;
-#pragma unroll
-    for (int mask = 16; mask >= 1; mask >>= 1) {
-        bool up = (lane & mask) != 0;
-#pragma unroll
-        for (int i = 0; i < NV / 2; ++i) {
-            if (i < n) {
-                float send = up ? v[i] : v[i + n];
-                float keep = up ? v[i + n] : v[i];
-                v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
-            }
-        }
-        n >>= 1;
-    }
-}
-
-
 // ------------------------------------------------------------------------------------------------
 // Asynchronous staging helpers (cp.async = LDGSTS): global -> shared memory without registers.
 // ------------------------------------------------------------------------------------------------
@@ -503,63 +479,6 @@ __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y
 __device__ __forceinline__ float2 f2mul(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 f2add(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 f2fma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
-
-constexpr int kPMax = kTMax / 2;  // sink pairs per pass
-
-struct __align__(16) WarpSmem3 {
-    float4 acc[kTMax * 32];       // [pair][half][lane]: {axA, axB, ayA, ayB}, {azA, azB, phiA, phiB}
-    float4 stage[8 * 32];         // [float4 of the record][lane]: the lane's cell of the NEXT P-C tile
-    float4 tgt[2][kTMax];         // raw sinks (x, y, z, m) of the current / the next bucket
-    float4 tp[(kPMax + 1) * 2];   // current pass, pair layout: {xA, xB, yA, yB}, {zA, zB, -, -}; +1 dummy pair
-    int32_t nidx[4][32];          // tiles 0, 1 of the P-P list and tiles 0, 1 of the P-C list
-    BucketDesc ndesc;             // descriptor of the next bucket
-    unsigned int bucket[2];       // index of the current / the next bucket (fix-up queue entries name it)
-};
-
-// The lane's cell record c (>= 0: valid) starts its way into the lane's staging slots (cp.async, 8 x 16 bytes).
-// (One cp.async.bulk of 128 bytes per lane with mbarrier completion was measured instead: 12 % SLOWER at N = 2^24 --
-// 32 single-lane bulk copies per tile serialise in the copy engine's issue path.)
-__device__ __forceinline__ void stage_cell(WarpSmem3& S, const EvalParams& p, int32_t c, int lane) {
-    if (c >= 0) {
-        const float4* q = p.cellq + (int64_t)c * 8;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) cp_async16(&S.stage[i * 32 + lane], q + i);
-    }
-}
-__device__ __forceinline__ float4 staged(const WarpSmem3& S, int src, int i) { return S.stage[i * 32 + src]; }
-
-// per-lane partial sums of sink t in the pair layout, as scalars (correction path, reduction)
-__device__ __forceinline__ int acc_idx(int t, int comp, int lane) {  // comp 0..3 = ax ay az phi
-    return (((t >> 1) * 2 + (comp >> 1)) * 32 + lane) * 4 + (comp & 1) * 2 + (t & 1);
-}
-
-// One source against one sink pair, Newtonian with r^2 clamped from below at h2c (so it is finite for
-// softened and coincident pairs; those are corrected afterwards, see pp_phase3).  With SELF the
-// accumulation is masked for the sink's own index (used only for tiles that hold own particles).
-// 13 packed FP instructions + 2 MUFU + min/max for 2 interactions; 19 flops per interaction.  minr2 (the
-// smallest r^2 between this lane's source and any sink of the pass) also feeds the conditioning bound.
-template <bool SELF>
-__device__ __forceinline__ void pp_fast2(const float4 txy, const float4 tz, const float4 s, bool selfA, bool selfB,
-                                         float h2c, float& minr2, float2& ax, float2& ay, float2& az, float2& aw) {
-    const float2 dx = f2add(make_float2(txy.x, txy.y), sp(-s.x));
-    const float2 dy = f2add(make_float2(txy.z, txy.w), sp(-s.y));
-    const float2 dz = f2add(make_float2(tz.x, tz.y), sp(-s.z));
-    float2 r2 = f2fma(dz, dz, f2fma(dy, dy, f2mul(dx, dx)));
-    const float2 ri = make_float2(rsqrt_approx(fmaxf(r2.x, h2c)), rsqrt_approx(fmaxf(r2.y, h2c)));
-    const float2 ri2 = f2mul(ri, ri);
-    float2 nm = sp(-s.w);
-    if (SELF) {
-        nm.x = selfA ? 0.0f : nm.x; nm.y = selfB ? 0.0f : nm.y;
-        r2.x = selfA ? 3.0e38f : r2.x; r2.y = selfB ? 3.0e38f : r2.y;
-    }
-    minr2 = fminf(minr2, fminf(r2.x, r2.y));
-    const float2 nmri = f2mul(nm, ri);
-    const float2 nmg = f2mul(nmri, ri2);
-    ax = f2fma(nmg, dx, ax);
-    ay = f2fma(nmg, dy, ay);
-    az = f2fma(nmg, dz, az);
-    aw = f2add(aw, nmri);
-}
 
 struct PcPre2 { float2 dx, dy, dz, ri; };
 
@@ -624,177 +543,6 @@ __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, floa
 #undef PKDG_T0
 #undef PKDG_T1
 
-// Raw sinks of pass t0 and index tiles 0, 1 of both lists by plain loads (first bucket of a warp, passes > 0).
-__device__ __forceinline__ void fill_direct3(WarpSmem3& S, const EvalParams& p, const BucketDesc& d, ListLens L, int t0,
-                                             int buf, int lane) {
-    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-    __syncwarp();
-    const int ntp = max(0, min(kTMax, d.count - t0));
-    if (lane < kTMax) S.tgt[buf][lane] = lane < ntp ? __ldg(p.xyzm + d.first + t0 + lane) : dummy_tgt;
-    S.nidx[0][lane] = L.pp > 0 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 0, lane) : -1;
-    S.nidx[1][lane] = L.pp > 32 ? tile_entry(p.pp_idx, d.pp_begin, L.pp, 1, lane) : -1;
-    S.nidx[2][lane] = L.pc > 0 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 0, lane) : -1;
-    S.nidx[3][lane] = L.pc > 32 ? tile_entry(p.pc_idx, d.pc_begin, L.pc, 1, lane) : -1;
-    __syncwarp();
-}
-
-// The same for the NEXT bucket (descriptor already in S.ndesc), asynchronously.
-__device__ __forceinline__ void stage_next_bucket3(WarpSmem3& S, const EvalParams& p, int nbuf, bool do_pp, bool do_pc,
-                                                   int lane) {
-    const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-    const BucketDesc nd = S.ndesc;
-    const ListLens L = eff_lens(nd, do_pp, do_pc);
-    const int ntp = max(0, min(kTMax, nd.count));
-    if (lane < kTMax) {
-        if (lane < ntp) cp_async16(&S.tgt[nbuf][lane], p.xyzm + nd.first + lane);
-        else S.tgt[nbuf][lane] = dummy_tgt;
-    }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int e = (q & 1) * 32 + lane;
-        const int len = q < 2 ? L.pp : L.pc;
-        const int32_t* src = q < 2 ? p.pp_idx + nd.pp_begin : p.pc_idx + nd.pc_begin;
-        if (e < len) cp_async4(&S.nidx[q][lane], src + e);
-        else S.nidx[q][lane] = -1;
-    }
-}
-
-// a2: raw sinks (visible to the warp) -> pair layout; pair kPMax is a dummy pair for the P-C pipeline.
-__device__ __forceinline__ void make_pairs(WarpSmem3& S, int buf, int lane) {
-    if (lane <= kPMax) {
-        const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-        const float4 A = lane < kPMax ? S.tgt[buf][2 * lane] : dummy_tgt;
-        const float4 B = lane < kPMax ? S.tgt[buf][2 * lane + 1] : dummy_tgt;
-        S.tp[2 * lane] = make_float4(A.x, B.x, A.y, B.y);
-        S.tp[2 * lane + 1] = make_float4(A.z, B.z, 0.0f, 0.0f);
-    }
-    __syncwarp();
-}
-
-// a3 for one pass, packed: NP sink pairs (4 or 8) in register accumulators.
-// LEAF (PKDG_PP_LEAVES): the list's entries are references to whole buckets.  A tile is then TWO
-// references: lanes 0-15 hold the particles of the first, lanes 16-31 those of the second (a bucket holds
-// at most 16), so the source gather is two contiguous runs and the list is 16 times shorter.
-template <int NP, bool LEAF>
-__device__ __forceinline__ void pp_phase3(const EvalParams& p, const BucketDesc& d, int pp_len, int t0, int ntp,
-                                          const float4* __restrict__ s_tgt, WarpSmem3& S, int lane, unsigned& bad,
-                                          float& s2_bound) {
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    const float4* __restrict__ tp = S.tp;
-    float4* __restrict__ s_acc = S.acc;
-    float* __restrict__ s_accf = reinterpret_cast<float*>(S.acc);
-    float2 ax[NP], ay[NP], az[NP], aw[NP];
-#pragma unroll
-    for (int q = 0; q < NP; ++q) ax[q] = ay[q] = az[q] = aw[q] = make_float2(0.f, 0.f);
-    // Conditioning of the P-P part: S2_i = sum_j |a_ij|^2 = sum_j m_j^2 / r_ij^4 <= sum_j m_j^2 / (min_i' r_i'j)^4, one
-    // bound for all sinks of the pass, from the minimum distance the tile loop tracks anyway.
-    float bsum = 0.0f;
-    bool smem_live = false;  // warp-uniform: s_acc already holds soft-pair corrections
-    const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
-    const int sink0 = d.first + t0;
-    const int half = lane >> 4, slot = lane & 15;
-    // LEAF helpers: reference of tile k for this half-warp (the first 64 are staged in shared memory),
-    // its (first, count), and the lane's particle in it
-    auto leaf_ref = [&](int k) -> int32_t {
-        const int r = 2 * k + half;
-        if (r >= pp_len) return -1;
-        return r < 64 ? S.nidx[r >> 5][r & 31] : __ldg(p.pp_idx + d.pp_begin + r);
-    };
-    auto leaf_fc = [&](int32_t g) -> int2 {
-        if ((uint32_t)g >= (uint64_t)p.n_gbuckets) return make_int2(0, 0);   // counted as a bad entry by the packer
-        const int2 fc = __ldg(p.gfc + g);
-        return fc.y > 16 ? make_int2(0, 0) : fc;
-    };
-    auto leaf_j = [&](int2 fc) -> int32_t { return slot < fc.y ? fc.x + slot : -1; };
-    int32_t j, jn, jnn = -1, gB = -1;
-    int2 fcA = make_int2(0, 0);
-    if (LEAF) {
-        j = ntile > 0 ? leaf_j(leaf_fc(leaf_ref(0))) : -1;
-        jn = ntile > 1 ? leaf_j(leaf_fc(leaf_ref(1))) : -1;
-        fcA = ntile > 2 ? leaf_fc(leaf_ref(2)) : make_int2(0, 0);
-        gB = ntile > 3 ? leaf_ref(3) : -1;
-    } else {
-        j = ntile > 0 ? S.nidx[0][lane] : -1;
-        jn = ntile > 1 ? S.nidx[1][lane] : -1;
-        jnn = ntile > 2 ? tile_entry(p.pp_idx, d.pp_begin, pp_len, 2, lane) : -1;
-    }
-    if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
-    if ((uint32_t)jn >= (uint64_t)p.n_particles) { bad += (jn >= 0); jn = -1; }
-    float4 s = j >= 0 ? __ldg(p.xyzm + j) : far4;
-    float4 sn = jn >= 0 ? __ldg(p.xyzm + jn) : far4;
-    for (int k = 0; k < ntile; ++k) {
-        // sources of the next two tiles and the index of the third are in flight during this tile
-        int32_t jn3 = -1;
-        if (LEAF) {
-            jnn = leaf_j(fcA);                                   // tile k+2
-            fcA = (k + 3 < ntile) ? leaf_fc(gB) : make_int2(0, 0);  // tile k+3
-            gB = (k + 4 < ntile) ? leaf_ref(k + 4) : -1;          // tile k+4
-        } else {
-            jn3 = (k + 3 < ntile) ? tile_entry(p.pp_idx, d.pp_begin, pp_len, k + 3, lane) : -1;
-        }
-        if ((uint32_t)jnn >= (uint64_t)p.n_particles) { bad += (jnn >= 0); jnn = -1; }
-        const float4 snn = jnn >= 0 ? __ldg(p.xyzm + jnn) : far4;
-        const int self_t = j - sink0;  // sink slot this source coincides with, if any
-        float minr2 = 3.0e38f;
-        if (__any_sync(0xffffffffu, (unsigned)self_t < (unsigned)(2 * NP))) {  // tile holds own particles
-#pragma unroll
-            for (int q = 0; q < NP; ++q)
-                pp_fast2<true>(tp[2 * q], tp[2 * q + 1], s, self_t == 2 * q, self_t == 2 * q + 1, p.h2c, minr2, ax[q],
-                               ay[q], az[q], aw[q]);
-        } else {
-#pragma unroll
-            for (int q = 0; q < NP; ++q)
-                pp_fast2<false>(tp[2 * q], tp[2 * q + 1], s, false, false, p.h2c, minr2, ax[q], ay[q], az[q], aw[q]);
-        }
-        {   // this lane's source pulls on no sink of the pass with more than m / max(min r^2, h^2)
-            const float ir = rsqrt_approx(fmaxf(minr2, p.h2c));
-            const float tb = s.w * ir * ir;
-            bsum = fmaf(tb, tb, bsum);
-        }
-        if (__any_sync(0xffffffffu, minr2 < p.h2c)) {
-            // rare: some pair of this tile is inside the softening (or coincident): replace its clamped
-            // Newtonian contribution by the spline one, through the shared accumulators.
-            if (!smem_live) {
-                for (int t = 0; t < kTMax; ++t) s_acc[t * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-                smem_live = true;
-            }
-            if (minr2 < p.h2c) {
-                for (int t = 0; t < ntp; ++t) {
-                    const float4 tg = s_tgt[t];
-                    float dx = tg.x - s.x, dy = tg.y - s.y, dz = tg.z - s.z;
-                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    if (r2 < p.h2c && self_t != t) {
-                        const float ri = rsqrt_approx(p.h2c);  // what pp_fast2 used for this pair
-                        const float2 dgw = pp_soft_correction(dx, dy, dz, p.eps, ri);
-                        const float mg = s.w * dgw.x, dw = dgw.y;
-                        s_accf[acc_idx(t, 0, lane)] = fmaf(-mg, dx, s_accf[acc_idx(t, 0, lane)]);
-                        s_accf[acc_idx(t, 1, lane)] = fmaf(-mg, dy, s_accf[acc_idx(t, 1, lane)]);
-                        s_accf[acc_idx(t, 2, lane)] = fmaf(-mg, dz, s_accf[acc_idx(t, 2, lane)]);
-                        s_accf[acc_idx(t, 3, lane)] = fmaf(s.w, dw, s_accf[acc_idx(t, 3, lane)]);
-                        // the bound above booked (m / h^2)^2 for this source; a softened pair pulls with up to
-                        // 2.6 m / h^2 and the correction is a difference of two terms: book (4 m / h^2)^2 in all
-                        const float tc = s.w * ri * ri;
-                        bsum = fmaf(15.0f * tc, tc, bsum);
-                    }
-                }
-            }
-        }
-        s = sn; sn = snn; j = jn; jn = jnn; jnn = jn3;
-    }
-#pragma unroll
-    for (int q = 0; q < NP; ++q) {
-        float4 a0 = make_float4(ax[q].x, ax[q].y, ay[q].x, ay[q].y), a1 = make_float4(az[q].x, az[q].y, aw[q].x, aw[q].y);
-        if (smem_live) {
-            const float4 b0 = s_acc[(2 * q) * 32 + lane], b1 = s_acc[(2 * q + 1) * 32 + lane];
-            a0.x += b0.x; a0.y += b0.y; a0.z += b0.z; a0.w += b0.w;
-            a1.x += b1.x; a1.y += b1.y; a1.z += b1.z; a1.w += b1.w;
-        }
-        s_acc[(2 * q) * 32 + lane] = a0;
-        s_acc[(2 * q + 1) * 32 + lane] = a1;
-    }
-    s2_bound = bsum;
-}
-
 // Queue one (bucket, pass) for the fp64 fix-up kernel (warp-uniform call).  Returns false if the queue is full
 // (cannot happen with the capacity the host sizes it to for non-overlapping buckets): the caller then writes
 // the fp32 result instead of dropping the rows.
@@ -806,212 +554,6 @@ __device__ __forceinline__ bool fix_push(const EvalParams& p, int bucket, int t0
     }
     k = __shfl_sync(0xffffffffu, k, 0);
     return k < p.fix_cap;
-}
-
-template <int WARPS, int MINB>
-__global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_eval3_kernel(const EvalParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    WarpSmem3& S = reinterpret_cast<WarpSmem3*>(smem_raw)[warp];
-    float4* s_acc = S.acc;
-    const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
-    const bool do_pp = !(p.flags & 0x2u), do_pc = !(p.flags & 0x4u), accumulate = (p.flags & 0x1u) != 0;
-    const bool pp_leaves = (p.flags & 0x8u) != 0;
-    unsigned bad = 0;
-    unsigned cur = 0;
-    if (lane == 0) cur = atomicAdd(p.work_counter, 1u);
-    cur = __shfl_sync(0xffffffffu, cur, 0);
-    if ((int64_t)cur >= p.n_buckets) return;
-    if (lane == 0) S.bucket[0] = cur;
-    BucketDesc d = p.desc[cur];
-    int buf = 0;
-    fill_direct3(S, p, d, eff_lens(d, do_pp, do_pc), 0, buf, lane);
-
-    for (;;) {
-        unsigned nxt = 0xffffffffu;
-        if (lane == 0) nxt = atomicAdd(p.work_counter, 1u);  // claimed now, looked at in the last pass
-        bool has_next = false;
-        const ListLens L = eff_lens(d, do_pp, do_pc);
-        const int npass = max(1, (d.count + kTMax - 1) / kTMax);
-
-        for (int pass = 0; pass < npass; ++pass) {
-            const int t0 = pass * kTMax;
-            const int ntp = max(0, min(kTMax, d.count - t0));
-            const bool last = pass == npass - 1;
-            if (pass > 0) fill_direct3(S, p, d, L, t0, buf, lane);
-            const float4* s_tgt = S.tgt[buf];
-
-            // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
-            const int pc_ntile = (L.pc + 31) >> 5;
-            int32_t c = pc_ntile > 0 ? S.nidx[2][lane] : -1;
-            int32_t cn = pc_ntile > 1 ? S.nidx[3][lane] : -1;
-            if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
-            stage_cell(S, p, c, lane);
-            cp_async_commit();
-
-            // ---- a2: pair layout of the sinks;  a3: P-P
-            make_pairs(S, buf, lane);
-            float s2_b = 0.0f;   // per-lane part of the conditioning bound of this pass (P-P, then P-C)
-            if (pp_leaves) {
-                if (ntp <= 8) pp_phase3<4, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
-                else pp_phase3<8, true>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
-            } else {
-                if (ntp <= 8) pp_phase3<4, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
-                else pp_phase3<8, false>(p, d, L.pp, t0, ntp, s_tgt, S, lane, bad, s2_b);
-            }
-
-            // ---- next bucket, stage 1: its descriptor
-            if (last) {
-                const unsigned nb = __shfl_sync(0xffffffffu, nxt, 0);
-                if (lane == 0) S.bucket[1] = nb;
-                has_next = (int64_t)nb < p.n_buckets;
-                if (has_next && lane < 2)
-                    cp_async16(reinterpret_cast<char*>(&S.ndesc) + 16 * lane,
-                               reinterpret_cast<const char*>(p.desc + nb) + 16 * lane);
-                cp_async_commit();
-            }
-
-            // ---- a4: P-C.  One sink pair per iteration; the lane's cell stays in registers for the tile.
-            {
-                const int npair = (ntp + 1) >> 1;  // odd count: the last pair's second half is a dummy sink
-                const float4* tp = S.tp;
-                // One tile.  LAST_TILE is a compile-time tag: only the last tile of a list can be partly filled, so only
-                // its copy of the code carries the sharing-out logic and the hand-over to the next bucket.
-                auto do_tile = [&](const int k, auto last_tag) {
-                    constexpr bool LAST_TILE = decltype(last_tag)::value;
-                    const int32_t c2 = (!LAST_TILE && k + 2 < pc_ntile) ? tile_entry(p.pc_idx, d.pc_begin, L.pc, k + 2, lane) : -1;
-                    cp_async_wait_all();  // this tile's record (own slots) and, in the last pass, ndesc
-                    // A last tile that is at most half (a quarter) full is shared out: 2 (4) groups of lanes take
-                    // the same cells and each group a half (a quarter) of the sink pairs, so the tile costs a
-                    // half (a quarter) of a full one.  Per-lane partial sums stay in the lane's own column.
-                    const int valid = LAST_TILE ? min(32, L.pc - 32 * k) : 32;   // warp-uniform
-                    const int rep = !LAST_TILE ? 1 : (valid <= 8 && npair >= 4) ? 4 : (valid <= 16 && npair >= 2) ? 2 : 1;
-                    int src = lane, q0 = 0, q1 = npair;
-                    int32_t cs = c;
-                    if (LAST_TILE && rep > 1) {
-                        const int width = 32 / rep, chunk = (npair + rep - 1) / rep;
-                        src = lane & (width - 1);
-                        q0 = min(npair, (lane / width) * chunk);
-                        q1 = min(npair, q0 + chunk);
-                        cs = __shfl_sync(0xffffffffu, c, src);
-                        __syncwarp();  // the record of lane `src` was copied by lane `src`
-                    }
-                    CellRegs cr;
-                    if (cs >= 0) {
-                        cell_unpack(cr, staged(S, src, 0), staged(S, src, 1), staged(S, src, 2), staged(S, src, 3),
-                                    staged(S, src, 4), staged(S, src, 5), staged(S, src, 6), staged(S, src, 7));
-                    } else {
-                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        cell_unpack(cr, far4, z4, z4, z4, z4, z4, z4, z4);
-                    }
-                    if (!LAST_TILE) {
-                        if ((uint32_t)cn >= (uint64_t)p.n_cells) { bad += (cn >= 0); cn = -1; }
-                        stage_cell(S, p, cn, lane);  // next tile's record; the slot was read into registers just above
-                    } else if (last && has_next) {   // next bucket, stage 2
-                        __syncwarp();
-                        stage_next_bucket3(S, p, buf ^ 1, do_pp, do_pc, lane);
-                    }
-                    cp_async_commit();
-                    // software pipeline, two pairs per trip so that no register copies are needed: the
-                    // displacement / rsqrt of the next pair is issued under the body of the current one
-                    float pc_minr2 = 3.0e38f;
-                    PcPre2 pA = pc_pre2(tp[2 * q0], tp[2 * q0 + 1], cr, pc_minr2);
-#pragma unroll 1
-                    for (int q = q0; q < q1; q += 2) {
-                        const PcPre2 pB = pc_pre2(tp[2 * q + 2], tp[2 * q + 3], cr, pc_minr2);
-                        {
-                            float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                            pc_body2(pA, cr, a0, a1);
-                            s_acc[(2 * q) * 32 + lane] = a0;
-                            s_acc[(2 * q + 1) * 32 + lane] = a1;
-                        }
-                        if (q + 1 < q1) {
-                            pA = pc_pre2(tp[2 * q + 4], tp[2 * q + 5], cr, pc_minr2);
-                            float4 a0 = s_acc[(2 * q + 2) * 32 + lane], a1 = s_acc[(2 * q + 3) * 32 + lane];
-                            pc_body2(pB, cr, a0, a1);
-                            s_acc[(2 * q + 2) * 32 + lane] = a0;
-                            s_acc[(2 * q + 3) * 32 + lane] = a1;
-                        }
-                    }
-                    {   // this lane's cell pulls on none of the sinks it was evaluated for with more than M / min r^2
-                        const float ir = rsqrt_approx(pc_minr2);
-                        const float tb = cr.M * ir * ir;
-                        s2_b = fmaf(tb, tb, s2_b);
-                    }
-                    c = cn; cn = c2;
-                };
-                for (int k = 0; k + 1 < pc_ntile; ++k) do_tile(k, std::false_type{});
-                if (pc_ntile > 0) do_tile(pc_ntile - 1, std::true_type{});
-                if (last && pc_ntile == 0 && has_next) {
-                    cp_async_wait_all();
-                    __syncwarp();
-                    stage_next_bucket3(S, p, buf ^ 1, do_pp, do_pc, lane);
-                    cp_async_commit();
-                }
-            }
-            // ---- a5: cross-lane reduction, conditioning test and write-back.  A sink whose sum cancels so far that
-            // fp32 terms cannot give the tolerance (S2_i > fix_k |a_i|^2) is not
-            // written here: its (bucket, pass) is queued and pkdg_fixup_kernel evaluates it with fp64 terms.
-            float* outf = reinterpret_cast<float*>(p.out + d.first + t0);
-            const bool fix_on = p.fix_k >= 0.0f;
-#pragma unroll
-            for (int o = 16; o; o >>= 1) s2_b += __shfl_xor_sync(0xffffffffu, s2_b, o);
-            if (ntp <= 8) {
-                float v[32];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                    v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
-                    v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
-                }
-                warp_transpose_reduce<32>(v, lane);       // lane l: component l & 3 of sink l >> 2
-                const bool valid = (lane >> 2) < ntp;
-                // with PKDG_ACCUMULATE the row already holds a part of the sum (the local expansion of
-                // pkdg_gravity_eval_fmm): the conditioning test is against the TOTAL acceleration
-                const float r = (accumulate && valid) ? v[0] + outf[lane] : v[0];
-                float sq = (lane & 3) < 3 ? r * r : 0.0f;
-                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
-                sq += __shfl_xor_sync(0xffffffffu, sq, 2);
-                bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
-                const unsigned ballot = __ballot_sync(0xffffffffu, flag);
-                if (ballot) {   // warp-uniform; every lane takes part in the push
-                    const bool queued = fix_push(p, (int)S.bucket[0], t0, ballot, lane);
-                    flag = flag && queued;
-                }
-                if (valid && !flag) outf[lane] = r;
-            } else {
-                float v[64];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const float4 a0 = s_acc[(2 * q) * 32 + lane], a1 = s_acc[(2 * q + 1) * 32 + lane];
-                    v[8 * q] = a0.x; v[8 * q + 1] = a0.z; v[8 * q + 2] = a1.x; v[8 * q + 3] = a1.z;
-                    v[8 * q + 4] = a0.y; v[8 * q + 5] = a0.w; v[8 * q + 6] = a1.y; v[8 * q + 7] = a1.w;
-                }
-                warp_transpose_reduce<64>(v, lane);        // lane l: components 2 (l & 1), 2 (l & 1) + 1 of sink l >> 1
-                const bool valid = (lane >> 1) < ntp;
-                float2* o2 = reinterpret_cast<float2*>(outf) + lane;
-                float2 r = make_float2(v[0], v[1]);
-                if (accumulate && valid) { const float2 old = *o2; r.x += old.x; r.y += old.y; }
-                float sq = (lane & 1) ? r.x * r.x : fmaf(r.x, r.x, r.y * r.y);
-                sq += __shfl_xor_sync(0xffffffffu, sq, 1);
-                bool flag = fix_on && valid && s2_b >= p.fix_k * sq;
-                const unsigned ballot = __ballot_sync(0xffffffffu, flag);
-                if (ballot) {
-                    const bool queued = fix_push(p, (int)S.bucket[0], (int)((unsigned)t0 | 0x80000000u), ballot, lane);
-                    flag = flag && queued;
-                }
-                if (valid && !flag) *o2 = r;
-            }
-        }
-        if (!has_next) break;
-        cp_async_wait_all();
-        __syncwarp();
-        d = S.ndesc;
-        if (lane == 0) S.bucket[0] = S.bucket[1];
-        buf ^= 1;
-    }
-    if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);
 }
 
 // ------------------------------------------------------------------------------------------------
