@@ -42,10 +42,14 @@ struct DevStats {
 // which is the truncated Taylor series of include/pkdg.h (d^n(1/r) is trace-free, so contracting the
 // raw moments with it equals contracting their trace-free part with d^n; the polynomials are
 // homogeneous, so evaluating them at tau absorbs every power of s/r).  Arithmetic in fp64: the
-// trace removal cancels leading digits.  Layout of the 32 floats:
-//   0-3 COM, M | 4 s | 5-9 q2 xx xy xz yy yz | 10-16 q3 xxx xxy xxz xyy xyz yyy yyz |
-//   17-25 q4 xxxx xxxy xxxz xxyy xxyz xyyy xyyz yyyy yyyz | 26 q2zz 27 q3xzz 28 q3yzz 29 q3zzz
-//   30 q4xxzz 31 q4yyzz          (the other four dependent q4 components are rebuilt in registers)
+// trace removal cancels leading digits.
+// Every slice q_i.. of a trace-free tensor is trace-free itself, so V_n,i = sum q_i jk.. tau_j tau_k .. needs no
+// component with two z indices among jk..: q_i..zz = -q_i..xx - q_i..yy moves the z^2 into the monomials
+// (pc_body2: 5 terms instead of 6 at order 3, 7 instead of 10 at order 4).  What is stored is therefore every
+// component with at most ONE z among the indices after the first -- the 5 + 7 + 9 independent ones and the six
+// the i = z slices need besides.  Layout of the 32 floats (one 128-byte line):
+//   0-3 COM, M | 4 s | 5-10 q2 xx xy xz yy yz zz | 11-19 q3 xxx xxy xxz xyy xyz yyy yyz xzz yzz |
+//   20-31 q4 xxxx xxxy xxxz xxyy xxyz xyyy xyyz yyyy yyyz xxzz xyzz yyzz
 // ------------------------------------------------------------------------------------------------
 // One thread per cell; the 36-float records of a block's 128 cells are staged through shared memory so
 // that global reads and writes are coalesced (a thread reading its own 144-byte record directly runs at
@@ -105,17 +109,15 @@ __device__ __forceinline__ void prep_cell_f64(const float* __restrict__ r, doubl
     }
     o[0] = r[0]; o[1] = r[1]; o[2] = r[2]; o[3] = r[3];
     o[4] = s;
-    o[5] = k2 * q2[0]; o[6] = k2 * q2[1]; o[7] = k2 * q2[2];
-    o[8] = k2 * q2[3]; o[9] = k2 * q2[4];
-    o[10] = k3 * q3[0]; o[11] = k3 * q3[1]; o[12] = k3 * q3[2];
-    o[13] = k3 * q3[3]; o[14] = k3 * q3[4]; o[15] = k3 * q3[6];
-    o[16] = k3 * q3[7];
-    o[17] = k4 * q4[0]; o[18] = k4 * q4[1]; o[19] = k4 * q4[2];
-    o[20] = k4 * q4[3]; o[21] = k4 * q4[4]; o[22] = k4 * q4[6];
-    o[23] = k4 * q4[7]; o[24] = k4 * q4[10]; o[25] = k4 * q4[11];
-    o[26] = k2 * q2[5];
-    o[27] = k3 * q3[5]; o[28] = k3 * q3[8]; o[29] = k3 * q3[9];
-    o[30] = k4 * q4[5]; o[31] = k4 * q4[12];
+    o[5] = k2 * q2[0]; o[6] = k2 * q2[1]; o[7] = k2 * q2[2];        // xx xy xz
+    o[8] = k2 * q2[3]; o[9] = k2 * q2[4]; o[10] = k2 * q2[5];       // yy yz zz
+    o[11] = k3 * q3[0]; o[12] = k3 * q3[1]; o[13] = k3 * q3[2];     // xxx xxy xxz
+    o[14] = k3 * q3[3]; o[15] = k3 * q3[4]; o[16] = k3 * q3[6];     // xyy xyz yyy
+    o[17] = k3 * q3[7]; o[18] = k3 * q3[5]; o[19] = k3 * q3[8];     // yyz xzz yzz
+    o[20] = k4 * q4[0]; o[21] = k4 * q4[1]; o[22] = k4 * q4[2];     // xxxx xxxy xxxz
+    o[23] = k4 * q4[3]; o[24] = k4 * q4[4]; o[25] = k4 * q4[6];     // xxyy xxyz xyyy
+    o[26] = k4 * q4[7]; o[27] = k4 * q4[10]; o[28] = k4 * q4[11];   // xyyz yyyy yyyz
+    o[29] = k4 * q4[5]; o[30] = k4 * q4[8]; o[31] = k4 * q4[12];    // xxzz xyzz yyzz
 }
 
 __device__ __forceinline__ void prep_one_cell(const float* __restrict__ r, float* __restrict__ o) {
@@ -412,12 +414,12 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 }
 
 
-// A cell held in registers by one lane (35 values; COM/M/s + 6 + 10 + 15 normalised components).
+// A cell held in registers by one lane: the 32 floats of its record.
 struct CellRegs {
     float cx, cy, cz, M, s;
     float xx, xy, xz, yy, yz, zz;
-    float xxx, xxy, xxz, xyy, xyz, xzz, yyy, yyz, yzz, zzz;
-    float xxxx, xxxy, xxxz, xxyy, xxyz, xxzz, xyyy, xyyz, xyzz, xzzz, yyyy, yyyz, yyzz, yzzz, zzzz;
+    float xxx, xxy, xxz, xyy, xyz, yyy, yyz, xzz, yzz;
+    float xxxx, xxxy, xxxz, xxyy, xxyz, xyyy, xyyz, yyyy, yyyz, xxzz, xyzz, yyzz;
 };
 
 __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const float4 f1, const float4 f2,
@@ -425,16 +427,12 @@ __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const 
                                             const float4 f6, const float4 f7) {
     c.cx = f0.x; c.cy = f0.y; c.cz = f0.z; c.M = f0.w;
     c.s = f1.x; c.xx = f1.y; c.xy = f1.z; c.xz = f1.w;
-    c.yy = f2.x; c.yz = f2.y; c.xxx = f2.z; c.xxy = f2.w;
-    c.xxz = f3.x; c.xyy = f3.y; c.xyz = f3.z; c.yyy = f3.w;
-    c.yyz = f4.x; c.xxxx = f4.y; c.xxxy = f4.z; c.xxxz = f4.w;
-    c.xxyy = f5.x; c.xxyz = f5.y; c.xyyy = f5.z; c.xyyz = f5.w;
-    c.yyyy = f6.x; c.yyyz = f6.y; c.zz = f6.z; c.xzz = f6.w;
-    c.yzz = f7.x; c.zzz = f7.y; c.xxzz = f7.z; c.yyzz = f7.w;
-    c.xyzz = -(c.xxxy + c.xyyy);
-    c.xzzz = -(c.xxxz + c.xyyz);
-    c.yzzz = -(c.xxyz + c.yyyz);
-    c.zzzz = -(c.xxzz + c.yyzz);
+    c.yy = f2.x; c.yz = f2.y; c.zz = f2.z; c.xxx = f2.w;
+    c.xxy = f3.x; c.xxz = f3.y; c.xyy = f3.z; c.xyz = f3.w;
+    c.yyy = f4.x; c.yyz = f4.y; c.xzz = f4.z; c.yzz = f4.w;
+    c.xxxx = f5.x; c.xxxy = f5.y; c.xxxz = f5.z; c.xxyy = f5.w;
+    c.xxyz = f6.x; c.xyyy = f6.y; c.xyyz = f6.z; c.yyyy = f6.w;
+    c.yyyz = f7.x; c.xxzz = f7.y; c.xyzz = f7.z; c.yyzz = f7.w;
 }
 
 
@@ -493,15 +491,18 @@ __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, con
     return q;
 }
 
-// One cell against one sink pair, packed.  Same truncated series as pc_body, arranged as ONE cumulative
-// chain per component: W2 = V2, W3 = W2 + V3, W4 = W3 + V4 = G (the order-3 chain starts from the
-// order-2 result, the order-4 chain from the order-3 one).  With E2 = W2.tau = e2, E3 = W3.tau = e2 + e3,
-// E4 = G.tau = e2 + e3 + e4:
+// One cell against one sink pair, packed.  ONE cumulative chain per component: W2 = V2, W3 = W2 + V3,
+// W4 = W3 + V4 = G (the order-3 chain starts from the order-2 result, the order-4 chain from the order-3 one).
+// With E2 = W2.tau = e2, E3 = W3.tau = e2 + e3, E4 = G.tau = e2 + e3 + e4:
 //   1 + sum e_n / n        = 1 + E2/6 + E3/12 + E4/4      (potential series fs)
 //   1 + sum (2n+1)/n e_n   = fs + 2 E4                     (radial factor S)
-// which needs no chain-start multiplies and no V2 + V3 + V4 sums, and the data dependence keeps the three
-// FFMA2 of a term (same monomial, x / y / z coefficient) adjacent, so the monomial pair is reused.
-// Per interaction: 5 FADD, 35 FMUL, 73 FFMA, 1 MUFU = 187 flops in 113 packed instructions per pair.
+// which needs no chain-start multiplies and no V2 + V3 + V4 sums.  The z^2 of every monomial is folded into the
+// x^2 and y^2 ones (the slices are trace-free, see the record layout): with A = xx - zz, B = yy - zz,
+//   V3_i = q_ixx A + q_iyy B + q_ixy 2xy + q_ixz 2xz + q_iyz 2yz
+//   V4_i = q_ixxx x(xx - 3zz) + q_ixxy 3yA + q_ixxz z(3xx - zz) + q_ixyy 3xB + q_ixyz 6xyz
+//        + q_iyyy y(yy - 3zz) + q_iyyz z(3yy - zz)
+// Per interaction: 7 FADD, 31 FMUL, 65 FFMA, 1 MUFU = 169 flops in 103 packed instructions per pair
+// (the textbook form with all 6 + 10 monomials: 187 flops in 113).
 #define PKDG_T0(CX, CY, CZ, M) vx = f2mul(sp(CX), M); vy = f2mul(sp(CY), M); vz = f2mul(sp(CZ), M);
 #define PKDG_T1(CX, CY, CZ, M) vx = f2fma(sp(CX), M, vx); vy = f2fma(sp(CY), M, vy); vz = f2fma(sp(CZ), M, vz);
 __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1) {
@@ -512,19 +513,20 @@ __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, floa
     PKDG_T0(c.xx, c.xy, c.xz, x) PKDG_T1(c.xy, c.yy, c.yz, y) PKDG_T1(c.xz, c.yz, c.zz, z)
     float2 E2 = f2mul(vx, x); E2 = f2fma(vy, y, E2); E2 = f2fma(vz, z, E2);
     const float2 xx = f2mul(x, x), yy = f2mul(y, y), zz = f2mul(z, z);
+    const float2 A = f2add(xx, neg2(zz)), B = f2add(yy, neg2(zz));
     const float2 x2 = f2add(x, x), y2 = f2add(y, y);
-    const float2 xy = f2mul(x2, y), xz = f2mul(x2, z), yz = f2mul(y2, z);
-    PKDG_T1(c.xxx, c.xxy, c.xxz, xx) PKDG_T1(c.xyy, c.yyy, c.yyz, yy) PKDG_T1(c.xzz, c.yzz, c.zzz, zz)
-    PKDG_T1(c.xxy, c.xyy, c.xyz, xy) PKDG_T1(c.xxz, c.xyz, c.xzz, xz) PKDG_T1(c.xyz, c.yyz, c.yzz, yz)
+    const float2 C = f2mul(x2, y), D = f2mul(x2, z), E = f2mul(y2, z);
+    PKDG_T1(c.xxx, c.xxy, c.xxz, A) PKDG_T1(c.xyy, c.yyy, c.yyz, B) PKDG_T1(c.xxy, c.xyy, c.xyz, C)
+    PKDG_T1(c.xxz, c.xyz, c.xzz, D) PKDG_T1(c.xyz, c.yyz, c.yzz, E)
     float2 E3 = f2mul(vx, x); E3 = f2fma(vy, y, E3); E3 = f2fma(vz, z, E3);
-    const float2 x3 = f2mul(sp(3.0f), x), y3 = f2mul(sp(3.0f), y), z3 = f2mul(sp(3.0f), z);
-    const float2 m0 = f2mul(xx, x), m1 = f2mul(yy, y), m2 = f2mul(zz, z);
-    const float2 m3 = f2mul(xx, y3), m4 = f2mul(xx, z3), m5 = f2mul(yy, x3), m6 = f2mul(yy, z3);
-    const float2 m7 = f2mul(zz, x3), m8 = f2mul(zz, y3), m9 = f2mul(xy, z3);
-    PKDG_T1(c.xxxx, c.xxxy, c.xxxz, m0) PKDG_T1(c.xxxy, c.xxyy, c.xxyz, m3) PKDG_T1(c.xxxz, c.xxyz, c.xxzz, m4)
-    PKDG_T1(c.xxyy, c.xyyy, c.xyyz, m5) PKDG_T1(c.xxyz, c.xyyz, c.xyzz, m9) PKDG_T1(c.xxzz, c.xyzz, c.xzzz, m7)
-    PKDG_T1(c.xyyy, c.yyyy, c.yyyz, m1) PKDG_T1(c.xyyz, c.yyyz, c.yyzz, m6) PKDG_T1(c.xyzz, c.yyzz, c.yzzz, m8)
-    PKDG_T1(c.xzzz, c.yzzz, c.zzzz, m2)
+    const float2 P1 = f2fma(sp(-3.0f), zz, xx), P2 = f2fma(sp(3.0f), xx, neg2(zz));
+    const float2 P3 = f2fma(sp(-3.0f), zz, yy), P4 = f2fma(sp(3.0f), yy, neg2(zz));
+    const float2 x3 = f2mul(sp(3.0f), x), y3 = f2mul(sp(3.0f), y);
+    const float2 K1 = f2mul(x, P1), K2 = f2mul(y3, A), K3 = f2mul(z, P2), K4 = f2mul(x3, B), K5 = f2mul(x3, E);
+    const float2 K6 = f2mul(y, P3), K7 = f2mul(z, P4);
+    PKDG_T1(c.xxxx, c.xxxy, c.xxxz, K1) PKDG_T1(c.xxxy, c.xxyy, c.xxyz, K2) PKDG_T1(c.xxxz, c.xxyz, c.xxzz, K3)
+    PKDG_T1(c.xxyy, c.xyyy, c.xyyz, K4) PKDG_T1(c.xxyz, c.xyyz, c.xyzz, K5) PKDG_T1(c.xyyy, c.yyyy, c.yyyz, K6)
+    PKDG_T1(c.xyyz, c.yyyz, c.yyzz, K7)
     float2 E4 = f2mul(vx, x); E4 = f2fma(vy, y, E4); E4 = f2fma(vz, z, E4);
     const float2 fs = f2fma(sp(0.25f), E4, f2fma(sp(0.083333333333f), E3, f2fma(sp(0.16666666667f), E2, sp(1.0f))));
     const float2 S = f2fma(sp(2.0f), E4, fs);
@@ -1110,19 +1112,19 @@ __device__ __noinline__ void pc_pair_f64(const double xi, const double yi, const
     const double r2 = dx * dx + dy * dy + dz * dz;
     const double ri = rsqrt(r2), ri2 = ri * ri, sr = sc * ri2;
     const double x = dx * sr, y = dy * sr, z = dz * sr;
-    const double qxx = q[5], qxy = q[6], qxz = q[7], qyy = q[8], qyz = q[9], qzz = q[26];
+    const double qxx = q[5], qxy = q[6], qxz = q[7], qyy = q[8], qyz = q[9], qzz = q[10];
     const double v2x = qxx * x + qxy * y + qxz * z, v2y = qxy * x + qyy * y + qyz * z, v2z = qxz * x + qyz * y + qzz * z;
     const double e2 = v2x * x + v2y * y + v2z * z;
-    const double xxx = q[10], xxy = q[11], xxz = q[12], xyy = q[13], xyz = q[14], yyy = q[15], yyz = q[16];
-    const double xzz = q[27], yzz = q[28], zzz = q[29];
+    const double xxx = q[11], xxy = q[12], xxz = q[13], xyy = q[14], xyz = q[15], yyy = q[16], yyz = q[17];
+    const double xzz = q[18], yzz = q[19], zzz = -(xxz + yyz);
     const double mxx = x * x, myy = y * y, mzz = z * z, mxy = 2 * x * y, mxz = 2 * x * z, myz = 2 * y * z;
     const double v3x = xxx * mxx + xyy * myy + xzz * mzz + xxy * mxy + xxz * mxz + xyz * myz;
     const double v3y = xxy * mxx + yyy * myy + yzz * mzz + xyy * mxy + xyz * mxz + yyz * myz;
     const double v3z = xxz * mxx + yyz * myy + zzz * mzz + xyz * mxy + xzz * mxz + yzz * myz;
     const double e3 = v3x * x + v3y * y + v3z * z;
-    const double xxxx = q[17], xxxy = q[18], xxxz = q[19], xxyy = q[20], xxyz = q[21], xyyy = q[22], xyyz = q[23];
-    const double yyyy = q[24], yyyz = q[25], xxzz = q[30], yyzz = q[31];
-    const double xyzz = -(xxxy + xyyy), xzzz = -(xxxz + xyyz), yzzz = -(xxyz + yyyz), zzzz = -(xxzz + yyzz);
+    const double xxxx = q[20], xxxy = q[21], xxxz = q[22], xxyy = q[23], xxyz = q[24], xyyy = q[25], xyyz = q[26];
+    const double yyyy = q[27], yyyz = q[28], xxzz = q[29], xyzz = q[30], yyzz = q[31];
+    const double xzzz = -(xxxz + xyyz), yzzz = -(xxyz + yyyz), zzzz = -(xxzz + yyzz);
     const double c0 = mxx * x, c1 = myy * y, c2 = mzz * z, c3 = 3 * mxx * y, c4 = 3 * mxx * z, c5 = 3 * myy * x;
     const double c6 = 3 * myy * z, c7 = 3 * mzz * x, c8 = 3 * mzz * y, c9 = 6 * x * y * z;
     const double v4x = xxxx * c0 + xxxy * c3 + xxxz * c4 + xxyy * c5 + xxyz * c9 + xxzz * c7 + xyyy * c1 + xyyz * c6 + xyzz * c8 + xzzz * c2;
