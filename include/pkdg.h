@@ -25,7 +25,7 @@
  * Precision ("single precision in calculating interactions, but all components are
  * accumulated in double precision").  Terms and per-lane
  * partial sums are fp32.  Beside a_i the kernel accumulates S2_i = sum_j |a_ij|^2; a sink whose sum cancels
- * so far that fp32 terms cannot give 2e-5 of |a_i| (sqrt(S2_i) > kappa2 |a_i|, default kappa2 = 8, option
+ * so far that fp32 terms cannot give 2e-5 of |a_i| (sqrt(S2_i) > kappa2 |a_i|, default kappa2 = 6, option
  * PKDG_OPT_KAPPA2) is re-evaluated over the same lists by a second kernel with fp64 terms and fp64
  * accumulators and its row is written by that kernel.  pkdg_stats.fixup_sinks counts them.
  *
@@ -139,7 +139,7 @@ typedef struct {
 pkdg_status pkdg_create(pkdg_ctx **ctx, int device);
 pkdg_status pkdg_destroy(pkdg_ctx *ctx);
 
-/* Options of a context.  PKDG_OPT_KAPPA2: conditioning threshold of the fp64 fix-up (> 0; default 8). */
+/* Options of a context.  PKDG_OPT_KAPPA2: conditioning threshold of the fp64 fix-up (> 0; default 6). */
 #define PKDG_OPT_KAPPA2 1
 pkdg_status pkdg_set_option(pkdg_ctx *ctx, int32_t option, double value);
 

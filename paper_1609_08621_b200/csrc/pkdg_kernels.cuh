@@ -825,18 +825,25 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
 }
 
 // ------------------------------------------------------------------------------------------------
-// Bucket kernel, generation 4 (a2-a5 for per-bucket lists).  The group kernel's idea -- a lane OWNS a sink pair,
-// sinks and accumulators stay in registers, sources stream through shared memory -- applied to ONE bucket per
-// warp: a bucket has at most 8 sink pairs per pass, so the 32 lanes are (source slot, sink pair) =
-// (lane >> LG, lane & (2^LG - 1)) with 2^LG = 8 or 4 pairs and NS = 4 or 8 source slots.  A tile of 32 source
-// particles / 32 cell records is staged by the whole warp (cp.async, double buffered, coalesced) and lane
-// (slot, pair) evaluates sources slot, slot + NS, ... of the tile against its pair.  Compared with generation 3
-// (a lane holds a source, per-lane partial sums of all 16 sinks in shared memory):
-//   - a list is padded to a multiple of NS (4 or 8) instead of 32: P-C lists fill 99 % of their slots, not 89 %;
-//   - no accumulator traffic through shared memory, and the cross-lane reduction is 2 (3) xor-shuffle rounds of 10
-//     values instead of a 64-value butterfly;
+// Bucket kernel (a2-a5 for per-bucket lists): one bucket per warp, buckets handed out in tree order through an
+// atomic counter (neighbouring buckets share most of their sources, so these come from L2 / L1).  A lane OWNS a
+// sink pair -- the two halves of every packed value are its two sinks -- and keeps sinks and accumulators in
+// registers; the sources stream through shared memory.  A pass of ntp <= 16 sinks has npp = ceil(ntp / 2) sink
+// pairs and the 32 lanes are laid out as npp pairs x ns = floor(32 / npp) source slots:
+//     13 - 16 sinks: 8 pairs x 4 slots;  11, 12: 6 x 5;  9, 10: 5 x 6;  7, 8: 4 x 8;  5, 6: 3 x 10;  3, 4: 2 x 16;  1, 2: 1 x 32
+// (30 of 32 lanes busy for 5 and 6 pairs, where a fixed 8-pair layout would leave 3 or 2 lanes of every 8 idle; a
+// binary tree over clustered particles fills its buckets to anything between 8 and 16).  A tile of T = ns *
+// floor(32 / ns) sources (32 or 30: a multiple of ns, so that every trip over a tile keeps all busy lanes busy) is
+// staged by the whole warp (cp.async, one source particle / one 128-byte cell record per lane) and lane (slot,
+// pair) evaluates sources slot, slot + ns, ... of the tile against its pair.
+//   - a list is padded to a multiple of ns, not of 32: P-C lists fill 99 % of their slots;
+//   - no accumulator traffic through shared memory; the cross-lane reduction at the end of a pass is a few shuffle
+//     rounds of 10 values;
 //   - the conditioning estimate is the exact per-sink S2_i = sum_j |a_ij|^2, a softened pair is corrected in place;
-//   - 112 registers: 16 warps per SM hide the load chain at the start of a bucket, no hand-built hand-over.
+//   - 96 registers, 20 warps per SM: the load chain at the start of a bucket (counter, descriptor, sinks, indices,
+//     sources) is hidden by the other warps, there is no hand-built hand-over between buckets.
+// P-P source tiles sit in a ring of 4 (three tiles in flight: a tile is only ~130 instructions per lane), P-C tiles
+// are double buffered and tile 0 is issued before the P-P phase.
 // ------------------------------------------------------------------------------------------------
 #ifndef PKDG_B_UNROLL
 #define PKDG_B_UNROLL 1
@@ -846,30 +853,45 @@ constexpr int kBUnroll = PKDG_B_UNROLL;
 constexpr int kBRing = 4;         // P-P source tiles in shared memory: one in use, kBRing - 1 in flight
 struct __align__(16) WarpSmemB {
     float4 cell[2][8 * 32];       // [float4 of the record][cell of the tile]: writes by lane = cell and reads by
-                                  // slot = cell mod NS are both conflict-free
+                                  // slot = cell mod ns are both conflict-free
     float4 src[kBRing][32];
     int32_t sidx[kBRing][32];
 };
 
-// One pass (<= 16 sinks = <= 2^LG pairs) of one bucket.
-template <int LG, bool LEAF>
+// entry e of a list of len entries that starts at idx[begin]; -1 (padding) beyond its end
+__device__ __forceinline__ int32_t list_entry(const int32_t* __restrict__ idx, int64_t begin, int32_t len, int32_t e) {
+    return e < len ? __ldg(idx + begin + e) : -1;
+}
+
+// floor(x / d) for 0 <= x <= 32, 1 <= d <= 8 without an integer division (the quotient's fractional part is a
+// multiple of 1 / d >= 1 / 8, so the reciprocal's rounding cannot move it across an integer)
+__device__ __forceinline__ int small_div(int x, int d) {
+    return __float2int_rd(fmaf((float)x, __frcp_rn((float)d), 0.01f));
+}
+
+// One pass (<= 16 sinks) of one bucket.
+template <bool LEAF>
 __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, const BucketDesc& d, const int bucket,
                                             const int t0, const int ntp, const int pp_len, const int pc_len,
                                             const int lane, unsigned& bad) {
-    constexpr int NPP = 1 << LG, NS = 32 >> LG;
+    const int npp = ntp > 12 ? 8 : (ntp + 1) >> 1;   // sink pairs of the layout
+    const int ns = small_div(32, npp);                // source slots
+    const int slot = small_div(lane, npp), pair = lane - slot * npp;
+    const bool busy = slot < ns;
+    const int lslot = busy ? slot : 0;                // idle lanes shadow slot 0 (their sinks are dummies, nothing is written)
+    const int T = (ns & (ns - 1)) ? 30 : 32;          // sources / cells per tile: ns * floor(32 / ns) (ns = 5, 6, 10: 30)
     const float4 far4 = make_float4(kFar, kFar, kFar, 0.0f);
     const bool accumulate = (p.flags & 0x1u) != 0, fix_on = p.fix_k >= 0.0f;
-    const int pair = lane & (NPP - 1), slot = lane >> LG;
     const int lo = d.first + t0, hi = lo + ntp;   // particle index range of the pass's sinks (self test per tile)
-    const int iA = 2 * pair < ntp ? lo + 2 * pair : -1, iB = 2 * pair + 1 < ntp ? lo + 2 * pair + 1 : -1;
+    const int iA = busy && 2 * pair < ntp ? lo + 2 * pair : -1, iB = busy && 2 * pair + 1 < ntp ? lo + 2 * pair + 1 : -1;
     const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
     const float4 tA = iA >= 0 ? __ldg(p.xyzm + iA) : dummy_tgt, tB = iB >= 0 ? __ldg(p.xyzm + iB) : dummy_tgt;
     const float2 X = make_float2(tA.x, tB.x), Y = make_float2(tA.y, tB.y), Z = make_float2(tA.z, tB.z);
     float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, aw = ax, s2 = ax;
 
     // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
-    const int pc_ntile = (pc_len + 31) >> 5;
-    auto cidx_of = [&](int k) -> int32_t { return tile_entry(p.pc_idx, d.pc_begin, pc_len, k, lane); };
+    const int pc_ntile = T == 32 ? (pc_len + 31) >> 5 : (pc_len + 29) / 30;
+    auto cidx_of = [&](int k) -> int32_t { return lane < T ? list_entry(p.pc_idx, d.pc_begin, pc_len, k * T + lane) : -1; };
     auto issue_cell = [&](int32_t c, int buf) {
         if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
         float4* dst = &S.cell[buf][lane];
@@ -891,11 +913,13 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
         cn = pc_ntile > 1 ? cidx_of(1) : -1;
     }
 
-    // ---- a3: P-P.  Tile k (32 sources) is computed from ring buffer k % kBRing while tiles k + 1 .. k + kBRing - 1 are
-    //      in flight (a tile is only ~130 instructions per lane: one tile of prefetch does not cover a global load).
+    // ---- a3: P-P.  Tile k is computed from ring buffer k % kBRing while tiles k + 1 .. k + kBRing - 1 are in flight.
+    //      LEAF (PKDG_PP_LEAVES): a tile is TWO bucket references, lanes 0-15 stage the particles of the first and
+    //      lanes 16-31 those of the second (a bucket holds at most 16), so a tile always has 32 slots.
     {
         constexpr int PD = kBRing - 1;
-        const int ntile = LEAF ? (pp_len + 1) >> 1 : (pp_len + 31) >> 5;
+        const int TP = LEAF ? 32 : T;
+        const int ntile = LEAF ? (pp_len + 1) >> 1 : TP == 32 ? (pp_len + 31) >> 5 : (pp_len + 29) / 30;
         const int half = lane >> 4, hslot = lane & 15;
         auto ref_of = [&](int k) -> int32_t {           // LEAF: bucket reference of this half-warp in tile k
             const int r = 2 * k + half;
@@ -906,7 +930,7 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             const int2 fc = __ldg(p.gfc + g);
             return fc.y > 16 ? make_int2(0, 0) : fc;
         };
-        auto idx_of = [&](int k) -> int32_t { return tile_entry(p.pp_idx, d.pp_begin, pp_len, k, lane); };
+        auto idx_of = [&](int k) -> int32_t { return lane < TP ? list_entry(p.pp_idx, d.pp_begin, pp_len, k * TP + lane) : -1; };
         auto issue = [&](int32_t j, int buf) {           // the lane's source of a tile starts its way to shared memory
             if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
             S.sidx[buf][lane] = j;
@@ -957,37 +981,46 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             } else {
                 cp_async_commit();
             }
-            // sources of this tile the lane visits: slot, slot + NS, ...; a short last tile ends early (warp-uniform)
-            const int nsrc = LEAF ? 32 : min(32, pp_len - 32 * k);
-            const int ntrip = (nsrc + NS - 1) >> (5 - LG);
+            // sources of this tile the lane visits: slot, slot + ns, ...; a short last tile ends early
+            const int nsrc = LEAF ? 32 : min(TP, pp_len - TP * k);
             const int32_t jl = S.sidx[buf][lane];
             const bool own = __any_sync(0xffffffffu, jl >= lo && jl < hi);   // tile holds sinks of this pass
-            const float4* src = S.src[buf] + slot;
-            const int32_t* sid = S.sidx[buf] + slot;
+            const float4* src = S.src[buf];
+            const int32_t* sid = S.sidx[buf];
+            // LEAF tiles have 32 slots whatever ns is: the last trip of a 30-slot layout runs past the tile for some lanes
+            auto ld_src = [&](int pos) -> float4 { return (LEAF && pos >= 32) ? far4 : src[pos]; };
+            auto ld_sid = [&](int pos) -> int32_t { return (LEAF && pos >= 32) ? -1 : sid[pos]; };
             float minr2 = 3.0e38f;
-            if (ntrip < 32 / NS || own) {   // a short last tile, or a tile with own particles: self test by index
-                if (ntrip == 32 / NS) {
+            if (npp == 8 && nsrc == 32) {   // a full tile of a full bucket: straight-line code
+                const float4* s8 = src + (lane >> 3);
+                if (!own) {
 #pragma unroll
-                    for (int it = 0; it < 32 / NS; ++it) {
-                        const int32_t sj = sid[it * NS];
-                        pp_pair_g<true>(X, Y, Z, src[it * NS], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
-                    }
+                    for (int it = 0; it < 8; ++it)
+                        pp_pair_g<false>(X, Y, Z, s8[4 * it], false, false, p.h2c, minr2, ax, ay, az, aw, s2);
                 } else {
-#pragma unroll 2
-                    for (int it = 0; it < ntrip; ++it) {
-                        const int32_t sj = sid[it * NS];
-                        pp_pair_g<true>(X, Y, Z, src[it * NS], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                    const int32_t* i8 = sid + (lane >> 3);
+#pragma unroll
+                    for (int it = 0; it < 8; ++it) {
+                        const int32_t sj = i8[4 * it];
+                        pp_pair_g<true>(X, Y, Z, s8[4 * it], sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
                     }
                 }
-            } else {   // the common tile: straight-line code over its 32 / NS sources, no guards, so that they interleave
-#pragma unroll
-                for (int it = 0; it < 32 / NS; ++it)
-                    pp_pair_g<false>(X, Y, Z, src[it * NS], false, false, p.h2c, minr2, ax, ay, az, aw, s2);
+            } else if (own) {                        // a tile with own particles: self test by index
+                // (trip counts are warp-uniform: slots beyond the end of a short tile hold padding, which contributes 0)
+#pragma unroll 2
+                for (int base = 0; base < nsrc; base += ns) {
+                    const int32_t sj = ld_sid(base + lslot);
+                    pp_pair_g<true>(X, Y, Z, ld_src(base + lslot), sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                }
+            } else {
+#pragma unroll 3
+                for (int base = 0; base < nsrc; base += ns)
+                    pp_pair_g<false>(X, Y, Z, ld_src(base + lslot), false, false, p.h2c, minr2, ax, ay, az, aw, s2);
             }
             if (minr2 < p.h2c) {   // rare: a pair of this lane inside the softening (or coincident): the lane owns its sinks
-                for (int it = 0; it < ntrip; ++it) {
-                    const float4 s = src[it * NS];
-                    const int32_t sj = sid[it * NS];
+                for (int base = 0; base < nsrc; base += ns) {
+                    const float4 s = ld_src(base + lslot);
+                    const int32_t sj = ld_sid(base + lslot);
                     if (sj < 0) continue;
                     if (sj != iA) pp_soft_fix_g(X.x, Y.x, Z.x, s, p, ax.x, ay.x, az.x, aw.x, s2.x);
                     if (sj != iB) pp_soft_fix_g(X.y, Y.y, Z.y, s, p, ax.y, ay.y, az.y, aw.y, s2.y);
@@ -996,7 +1029,7 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
         }
     }
 
-    // ---- a4: P-C.  Tile k = 32 cell records, one per lane (8 x cp.async of 16 bytes), in buffer k & 1; tile 0 was
+    // ---- a4: P-C.  Tile k = T cell records, one per lane (8 x cp.async of 16 bytes), in buffer k & 1; tile 0 was
     //      issued before the P-P phase.
     {
         for (int k = 0; k < pc_ntile; ++k) {
@@ -1007,12 +1040,11 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
                 issue_cell(cn, buf ^ 1);
                 cn = (k + 2 < pc_ntile) ? cidx_of(k + 2) : -1;
             }
-            const int ncell = min(32, pc_len - 32 * k);
-            const int ntrip = (ncell + NS - 1) >> (5 - LG);
-            const float4* rec = S.cell[buf] + slot;
+            const int ncell = min(T, pc_len - T * k);
+            const float4* rec = S.cell[buf];
 #pragma unroll kBUnroll
-            for (int it = 0; it < ntrip; ++it) {
-                const float4* r = rec + it * NS;
+            for (int base = 0; base < ncell; base += ns) {   // warp-uniform trips; a short tile ends in padding cells
+                const float4* r = rec + base + lslot;
                 CellRegs cr;
                 cell_unpack(cr, r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]);
                 pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
@@ -1020,14 +1052,24 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
         }
     }
 
-    // ---- a5: the NS source slots of every sink pair are summed by xor-shuffles; lanes of slot 0 test and write
+    // ---- a5: the source slots of every sink pair are summed by shuffles; lanes of slot 0 test and write
+    if (npp == 8) {
 #pragma unroll
-    for (int o = 16; o >= NPP; o >>= 1) {
-        ax.x += __shfl_xor_sync(0xffffffffu, ax.x, o); ax.y += __shfl_xor_sync(0xffffffffu, ax.y, o);
-        ay.x += __shfl_xor_sync(0xffffffffu, ay.x, o); ay.y += __shfl_xor_sync(0xffffffffu, ay.y, o);
-        az.x += __shfl_xor_sync(0xffffffffu, az.x, o); az.y += __shfl_xor_sync(0xffffffffu, az.y, o);
-        aw.x += __shfl_xor_sync(0xffffffffu, aw.x, o); aw.y += __shfl_xor_sync(0xffffffffu, aw.y, o);
-        s2.x += __shfl_xor_sync(0xffffffffu, s2.x, o); s2.y += __shfl_xor_sync(0xffffffffu, s2.y, o);
+        for (int o = 16; o >= 8; o >>= 1) {
+            ax.x += __shfl_xor_sync(0xffffffffu, ax.x, o); ax.y += __shfl_xor_sync(0xffffffffu, ax.y, o);
+            ay.x += __shfl_xor_sync(0xffffffffu, ay.x, o); ay.y += __shfl_xor_sync(0xffffffffu, ay.y, o);
+            az.x += __shfl_xor_sync(0xffffffffu, az.x, o); az.y += __shfl_xor_sync(0xffffffffu, az.y, o);
+            aw.x += __shfl_xor_sync(0xffffffffu, aw.x, o); aw.y += __shfl_xor_sync(0xffffffffu, aw.y, o);
+            s2.x += __shfl_xor_sync(0xffffffffu, s2.x, o); s2.y += __shfl_xor_sync(0xffffffffu, s2.y, o);
+        }
+    } else {   // any number of slots: slot s < step takes slot s + step, step = 16, 8, .. 1
+        for (int step = 16; step >= 1; step >>= 1) {
+            if (step >= ns) continue;   // warp-uniform
+            const int o = step * npp;
+            const bool take = slot < step && slot + step < ns;   // then lane + o <= 31
+            auto add = [&](float& v) { const float t = __shfl_down_sync(0xffffffffu, v, o & 31); v += take ? t : 0.0f; };
+            add(ax.x); add(ax.y); add(ay.x); add(ay.y); add(az.x); add(az.y); add(aw.x); add(aw.y); add(s2.x); add(s2.y);
+        }
     }
     float4 rA = make_float4(ax.x, ay.x, az.x, aw.x), rB = make_float4(ax.y, ay.y, az.y, aw.y);
     const bool wA = slot == 0 && iA >= 0, wB = slot == 0 && iB >= 0;
@@ -1063,8 +1105,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalb_kernel(const Eval
         const int pp_len = do_pp ? d.pp_len : 0, pc_len = do_pc ? d.pc_len : 0;
         for (int t0 = 0; t0 < d.count; t0 += kTMax) {
             const int ntp = min(kTMax, d.count - t0);
-            if (ntp > 8) bucket_pass<3, LEAF>(p, S, d, (int)bu, t0, ntp, pp_len, pc_len, lane, bad);
-            else bucket_pass<2, LEAF>(p, S, d, (int)bu, t0, ntp, pp_len, pc_len, lane, bad);
+            bucket_pass<LEAF>(p, S, d, (int)bu, t0, ntp, pp_len, pc_len, lane, bad);
         }
     }
     if (bad) atomicAdd(&p.stats->bad_entries, (unsigned long long)bad);

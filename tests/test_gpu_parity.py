@@ -372,7 +372,7 @@ def test_fixup_threshold_option_and_accumulate(ctx, torch, cfg1):
         acc = run_resident(ctx, p, torch, flags=binding.ACCUMULATE, fill=1.0)
         assert np.allclose(acc, mixed + 1.0, rtol=1e-6, atol=1e-6)
     finally:
-        ctx.set_option(binding.OPT_KAPPA2, 8.0)
+        ctx.set_option(binding.OPT_KAPPA2, 6.0)   # the library default (kDefaultKappa2)
 
 
 def test_validate_flag_checks_the_value_range_contract(ctx, torch, cfg1):
