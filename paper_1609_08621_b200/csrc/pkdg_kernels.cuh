@@ -916,9 +916,11 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
     // ---- a3: P-P.  Tile k is computed from ring buffer k % kBRing while tiles k + 1 .. k + kBRing - 1 are in flight.
     //      LEAF (PKDG_PP_LEAVES): a tile is TWO bucket references, lanes 0-15 stage the particles of the first and
     //      lanes 16-31 those of the second (a bucket holds at most 16), so a tile always has 32 slots.
-    {
+    auto pp_phase = [&](auto full_tag) {   // two copies of the P-P loop: full buckets (8 x 4 lanes, everything a constant) and the rest
+        constexpr bool FULL = decltype(full_tag)::value;
+        const int nsl = FULL ? 4 : ns, Tl = FULL ? 32 : T, lsl = FULL ? (lane >> 3) : lslot;
         constexpr int PD = kBRing - 1;
-        const int TP = LEAF ? 32 : T;
+        const int TP = LEAF ? 32 : Tl;
         const int ntile = LEAF ? (pp_len + 1) >> 1 : TP == 32 ? (pp_len + 31) >> 5 : (pp_len + 29) / 30;
         const int half = lane >> 4, hslot = lane & 15;
         auto ref_of = [&](int k) -> int32_t {           // LEAF: bucket reference of this half-warp in tile k
@@ -991,7 +993,7 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             auto ld_src = [&](int pos) -> float4 { return (LEAF && pos >= 32) ? far4 : src[pos]; };
             auto ld_sid = [&](int pos) -> int32_t { return (LEAF && pos >= 32) ? -1 : sid[pos]; };
             float minr2 = 3.0e38f;
-            if (npp == 8 && nsrc == 32) {   // a full tile of a full bucket: straight-line code
+            if (FULL && nsrc == 32) {   // a full tile of a full bucket: straight-line code
                 const float4* s8 = src + (lane >> 3);
                 if (!own) {
 #pragma unroll
@@ -1008,26 +1010,28 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             } else if (own) {                        // a tile with own particles: self test by index
                 // (trip counts are warp-uniform: slots beyond the end of a short tile hold padding, which contributes 0)
 #pragma unroll 2
-                for (int base = 0; base < nsrc; base += ns) {
-                    const int32_t sj = ld_sid(base + lslot);
-                    pp_pair_g<true>(X, Y, Z, ld_src(base + lslot), sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
+                for (int base = 0; base < nsrc; base += nsl) {
+                    const int32_t sj = ld_sid(base + lsl);
+                    pp_pair_g<true>(X, Y, Z, ld_src(base + lsl), sj == iA, sj == iB, p.h2c, minr2, ax, ay, az, aw, s2);
                 }
             } else {
 #pragma unroll 3
-                for (int base = 0; base < nsrc; base += ns)
-                    pp_pair_g<false>(X, Y, Z, ld_src(base + lslot), false, false, p.h2c, minr2, ax, ay, az, aw, s2);
+                for (int base = 0; base < nsrc; base += nsl)
+                    pp_pair_g<false>(X, Y, Z, ld_src(base + lsl), false, false, p.h2c, minr2, ax, ay, az, aw, s2);
             }
             if (minr2 < p.h2c) {   // rare: a pair of this lane inside the softening (or coincident): the lane owns its sinks
-                for (int base = 0; base < nsrc; base += ns) {
-                    const float4 s = ld_src(base + lslot);
-                    const int32_t sj = ld_sid(base + lslot);
+                for (int base = 0; base < nsrc; base += nsl) {
+                    const float4 s = ld_src(base + lsl);
+                    const int32_t sj = ld_sid(base + lsl);
                     if (sj < 0) continue;
                     if (sj != iA) pp_soft_fix_g(X.x, Y.x, Z.x, s, p, ax.x, ay.x, az.x, aw.x, s2.x);
                     if (sj != iB) pp_soft_fix_g(X.y, Y.y, Z.y, s, p, ax.y, ay.y, az.y, aw.y, s2.y);
                 }
             }
         }
-    }
+    
+    };
+    if (npp == 8) pp_phase(std::true_type{}); else pp_phase(std::false_type{});
 
     // ---- a4: P-C.  Tile k = T cell records, one per lane (8 x cp.async of 16 bytes), in buffer k & 1; tile 0 was
     //      issued before the P-P phase.
