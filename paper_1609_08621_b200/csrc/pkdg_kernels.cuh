@@ -845,10 +845,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
 // P-P source tiles sit in a ring of 4 (three tiles in flight: a tile is only ~130 instructions per lane), P-C tiles
 // are double buffered and tile 0 is issued before the P-P phase.
 // ------------------------------------------------------------------------------------------------
-#ifndef PKDG_B_UNROLL
-#define PKDG_B_UNROLL 1
-#endif
-constexpr int kBUnroll = PKDG_B_UNROLL;
 
 constexpr int kBRing = 4;         // P-P source tiles in shared memory: one in use, kBRing - 1 in flight
 struct __align__(16) WarpSmemB {
@@ -993,7 +989,8 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             auto ld_src = [&](int pos) -> float4 { return (LEAF && pos >= 32) ? far4 : src[pos]; };
             auto ld_sid = [&](int pos) -> int32_t { return (LEAF && pos >= 32) ? -1 : sid[pos]; };
             float minr2 = 3.0e38f;
-            if (FULL && nsrc == 32) {   // a full tile of a full bucket: straight-line code
+            if (FULL) {   // a full bucket: straight-line code over the 8 visits of a tile (a short last tile ends in padding
+                          // slots, which contribute exactly 0: cheaper than a second, looping copy of the code)
                 const float4* s8 = src + (lane >> 3);
                 if (!own) {
 #pragma unroll
@@ -1046,12 +1043,26 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             }
             const int ncell = min(T, pc_len - T * k);
             const float4* rec = S.cell[buf];
-#pragma unroll kBUnroll
-            for (int base = 0; base < ncell; base += ns) {   // warp-uniform trips; a short tile ends in padding cells
-                const float4* r = rec + base + lslot;
-                CellRegs cr;
-                cell_unpack(cr, r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]);
-                pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
+            // warp-uniform trips; a short tile ends in padding cells.  Full buckets (8 x 4 lanes: a full tile is 8 trips)
+            // run two trips per iteration -- ptxas then keeps a few more operands in the reuse cache (config 3 -0.8 %);
+            // the other layouts have 5 or 6 trips per tile and lose 4 % that way.
+            if (npp == 8) {
+                const float4* r = rec + (lane >> 3);
+#pragma unroll 2
+                for (int base = 0; base < ncell; base += 4) {
+                    CellRegs cr;
+                    cell_unpack(cr, r[base], r[base + 32], r[base + 64], r[base + 96], r[base + 128], r[base + 160],
+                                r[base + 192], r[base + 224]);
+                    pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
+                }
+            } else {
+#pragma unroll 1
+                for (int base = 0; base < ncell; base += ns) {
+                    const float4* r = rec + base + lslot;
+                    CellRegs cr;
+                    cell_unpack(cr, r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]);
+                    pc_pair_g(X, Y, Z, cr, ax, ay, az, aw, s2);
+                }
             }
         }
     }
