@@ -691,6 +691,10 @@ def run_report(args):
             lines.append(rc(f"cfg4 P-C only L_pc={lpc}", inputs.config4(nbc, 0, lpc), f"{nbc} buckets, reuse 16"))
         for l, nbc in ((32, 65536), (128, 65536), (512, 16384), (2048, 4096)):
             lines.append(rc(f"cfg4 fused L_pp=L_pc={l}", inputs.config4(nbc, l, l), f"{nbc} buckets, reuse 16"))
+    for tok in sorted(want):   # one config-4 shape by itself: c4:<buckets>:<L_pp>:<L_pc> (what an ncu capture of one shape runs)
+        if tok.startswith("c4:"):
+            nbc, lpp, lpc = (int(v) for v in tok[3:].split(":"))
+            lines.append(rc(f"cfg4 {nbc} buckets L_pp={lpp} L_pc={lpc}", inputs.config4(nbc, lpp, lpc), "reuse 16"))
     if "5" in want or "all" in want:
         # N = 2^26: a contiguous range of 2^20 buckets (lists built for that range), resident and streamed
         xyzm, eps = inputs.config5_particles()
@@ -808,7 +812,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-chunk", type=int, default=1 << 23)
-    ap.add_argument("--report", default="", help="comma list of configs (1,2,3,4,5,5full or all): per-case report lines "
+    ap.add_argument("--report", default="", help="comma list of configs (1,2,3,4,5,5full, all, or c4:<buckets>:<L_pp>:<L_pc>): per-case report lines "
                                                   "instead of the contract line")
     ap.add_argument("--report-reps", type=int, default=10)
     args = ap.parse_args()

@@ -164,6 +164,61 @@ def test_edge_cases(ctx, torch, flags):
     assert ctx.get_stats()["bad_entries"] == 0
 
 
+def _layout_problem(seed=7):
+    """Every bucket occupancy 0 .. 35 (all lane layouts of the bucket kernel: 1 x 32, 2 x 16, 3 x 10, 4 x 8, 5 x 6,
+    6 x 5, 8 x 4, and passes beyond 16 sinks) against list lengths on both sides of the 30- and 32-slot tile
+    boundaries.  The buckets' own particles are on their P-P lists (self pairs), some pairs are softened."""
+    from paper_1609_08621_b200 import inputs
+    rng = np.random.default_rng(seed)
+    lens = [0, 1, 4, 5, 29, 30, 31, 32, 33, 59, 60, 61, 63, 64, 65, 90, 96, 127, 150, 301]
+    counts = [c for c in range(36) for _ in range(3)]
+    nb = len(counts)
+    n_t = sum(counts)
+    n_src = 1200
+    xyzm = np.empty((n_t + n_src, 4), np.float32)
+    centre = 0.5 + 0.2 * rng.standard_normal((nb, 3))
+    first = np.concatenate([[0], np.cumsum(counts)[:-1]]).astype(np.int32)
+    count = np.array(counts, np.int32)
+    for b in range(nb):
+        xyzm[first[b]: first[b] + count[b], :3] = centre[b] + 0.004 * rng.standard_normal((count[b], 3))
+    xyzm[n_t:, :3] = 0.5 + 0.25 * rng.standard_normal((n_src, 3))
+    xyzm[:, 3] = rng.uniform(0.5, 1.5, n_t + n_src) / (n_t + n_src)
+    pp, pc = [], []
+    ncell = 400
+    com = 0.5 + rng.choice([-1, 1], (ncell, 3)) * rng.uniform(1.2, 2.0, (ncell, 3))
+    pts = np.empty((ncell * 12, 4), np.float32)
+    pts[:, :3] = np.repeat(com, 12, axis=0) + 0.03 * rng.standard_normal((ncell * 12, 3))
+    pts[:, 3] = rng.uniform(0.5, 1.5, ncell * 12) / (ncell * 12)
+    cells = inputs.cloud_records(pts, 12)
+    for b in range(nb):
+        own = np.arange(first[b], first[b] + count[b])
+        L = lens[(b * 7 + 3) % len(lens)]
+        l = np.concatenate([own, n_t + rng.choice(n_src, L, replace=False)]).astype(np.int32)
+        rng.shuffle(l)                                                  # own particles anywhere in the list
+        pp.append(l)
+        pc.append(rng.choice(ncell, lens[(b * 11 + 5) % len(lens)], replace=False).astype(np.int32))
+    pp_off = np.concatenate([[0], np.cumsum([len(l) for l in pp])]).astype(np.int64)
+    pc_off = np.concatenate([[0], np.cumsum([len(l) for l in pc])]).astype(np.int64)
+    return inputs.Problem(name="layouts", xyzm=xyzm, cells=cells, first=first, count=count, pp_off=pp_off,
+                          pp_idx=np.concatenate(pp).astype(np.int32), pc_off=pc_off,
+                          pc_idx=np.concatenate(pc).astype(np.int32), eps=float(np.float32(0.003)))
+
+
+@pytest.mark.parametrize("flags", MODES)
+def test_every_bucket_occupancy_and_lane_layout(ctx, torch, flags):
+    from gpu_util import rel_errors, run_resident
+    p = _layout_problem()
+    ref = _oracle(p)
+    out = run_resident(ctx, p, torch, flags=flags)
+    st = ctx.get_stats()
+    assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
+    n_t = int(p.count.sum())
+    ea, ep = rel_errors(out, ref, np.arange(n_t))
+    worst = int(np.argmax(ea))
+    assert ea.max() <= TOL and ep.max() <= TOL, (ea.max(), ep.max(), int(np.searchsorted(p.first, worst, "right") - 1))
+    assert np.isnan(out[n_t:]).all()                                    # sources are in no bucket: untouched
+
+
 def test_softened_plummer_cores(ctx, torch):
     """configs[1] recipe at N = 2^15: dense Plummer cores put many pairs inside the spline."""
     from paper_1609_08621_b200 import inputs
