@@ -584,7 +584,14 @@ struct __align__(16) WarpSmemG {
     int32_t sslot[kGSinks];
 };
 
-// One source against the lane's sink pair; as pp_fast2 plus the exact conditioning estimate.
+// Coordinate c (0, 1, 2) of the sinks iA, iB of a lane as one packed pair; an unused slot (index < 0) is a dummy
+// sink at -1e15 that no source comes near.
+__device__ __forceinline__ float2 sink_pair_coord(const float4* __restrict__ xyzm, int iA, int iB, int c) {
+    const float* f = reinterpret_cast<const float*>(xyzm);
+    return make_float2(iA >= 0 ? __ldg(f + 4 * (int64_t)iA + c) : -kFar, iB >= 0 ? __ldg(f + 4 * (int64_t)iB + c) : -kFar);
+}
+
+// One source against the lane's sink pair, Newtonian with r^2 clamped from below at h2c, plus the exact conditioning estimate.
 template <bool SELF>
 __device__ __forceinline__ void pp_pair_g(const float2 X, const float2 Y, const float2 Z, const float4 s, bool selfA,
                                           bool selfB, float h2c, float& minr2, float2& ax, float2& ay, float2& az,
@@ -680,8 +687,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
             __syncwarp();
             const int iA = S.sink[2 * lane], iB = S.sink[2 * lane + 1];
             const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-            const float4 tA = iA >= 0 ? __ldg(p.xyzm + iA) : dummy_tgt, tB = iB >= 0 ? __ldg(p.xyzm + iB) : dummy_tgt;
-            const float2 X = make_float2(tA.x, tB.x), Y = make_float2(tA.y, tB.y), Z = make_float2(tA.z, tB.z);
+            const float2 X = sink_pair_coord(p.xyzm, iA, iB, 0), Y = sink_pair_coord(p.xyzm, iA, iB, 1), Z = sink_pair_coord(p.xyzm, iA, iB, 2);
             float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, aw = ax, s2 = ax;
 
             // ---- a3: P-P.  Tile k (32 sources) is computed from buffer k & 1 while tile k + 1 lands in the other.
@@ -881,8 +887,9 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
     const int lo = d.first + t0, hi = lo + ntp;   // particle index range of the pass's sinks (self test per tile)
     const int iA = busy && 2 * pair < ntp ? lo + 2 * pair : -1, iB = busy && 2 * pair + 1 < ntp ? lo + 2 * pair + 1 : -1;
     const float4 dummy_tgt = make_float4(-kFar, -kFar, -kFar, 0.0f);
-    const float4 tA = iA >= 0 ? __ldg(p.xyzm + iA) : dummy_tgt, tB = iB >= 0 ? __ldg(p.xyzm + iB) : dummy_tgt;
-    const float2 X = make_float2(tA.x, tB.x), Y = make_float2(tA.y, tB.y), Z = make_float2(tA.z, tB.z);
+    // scalar loads: a float4 load would tie (x_A, x_B) to two different register quads and ptxas would re-pack the
+    // pair with two MOVs in front of every packed instruction that reads it (4.5 MOVs per P-P visit)
+    const float2 X = sink_pair_coord(p.xyzm, iA, iB, 0), Y = sink_pair_coord(p.xyzm, iA, iB, 1), Z = sink_pair_coord(p.xyzm, iA, iB, 2);
     float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, aw = ax, s2 = ax;
 
     // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
