@@ -860,11 +860,6 @@ struct __align__(16) WarpSmemB {
     int32_t sidx[kBRing][32];
 };
 
-// entry e of a list of len entries that starts at idx[begin]; -1 (padding) beyond its end
-__device__ __forceinline__ int32_t list_entry(const int32_t* __restrict__ idx, int64_t begin, int32_t len, int32_t e) {
-    return e < len ? __ldg(idx + begin + e) : -1;
-}
-
 // floor(x / d) for 0 <= x <= 32, 1 <= d <= 8 without an integer division (the quotient's fractional part is a
 // multiple of 1 / d >= 1 / 8, so the reciprocal's rounding cannot move it across an integer)
 __device__ __forceinline__ int small_div(int x, int d) {
@@ -894,9 +889,11 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
 
     // ---- the lane's cell of P-C tile 0 starts its way to shared memory under the P-P phase
     const int pc_ntile = T == 32 ? (pc_len + 31) >> 5 : (pc_len + 29) / 30;
-    auto cidx_of = [&](int k) -> int32_t { return lane < T ? list_entry(p.pc_idx, d.pc_begin, pc_len, k * T + lane) : -1; };
+    const int32_t* __restrict__ pc_list = p.pc_idx + d.pc_begin;   // n_particles, n_cells < 2^31 (checked by the host): 32-bit tests
+    const uint32_t np32 = (uint32_t)p.n_particles, nc32 = (uint32_t)p.n_cells;
+    auto cidx_of = [&](int k) -> int32_t { const int e = k * T + lane; return (lane < T && e < pc_len) ? __ldg(pc_list + e) : -1; };
     auto issue_cell = [&](int32_t c, int buf) {
-        if ((uint32_t)c >= (uint64_t)p.n_cells) { bad += (c >= 0); c = -1; }
+        if ((uint32_t)c >= nc32) { bad += (c >= 0); c = -1; }
         float4* dst = &S.cell[buf][lane];
         if (c >= 0) {
             const float4* q = p.cellq + (int64_t)c * 8;
@@ -935,9 +932,10 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
             const int2 fc = __ldg(p.gfc + g);
             return fc.y > 16 ? make_int2(0, 0) : fc;
         };
-        auto idx_of = [&](int k) -> int32_t { return lane < TP ? list_entry(p.pp_idx, d.pp_begin, pp_len, k * TP + lane) : -1; };
+        const int32_t* __restrict__ pp_list = p.pp_idx + d.pp_begin;
+        auto idx_of = [&](int k) -> int32_t { const int e = k * TP + lane; return (lane < TP && e < pp_len) ? __ldg(pp_list + e) : -1; };
         auto issue = [&](int32_t j, int buf) {           // the lane's source of a tile starts its way to shared memory
-            if ((uint32_t)j >= (uint64_t)p.n_particles) { bad += (j >= 0); j = -1; }
+            if ((uint32_t)j >= np32) { bad += (j >= 0); j = -1; }
             S.sidx[buf][lane] = j;
             if (j >= 0) cp_async16(&S.src[buf][lane], p.xyzm + j);
             else S.src[buf][lane] = far4;
