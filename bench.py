@@ -32,7 +32,7 @@ sys.path.insert(0, ROOT)
 # line by line in DESIGN.md "Flop audit".  The paper's own convention (Table 3: 53 / 215, rsqrt = 7)
 # is reported beside it as context only.
 F_PP = 19
-F_PC = 169
+F_PC = 167
 PAPER_F_PP, PAPER_F_PC = 53, 215
 # C-C / C-P path (pkdg_fmm.cuh, formulas as executed): per C-C entry, per C-P entry, per sink evaluated, per bucket
 F_CC, F_CP, F_LOC_SINK, F_LOC_BUCKET = 1091, 468, 488, 1848

@@ -478,6 +478,13 @@ __device__ __forceinline__ float2 f2mul(float2 a, float2 b) { return __fmul2_rn(
 __device__ __forceinline__ float2 f2add(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 f2fma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 
+// 2 v by an integer add to the exponent field: runs on the ALU pipe, not on the FMA pipe the kernel is bound by.
+// Exact for normal numbers; 0 (a padding cell's tau) becomes 1.2e-38, which the products that follow flush to nothing.
+// |v| < 1 here (tau = s d / r^2), so the exponent cannot overflow.
+__device__ __forceinline__ float2 twice2(float2 v) {
+    return make_float2(__int_as_float(__float_as_int(v.x) + 0x00800000), __int_as_float(__float_as_int(v.y) + 0x00800000));
+}
+
 struct PcPre2 { float2 dx, dy, dz, ri; };
 
 __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, const CellRegs& c, float& minr2) {
@@ -501,8 +508,8 @@ __device__ __forceinline__ PcPre2 pc_pre2(const float4 txy, const float4 tz, con
 //   V3_i = q_ixx A + q_iyy B + q_ixy 2xy + q_ixz 2xz + q_iyz 2yz
 //   V4_i = q_ixxx x(xx - 3zz) + q_ixxy 3yA + q_ixxz z(3xx - zz) + q_ixyy 3xB + q_ixyz 6xyz
 //        + q_iyyy y(yy - 3zz) + q_iyyz z(3yy - zz)
-// Per interaction: 7 FADD, 31 FMUL, 65 FFMA, 1 MUFU = 169 flops in 103 packed instructions per pair
-// (the textbook form with all 6 + 10 monomials: 187 flops in 113).
+// Per interaction: 5 FADD, 31 FMUL, 65 FFMA, 1 MUFU = 167 flops in 101 packed instructions per pair, plus two
+// doublings done as integer adds on the ALU pipe (the textbook form with all 6 + 10 monomials: 187 flops in 113).
 #define PKDG_T0(CX, CY, CZ, M) vx = f2mul(sp(CX), M); vy = f2mul(sp(CY), M); vz = f2mul(sp(CZ), M);
 #define PKDG_T1(CX, CY, CZ, M) vx = f2fma(sp(CX), M, vx); vy = f2fma(sp(CY), M, vy); vz = f2fma(sp(CZ), M, vz);
 __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, float4& a0, float4& a1) {
@@ -514,7 +521,7 @@ __device__ __forceinline__ void pc_body2(const PcPre2 q, const CellRegs& c, floa
     float2 E2 = f2mul(vx, x); E2 = f2fma(vy, y, E2); E2 = f2fma(vz, z, E2);
     const float2 xx = f2mul(x, x), yy = f2mul(y, y), zz = f2mul(z, z);
     const float2 A = f2add(xx, neg2(zz)), B = f2add(yy, neg2(zz));
-    const float2 x2 = f2add(x, x), y2 = f2add(y, y);
+    const float2 x2 = twice2(x), y2 = twice2(y);
     const float2 C = f2mul(x2, y), D = f2mul(x2, z), E = f2mul(y2, z);
     PKDG_T1(c.xxx, c.xxy, c.xxz, A) PKDG_T1(c.xyy, c.yyy, c.yyz, B) PKDG_T1(c.xxy, c.xyy, c.xyz, C)
     PKDG_T1(c.xxz, c.xyz, c.xzz, D) PKDG_T1(c.xyz, c.yyz, c.yzz, E)

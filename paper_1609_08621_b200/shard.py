@@ -16,7 +16,7 @@ import numpy as np
 
 # cost model: flops per (sink, list entry) as executed by the default kernel
 W_PP = 19
-W_PC = 169
+W_PC = 167
 
 
 def bucket_cost(count, pp_off, pc_off, pp_weights=None):
