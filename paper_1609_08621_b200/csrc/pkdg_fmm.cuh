@@ -66,28 +66,104 @@ __device__ __forceinline__ void fmm_source_derivs(const float Rx, const float Ry
     fmm_derivs(p, g, d);
 }
 
+// Per-warp shared memory: while the source lists are walked it holds the lane's NEXT cell record (cp.async, two
+// buffers of 9 x 16 bytes per lane, [buffer][part][lane]: conflict-free) -- a lane needs ~800 clocks for one C-C
+// entry and two warps per scheduler cannot hide a global load behind that; afterwards the same bytes hold the
+// 32 lane partials of the 56 coefficients for the reduction.
+constexpr int kFmmStageF4 = 2 * 9 * 32;                                        // float4 per warp
+constexpr int kFmmWarpFloats = kFmmStageF4 * 4 > kNLoc * kFmmRow ? kFmmStageF4 * 4 : kNLoc * kFmmRow;
+
+// What is fetched ahead for a bucket, in three dependent steps (A: its ranges, B: the first list entries and the
+// lane's sink, C: the first sources), each issued one phase of arithmetic before the next needs it: a bucket has only
+// ~3 + 2 trips over its lists, so without this seven dependent global loads would sit in front of ~4000 clocks of
+// arithmetic and two warps per scheduler cannot hide them.
+struct FmmAhead {
+    unsigned bu;
+    int first, count;
+    float zx, zy, zz;
+    int64_t cc0, cc1, cp0, cp1;
+    int32_t icc0, icc1, jcp0, jcp1;   // first list entries of the lane, as loaded (validated when they are used)
+    float4 sink, pcp0;
+};
+
 __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmParams p) {
-    __shared__ float s_part[kFmmWarps][kNLoc * kFmmRow];
+    __shared__ __align__(16) float s_part[kFmmWarps][kFmmWarpFloats];
     __shared__ float s_lam[kFmmWarps][64];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* part = s_part[warp];
+    float4* stage = reinterpret_cast<float4*>(s_part[warp]);
     float* Lam = s_lam[warp];
     const bool accumulate = (p.flags & 0x1u) != 0;
     unsigned long long n_cc = 0, n_cp = 0, bad = 0;   // lane 0 counts list lengths, every lane its bad entries
 
+    // Entry e of a list as it is stored (-1 beyond the end).  Nothing looks at the value here: a load whose result is
+    // tested at once stalls the warp for the whole memory latency; cc_valid / cp_valid test it one trip later.
+    auto cc_entry = [&](const FmmAhead& m, int64_t e) -> int32_t { return e < m.cc1 ? __ldg(p.cc_idx + e) : -1; };
+    auto cp_entry = [&](const FmmAhead& m, int64_t e) -> int32_t { return e < m.cp1 ? __ldg(p.cp_idx + e) : -1; };
+    auto cc_valid = [&](int32_t c) -> int32_t {
+        if (c >= 0 && (int64_t)c >= p.n_cells) { ++bad; return -1; }
+        return c;
+    };
+    auto cp_valid = [&](int32_t j) -> int32_t {
+        if (j >= 0 && (int64_t)j >= p.n_particles) { ++bad; return -1; }
+        return j;
+    };
+    auto issue_rec = [&](int32_t c, int buf) {   // rec_vec4: records are 16-byte aligned with a stride that keeps them so
+        if (c >= 0 && p.rec_vec4) {
+            const float4* r4 = reinterpret_cast<const float4*>(p.rec + (int64_t)c * p.stride);
+#pragma unroll
+            for (int i = 0; i < 9; ++i) cp_async16(stage + (buf * 9 + i) * 32 + lane, r4 + i);
+        }
+        cp_async_commit();
+    };
+    auto step_a = [&](FmmAhead& m) {   // needs m.bu
+        const int64_t b = m.bu;
+        m.first = __ldg(p.first + b); m.count = __ldg(p.count + b);
+        m.zx = __ldg(p.centre + 3 * b); m.zy = __ldg(p.centre + 3 * b + 1); m.zz = __ldg(p.centre + 3 * b + 2);
+        m.cc0 = m.cc1 = m.cp0 = m.cp1 = 0;
+        if (p.cc_off) { m.cc0 = __ldg(p.cc_off + b); m.cc1 = __ldg(p.cc_off + b + 1); }
+        if (p.cp_off) { m.cp0 = __ldg(p.cp_off + b); m.cp1 = __ldg(p.cp_off + b + 1); }
+    };
+    auto step_b = [&](FmmAhead& m) {   // needs step A
+        if (m.count < 0 || m.first < 0 || (int64_t)m.first + m.count > p.n_particles) { bad += (lane == 0); m.count = 0; }
+        if (m.cc1 < m.cc0) { bad += (lane == 0); m.cc1 = m.cc0; }
+        if (m.cp1 < m.cp0) { bad += (lane == 0); m.cp1 = m.cp0; }
+        m.icc0 = cc_entry(m, m.cc0 + lane); m.icc1 = cc_entry(m, m.cc0 + lane + 32);
+        m.jcp0 = cp_entry(m, m.cp0 + lane); m.jcp1 = cp_entry(m, m.cp0 + lane + 32);
+        m.sink = lane < m.count ? __ldg(p.xyzm + m.first + lane) : make_float4(m.zx, m.zy, m.zz, 0.0f);
+    };
+    auto step_c = [&](FmmAhead& m) {   // needs step B; the staging memory must be free
+        m.icc0 = cc_valid(m.icc0);
+        issue_rec(m.icc0, 0);
+        m.jcp0 = cp_valid(m.jcp0);
+        m.pcp0 = m.jcp0 >= 0 ? __ldg(p.xyzm + m.jcp0) : make_float4(0.f, 0.f, 0.f, 0.f);
+    };
+    auto claim = [&]() -> unsigned {
+        unsigned v = 0;
+        if (lane == 0) v = atomicAdd(p.work_counter, 1u);
+        return v;
+    };
+
+    FmmAhead cur;
+    cur.bu = __shfl_sync(0xffffffffu, claim(), 0);
+    if ((int64_t)cur.bu >= p.n_buckets) return;
+    step_a(cur); step_b(cur); step_c(cur);
+    unsigned claimed = claim();   // buckets are claimed one iteration before they are looked at
+
     for (;;) {
-        unsigned bu = 0;
-        if (lane == 0) bu = atomicAdd(p.work_counter, 1u);
-        bu = __shfl_sync(0xffffffffu, bu, 0);
-        if ((int64_t)bu >= p.n_buckets) break;
-        const int64_t b = bu;
-        int first = __ldg(p.first + b), count = __ldg(p.count + b);
-        if (count < 0 || first < 0 || (int64_t)first + count > p.n_particles) { bad += (lane == 0); count = 0; }
-        const float zx = __ldg(p.centre + 3 * b), zy = __ldg(p.centre + 3 * b + 1), zz = __ldg(p.centre + 3 * b + 2);
+        FmmAhead nxt;
+        nxt.bu = __shfl_sync(0xffffffffu, claimed, 0);
+        claimed = claim();
+        const int first = cur.first, count = cur.count;
+        const float zx = cur.zx, zy = cur.zy, zz = cur.zz;
 
         // lambda = the largest distance of a sink from the centre (1 if the bucket is a point at its centre)
-        float lam2 = 0.0f;
-        for (int t = lane; t < count; t += 32) {
+        float lam2;
+        {
+            const float sx = cur.sink.x - zx, sy = cur.sink.y - zy, sz = cur.sink.z - zz;
+            lam2 = fmaf(sz, sz, fmaf(sy, sy, sx * sx));
+        }
+        for (int t = lane + 32; t < count; t += 32) {
             const float4 x = __ldg(p.xyzm + first + t);
             const float sx = x.x - zx, sy = x.y - zy, sz = x.z - zz;
             lam2 = fmaxf(lam2, fmaf(sz, sz, fmaf(sy, sy, sx * sx)));
@@ -97,33 +173,42 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
         const float lam = lam2 > 0.0f ? sqrtf(lam2) : 1.0f;
         const float il = 1.0f / lam;
 
+        const bool has_next = (int64_t)nxt.bu < p.n_buckets;
+        if (has_next) step_a(nxt);
+
         float L[kNLoc];
 #pragma unroll
         for (int i = 0; i < kNLoc; ++i) L[i] = 0.0f;
 
-        // ---- C-C: one source cell per lane and trip
+        // ---- C-C: one source cell per lane and trip; the record of trip t + 1 and the index of trip t + 2 are in
+        //      flight during trip t (the record of trip 0 since step C)
         if (p.cc_off) {
-            int64_t e0 = __ldg(p.cc_off + b), e1 = __ldg(p.cc_off + b + 1);
-            if (e1 < e0) { bad += (lane == 0); e1 = e0; }
+            const int64_t e0 = cur.cc0, e1 = cur.cc1;
             if (lane == 0) n_cc += (unsigned long long)(e1 - e0);
             // -(-1)^|m| / lambda^|m| for |m| = 0, 2, 3, 4
             const float il2 = il * il;
             const float sc0 = -1.0f, sc2 = -il2, sc3 = il2 * il, sc4 = -il2 * il2;
+            int32_t c_cur = cur.icc0, c_nxt = cur.icc1;
+            int buf = 0;
 #pragma unroll 1
-            for (int64_t e = e0 + lane; e < e1; e += 32) {
-                const int32_t c = __ldg(p.cc_idx + e);
-                if (c < 0) continue;                                   // padding
-                if ((int64_t)c >= p.n_cells) { ++bad; continue; }
-                const float* r = p.rec + (int64_t)c * p.stride;
+            for (int64_t e = e0; e < e1; e += 32) {   // warp-uniform trips
+                const int32_t c = c_cur;
+                c_cur = cc_valid(c_nxt);
+                issue_rec(c_cur, buf ^ 1);
+                c_nxt = cc_entry(cur, e + lane + 64);
+                cp_async_wait_pending<1>();            // this trip's record has landed (only the lane itself reads it)
+                const int bsel = buf;
+                buf ^= 1;
+                if (c < 0) continue;                   // padding, bad entry, or past the end of the list
                 float q[36];
                 if (p.rec_vec4) {
-                    const float4* r4 = reinterpret_cast<const float4*>(r);
 #pragma unroll
                     for (int i = 0; i < 9; ++i) {
-                        const float4 v = __ldg(r4 + i);
+                        const float4 v = stage[(bsel * 9 + i) * 32 + lane];
                         q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
                     }
                 } else {
+                    const float* r = p.rec + (int64_t)c * p.stride;
 #pragma unroll
                     for (int i = 0; i < 35; ++i) q[i] = __ldg(r + i);
                 }
@@ -138,20 +223,28 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
                 fmm_m2l_cell(d, mu, L);
             }
         }
-        // ---- C-P: one source particle per lane and trip
+        cp_async_wait_all();
+        if (has_next) step_b(nxt);
+
+        // ---- C-P: one source particle per lane and trip; the particle of the next trip is loaded before this trip's
+        //      arithmetic (the one of trip 0 since step C)
         if (p.cp_off) {
-            int64_t e0 = __ldg(p.cp_off + b), e1 = __ldg(p.cp_off + b + 1);
-            if (e1 < e0) { bad += (lane == 0); e1 = e0; }
+            const int64_t e0 = cur.cp0, e1 = cur.cp1;
             if (lane == 0) n_cp += (unsigned long long)(e1 - e0);
+            float4 s_cur = cur.pcp0;
+            bool ok_cur = cur.jcp0 >= 0;
+            int32_t j_nxt = cur.jcp1;   // index of trip t + 1 (loaded a trip ago), particle of trip t + 1 loaded now
 #pragma unroll 1
-            for (int64_t e = e0 + lane; e < e1; e += 32) {
-                const int32_t j = __ldg(p.cp_idx + e);
-                if (j < 0) continue;
-                if ((int64_t)j >= p.n_particles) { ++bad; continue; }
-                const float4 s = __ldg(p.xyzm + j);
-                float d[kNLoc];
-                fmm_source_derivs(zx - s.x, zy - s.y, zz - s.z, lam, d);
-                fmm_m2l_particle(d, -s.w, L);
+            for (int64_t e = e0; e < e1; e += 32) {
+                const int32_t jn = cp_valid(j_nxt);
+                const float4 s_nxt = jn >= 0 ? __ldg(p.xyzm + jn) : make_float4(0.f, 0.f, 0.f, 0.f);
+                j_nxt = cp_entry(cur, e + lane + 64);
+                if (ok_cur) {
+                    float d[kNLoc];
+                    fmm_source_derivs(zx - s_cur.x, zy - s_cur.y, zz - s_cur.z, lam, d);
+                    fmm_m2l_particle(d, -s_cur.w, L);
+                }
+                s_cur = s_nxt; ok_cur = jn >= 0;
             }
         }
 
@@ -170,11 +263,12 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
                 Lam[i] = sum * kLocInvFact[i];
             }
         }
-        __syncwarp();
+        __syncwarp();   // the staging memory is free again, Lam is visible
+        if (has_next) step_c(nxt);
 
         // ---- lanes = sinks: the polynomial in sigma = s / lambda and its gradient
         for (int t = lane; t < count; t += 32) {
-            const float4 x = __ldg(p.xyzm + first + t);
+            const float4 x = t == lane ? cur.sink : __ldg(p.xyzm + first + t);
             float m[kNLoc];
             fmm_monomials((x.x - zx) * il, (x.y - zy) * il, (x.z - zz) * il, m);
             float phi, gx, gy, gz;
@@ -183,7 +277,11 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
             if (accumulate) { const float4 o = p.out[first + t]; r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w; }
             p.out[first + t] = r;
         }
+        if (!has_next) break;
+        __syncwarp();   // Lam is rewritten by the next bucket only after every lane has evaluated its sinks
+        cur = nxt;
     }
+    cp_async_wait_all();
     n_cc = warp_sum_u64(n_cc); n_cp = warp_sum_u64(n_cp); bad = warp_sum_u64(bad);
     if (lane == 0) {
         if (n_cc) atomicAdd(&p.stats->interactions_cc, n_cc);
