@@ -5,11 +5,13 @@
 //   pkdg_prep_cells_kernel   canonical raw-moment records -> normalised trace-free records (128 B)
 //   pkdg_pack_kernel         a1: bucket work descriptors, tile counts, validation, I_pp / I_pc
 //   pkdg_tiles_kernel        a1: materialised 32-entry tiles (pkdg_pack_export)
-//   pkdg_eval3_kernel        a2-a5, library default: one warp per bucket, lanes stride the source
-//                            lists, packed FP32x2 arithmetic over sink pairs, cp.async staging of
-//                            cell records and of the next bucket, butterfly transpose-reduction
-//                            + per-sink conditioning estimate; ill-conditioned sinks are queued
+//   pkdg_evalb_kernel        a2-a5 for per-bucket lists (the headline kernel): one warp per bucket, a lane owns a
+//                            sink pair (packed FP32x2 arithmetic), sources stream through shared memory (cp.async);
+//                            per-sink conditioning estimate, ill-conditioned sinks are queued
+//   pkdg_evalg_kernel        the same for lists shared by a group of <= 64 sinks: one warp per group
 //   pkdg_fixup_kernel        queued sinks re-evaluated with fp64 terms and fp64 accumulators
+//   pkdg_walk_kernel         list construction: the tree walk with the opening criterion, bit-identical to the host's
+//   pkdg_validate_*_kernel   PKDG_VALIDATE
 //   pkdg_fma_probe_kernel    FFMA-only probe (roofline denominator check)
 #pragma once
 #include <cuda_runtime.h>
@@ -329,18 +331,9 @@ __global__ void pkdg_tiles_kernel(const int64_t* __restrict__ off, const int32_t
 }
 
 // ------------------------------------------------------------------------------------------------
-// Evaluation kernel (a2-a5).  One warp per bucket, buckets handed out in tree order through an
-// atomic counter.  Lanes stride the SOURCE lists (lists are cut at warp multiples;
-// here the remainder is masked instead of being shunted to the CPU).  Sinks are processed in
-// passes of up to 16:
-//   a2  the pass's sinks are staged in shared memory (broadcast reads);
-//   a3  P-P: each lane keeps ONE source in registers and visits all sinks of the pass, unrolled,
-//       with per-lane register accumulators (8 or 16 sink slots);
-//   a4  P-C: each lane keeps ONE cell (35 registers) and visits the sinks in a run-time loop (one or
-//       two per iteration, software-pipelined); per-lane partial sums live in shared memory (s_acc[sink][lane], float4), so
-//       the body is not unrolled 16 times (instruction cache) and any sink count works;
-//   a5  the 32 per-lane partials of every (sink, component) are reduced with a butterfly
-//       transpose-reduction and written as float4 {ax, ay, az, phi}.
+// Evaluation kernels (a2-a5): shared parameters and pieces.  Sinks are processed in passes of up to 16 per bucket
+// (pkdg_evalb_kernel) or 64 per group (pkdg_evalg_kernel); PAPER.md:L188 cuts lists at warp multiples and sends the
+// remainder to the CPU -- here remainders are masked in place.
 // ------------------------------------------------------------------------------------------------
 constexpr int kTMax = 16;  // sinks per pass
 
@@ -460,17 +453,15 @@ __device__ __forceinline__ ListLens eff_lens(const BucketDesc& d, bool do_pp, bo
 }
 
 // ------------------------------------------------------------------------------------------------
-// Generation 3: packed FP32x2 arithmetic (sm_100 FFMA2 / FMUL2 / FADD2).
+// Packed FP32x2 arithmetic (sm_100 FFMA2 / FMUL2 / FADD2).
 //
-// Measured on B200 (pkdg_fma_probe, profiles/r01_bench_ng256.md): the register file delivers one 32-bit operand
-// per bank (even / odd register) per clock, so a scalar FFMA with three distinct register operands
-// issues every 1.5 clocks (0.66 of the FMA peak) and the scalar P-C body tops out at 0.76.  A packed
-// FFMA2 computes two FMAs in two clocks from 64-bit register pairs (one read of each bank per
-// operand) and accepts a scalar register broadcast to both halves: coefficient (scalar) x monomial
-// (pair) + accumulator (pair) needs <= 2 reads per bank whenever one operand is reused from the
-// previous instruction -- full FMA rate with half the issue slots, independent of register allocation.
-// So one lane still holds ONE source (particle or cell) in scalar registers, and the two halves of
-// every packed value are two SINKS of the bucket (sink pair p = sinks 2p, 2p+1).
+// Measured on B200 (round 1, profiles/r01_bench_ng256.md): the register file delivers one 32-bit operand per bank
+// (even / odd register) per clock, so a scalar FFMA with three distinct register operands issues every 1.5 clocks
+// (0.66 of the FMA peak).  A packed FFMA2 computes two FMAs in two clocks from 64-bit register pairs (one read of
+// each bank per operand) and accepts a scalar register broadcast to both halves: coefficient (scalar) x monomial
+// (pair) + accumulator (pair) needs <= 2 reads per bank whenever one operand is reused from the previous
+// instruction -- full FMA rate with half the issue slots -- and three clocks otherwise.  So the two halves of every
+// packed value are two SINKS (a sink pair) and everything that belongs to a source is a scalar.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float2 sp(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
