@@ -163,14 +163,18 @@ def run_reference(args, rank, world):
 
 
 def kernel_source_hash():
-    """sha256 (first 16 hex digits) of the CUDA sources the evaluation kernel is built from: the key
-    profiles/traffic.json is stamped with, so that a measured DRAM-traffic figure is dropped (null) as soon as
-    the kernel it was measured on has changed."""
+    """sha256 (first 16 hex digits) of the CUDA sources the evaluation kernel is built from, comments and white space
+    removed: the key profiles/traffic.json is stamped with, so that a measured DRAM-traffic figure is dropped (null)
+    as soon as the code it was measured on has changed."""
     import hashlib
+    import re
     h = hashlib.sha256()
     for rel in ("paper_1609_08621_b200/csrc/pkdg_kernels.cuh", "paper_1609_08621_b200/csrc/pkdg.cu", "include/pkdg.h"):
-        with open(os.path.join(ROOT, rel), "rb") as f:
-            h.update(f.read())
+        with open(os.path.join(ROOT, rel), "r") as f:
+            text = f.read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        text = re.sub(r"//[^\n]*", "", text)
+        h.update(re.sub(r"\s+", "", text).encode())
     return h.hexdigest()[:16]
 
 
