@@ -154,7 +154,7 @@ def run_reference(args, rank, world):
     sample = f"{nb_s} of {p.n_buckets} buckets (evenly spread in tree order) per step, ~{per_step:.1f} s of CPU work each"
     line = {"impl": "reference", "metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(p, args.ng),
             "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
