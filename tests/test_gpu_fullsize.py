@@ -281,3 +281,87 @@ def test_config5_streamed_range(ctx, torch):
     lo, hi = int(first[0]), int(first[-1] + count[-1])
     o = out.cpu().numpy()
     assert np.isfinite(o[lo:hi]).all() and np.isnan(o[:lo]).all() and np.isnan(o[hi:]).all()
+
+
+def _sub_csr(off, idx, sel):
+    """The CSR list restricted to buckets sel (pure indexing)."""
+    lens = np.diff(off)[sel]
+    o = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    start = np.repeat(off[:-1][sel] - o[:-1], lens)
+    return o, np.ascontiguousarray(idx[start + np.arange(int(lens.sum()), dtype=np.int64)], np.int32)
+
+
+def test_config3_group_lists_sampled(ctx, torch, cfg3):
+    """The headline configuration with lists shared by groups of <= 64 particles and P-P entries as bucket references
+    (the launch configuration of bench.py's group_lists key): counters bit-exact, 8192 evenly spread
+    buckets + the 64 longest group lists against the oracle on the per-bucket lists the group lists stand for."""
+    import oracle
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors
+    p = cfg3
+    gc, gf, gn = inputs.build_groups(p, 64)
+    ppo, ppi, pco, pci = inputs.build_group_lists(p, gc, p.theta, p.eps)
+    lo, li = inputs.pp_leaves(p.n, p.first, p.count, ppo, ppi)
+    gcount = np.add.reduceat(p.count.astype(np.int64), gf)
+    I_pp, I_pc = int(np.dot(gcount, np.diff(ppo))), int(np.dot(gcount, np.diff(pco)))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+    out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda:0")
+    ctx.gravity_eval_groups(t(p.xyzm), t(p.cells), t(p.first), t(p.count), t(gf), t(gn), t(lo), t(li), t(pco), t(pci), p.eps,
+                            out, flags=binding.PP_LEAVES)
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    assert st["interactions_pp"] == I_pp and st["interactions_pc"] == I_pc and st["bad_entries"] == 0
+    group_of = np.repeat(np.arange(gf.shape[0]), gn)
+    longest = np.argsort(np.diff(ppo) + np.diff(pco))[-64:]
+    sel = np.unique(np.concatenate([np.linspace(0, p.n_buckets - 1, 8192).astype(np.int64),
+                                    np.flatnonzero(np.isin(group_of, longest))]))
+    s_ppo, s_ppi = inputs.expand_groups(gf, gn, ppo, ppi, sel=sel)
+    s_pco, s_pci = inputs.expand_groups(gf, gn, pco, pci, sel=sel)
+    first = np.ascontiguousarray(p.first[sel]); count = np.ascontiguousarray(p.count[sel])
+    ref = oracle.gravity_eval(p.xyzm, p.cells, first, count, s_ppo, s_ppi, s_pco, s_pci, p.eps)
+    rows = _rows_of(first, count, np.arange(len(sel)))
+    got = out[torch.from_numpy(rows).to("cuda:0")].cpu().numpy()
+    ea, ep = rel_errors(got, ref[rows])
+    print(f"\n[cfg3 group lists] compared {len(rows)} particles in {len(sel)} buckets: acc max {ea.max():.2e} rms "
+          f"{np.sqrt(np.mean(ea ** 2)):.2e} | pot max {ep.max():.2e} | fp64 fix-up: {st['fixup_sinks']} sinks")
+    assert ea.max() <= TOL and ep.max() <= TOL, (float(ea.max()), float(ep.max()))
+    o = out.cpu().numpy()
+    assert np.isfinite(o).all() and (o[:, 3] < 0).all()
+
+
+def test_config3_four_lists_sampled(ctx, torch, cfg3):
+    """The headline configuration through pkdg_gravity_eval_fmm (C-C / C-P lists into the 5th-order local expansion of
+    every bucket + the remaining P-P / P-C lists; the launch configuration of bench.py's fmm key): list counters
+    bit-exact, 8192 evenly spread buckets + the 64 with the longest C-C lists against the oracle, errors relative to
+    the TOTAL of the four lists."""
+    import oracle
+    from paper_1609_08621_b200 import inputs
+    p = cfg3
+    F = inputs.build_fmm_lists(p, p.theta, p.eps)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+    out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device="cuda:0")
+    ctx.gravity_eval_fmm(t(p.xyzm), t(p.cells), t(p.first), t(p.count), t(F["centre"]), t(F["pp"][0]), t(F["pp"][1]),
+                         t(F["pc"][0]), t(F["pc"][1]), t(F["cp"][0]), t(F["cp"][1]), t(F["cc"][0]), t(F["cc"][1]), F["eps"], out)
+    torch.cuda.synchronize()
+    st = ctx.get_stats()
+    cnt = p.count.astype(np.int64)
+    assert st["interactions_cc"] == len(F["cc"][1]) and st["interactions_cp"] == len(F["cp"][1])
+    assert st["interactions_pp"] == int(np.dot(cnt, np.diff(F["pp"][0]))) and st["interactions_pc"] == int(np.dot(cnt, np.diff(F["pc"][0])))
+    assert st["bad_entries"] == 0
+    sel = np.unique(np.concatenate([np.linspace(0, p.n_buckets - 1, 8192).astype(np.int64),
+                                    np.argsort(np.diff(F["cc"][0]))[-64:]]))
+    sub = {k: _sub_csr(F[k][0], F[k][1], sel) for k in ("pp", "pc", "cp", "cc")}
+    first = np.ascontiguousarray(p.first[sel]); count = np.ascontiguousarray(p.count[sel])
+    ref = oracle.gravity_eval(p.xyzm, p.cells, first, count, sub["pp"][0], sub["pp"][1], sub["pc"][0], sub["pc"][1], F["eps"])
+    ref = oracle.fmm_eval(p.xyzm, p.cells, first, count, np.ascontiguousarray(F["centre"][sel]), sub["cc"][0], sub["cc"][1],
+                          sub["cp"][0], sub["cp"][1], out=ref)
+    rows = _rows_of(first, count, np.arange(len(sel)))
+    got = out[torch.from_numpy(rows).to("cuda:0")].cpu().numpy().astype(np.float64)
+    r = ref[rows]
+    ea = np.linalg.norm(got[:, :3] - r[:, :3], axis=1) / np.linalg.norm(r[:, :3], axis=1)
+    ep = np.abs(got[:, 3] - r[:, 3]) / np.abs(r[:, 3])
+    print(f"\n[cfg3 four lists] compared {len(rows)} particles in {len(sel)} buckets: acc max {ea.max():.2e} rms "
+          f"{np.sqrt(np.mean(ea ** 2)):.2e} | pot max {ep.max():.2e} | fp64 fix-up: {st['fixup_sinks']} sinks")
+    assert ea.max() <= TOL and ep.max() <= TOL, (float(ea.max()), float(ep.max()))
+    o = out.cpu().numpy()
+    assert np.isfinite(o).all() and (o[:, 3] < 0).all()
