@@ -61,6 +61,8 @@ struct pkdg_ctx {
     int64_t e2e_np = 0, e2e_nc = 0, e2e_no = 0;
     int64_t* scan_tmp = nullptr;
     int64_t scan_cap = 0;
+    WalkNode* wnodes = nullptr;        // pkdg_build_lists_*: one 64-byte record per tree cell
+    int64_t wnodes_cap = 0;
     int2* gfc = nullptr;               // PKDG_PP_LEAVES: (first, count) of every bucket
     int64_t gfc_cap = 0;
     int32_t *g_first = nullptr, *g_count = nullptr;  // streamed variants: device copy of the bucket arrays
@@ -322,7 +324,7 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
     cudaDeviceSynchronize();
     cudaFree(ctx->cellq); cudaFree(ctx->desc); cudaFree(ctx->stats); cudaFree(ctx->counters);
     cudaFree(ctx->e2e_xyzm); cudaFree(ctx->e2e_cells); cudaFree(ctx->e2e_out); cudaFree(ctx->scan_tmp);
-    cudaFree(ctx->gfc); cudaFree(ctx->g_first); cudaFree(ctx->g_count); cudaFree(ctx->fixq);
+    cudaFree(ctx->gfc); cudaFree(ctx->wnodes); cudaFree(ctx->g_first); cudaFree(ctx->g_count); cudaFree(ctx->fixq);
     for (int i = 0; i < ctx->n_slots_live; ++i) {
         Slot& s = ctx->slots[i];
         cudaFree(s.pp_idx); cudaFree(s.pc_idx); cudaFree(s.first); cudaFree(s.count);
@@ -799,6 +801,16 @@ static TreeView tree_view(const pkdg_tree* T, const pkdg_cells* C, bool leaves) 
     return v;
 }
 
+// the walk's 64-byte cell records (workspace of the context)
+static pkdg_status walk_nodes(pkdg_ctx* ctx, const TreeView& v, cudaStream_t st) {
+    pkdg_status s = ensure(ctx, &ctx->wnodes, &ctx->wnodes_cap, v.n_cells);
+    if (s != PKDG_OK || v.n_cells == 0) return s;
+    pkdg_walk_nodes_kernel<<<(unsigned)((v.n_cells + 255) / 256), 256, 0, st>>>(v, ctx->wnodes);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return PKDG_OK;
+}
+
 pkdg_status pkdg_build_lists_count(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_cells* C, const int32_t* sink_cell,
                                    int64_t n_sinks, double theta, double eps, uint32_t flags, int64_t* pp_off,
                                    int64_t* pc_off, int64_t* totals_host, void* stream) {
@@ -809,9 +821,11 @@ pkdg_status pkdg_build_lists_count(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
+    if ((s = walk_nodes(ctx, v, st)) != PKDG_OK) return s;
     if (n_sinks > 0) {
-        pkdg_walk_kernel<false><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(v, sink_cell, n_sinks, theta, eps, pp_off,
-                                                                                   pc_off, nullptr, nullptr, nullptr, nullptr);
+        pkdg_walk_kernel<false><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
+            ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, pp_off, pc_off, nullptr,
+            nullptr, nullptr, nullptr);
         ctx->launches++;
         CK(cudaGetLastError());
     }
@@ -836,8 +850,10 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
-    pkdg_walk_kernel<true><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(v, sink_cell, n_sinks, theta, eps, nullptr,
-                                                                              nullptr, pp_off, pc_off, pp_idx, pc_idx);
+    if ((s = walk_nodes(ctx, v, st)) != PKDG_OK) return s;   // rebuilt here: the caller may have changed the tree since _count
+    pkdg_walk_kernel<true><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
+        ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, nullptr, nullptr, pp_off,
+        pc_off, pp_idx, pc_idx);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;

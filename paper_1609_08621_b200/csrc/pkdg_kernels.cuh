@@ -1288,33 +1288,61 @@ struct TreeView {
     const int32_t* leaf_rank;               // NULL, or [n_cells]: bucket index of a leaf cell (PKDG_PP_LEAVES output)
 };
 
+// What the walk needs of a cell, gathered once per call into one 64-byte record (one cache line per visited cell
+// instead of six: the canonical record's COM and b_max sit in two different lines, the boxes in two arrays, count /
+// end / isleaf / first in four more).  The values are copies, so every decision stays bit-identical.
+struct __align__(16) WalkNode {
+    float cx, cy, cz, bmax;        // centre of mass, b_max
+    float lox, loy, loz, hix;      // bounding box
+    float hiy, hiz; int32_t count, end;
+    int32_t first, leaf;           // leaf: -1 = internal cell, else what a P-P entry for this leaf is (its rank, or 0)
+    int32_t pad0, pad1;
+};
+
+__global__ void pkdg_walk_nodes_kernel(const TreeView T, WalkNode* __restrict__ nodes) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= T.n_cells) return;
+    const float* r = T.rec + k * (int64_t)T.stride;
+    WalkNode w;
+    w.cx = r[0]; w.cy = r[1]; w.cz = r[2]; w.bmax = r[35];
+    w.lox = T.bblo[3 * k]; w.loy = T.bblo[3 * k + 1]; w.loz = T.bblo[3 * k + 2];
+    w.hix = T.bbhi[3 * k]; w.hiy = T.bbhi[3 * k + 1]; w.hiz = T.bbhi[3 * k + 2];
+    w.count = T.count[k]; w.end = T.end[k]; w.first = T.first[k];
+    w.leaf = T.isleaf[k] ? (T.leaf_rank ? T.leaf_rank[k] : 0) : -1;
+    w.pad0 = w.pad1 = 0;
+    nodes[k] = w;
+}
+
 template <bool FILL>
-__global__ void pkdg_walk_kernel(const TreeView T, const int32_t* __restrict__ sink_cell, int64_t n_sinks, double theta,
+__global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_cells, bool leaf_refs,
+                                 const int32_t* __restrict__ sink_cell, int64_t n_sinks, double theta,
                                  double eps, int64_t* __restrict__ pp_len, int64_t* __restrict__ pc_len,
                                  const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
                                  int32_t* __restrict__ pp_idx, int32_t* __restrict__ pc_idx) {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_sinks) return;
     const int64_t cb = sink_cell[s];
-    const float* rb = T.rec + cb * (int64_t)T.stride;
-    const double bx = rb[0], by = rb[1], bz = rb[2], bmaxB = rb[35];
-    const double lob0 = T.bblo[3 * cb], lob1 = T.bblo[3 * cb + 1], lob2 = T.bblo[3 * cb + 2];
-    const double hib0 = T.bbhi[3 * cb], hib1 = T.bbhi[3 * cb + 1], hib2 = T.bbhi[3 * cb + 2];
+    const float4* nq = reinterpret_cast<const float4*>(nodes);
+    const float4 b0 = __ldg(nq + 4 * cb), b1 = __ldg(nq + 4 * cb + 1), b2 = __ldg(nq + 4 * cb + 2);
+    const double bx = b0.x, by = b0.y, bz = b0.z, bmaxB = b0.w;
+    const double lob0 = b1.x, lob1 = b1.y, lob2 = b1.z;
+    const double hib0 = b1.w, hib1 = b2.x, hib2 = b2.y;
     const double gap_min2 = __dmul_rn(__dmul_rn(4.0, eps), eps);
     int64_t npp = 0, npc = 0;
     int64_t wpp = FILL ? pp_off[s] : 0, wpc = FILL ? pc_off[s] : 0;
     int64_t k = 0;
-    while (k < T.n_cells) {
+    while (k < n_cells) {
+        const float4 q0 = __ldg(nq + 4 * k), q2 = __ldg(nq + 4 * k + 2);
+        const int4 q3 = __ldg(reinterpret_cast<const int4*>(nq + 4 * k + 3));
+        const int32_t cnt = __float_as_int(q2.z), end = __float_as_int(q2.w);
         bool accept = false;
-        const int32_t cnt = __ldg(T.count + k);
         if (k != cb && cnt >= 2) {
-            const float* rk = T.rec + k * (int64_t)T.stride;
-            const double dx = __dsub_rn(bx, (double)__ldg(rk)), dy = __dsub_rn(by, (double)__ldg(rk + 1)),
-                         dz = __dsub_rn(bz, (double)__ldg(rk + 2));
+            const double dx = __dsub_rn(bx, (double)q0.x), dy = __dsub_rn(by, (double)q0.y), dz = __dsub_rn(bz, (double)q0.z);
             const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
-            if (d > __dadd_rn(bmaxB, __ddiv_rn((double)__ldg(rk + 35), theta))) {
-                const double lok0 = __ldg(T.bblo + 3 * k), lok1 = __ldg(T.bblo + 3 * k + 1), lok2 = __ldg(T.bblo + 3 * k + 2);
-                const double hik0 = __ldg(T.bbhi + 3 * k), hik1 = __ldg(T.bbhi + 3 * k + 1), hik2 = __ldg(T.bbhi + 3 * k + 2);
+            if (d > __dadd_rn(bmaxB, __ddiv_rn((double)q0.w, theta))) {
+                const float4 q1 = __ldg(nq + 4 * k + 1);
+                const double lok0 = q1.x, lok1 = q1.y, lok2 = q1.z;
+                const double hik0 = q1.w, hik1 = q2.x, hik2 = q2.y;
                 double g0 = 0.0, g1 = 0.0, g2 = 0.0, t;
                 t = __dsub_rn(lok0, hib0); if (t > g0) g0 = t;
                 t = __dsub_rn(lob0, hik0); if (t > g0) g0 = t;
@@ -1329,19 +1357,19 @@ __global__ void pkdg_walk_kernel(const TreeView T, const int32_t* __restrict__ s
         if (accept) {
             if (FILL) pc_idx[wpc++] = (int32_t)k;
             ++npc;
-            k = __ldg(T.end + k);
-        } else if (__ldg(T.isleaf + k)) {
-            if (T.leaf_rank) {
-                if (FILL) pp_idx[wpp++] = __ldg(T.leaf_rank + k);
+            k = end;
+        } else if (q3.y >= 0) {   // a leaf joins the P-P list whole
+            if (leaf_refs) {
+                if (FILL) pp_idx[wpp++] = q3.y;
                 ++npp;
             } else {
                 if (FILL) {
-                    const int32_t f = __ldg(T.first + k);
+                    const int32_t f = q3.x;
                     for (int32_t j = 0; j < cnt; ++j) pp_idx[wpp++] = f + j;
                 }
                 npp += cnt;
             }
-            k = __ldg(T.end + k);
+            k = end;
         } else {
             k = k + 1;
         }
