@@ -1291,12 +1291,11 @@ struct TreeView {
 // What the walk needs of a cell, gathered once per call into one 64-byte record (one cache line per visited cell
 // instead of six: the canonical record's COM and b_max sit in two different lines, the boxes in two arrays, count /
 // end / isleaf / first in four more).  The values are copies, so every decision stays bit-identical.
-struct __align__(16) WalkNode {
-    float cx, cy, cz, bmax;        // centre of mass, b_max
+struct __align__(16) WalkNode {     // first 32-byte sector: what every visit reads; second: the box, read only by
+    float cx, cy, cz, bmax;        // cells that pass the distance test.  Centre of mass, b_max
+    int32_t count, end, first, leaf;   // leaf: -1 = internal cell, else what a P-P entry for this leaf is (its rank, or 0)
     float lox, loy, loz, hix;      // bounding box
-    float hiy, hiz; int32_t count, end;
-    int32_t first, leaf;           // leaf: -1 = internal cell, else what a P-P entry for this leaf is (its rank, or 0)
-    int32_t pad0, pad1;
+    float hiy, hiz, pad0, pad1;
 };
 
 __global__ void pkdg_walk_nodes_kernel(const TreeView T, WalkNode* __restrict__ nodes) {
@@ -1309,7 +1308,7 @@ __global__ void pkdg_walk_nodes_kernel(const TreeView T, WalkNode* __restrict__ 
     w.hix = T.bbhi[3 * k]; w.hiy = T.bbhi[3 * k + 1]; w.hiz = T.bbhi[3 * k + 2];
     w.count = T.count[k]; w.end = T.end[k]; w.first = T.first[k];
     w.leaf = T.isleaf[k] ? (T.leaf_rank ? T.leaf_rank[k] : 0) : -1;
-    w.pad0 = w.pad1 = 0;
+    w.pad0 = w.pad1 = 0.0f;
     nodes[k] = w;
 }
 
@@ -1323,7 +1322,7 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
     if (s >= n_sinks) return;
     const int64_t cb = sink_cell[s];
     const float4* nq = reinterpret_cast<const float4*>(nodes);
-    const float4 b0 = __ldg(nq + 4 * cb), b1 = __ldg(nq + 4 * cb + 1), b2 = __ldg(nq + 4 * cb + 2);
+    const float4 b0 = __ldg(nq + 4 * cb), b1 = __ldg(nq + 4 * cb + 2), b2 = __ldg(nq + 4 * cb + 3);
     const double bx = b0.x, by = b0.y, bz = b0.z, bmaxB = b0.w;
     const double lob0 = b1.x, lob1 = b1.y, lob2 = b1.z;
     const double hib0 = b1.w, hib1 = b2.x, hib2 = b2.y;
@@ -1332,15 +1331,15 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
     int64_t wpp = FILL ? pp_off[s] : 0, wpc = FILL ? pc_off[s] : 0;
     int64_t k = 0;
     while (k < n_cells) {
-        const float4 q0 = __ldg(nq + 4 * k), q2 = __ldg(nq + 4 * k + 2);
-        const int4 q3 = __ldg(reinterpret_cast<const int4*>(nq + 4 * k + 3));
-        const int32_t cnt = __float_as_int(q2.z), end = __float_as_int(q2.w);
+        const float4 q0 = __ldg(nq + 4 * k);
+        const int4 q3 = __ldg(reinterpret_cast<const int4*>(nq + 4 * k + 1));   // count, end, first, leaf
+        const int32_t cnt = q3.x, end = q3.y;
         bool accept = false;
         if (k != cb && cnt >= 2) {
             const double dx = __dsub_rn(bx, (double)q0.x), dy = __dsub_rn(by, (double)q0.y), dz = __dsub_rn(bz, (double)q0.z);
             const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
             if (d > __dadd_rn(bmaxB, __ddiv_rn((double)q0.w, theta))) {
-                const float4 q1 = __ldg(nq + 4 * k + 1);
+                const float4 q1 = __ldg(nq + 4 * k + 2), q2 = __ldg(nq + 4 * k + 3);
                 const double lok0 = q1.x, lok1 = q1.y, lok2 = q1.z;
                 const double hik0 = q1.w, hik1 = q2.x, hik2 = q2.y;
                 double g0 = 0.0, g1 = 0.0, g2 = 0.0, t;
@@ -1358,13 +1357,13 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
             if (FILL) pc_idx[wpc++] = (int32_t)k;
             ++npc;
             k = end;
-        } else if (q3.y >= 0) {   // a leaf joins the P-P list whole
+        } else if (q3.w >= 0) {   // a leaf joins the P-P list whole
             if (leaf_refs) {
-                if (FILL) pp_idx[wpp++] = q3.y;
+                if (FILL) pp_idx[wpp++] = q3.w;
                 ++npp;
             } else {
                 if (FILL) {
-                    const int32_t f = q3.x;
+                    const int32_t f = q3.z;
                     for (int32_t j = 0; j < cnt; ++j) pp_idx[wpp++] = f + j;
                 }
                 npp += cnt;
