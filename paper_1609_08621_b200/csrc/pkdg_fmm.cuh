@@ -20,7 +20,7 @@
 // exact differentiation -- not from a recurrence).  The 32 lane partials of each coefficient are summed through
 // shared memory in a fixed order, then lanes = sinks evaluate the polynomial and its gradient.
 // Flops as executed (add / mul = 1, FMA = 2, rsqrt = 1): per C-C entry 23 (geometry, Newton step) + 52 (monomials)
-// + 280 (derivative polynomials: 140 terms, 56 scalings) + 64 (moments) + 672 (shift: 336 FMA) = 1091; per C-P entry
+// + 280 (derivative polynomials: 140 terms, 56 scalings) + 32 (moments) + 672 (shift: 336 FMA) = 1059; per C-P entry
 // 23 + 52 + 280 + 113 = 468; per sink 6 + 52 + 112 + 315 + 3 = 488; per bucket 1848 (reduction).  The paper's
 // audit of its own CPU code gives 472 + rsqrt / 206 + rsqrt (Table 3).
 #pragma once
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
 #pragma unroll
                 for (int s = 0; s < 32; ++s) {
                     const float sc = kMuOrder[s] == 0 ? sc0 : kMuOrder[s] == 2 ? sc2 : kMuOrder[s] == 3 ? sc3 : sc4;
-                    mu[s] = (q[kMuRec[s]] * kMuInvFact[s]) * sc;
+                    mu[s] = q[kMuRec[s]] * (kMuInvFact[s] * sc);   // the factor is the same for every entry of the bucket: hoisted
                 }
                 fmm_m2l_cell(d, mu, L);
             }
