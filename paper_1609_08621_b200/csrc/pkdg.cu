@@ -198,9 +198,7 @@ void fill_params(EvalParams& p, pkdg_ctx* ctx, const float* xyzm, int64_t np, in
     p.n_cells = nc;
     float h = 2.0f * eps;
     p.eps = eps;
-    p.h2 = h * h;
     p.h2c = fmaxf(h * h, 1.0e-24f);
-    p.hinv = h > 0.0f ? 1.0f / h : 0.0f;
     p.flags = flags;
     p.cells_raw = nullptr;
     p.cells_stride = PKDG_CELL_FLOATS;

@@ -349,9 +349,7 @@ struct EvalParams {
     DevStats* stats;
     unsigned int* work_counter;
     int64_t n_buckets, n_particles, n_cells;
-    float h2;     // (2 eps)^2
-    float h2c;    // clamp of r^2 in the Newtonian fast path: max(h2, 1e-24)
-    float hinv;   // 1/h, 0 if eps == 0
+    float h2c;    // (2 eps)^2, the clamp of r^2 in the Newtonian fast path; at least 1e-24
     float eps;
     uint32_t flags;
     // conditioning estimate and fix-up queue
@@ -435,9 +433,6 @@ __device__ __forceinline__ void cell_unpack(CellRegs& c, const float4 f0, const 
 __device__ __forceinline__ uint32_t smem_u32(const void* q) { return (uint32_t)__cvta_generic_to_shared(q); }
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async4(void* dst, const void* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
