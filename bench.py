@@ -35,7 +35,7 @@ F_PP = 19
 F_PC = 167
 PAPER_F_PP, PAPER_F_PC = 53, 215
 # C-C / C-P path (pkdg_fmm.cuh, formulas as executed): per C-C entry, per C-P entry, per sink evaluated, per bucket
-F_CC, F_CP, F_LOC_SINK, F_LOC_BUCKET = 1059, 468, 488, 1848
+F_CC, F_CP, F_LOC_SINK, F_LOC_BUCKET = 815, 372, 488, 1488
 PAPER_F_CC, PAPER_F_CP = 479, 213       # PAPER.md Table 3 (L216-217), context only
 SM_COUNT_NOMINAL, FP32_LANES_PER_SM = 148, 128
 

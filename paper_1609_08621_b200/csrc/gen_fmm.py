@@ -7,8 +7,10 @@ What is generated (DESIGN.md 
   fmm_monomials(x, y, z, p)        p[i] = x^a y^b z^c for the 56 multi-indices |k| <= 5 in the library's order
   fmm_derivs(p, g, d)              d[i] = lambda^|k| D_k(R), D_k = d^k (1/|R|), from the monomials p of the unit
                                    vector u = R / |R| and g[n] = (lambda / |R|)^n / |R|
-  fmm_m2l_cell(d, mu, L)           L[n] += sum_m mu[m] d[n + m],  |m| in {0, 2, 3, 4},  |n| + |m| <= 5
-  fmm_m2l_particle(d, mu0, L)      L[n] += mu0 d[n]
+  fmm_fold_moments(q, sc, F)       the 22 folded moments of a cell record (see "Trace-free" below)
+  fmm_m2l_cell(d, F, L)            L[n] += sum_m F[m] d[n + m],  |m| in {0, 2, 3, 4},  |n| + |m| <= 5, n and m with at most one z
+  fmm_m2l_particle(d, mu0, L)      L[n] += mu0 d[n], the 36 n with at most one z
+  kExp*                            the table that rebuilds all 56 coefficients from those 36
   fmm_eval(p, Lam, phi, gx, gy, gz)  polynomial sum_n Lam[n] sigma^n and its gradient from the monomials p of sigma
 
 The derivative tensors come from the DEFINITION, not from a recurrence: D_k = N_k(x, rho) / r^(2|k|+1) with
@@ -20,6 +22,13 @@ cell record (include/pkdg.h): for n = 0..5, a = n..0, b = n-a..0, c = n-a-b.
 With D_k = k! t_k the shift of a multipole expansion to a local one (Taylor's theorem) reads
     L_n = -(1/n!) sum_m (-1)^|m| (M_m / m!) D_{n+m}(R),      R = z_sink - z_source,
 so the kernel feeds mu[m] = -(-1)^|m| M_m / (m! lambda^|m|) and divides by n! once, after the whole list.
+
+Trace-free.  1/|R| is harmonic, so D_{k+2ex} + D_{k+2ey} + D_{k+2ez} = 0 for every k.  Two consequences, both exact:
+(1) in sum_m mu[m] D_{n+m} every m with two or more z can be moved onto the m with fewer (D_{n+m0+2ez} = -D_{n+m0+2ex}
+- D_{n+m0+2ey}), so only the 1 + 5 + 7 + 9 = 22 FOLDED moments F[m], m_z <= 1, are needed (linear combinations of the
+record's 32, made once per cell); (2) the accumulated coefficients obey the same identity (the truncation is by the
+total order |n| + |m|, so all three terms of it are always present together), hence only the 36 coefficients with
+n_z <= 1 are accumulated and the other 20 are rebuilt once per bucket.  215 multiply-adds per cell instead of 336.
 """
 from __future__ import annotations
 
@@ -39,6 +48,21 @@ def multi_indices(nmax):
 IDX = multi_indices(ORDER)
 POS = {k: i for i, k in enumerate(IDX)}
 MOM = multi_indices(4)          # record layout: 35 moments (the 3 dipole slots are absent from the record)
+IND = [k for k in IDX if k[2] <= 1]                         # the 36 coefficients that are accumulated
+POSI = {k: i for i, k in enumerate(IND)}
+MOMF = [m for m in MOM if sum(m) != 1 and m[2] <= 1]        # the 22 folded moments
+POSF = {m: i for i, m in enumerate(MOMF)}
+
+
+def reduce_z(k):
+    """k -> {k' with k'_z <= 1: integer coefficient}: repeated use of T[k + 2ez] = -T[k + 2ex] - T[k + 2ey]."""
+    if k[2] <= 1:
+        return {k: 1}
+    out = defaultdict(int)
+    for kk in ((k[0] + 2, k[1], k[2] - 2), (k[0], k[1] + 2, k[2] - 2)):
+        for key, c in reduce_z(kk).items():
+            out[key] -= c
+    return {key: c for key, c in out.items() if c != 0}
 
 
 # --- exact polynomial algebra in (x, y, z, rho): dict {(ex, ey, ez, erho): int} ---------------------------------
@@ -115,6 +139,8 @@ def emit():
     w("__device__ __forceinline__ void fmm_derivs(const float (&p)[kNLoc], const float (&g)[%d], float (&d)[kNLoc]) {" % (ORDER + 1))
     nterms = 0
     for i, k in enumerate(IDX):
+        if k[2] > 2:
+            continue            # n and m have at most one z each: no D with three or more z is ever read
         poly = on_unit_sphere(N[k])
         terms = sorted(poly.items(), key=lambda kv: -sum(kv[0]))
         nterms += len(terms)
@@ -125,44 +151,57 @@ def emit():
         w("    d[%d] = g[%d] * (%s);" % (i, sum(k), expr))
     w("}")
     w("")
-    pairs = [(n, m) for n in IDX for m in MOM if sum(m) != 1 and sum(n) + sum(m) <= ORDER]
-    w("// L[n] += sum_m mu[m] d[n + m]: %d multiply-adds.  mu = the 35 slots of the canonical record from [3] on" % len(pairs))
-    w("// (mass, 6 + 10 + 15 moments), already scaled: mu[m] = -(-1)^|m| M_m / (m! lambda^|m|)")
-    w("__device__ __forceinline__ void fmm_m2l_cell(const float (&d)[kNLoc], const float (&mu)[32], float (&L)[kNLoc]) {")
-    slot = {}
-    s = 0
-    for m in MOM:
-        if sum(m) == 1:
-            continue
-        slot[m] = s; s += 1
-    assert s == 32
-    for n in IDX:
-        for m in MOM:
-            if sum(m) == 1 or sum(n) + sum(m) > ORDER:
+    pairs = [(n, m) for n in IND for m in MOMF if sum(n) + sum(m) <= ORDER]
+    w("// L[n] += sum_m F[m] d[n + m] over the 36 n and 22 folded m with at most one z: %d multiply-adds." % len(pairs))
+    w("constexpr int kNRed = %d;   // accumulated local coefficients (n_z <= 1)" % len(IND))
+    w("constexpr int kNFold = %d;  // folded moments (m_z <= 1)" % len(MOMF))
+    w("__device__ __forceinline__ void fmm_m2l_cell(const float (&d)[kNLoc], const float (&F)[kNFold], float (&L)[kNRed]) {")
+    for n in IND:
+        for m in MOMF:
+            if sum(n) + sum(m) > ORDER:
                 continue
             nm = tuple(a + b for a, b in zip(n, m))
-            w("    L[%d] = fmaf(mu[%d], d[%d], L[%d]);" % (POS[n], slot[m], POS[nm], POS[n]))
+            w("    L[%d] = fmaf(F[%d], d[%d], L[%d]);" % (POSI[n], POSF[m], POS[nm], POSI[n]))
     w("}")
     w("")
-    w("// scale factors of the record's moments: mu[s] = rec[3 + s'] * kMuScale[s] * (-1 / lambda)^|m| * (-1)")
-    w("// kMuOrder[s] = |m| of slot s, kMuRec[s] = its float in the canonical record, kMuInvFact[s] = 1 / m!")
-    w("__device__ constexpr int kMuOrder[32] = {%s};" % ", ".join(str(sum(m)) for m in MOM if sum(m) != 1))
-    rec_pos = []
-    for m in MOM:
-        if sum(m) == 1:
-            continue
+    # folded moments: F[m] = sc[|m|] * sum_{m'} c(m', m) / m'! * q[rec(m')]
+    def rec_of(m):
         n = sum(m)
         base = {0: 3, 2: 4, 3: 10, 4: 20}[n]
-        within = [k for k in multi_indices(n) if sum(k) == n].index(m)
-        rec_pos.append(base + within)
-    w("__device__ constexpr int kMuRec[32] = {%s};" % ", ".join(map(str, rec_pos)))
-    w("__device__ constexpr float kMuInvFact[32] = {%s};" % ", ".join(
-        flit(Fraction(1, math.factorial(m[0]) * math.factorial(m[1]) * math.factorial(m[2]))) for m in MOM if sum(m) != 1))
-    w("")
-    w("__device__ __forceinline__ void fmm_m2l_particle(const float (&d)[kNLoc], const float mu0, float (&L)[kNLoc]) {")
-    w("#pragma unroll")
-    w("    for (int i = 0; i < kNLoc; ++i) L[i] = fmaf(mu0, d[i], L[i]);")
+        return base + [k for k in multi_indices(n) if sum(k) == n].index(m)
+    w("// F[m] = sc[|m|] * sum_m' c(m', m) q[m'] / m'!  (q = the canonical record; sc[r] = -(-1)^r / lambda^r)")
+    w("__device__ __forceinline__ void fmm_fold_moments(const float (&q)[36], const float sc0, const float sc2, const float sc3,")
+    w("                                                 const float sc4, float (&F)[kNFold]) {")
+    nfold_terms = 0
+    for m in MOMF:
+        terms = []
+        for mp in MOM:
+            if sum(mp) != sum(m) or sum(mp) == 1:
+                continue
+            c = reduce_z(mp).get(m, 0)
+            if c:
+                terms.append((Fraction(c, math.factorial(mp[0]) * math.factorial(mp[1]) * math.factorial(mp[2])), rec_of(mp)))
+        nfold_terms += len(terms)
+        expr = None
+        for c, r in terms:
+            expr = "%s * q[%d]" % (flit(c), r) if expr is None else "fmaf(%s, q[%d], %s)" % (flit(c), r, expr)
+        w("    F[%d] = sc%d * (%s);" % (POSF[m], sum(m), expr))
     w("}")
+    w("")
+    w("__device__ __forceinline__ void fmm_m2l_particle(const float (&d)[kNLoc], const float mu0, float (&L)[kNRed]) {")
+    for n in IND:
+        w("    L[%d] = fmaf(mu0, d[%d], L[%d]);" % (POSI[n], POS[n], POSI[n]))
+    w("}")
+    w("")
+    w("// all 56 coefficients from the 36 accumulated ones: full[k] = sum_j kExpCoef[k][j] * red[kExpIdx[k][j]]")
+    exp = []
+    for k in IDX:
+        t = sorted(reduce_z(k).items(), key=lambda kv: POSI[kv[0]])
+        assert 1 <= len(t) <= 3
+        t = t + [(IND[0], 0)] * (3 - len(t))
+        exp.append(t)
+    w("__device__ constexpr int kExpIdx[kNLoc][3] = {%s};" % ", ".join("{%s}" % ", ".join(str(POSI[n]) for n, _ in t) for t in exp))
+    w("__device__ constexpr float kExpCoef[kNLoc][3] = {%s};" % ", ".join("{%s}" % ", ".join(flit(c) for _, c in t) for t in exp))
     w("")
     w("// 1 / n! of the 56 local coefficients")
     w("__device__ constexpr float kLocInvFact[kNLoc] = {%s};" % ", ".join(
@@ -182,14 +221,14 @@ def emit():
         w("    }")
     w("}")
     w("}  // namespace pkdg")
-    return "\n".join(out) + "\n", nterms, len(pairs)
+    return "\n".join(out) + "\n", nterms, len(pairs), nfold_terms
 
 
 def main():
-    text, nterms, npairs = emit()
+    text, nterms, npairs, nfold = emit()
     with open(os.path.join(HERE, "pkdg_fmm_gen.cuh"), "w") as f:
         f.write(text)
-    print("pkdg_fmm_gen.cuh: %d derivative terms, %d shift multiply-adds" % (nterms, npairs))
+    print("pkdg_fmm_gen.cuh: %d derivative terms, %d shift multiply-adds, %d moment-folding terms" % (nterms, npairs, nfold))
 
 
 if __name__ == "__main__":

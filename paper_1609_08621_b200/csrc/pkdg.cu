@@ -476,7 +476,7 @@ pkdg_status pkdg_gravity_eval_fmm(pkdg_ctx* ctx, const pkdg_particles* P, const 
     f.work_counter = ctx->counters + 2 * (kMaxSlots + 1);
     f.flags = flags;
     CK(cudaMemsetAsync(f.work_counter, 0, sizeof(unsigned int), st));
-    int64_t grid = (int64_t)ctx->num_sms * 2;
+    int64_t grid = (int64_t)ctx->num_sms * 4;   // 128 registers: four CTAs of four warps per SM
     const int64_t want = (B->n + kFmmWarps - 1) / kFmmWarps;
     if (grid > want) grid = want;
     pkdg_fmm_kernel<<<(unsigned)grid, kFmmWarps * 32, 0, st>>>(f);

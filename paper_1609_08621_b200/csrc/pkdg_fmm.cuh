@@ -11,18 +11,22 @@
 //     phi(x_i) += sum_n L_n s^n,   a(x_i) -= grad of that polynomial,   s = x_i - z_B.
 //
 // Mapping.  One warp per sink bucket (buckets from an atomic counter, tree order).  Lanes stride the two source
-// lists; a lane keeps its partial sum of the 56 coefficients in registers across both lists.  Everything is
+// lists; a lane keeps its partial sums of the local coefficients in registers across both lists.  Everything is
 // made dimensionless with ONE length per bucket, lambda = max_i |x_i - z_B|: the lane accumulates
 // lambda^|n| n! L_n from D_k lambda^|k| = (lambda/|R|)^|k| / |R| x (polynomial in the unit vector R/|R|) and
 // moments divided by lambda^|m|, so no intermediate leaves the fp32 range for any |R| and the sinks evaluate a
-// polynomial in sigma = s / lambda, |sigma| <= 1.  The derivative polynomials and the 336 multiply-adds of the
-// shift are generated straight-line code (pkdg_fmm_gen.cuh, written by gen_fmm.py from the definition of D_k by
-// exact differentiation -- not from a recurrence).  The 32 lane partials of each coefficient are summed through
-// shared memory in a fixed order, then lanes = sinks evaluate the polynomial and its gradient.
+// polynomial in sigma = s / lambda, |sigma| <= 1.  1/|R| is harmonic, so only the 36 coefficients with at most one
+// z index are accumulated, from 22 folded moments per cell (gen_fmm.py "Trace-free"): 215 multiply-adds per cell
+// instead of 336, 128 registers and 16 warps per SM instead of 255 and 8; the other 20 coefficients are rebuilt once
+// per bucket.  The derivative polynomials, the moment folding and the shift are generated straight-line code
+// (pkdg_fmm_gen.cuh, written by gen_fmm.py from the definition of D_k by exact differentiation -- not from a
+// recurrence).  The 32 lane partials of each coefficient are summed through shared memory in a fixed order, then
+// lanes = sinks evaluate the polynomial and its gradient.
 // Flops as executed (add / mul = 1, FMA = 2, rsqrt = 1): per C-C entry 23 (geometry, Newton step) + 52 (monomials)
-// + 280 (derivative polynomials: 140 terms, 56 scalings) + 32 (moments) + 672 (shift: 336 FMA) = 1059; per C-P entry
-// 23 + 52 + 280 + 113 = 468; per sink 6 + 52 + 112 + 315 + 3 = 488; per bucket 1848 (reduction).  The paper's
-// audit of its own CPU code gives 472 + rsqrt / 206 + rsqrt (Table 3).
+// + 224 (derivative polynomials: 112 terms, 46 scalings) + 86 (folded moments: 43 terms, 22 scalings) + 430 (shift:
+// 215 FMA) = 815; per C-P entry 23 + 52 + 224 + 73 = 372; per sink 6 + 52 + 112 + 315 + 3 = 488; per bucket 1488
+// (reduction of 36 x 32 partials, rebuilding the 56).  The paper's audit of its own CPU code gives 472 + rsqrt /
+// 206 + rsqrt (Table 3).
 #pragma once
 #include "pkdg_fmm_gen.cuh"
 
@@ -86,7 +90,7 @@ struct FmmAhead {
     float4 sink, pcp0;
 };
 
-__global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmParams p) {
+__global__ void __launch_bounds__(kFmmWarps * 32, 4) pkdg_fmm_kernel(const FmmParams p) {
     __shared__ __align__(16) float s_part[kFmmWarps][kFmmWarpFloats];
     __shared__ float s_lam[kFmmWarps][64];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -176,9 +180,9 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
         const bool has_next = (int64_t)nxt.bu < p.n_buckets;
         if (has_next) step_a(nxt);
 
-        float L[kNLoc];
+        float L[kNRed];   // the 36 coefficients with at most one z; the other 20 follow from them (1/|R| is harmonic)
 #pragma unroll
-        for (int i = 0; i < kNLoc; ++i) L[i] = 0.0f;
+        for (int i = 0; i < kNRed; ++i) L[i] = 0.0f;
 
         // ---- C-C: one source cell per lane and trip; the record of trip t + 1 and the index of trip t + 2 are in
         //      flight during trip t (the record of trip 0 since step C)
@@ -214,13 +218,9 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
                 }
                 float d[kNLoc];
                 fmm_source_derivs(zx - q[0], zy - q[1], zz - q[2], lam, d);
-                float mu[32];
-#pragma unroll
-                for (int s = 0; s < 32; ++s) {
-                    const float sc = kMuOrder[s] == 0 ? sc0 : kMuOrder[s] == 2 ? sc2 : kMuOrder[s] == 3 ? sc3 : sc4;
-                    mu[s] = q[kMuRec[s]] * (kMuInvFact[s] * sc);   // the factor is the same for every entry of the bucket: hoisted
-                }
-                fmm_m2l_cell(d, mu, L);
+                float F[kNFold];
+                fmm_fold_moments(q, sc0, sc2, sc3, sc4, F);
+                fmm_m2l_cell(d, F, L);
             }
         }
         cp_async_wait_all();
@@ -248,19 +248,30 @@ __global__ void __launch_bounds__(kFmmWarps * 32, 2) pkdg_fmm_kernel(const FmmPa
             }
         }
 
-        // ---- the 32 lane partials of each coefficient, summed in a fixed order; 1 / n!
+        // ---- the 32 lane partials of each accumulated coefficient, summed in a fixed order; then all 56 coefficients
+        //      from the 36 (full[k + 2ez] = -full[k + 2ex] - full[k + 2ey], as a table) and 1 / n!
         __syncwarp();
 #pragma unroll
-        for (int i = 0; i < kNLoc; ++i) part[i * kFmmRow + lane] = L[i];
+        for (int i = 0; i < kNRed; ++i) part[i * kFmmRow + lane] = L[i];
+        __syncwarp();
+        float red0 = 0.0f, red1 = 0.0f;
+#pragma unroll 8
+        for (int j = 0; j < 32; ++j) red0 += part[lane * kFmmRow + j];
+        if (lane + 32 < kNRed) {
+#pragma unroll 8
+            for (int j = 0; j < 32; ++j) red1 += part[(lane + 32) * kFmmRow + j];
+        }
+        __syncwarp();
+        part[lane] = red0;                       // the reduced coefficients, in the first floats of the same memory
+        if (lane + 32 < kNRed) part[lane + 32] = red1;
         __syncwarp();
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int i = lane + 32 * h;
             if (i < kNLoc) {
-                float sum = 0.0f;
-#pragma unroll 8
-                for (int j = 0; j < 32; ++j) sum += part[i * kFmmRow + j];
-                Lam[i] = sum * kLocInvFact[i];
+                const float full = kExpCoef[i][0] * part[kExpIdx[i][0]] + kExpCoef[i][1] * part[kExpIdx[i][1]] +
+                                   kExpCoef[i][2] * part[kExpIdx[i][2]];
+                Lam[i] = full * kLocInvFact[i];
             }
         }
         __syncwarp();   // the staging memory is free again, Lam is visible
