@@ -784,7 +784,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
                     }
                     const int ncell = min(32, pc_len - 32 * k);
                     const float4* rec = S.cell[buf];
-#pragma unroll 1
+#pragma unroll 2
                     for (int c = 0; c < ncell; ++c) {
                         CellRegs cr;
                         cell_unpack(cr, rec[8 * c], rec[8 * c + 1], rec[8 * c + 2], rec[8 * c + 3], rec[8 * c + 4],
