@@ -191,6 +191,12 @@ def measured_traffic(key):
     return t.get(key), f"ncu capture {t.get('capture', '?')}"
 
 
+def _leaf_lists(p):
+    """The P-P lists of problem p with bucket references as entries (what the host generator gives with leaf form)."""
+    from paper_1609_08621_b200 import inputs
+    return inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+
+
 def _max_over_ranks(x, dist, torch, dev):
     if dist is None:
         return x
@@ -478,12 +484,97 @@ def run_ours(args, rank, world, local_rank):
             dl_e2e()
         dt = (time.perf_counter() - t0) / k2
         h2d = sum(int(v.numel() * v.element_size()) for v in list(tree_h.values()) + [sink_h, xy_h, ce_h, fb_h, cb_h])
+        # the same with P-P entries as bucket references (PKDG_PP_LEAVES): 16 x fewer P-P entries to write and to read
+        leaf_rank = (np.cumsum(tr["isleaf"] != 0) - 1).astype(np.int32)
+        lr_h = torch.from_numpy(leaf_rank).pin_memory()
+        tree_d["leaf_rank"] = lr_h.to(dev)
+        lo_h, li_h = _leaf_lists(p)
+        d_lli = torch.empty(li_h.shape[0], dtype=torch.int32, device=dev)
+        lfl = flags | binding.PP_LEAVES
+
+        def walk_leaf():
+            npp, npc = ctx.build_lists_count(tree_d, g.cells, sink_d, p.theta, p.eps, d_ppo, d_pco, flags=binding.PP_LEAVES)
+            assert npp == li_h.shape[0] and npc == p.pc_idx.shape[0]
+            ctx.build_lists_fill(tree_d, g.cells, sink_d, p.theta, p.eps, d_ppo, d_pco, d_lli, d_pci, flags=binding.PP_LEAVES)
+        for _ in range(2):
+            walk_leaf()
+        walk_leaf_ms = timed(walk_leaf, max(3, args.steps // 2))
+        same_leaf = bool(torch.equal(d_lli.cpu(), torch.from_numpy(li_h)) and torch.equal(d_ppo.cpu(), torch.from_numpy(lo_h))
+                         and torch.equal(d_pci, g.pc_idx))
+
+        def dl_e2e_leaf():
+            x = xy_h.to(dev, non_blocking=True); c = ce_h.to(dev, non_blocking=True)
+            td = {k: v.to(dev, non_blocking=True) for k, v in tree_h.items()}
+            td["leaf_rank"] = lr_h.to(dev, non_blocking=True)
+            sk = sink_h.to(dev, non_blocking=True); fb = fb_h.to(dev, non_blocking=True); cb = cb_h.to(dev, non_blocking=True)
+            ctx.build_lists_count(td, c, sk, p.theta, p.eps, d_ppo, d_pco, flags=binding.PP_LEAVES)
+            ctx.build_lists_fill(td, c, sk, p.theta, p.eps, d_ppo, d_pco, d_lli, d_pci, flags=binding.PP_LEAVES)
+            ctx.gravity_eval(x, c, fb, cb, d_ppo, d_lli, d_pco, d_pci, g.eps, out, flags=lfl)
+            out_h.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        for _ in range(2):
+            dl_e2e_leaf()
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            dl_e2e_leaf()
+        dt_leaf = (time.perf_counter() - t0) / k2
+        lst = ctx.get_stats()
+        assert lst["interactions_pp"] == p.I_pp and lst["interactions_pc"] == p.I_pc and lst["bad_entries"] == 0
+
+        # the same again with the copies overlapped: tree and cells first, the walk starts while the particles are
+        # still crossing the bus; the evaluation runs in four bucket ranges (pkdg_gravity_eval_range) and the rows of a
+        # range go back while the next range is evaluated.
+        s1, s2 = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+        n_rng = 4
+        rb = [int(v) for v in np.linspace(0, p.n_buckets, n_rng + 1)]
+        row_of = lambda b: int(p.first[b]) if b < p.n_buckets else int(p.first[-1] + p.count[-1])
+
+        def dl_e2e_overlapped():
+            with torch.cuda.stream(s1):
+                c = ce_h.to(dev, non_blocking=True)
+                td = {k: v.to(dev, non_blocking=True) for k, v in tree_h.items()}
+                td["leaf_rank"] = lr_h.to(dev, non_blocking=True)
+                sk = sink_h.to(dev, non_blocking=True); fb = fb_h.to(dev, non_blocking=True); cb = cb_h.to(dev, non_blocking=True)
+            with torch.cuda.stream(s2):
+                x = xy_h.to(dev, non_blocking=True)
+                ev_x = s2.record_event()
+            with torch.cuda.stream(s1):
+                ctx.build_lists_count(td, c, sk, p.theta, p.eps, d_ppo, d_pco, flags=binding.PP_LEAVES, stream=s1)
+                ctx.build_lists_fill(td, c, sk, p.theta, p.eps, d_ppo, d_pco, d_lli, d_pci, flags=binding.PP_LEAVES, stream=s1)
+                s1.wait_event(ev_x)
+                for r in range(n_rng):
+                    b0, b1 = rb[r], rb[r + 1]
+                    ctx.gravity_eval_range(x, c, fb, cb, b0, b1, d_ppo[b0:b1 + 1], d_lli, d_pco[b0:b1 + 1], d_pci, g.eps, out,
+                                           flags=lfl, stream=s1)
+                    ev = s1.record_event()
+                    with torch.cuda.stream(s2):
+                        s2.wait_event(ev)
+                        r0, r1 = row_of(b0), row_of(b1)
+                        out_h[r0:r1].copy_(out[r0:r1], non_blocking=True)
+            s1.synchronize(); s2.synchronize()
+        ref_rows = out_h.clone()     # the result of the plain sequence above: ranges give the same bits
+        out_h.zero_()
+        for _ in range(2):
+            dl_e2e_overlapped()
+        same_rows = bool(torch.equal(out_h, ref_rows))
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            dl_e2e_overlapped()
+        dt_ovl = (time.perf_counter() - t0) / k2
         devlists = {"walk_ms": walk_ms, "bit_identical_to_host_generator": same,
+                    "leaf_form": {"walk_ms": walk_leaf_ms, "bit_identical_to_host_generator": same_leaf,
+                                  "list_entries": int(li_h.shape[0] + p.pc_idx.shape[0]),
+                                  "e2e_ms_per_step": dt_leaf * 1e3, "e2e_value": inter / dt_leaf,
+                                  "e2e_overlapped_ms_per_step": dt_ovl * 1e3, "e2e_overlapped_value": inter / dt_ovl,
+                                  "e2e_overlapped_rows_complete": same_rows,
+                                  "e2e_overlapped_api": "H2D of tree and cells, walk while the particles arrive, four "
+                                                        "pkdg_gravity_eval_range calls, rows of a range copied back under the next",
+                                  "h2d_bytes_per_step": h2d + int(lr_h.numel() * 4)},
                     "list_entries": int(p.pp_idx.shape[0] + p.pc_idx.shape[0]),
                     "e2e": {"value": inter / dt, "unit": "interactions/s", "ms_per_step": dt * 1e3, "h2d_bytes_per_step": h2d,
                             "d2h_bytes_per_step": int(out_h.numel() * 4),
                             "api": "H2D of particles, cells, tree; pkdg_build_lists_count + _fill; pkdg_gravity_eval; D2H"}}
-        del tree_d, sink_d, d_ppo, d_pco, d_ppi, d_pci, out_h
+        del tree_d, sink_d, d_ppo, d_pco, d_ppi, d_pci, d_lli, out_h
 
     # ---- FMM form of the path: four lists per bucket, C-C / C-P through the 5th-order local
     #      expansion.  Extra key, N = 1: the whole call and the local-expansion kernel alone.
