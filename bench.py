@@ -561,7 +561,26 @@ def run_ours(args, rank, world, local_rank):
         for _ in range(k2):
             dl_e2e_overlapped()
         dt_ovl = (time.perf_counter() - t0) / k2
+        # the same sequence as ONE call of the library: pkdg_gravity_eval_tree_host
+        tree_np = {k: v for k, v in tree_h.items()}
+        out_t = torch.zeros((p.n, 4), dtype=torch.float32).pin_memory()
+
+        def tree_call():
+            ctx.gravity_eval_tree_host(xy_h, ce_h, tree_np, fb_h, cb_h, sink_h, p.theta, p.eps, out_t, flags=flags, n_ranges=4)
+        for _ in range(2):
+            tree_call()
+        same_tree = bool(torch.equal(out_t, ref_rows))
+        tst = ctx.get_stats()
+        assert tst["interactions_pp"] == p.I_pp and tst["interactions_pc"] == p.I_pc and tst["bad_entries"] == 0
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            tree_call()
+        dt_tree = (time.perf_counter() - t0) / k2
         devlists = {"walk_ms": walk_ms, "bit_identical_to_host_generator": same,
+                    "tree_host_call": {"api": "pkdg_gravity_eval_tree_host (host buffers in, device-built leaf-form lists, 4 ranges)",
+                                       "ms_per_step": dt_tree * 1e3, "value": inter / dt_tree, "unit": "interactions/s",
+                                       "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(out_t.numel() * 4),
+                                       "rows_equal_to_plain_sequence": same_tree},
                     "leaf_form": {"walk_ms": walk_leaf_ms, "bit_identical_to_host_generator": same_leaf,
                                   "list_entries": int(li_h.shape[0] + p.pc_idx.shape[0]),
                                   "e2e_ms_per_step": dt_leaf * 1e3, "e2e_value": inter / dt_leaf,

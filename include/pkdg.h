@@ -259,6 +259,19 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx *ctx, const pkdg_tree *tree, const pk
                                   uint32_t flags, const int64_t *pp_offsets, const int64_t *pc_offsets,
                                   int32_t *pp_idx, int32_t *pc_idx, void *stream);
 
+/* End to end from the TREE (every buffer on the host, pinned for full speed): the lists are built on the device
+ * (pkdg_build_lists_*, P-P entries as bucket references) and evaluated, so only particles, cells and the tree cross the
+ * bus, not the lists.  tree_host holds host arrays (leaf_rank is ignored); buckets_host are the leaves as sinks,
+ * contiguous runs of particles in ascending order, and bucket_cell_host[b] is the tree cell of bucket b.
+ * Tree, cells and buckets are copied first; the walk runs while the particles are still arriving; the evaluation is
+ * cut into n_ranges (1..64; 4 is a good value) bucket ranges and the rows of a range are copied back while the next
+ * range is evaluated.  Synchronous; rows of particles in no bucket keep the caller's values.  Flags: PKDG_NO_FIXUP,
+ * PKDG_FIXUP_ALL, PKDG_VALIDATE.  pkdg_stats holds the totals of the call (chunks = n_ranges). */
+pkdg_status pkdg_gravity_eval_tree_host(pkdg_ctx *ctx, const pkdg_particles *particles_host, const pkdg_cells *cells_host,
+                                        const pkdg_tree *tree_host, const pkdg_buckets *buckets_host,
+                                        const int32_t *bucket_cell_host, double theta, float eps, uint32_t flags,
+                                        float *out_acc_pot_host, int32_t n_ranges);
+
 /* Packer made visible for bit-exact checks (SURVEY.md sec 8(c) "Integer side"): the tiles the
  * evaluation kernel consumes.  tile_offsets = [n_buckets+1] int64 (first tile of each bucket);
  * tiles = [tile_capacity][32] int32, list order, last tile of a bucket padded with PKDG_PAD.

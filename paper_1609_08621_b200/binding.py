@@ -30,7 +30,8 @@ CELLQ_FLOATS = 32
 
 EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_gravity_eval_host_range", "pkdg_gravity_eval_groups",
-           "pkdg_gravity_eval_host_groups", "pkdg_gravity_eval_fmm", "pkdg_build_lists_count", "pkdg_build_lists_fill", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
+           "pkdg_gravity_eval_host_groups", "pkdg_gravity_eval_fmm", "pkdg_build_lists_count", "pkdg_build_lists_fill",
+           "pkdg_gravity_eval_tree_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
            "pkdg_get_stats", "pkdg_set_option", "pkdg_profile_enable", "pkdg_profile_read", "pkdg_launch_count",
            "pkdg_status_string", "pkdg_last_error", "pkdg_version", "pkdg_fma_peak_probe"]
 
@@ -108,6 +109,8 @@ def _load():
                                          c_uint32, c_void_p, c_void_p, c_void_p, c_void_p]
     L.pkdg_build_lists_fill.argtypes = [c_void_p, POINTER(_Tree), POINTER(_Cells), c_void_p, c_int64, c_double, c_double,
                                         c_uint32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    L.pkdg_gravity_eval_tree_host.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Tree),
+                                              POINTER(_Buckets), c_void_p, c_double, c_float, c_uint32, c_void_p, c_int32]
     L.pkdg_pack_export.argtypes = [c_void_p, c_int64, POINTER(_List), c_void_p, c_void_p, c_int64, c_void_p]
     L.pkdg_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int64)]
     L.pkdg_prepare_cells_export.argtypes = [c_void_p, POINTER(_Cells), c_void_p, c_void_p]
@@ -346,6 +349,20 @@ class Context:
                                        float(theta), float(eps), int(flags), _ptr(pp_off), _ptr(pc_off), _ptr(pp_idx),
                                        _ptr(pc_idx), _stream_ptr(stream))
         self._check(s, "pkdg_build_lists_fill")
+
+    def gravity_eval_tree_host(self, xyzm_h, cells_h, tree_h, first_h, count_h, bucket_cell_h, theta, eps, out_h, flags=0,
+                               n_ranges=4):
+        """pkdg_gravity_eval_tree_host: every buffer on the host (numpy or CPU tensors, pinned for full speed); the
+        lists are built on the device.  tree_h: dict of first, count, end, isleaf (int32), bblo, bbhi (float32 [n,3])."""
+        T, C = self._tree(tree_h, cells_h)
+        _dt(xyzm_h, "float32", "xyzm"); _dt(first_h, "int32", "first"); _dt(count_h, "int32", "count")
+        _dt(bucket_cell_h, "int32", "bucket_cell"); _dt(out_h, "float32", "out")
+        P = _Particles(_ptr(xyzm_h), int(xyzm_h.shape[0]))
+        B = _Buckets(_ptr(first_h), _ptr(count_h), int(first_h.shape[0]))
+        s = _lib.pkdg_gravity_eval_tree_host(self._h, byref(P), byref(C), byref(T), byref(B), _ptr(bucket_cell_h),
+                                             float(theta), float(eps), int(flags), _ptr(out_h), int(n_ranges))
+        self._check(s, "pkdg_gravity_eval_tree_host")
+        return out_h
 
     def pack_export(self, n_buckets, off, idx, tile_offsets, tiles, stream=None):
         """pkdg_pack_export: tile_offsets[n_buckets+1] int64 and tiles[cap,32] int32 (device)."""

@@ -61,6 +61,14 @@ struct pkdg_ctx {
     int64_t e2e_np = 0, e2e_nc = 0, e2e_no = 0;
     int64_t* scan_tmp = nullptr;
     int64_t scan_cap = 0;
+    // pkdg_gravity_eval_tree_host: device copies of the tree and the lists built from it
+    int32_t *t_first = nullptr, *t_count = nullptr, *t_end = nullptr, *t_isleaf = nullptr, *t_rank = nullptr, *t_sink = nullptr;
+    float *t_bblo = nullptr, *t_bbhi = nullptr;
+    int64_t t_cap[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int32_t *t_bfirst = nullptr, *t_bcount = nullptr, *t_ppi = nullptr, *t_pci = nullptr;
+    int64_t *t_ppo = nullptr, *t_pco = nullptr;
+    int64_t t_bcap[6] = {0, 0, 0, 0, 0, 0};
+    cudaEvent_t t_ev[2] = {nullptr, nullptr};
     WalkNode* wnodes = nullptr;        // pkdg_build_lists_*: one 64-byte record per tree cell
     int64_t wnodes_cap = 0;
     int2* gfc = nullptr;               // PKDG_PP_LEAVES: (first, count) of every bucket
@@ -322,6 +330,11 @@ pkdg_status pkdg_destroy(pkdg_ctx* ctx) {
     cudaDeviceSynchronize();
     cudaFree(ctx->cellq); cudaFree(ctx->desc); cudaFree(ctx->stats); cudaFree(ctx->counters);
     cudaFree(ctx->e2e_xyzm); cudaFree(ctx->e2e_cells); cudaFree(ctx->e2e_out); cudaFree(ctx->scan_tmp);
+    cudaFree(ctx->t_first); cudaFree(ctx->t_count); cudaFree(ctx->t_end); cudaFree(ctx->t_isleaf); cudaFree(ctx->t_rank);
+    cudaFree(ctx->t_sink); cudaFree(ctx->t_bblo); cudaFree(ctx->t_bbhi); cudaFree(ctx->t_bfirst); cudaFree(ctx->t_bcount);
+    cudaFree(ctx->t_ppi); cudaFree(ctx->t_pci); cudaFree(ctx->t_ppo); cudaFree(ctx->t_pco);
+    for (cudaEvent_t e : ctx->t_ev)
+        if (e) cudaEventDestroy(e);
     cudaFree(ctx->gfc); cudaFree(ctx->wnodes); cudaFree(ctx->g_first); cudaFree(ctx->g_count); cudaFree(ctx->fixq);
     for (int i = 0; i < ctx->n_slots_live; ++i) {
         Slot& s = ctx->slots[i];
@@ -855,6 +868,98 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
+}
+
+// End to end from the TREE: every buffer on the host, lists built on the device.  Tree, cells and buckets go first;
+// the walk runs while the particles are still crossing the bus; the evaluation is cut into n_ranges bucket ranges and
+// the rows of a range go back while the next range is evaluated.
+pkdg_status pkdg_gravity_eval_tree_host(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg_cells* Ch, const pkdg_tree* Th,
+                                        const pkdg_buckets* Bh, const int32_t* bucket_cell_host, double theta, float eps,
+                                        uint32_t flags, float* out_host, int32_t n_ranges) {
+    if (!ctx) return PKDG_EINVAL;
+    if (!Ph || !Ch || !Th || !Bh || !out_host) return fail(ctx, PKDG_EINVAL, "particles, cells, tree, buckets and out must not be NULL");
+    pkdg_status s = check_tree(ctx, Th, Ch, bucket_cell_host, Bh->n, theta);
+    if (s != PKDG_OK) return s;
+    if ((s = check_common(ctx, Ph, Ch, Bh, nullptr, nullptr, out_host)) != PKDG_OK) return s;
+    if (n_ranges < 1 || n_ranges > 64) return fail(ctx, PKDG_EINVAL, "n_ranges must be in 1..64");
+    if (flags & (PKDG_ACCUMULATE | PKDG_SKIP_PP | PKDG_SKIP_PC))
+        return fail(ctx, PKDG_EINVAL, "pkdg_gravity_eval_tree_host takes PKDG_NO_FIXUP, PKDG_FIXUP_ALL and PKDG_VALIDATE only");
+    const int64_t nb = Bh->n, ncell = Th->n_cells, np = Ph->n;
+    for (int64_t b = 0; b < nb; ++b) {   // rows go back range by range: the buckets must be the contiguous runs of tree order
+        const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
+        if (Bh->count[b] < 0 || Bh->first[b] < 0 || end > np || (b + 1 < nb && end != (int64_t)Bh->first[b + 1]) ||
+            bucket_cell_host[b] < 0 || bucket_cell_host[b] >= ncell)
+            return fail(ctx, PKDG_EINVAL, "buckets must be contiguous runs in ascending order and name cells of the tree");
+    }
+    CK(cudaSetDevice(ctx->device));
+    if (!ctx->own_stream) CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+    if ((s = ensure_slots(ctx, 1)) != PKDG_OK) return s;
+    for (cudaEvent_t& e : ctx->t_ev)
+        if (!e) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    cudaStream_t sa = ctx->own_stream, sb = ctx->slots[0].st;
+    if (nb == 0 || np == 0) return PKDG_OK;
+    // workspace
+    if ((s = ensure(ctx, &ctx->e2e_xyzm, &ctx->e2e_np, np * 4)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->e2e_out, &ctx->e2e_no, np * 4)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->e2e_cells, &ctx->e2e_nc, ncell * (int64_t)Ch->stride_floats)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_first, &ctx->t_cap[0], ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_count, &ctx->t_cap[1], ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_end, &ctx->t_cap[2], ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_isleaf, &ctx->t_cap[3], ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_rank, &ctx->t_cap[4], ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_sink, &ctx->t_cap[5], nb)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_bblo, &ctx->t_cap[6], 3 * ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_bbhi, &ctx->t_cap[7], 3 * ncell)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_bfirst, &ctx->t_bcap[0], nb)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_bcount, &ctx->t_bcap[1], nb)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_ppo, &ctx->t_bcap[2], nb + 1)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_pco, &ctx->t_bcap[3], nb + 1)) != PKDG_OK) return s;
+    // tree, cells, buckets on stream a; particles on stream b
+    auto h2d = [&](void* d, const void* h, size_t bytes, cudaStream_t st) { return cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, st); };
+    CK(h2d(ctx->e2e_cells, Ch->rec, sizeof(float) * ncell * Ch->stride_floats, sa));
+    CK(h2d(ctx->t_first, Th->first, 4 * ncell, sa)); CK(h2d(ctx->t_count, Th->count, 4 * ncell, sa));
+    CK(h2d(ctx->t_end, Th->end, 4 * ncell, sa)); CK(h2d(ctx->t_isleaf, Th->isleaf, 4 * ncell, sa));
+    CK(h2d(ctx->t_bblo, Th->bblo, 12 * ncell, sa)); CK(h2d(ctx->t_bbhi, Th->bbhi, 12 * ncell, sa));
+    CK(h2d(ctx->t_sink, bucket_cell_host, 4 * nb, sa));
+    CK(h2d(ctx->t_bfirst, Bh->first, 4 * nb, sa)); CK(h2d(ctx->t_bcount, Bh->count, 4 * nb, sa));
+    CK(h2d(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * np, sb));
+    CK(cudaEventRecord(ctx->t_ev[0], sb));
+    // leaf_rank[cell of bucket b] = b, then the walk (P-P entries as bucket references)
+    pkdg_leaf_rank_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, sa>>>(ctx->t_sink, nb, ctx->t_rank);
+    ctx->launches++;
+    pkdg_tree Td = {ctx->t_first, ctx->t_count, ctx->t_end, ctx->t_isleaf, ctx->t_bblo, ctx->t_bbhi, ctx->t_rank, ncell};
+    pkdg_cells Cd = {ctx->e2e_cells, ncell, Ch->stride_floats};
+    int64_t tot[2] = {0, 0};
+    if ((s = pkdg_build_lists_count(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
+                                    tot, sa)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_ppi, &ctx->t_bcap[4], tot[0] + 1)) != PKDG_OK) return s;
+    if ((s = ensure(ctx, &ctx->t_pci, &ctx->t_bcap[5], tot[1] + 1)) != PKDG_OK) return s;
+    if ((s = pkdg_build_lists_fill(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
+                                   ctx->t_ppi, ctx->t_pci, sa)) != PKDG_OK) return s;
+    CK(cudaStreamWaitEvent(sa, ctx->t_ev[0], 0));
+    // evaluation in bucket ranges; rows of a range go back on stream b while the next range runs
+    pkdg_particles Pd = {ctx->e2e_xyzm, np};
+    pkdg_buckets Bd = {ctx->t_bfirst, ctx->t_bcount, nb};
+    pkdg_status rc = PKDG_OK;
+    bool first_range = true;
+    for (int r = 0; r < n_ranges && rc == PKDG_OK; ++r) {
+        const int64_t b0 = nb * r / n_ranges, b1 = nb * (r + 1) / n_ranges;
+        if (b1 <= b0) continue;
+        pkdg_list pp = {ctx->t_ppo + b0, ctx->t_ppi}, pc = {ctx->t_pco + b0, ctx->t_pci};
+        // the counters are reset by the first range only: they add up over the call
+        rc = resident_impl(ctx, &Pd, &Cd, &Bd, b0, b1, nullptr, &pp, &pc, eps, flags | PKDG_PP_LEAVES, ctx->e2e_out, sa, first_range);
+        first_range = false;
+        if (rc != PKDG_OK) break;
+        if (cudaEventRecord(ctx->t_ev[1], sa) != cudaSuccess || cudaStreamWaitEvent(sb, ctx->t_ev[1], 0) != cudaSuccess) { rc = PKDG_ECUDA; break; }
+        const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];
+        if (r1 > r0 && cudaMemcpyAsync(out_host + 4 * r0, ctx->e2e_out + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
+                                       cudaMemcpyDeviceToHost, sb) != cudaSuccess) { rc = PKDG_ECUDA; break; }
+    }
+    cudaError_t e1 = cudaStreamSynchronize(sa), e2 = cudaStreamSynchronize(sb);   // also on the error path
+    if (rc == PKDG_OK && (e1 != cudaSuccess || e2 != cudaSuccess)) rc = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+    if (rc == PKDG_ECUDA && ctx->err.empty()) ctx->err = cudaGetErrorString(cudaGetLastError());
+    ctx->last_stream = sa; ctx->last_chunks = n_ranges; ctx->last_buckets = nb;
+    return rc;
 }
 
 pkdg_status pkdg_chunk_bounds(int64_t n_buckets, const int64_t* pp_off, const int64_t* pc_off, int64_t max_entries,

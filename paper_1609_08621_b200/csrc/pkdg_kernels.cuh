@@ -1307,6 +1307,12 @@ __global__ void pkdg_walk_nodes_kernel(const TreeView T, WalkNode* __restrict__ 
     nodes[k] = w;
 }
 
+// leaf_rank[cell of bucket b] = b: what a P-P entry for that leaf is with PKDG_PP_LEAVES (only leaves are ever read)
+__global__ void pkdg_leaf_rank_kernel(const int32_t* __restrict__ bucket_cell, int64_t n_buckets, int32_t* __restrict__ leaf_rank) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < n_buckets) leaf_rank[bucket_cell[b]] = (int32_t)b;
+}
+
 template <bool FILL>
 __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_cells, bool leaf_refs,
                                  const int32_t* __restrict__ sink_cell, int64_t n_sinks, double theta,

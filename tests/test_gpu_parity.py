@@ -628,3 +628,44 @@ def test_device_list_construction_is_bit_exact(ctx, torch, cfg1):
     assert list(z[0]) == [0] and list(z[2]) == [0] and z[1].size == 0
     with pytest.raises(binding.PkdgError):
         _device_lists(ctx, torch, p, p.tree["leaf_cell"], -1.0, p.eps)
+
+
+def test_tree_host_call_builds_lists_and_evaluates(ctx, torch, cfg1):
+    """pkdg_gravity_eval_tree_host: every buffer on the host, lists built on the device.  Same bits as the resident
+    call on the host generator's leaf-form lists (the device walk is bit-identical and ranges do not change a
+    bucket's sums), the oracle's result within the tolerance, counters of the whole call, 1 / 3 / 4 ranges; rows in
+    no bucket keep the caller's values; bad arguments fail loudly."""
+    from paper_1609_08621_b200 import binding, inputs
+    from gpu_util import rel_errors, run_resident
+    for p in (cfg1, inputs.config2(n=1 << 15), inputs.config3(32)):
+        q = _leaf_problem(p)
+        base = run_resident(ctx, q, torch, flags=binding.PP_LEAVES)
+        ref = _oracle(p)
+        tr = p.tree
+        tree = {k: np.ascontiguousarray(tr[k]) for k in ("first", "count", "end", "isleaf", "bblo", "bbhi")}
+        cell_of = np.ascontiguousarray(tr["leaf_cell"].astype(np.int32))
+        for n_ranges in (1, 3, 4):
+            out = np.full((p.n, 4), np.nan, np.float32)
+            ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, p.first, p.count, cell_of, p.theta, p.eps, out, n_ranges=n_ranges)
+            st = ctx.get_stats()
+            assert np.array_equal(out, base), (p.name, n_ranges)
+            assert st["interactions_pp"] == p.I_pp and st["interactions_pc"] == p.I_pc and st["bad_entries"] == 0
+            assert st["chunks"] == n_ranges and st["n_buckets"] == p.n_buckets
+        ea, ep = rel_errors(out, ref)
+        assert ea.max() <= TOL and ep.max() <= TOL, (p.name, ea.max(), ep.max())
+    # a subset of the buckets (a contiguous run): other rows untouched
+    p = cfg1
+    tr = p.tree
+    tree = {k: np.ascontiguousarray(tr[k]) for k in ("first", "count", "end", "isleaf", "bblo", "bbhi")}
+    b0, b1 = 100, 300
+    out = np.full((p.n, 4), np.nan, np.float32)
+    ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, np.ascontiguousarray(p.first[b0:b1]), np.ascontiguousarray(p.count[b0:b1]),
+                               np.ascontiguousarray(tr["leaf_cell"][b0:b1].astype(np.int32)), p.theta, p.eps, out, n_ranges=2)
+    lo, hi = int(p.first[b0]), int(p.first[b1 - 1] + p.count[b1 - 1])
+    assert np.isfinite(out[lo:hi]).all() and np.isnan(out[:lo]).all() and np.isnan(out[hi:]).all()
+    with pytest.raises(binding.PkdgError):      # buckets out of order
+        ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, np.ascontiguousarray(p.first[::-1]), np.ascontiguousarray(p.count[::-1]),
+                                   np.ascontiguousarray(tr["leaf_cell"][::-1].astype(np.int32)), p.theta, p.eps, out)
+    with pytest.raises(binding.PkdgError):
+        ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, p.first, p.count, np.ascontiguousarray(tr["leaf_cell"].astype(np.int32)),
+                                   p.theta, p.eps, out, n_ranges=0)
