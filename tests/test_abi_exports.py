@@ -61,3 +61,16 @@ def test_product_package_does_not_import_the_oracle():
         text = open(os.path.join(pkg, src)).read()
         assert "oracle" not in text.lower().replace("the oracle", "")  # comments may mention it; no include
         assert "#include \"../../oracle" not in text and "pkdg_oracle" not in text
+
+
+def test_generated_fmm_header_is_current():
+    """pkdg_fmm_gen.cuh is what gen_fmm.py writes (the header is committed; the generator is its source)."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_1609_08621_b200", "csrc")
+    spec = importlib.util.spec_from_file_location("gen_fmm", os.path.join(here, "gen_fmm.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    text = gen.emit()[0]
+    with open(os.path.join(here, "pkdg_fmm_gen.cuh")) as f:
+        assert f.read() == text
