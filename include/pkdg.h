@@ -305,6 +305,7 @@ pkdg_status pkdg_profile_read(pkdg_ctx *ctx, int64_t *n_launches_host, double *e
 int64_t pkdg_launch_count(const pkdg_ctx *ctx);
 
 const char *pkdg_status_string(pkdg_status s);
+/* Text of the last error on ctx; with ctx == NULL, why the calling thread's last pkdg_create failed. */
 const char *pkdg_last_error(const pkdg_ctx *ctx);
 void pkdg_version(int32_t *major, int32_t *minor);
 

@@ -197,7 +197,7 @@ class Context:
         s = _lib.pkdg_create(byref(self._h), int(device))
         if s != 0:
             self._h = c_void_p()
-            raise PkdgError(f"pkdg_create: {status_string(s)}")
+            raise PkdgError(f"pkdg_create: {status_string(s)}: {_lib.pkdg_last_error(None).decode()}")
         self.device = device
 
     def close(self):

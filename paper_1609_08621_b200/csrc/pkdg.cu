@@ -40,6 +40,8 @@ struct Slot {
 
 }  // namespace
 
+static thread_local std::string g_create_err;   // why the last pkdg_create of this thread failed
+
 struct pkdg_ctx {
     int device = 0;
     int num_sms = 0;
@@ -316,7 +318,7 @@ pkdg_status pkdg_create(pkdg_ctx** out, int device) {
     if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(unsigned int) * (2 * (kMaxSlots + 1) + 1));
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_ready, cudaEventDisableTiming);
     if (e != cudaSuccess) {
-        fprintf(stderr, "pkdg_create: %s\n", cudaGetErrorString(e));
+        g_create_err = std::string("pkdg_create: ") + cudaGetErrorString(e);   // read with pkdg_last_error(NULL)
         delete ctx;
         return PKDG_ECUDA;
     }
@@ -1051,7 +1053,7 @@ const char* pkdg_status_string(pkdg_status s) {
     }
 }
 
-const char* pkdg_last_error(const pkdg_ctx* ctx) { return ctx ? ctx->err.c_str() : "no context"; }
+const char* pkdg_last_error(const pkdg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 void pkdg_version(int32_t* major, int32_t* minor) {
     if (major) *major = PKDG_VERSION_MAJOR;

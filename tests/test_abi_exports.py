@@ -74,3 +74,15 @@ def test_generated_fmm_header_is_current():
     text = gen.emit()[0]
     with open(os.path.join(here, "pkdg_fmm_gen.cuh")) as f:
         assert f.read() == text
+
+
+def test_create_failure_is_reported_through_the_abi():
+    """Without a CUDA device pkdg_create fails and pkdg_last_error(NULL) says why (nothing is printed to stderr)."""
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    from paper_1609_08621_b200 import binding
+    with pytest.raises(binding.PkdgError) as e:
+        binding.Context(0)
+    assert "PKDG_ECUDA" in str(e.value) and "pkdg_create:" in str(e.value) and len(str(e.value)) > 40
