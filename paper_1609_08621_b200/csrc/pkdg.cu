@@ -900,63 +900,70 @@ pkdg_status pkdg_gravity_eval_tree_host(pkdg_ctx* ctx, const pkdg_particles* Ph,
         if (!e) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     cudaStream_t sa = ctx->own_stream, sb = ctx->slots[0].st;
     if (nb == 0 || np == 0) return PKDG_OK;
-    // workspace
-    if ((s = ensure(ctx, &ctx->e2e_xyzm, &ctx->e2e_np, np * 4)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->e2e_out, &ctx->e2e_no, np * 4)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->e2e_cells, &ctx->e2e_nc, ncell * (int64_t)Ch->stride_floats)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_first, &ctx->t_cap[0], ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_count, &ctx->t_cap[1], ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_end, &ctx->t_cap[2], ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_isleaf, &ctx->t_cap[3], ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_rank, &ctx->t_cap[4], ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_sink, &ctx->t_cap[5], nb)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_bblo, &ctx->t_cap[6], 3 * ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_bbhi, &ctx->t_cap[7], 3 * ncell)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_bfirst, &ctx->t_bcap[0], nb)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_bcount, &ctx->t_bcap[1], nb)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_ppo, &ctx->t_bcap[2], nb + 1)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_pco, &ctx->t_bcap[3], nb + 1)) != PKDG_OK) return s;
-    // tree, cells, buckets on stream a; particles on stream b
-    auto h2d = [&](void* d, const void* h, size_t bytes, cudaStream_t st) { return cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, st); };
-    CK(h2d(ctx->e2e_cells, Ch->rec, sizeof(float) * ncell * Ch->stride_floats, sa));
-    CK(h2d(ctx->t_first, Th->first, 4 * ncell, sa)); CK(h2d(ctx->t_count, Th->count, 4 * ncell, sa));
-    CK(h2d(ctx->t_end, Th->end, 4 * ncell, sa)); CK(h2d(ctx->t_isleaf, Th->isleaf, 4 * ncell, sa));
-    CK(h2d(ctx->t_bblo, Th->bblo, 12 * ncell, sa)); CK(h2d(ctx->t_bbhi, Th->bbhi, 12 * ncell, sa));
-    CK(h2d(ctx->t_sink, bucket_cell_host, 4 * nb, sa));
-    CK(h2d(ctx->t_bfirst, Bh->first, 4 * nb, sa)); CK(h2d(ctx->t_bcount, Bh->count, 4 * nb, sa));
-    CK(h2d(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * np, sb));
-    CK(cudaEventRecord(ctx->t_ev[0], sb));
-    // leaf_rank[cell of bucket b] = b, then the walk (P-P entries as bucket references)
-    pkdg_leaf_rank_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, sa>>>(ctx->t_sink, nb, ctx->t_rank);
-    ctx->launches++;
-    pkdg_tree Td = {ctx->t_first, ctx->t_count, ctx->t_end, ctx->t_isleaf, ctx->t_bblo, ctx->t_bbhi, ctx->t_rank, ncell};
-    pkdg_cells Cd = {ctx->e2e_cells, ncell, Ch->stride_floats};
-    int64_t tot[2] = {0, 0};
-    if ((s = pkdg_build_lists_count(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
-                                    tot, sa)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_ppi, &ctx->t_bcap[4], tot[0] + 1)) != PKDG_OK) return s;
-    if ((s = ensure(ctx, &ctx->t_pci, &ctx->t_bcap[5], tot[1] + 1)) != PKDG_OK) return s;
-    if ((s = pkdg_build_lists_fill(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
-                                   ctx->t_ppi, ctx->t_pci, sa)) != PKDG_OK) return s;
-    CK(cudaStreamWaitEvent(sa, ctx->t_ev[0], 0));
-    // evaluation in bucket ranges; rows of a range go back on stream b while the next range runs
-    pkdg_particles Pd = {ctx->e2e_xyzm, np};
-    pkdg_buckets Bd = {ctx->t_bfirst, ctx->t_bcount, nb};
-    pkdg_status rc = PKDG_OK;
-    bool first_range = true;
-    for (int r = 0; r < n_ranges && rc == PKDG_OK; ++r) {
-        const int64_t b0 = nb * r / n_ranges, b1 = nb * (r + 1) / n_ranges;
-        if (b1 <= b0) continue;
-        pkdg_list pp = {ctx->t_ppo + b0, ctx->t_ppi}, pc = {ctx->t_pco + b0, ctx->t_pci};
-        // the counters are reset by the first range only: they add up over the call
-        rc = resident_impl(ctx, &Pd, &Cd, &Bd, b0, b1, nullptr, &pp, &pc, eps, flags | PKDG_PP_LEAVES, ctx->e2e_out, sa, first_range);
-        first_range = false;
-        if (rc != PKDG_OK) break;
-        if (cudaEventRecord(ctx->t_ev[1], sa) != cudaSuccess || cudaStreamWaitEvent(sb, ctx->t_ev[1], 0) != cudaSuccess) { rc = PKDG_ECUDA; break; }
-        const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];
-        if (r1 > r0 && cudaMemcpyAsync(out_host + 4 * r0, ctx->e2e_out + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
-                                       cudaMemcpyDeviceToHost, sb) != cudaSuccess) { rc = PKDG_ECUDA; break; }
-    }
+    // everything that queues work runs in this lambda, so that every way out of it passes the synchronisation below:
+    // no copy that touches the caller's host buffers may still be in flight when the call returns
+    auto run = [&]() -> pkdg_status {
+        pkdg_status s = PKDG_OK;
+        // workspace
+        if ((s = ensure(ctx, &ctx->e2e_xyzm, &ctx->e2e_np, np * 4)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->e2e_out, &ctx->e2e_no, np * 4)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->e2e_cells, &ctx->e2e_nc, ncell * (int64_t)Ch->stride_floats)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_first, &ctx->t_cap[0], ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_count, &ctx->t_cap[1], ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_end, &ctx->t_cap[2], ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_isleaf, &ctx->t_cap[3], ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_rank, &ctx->t_cap[4], ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_sink, &ctx->t_cap[5], nb)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_bblo, &ctx->t_cap[6], 3 * ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_bbhi, &ctx->t_cap[7], 3 * ncell)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_bfirst, &ctx->t_bcap[0], nb)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_bcount, &ctx->t_bcap[1], nb)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_ppo, &ctx->t_bcap[2], nb + 1)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_pco, &ctx->t_bcap[3], nb + 1)) != PKDG_OK) return s;
+        // tree, cells, buckets on stream a; particles on stream b
+        auto h2d = [&](void* d, const void* h, size_t bytes, cudaStream_t st) { return cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, st); };
+        CK(h2d(ctx->e2e_cells, Ch->rec, sizeof(float) * ncell * Ch->stride_floats, sa));
+        CK(h2d(ctx->t_first, Th->first, 4 * ncell, sa)); CK(h2d(ctx->t_count, Th->count, 4 * ncell, sa));
+        CK(h2d(ctx->t_end, Th->end, 4 * ncell, sa)); CK(h2d(ctx->t_isleaf, Th->isleaf, 4 * ncell, sa));
+        CK(h2d(ctx->t_bblo, Th->bblo, 12 * ncell, sa)); CK(h2d(ctx->t_bbhi, Th->bbhi, 12 * ncell, sa));
+        CK(h2d(ctx->t_sink, bucket_cell_host, 4 * nb, sa));
+        CK(h2d(ctx->t_bfirst, Bh->first, 4 * nb, sa)); CK(h2d(ctx->t_bcount, Bh->count, 4 * nb, sa));
+        CK(h2d(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * np, sb));
+        CK(cudaEventRecord(ctx->t_ev[0], sb));
+        // leaf_rank[cell of bucket b] = b, then the walk (P-P entries as bucket references)
+        pkdg_leaf_rank_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, sa>>>(ctx->t_sink, nb, ctx->t_rank);
+        ctx->launches++;
+        pkdg_tree Td = {ctx->t_first, ctx->t_count, ctx->t_end, ctx->t_isleaf, ctx->t_bblo, ctx->t_bbhi, ctx->t_rank, ncell};
+        pkdg_cells Cd = {ctx->e2e_cells, ncell, Ch->stride_floats};
+        int64_t tot[2] = {0, 0};
+        if ((s = pkdg_build_lists_count(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
+                                        tot, sa)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_ppi, &ctx->t_bcap[4], tot[0] + 1)) != PKDG_OK) return s;
+        if ((s = ensure(ctx, &ctx->t_pci, &ctx->t_bcap[5], tot[1] + 1)) != PKDG_OK) return s;
+        if ((s = pkdg_build_lists_fill(ctx, &Td, &Cd, ctx->t_sink, nb, theta, (double)eps, PKDG_PP_LEAVES, ctx->t_ppo, ctx->t_pco,
+                                       ctx->t_ppi, ctx->t_pci, sa)) != PKDG_OK) return s;
+        CK(cudaStreamWaitEvent(sa, ctx->t_ev[0], 0));
+        // evaluation in bucket ranges; rows of a range go back on stream b while the next range runs
+        pkdg_particles Pd = {ctx->e2e_xyzm, np};
+        pkdg_buckets Bd = {ctx->t_bfirst, ctx->t_bcount, nb};
+        pkdg_status rc = PKDG_OK;
+        bool first_range = true;
+        for (int r = 0; r < n_ranges && rc == PKDG_OK; ++r) {
+            const int64_t b0 = nb * r / n_ranges, b1 = nb * (r + 1) / n_ranges;
+            if (b1 <= b0) continue;
+            pkdg_list pp = {ctx->t_ppo + b0, ctx->t_ppi}, pc = {ctx->t_pco + b0, ctx->t_pci};
+            // the counters are reset by the first range only: they add up over the call
+            rc = resident_impl(ctx, &Pd, &Cd, &Bd, b0, b1, nullptr, &pp, &pc, eps, flags | PKDG_PP_LEAVES, ctx->e2e_out, sa, first_range);
+            first_range = false;
+            if (rc != PKDG_OK) break;
+            if (cudaEventRecord(ctx->t_ev[1], sa) != cudaSuccess || cudaStreamWaitEvent(sb, ctx->t_ev[1], 0) != cudaSuccess) { rc = PKDG_ECUDA; break; }
+            const int64_t r0 = Bh->first[b0], r1 = (int64_t)Bh->first[b1 - 1] + Bh->count[b1 - 1];
+            if (r1 > r0 && cudaMemcpyAsync(out_host + 4 * r0, ctx->e2e_out + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
+                                           cudaMemcpyDeviceToHost, sb) != cudaSuccess) { rc = PKDG_ECUDA; break; }
+        }
+        return rc;
+    };
+    pkdg_status rc = run();
     cudaError_t e1 = cudaStreamSynchronize(sa), e2 = cudaStreamSynchronize(sb);   // also on the error path
     if (rc == PKDG_OK && (e1 != cudaSuccess || e2 != cudaSuccess)) rc = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
     if (rc == PKDG_ECUDA && ctx->err.empty()) ctx->err = cudaGetErrorString(cudaGetLastError());
