@@ -815,10 +815,10 @@ static TreeView tree_view(const pkdg_tree* T, const pkdg_cells* C, bool leaves) 
 }
 
 // the walk's 64-byte cell records (workspace of the context)
-static pkdg_status walk_nodes(pkdg_ctx* ctx, const TreeView& v, cudaStream_t st) {
+static pkdg_status walk_nodes(pkdg_ctx* ctx, const TreeView& v, double theta, cudaStream_t st) {
     pkdg_status s = ensure(ctx, &ctx->wnodes, &ctx->wnodes_cap, v.n_cells);
     if (s != PKDG_OK || v.n_cells == 0) return s;
-    pkdg_walk_nodes_kernel<<<(unsigned)((v.n_cells + 255) / 256), 256, 0, st>>>(v, ctx->wnodes);
+    pkdg_walk_nodes_kernel<<<(unsigned)((v.n_cells + 255) / 256), 256, 0, st>>>(v, theta, ctx->wnodes);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -834,7 +834,7 @@ pkdg_status pkdg_build_lists_count(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
-    if ((s = walk_nodes(ctx, v, st)) != PKDG_OK) return s;
+    if ((s = walk_nodes(ctx, v, theta, st)) != PKDG_OK) return s;
     if (n_sinks > 0) {
         pkdg_walk_kernel<false><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
             ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, pp_off, pc_off, nullptr,
@@ -863,7 +863,7 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
-    if ((s = walk_nodes(ctx, v, st)) != PKDG_OK) return s;   // rebuilt here: the caller may have changed the tree since _count
+    if ((s = walk_nodes(ctx, v, theta, st)) != PKDG_OK) return s;   // rebuilt here: the caller may have changed the tree since _count
     pkdg_walk_kernel<true><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
         ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, nullptr, nullptr, pp_off,
         pc_off, pp_idx, pc_idx);

@@ -1286,24 +1286,29 @@ struct TreeView {
 // What the walk needs of a cell, gathered once per call into one 64-byte record (one cache line per visited cell
 // instead of six: the canonical record's COM and b_max sit in two different lines, the boxes in two arrays, count /
 // end / isleaf / first in four more).  The values are copies, so every decision stays bit-identical.
-struct __align__(16) WalkNode {     // first 32-byte sector: what every visit reads; second: the box, read only by
-    float cx, cy, cz, bmax;        // cells that pass the distance test.  Centre of mass, b_max
-    int32_t count, end, first, leaf;   // leaf: -1 = internal cell, else what a P-P entry for this leaf is (its rank, or 0)
+struct __align__(16) WalkNode {     // first 32-byte sector: what every visit reads; second: the box (read only by cells that
+    float cx, cy, cz;              // pass the distance test) and b_max (read for the sink cell).  Centre of mass;
+    int32_t count;                 // particles of the cell; bit 31 set = a leaf
+    double ro;                     // b_max / theta (fp64, IEEE division: the value the host walk computes at every visit)
+    int32_t end, entry;            // end of the subtree; a leaf's P-P entry: its first particle, or its rank (leaf references)
     float lox, loy, loz, hix;      // bounding box
-    float hiy, hiz, pad0, pad1;
+    float hiy, hiz, bmax, pad;
 };
 
-__global__ void pkdg_walk_nodes_kernel(const TreeView T, WalkNode* __restrict__ nodes) {
+__global__ void pkdg_walk_nodes_kernel(const TreeView T, double theta, WalkNode* __restrict__ nodes) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= T.n_cells) return;
     const float* r = T.rec + k * (int64_t)T.stride;
     WalkNode w;
     w.cx = r[0]; w.cy = r[1]; w.cz = r[2]; w.bmax = r[35];
+    w.ro = __ddiv_rn((double)r[35], theta);
     w.lox = T.bblo[3 * k]; w.loy = T.bblo[3 * k + 1]; w.loz = T.bblo[3 * k + 2];
     w.hix = T.bbhi[3 * k]; w.hiy = T.bbhi[3 * k + 1]; w.hiz = T.bbhi[3 * k + 2];
-    w.count = T.count[k]; w.end = T.end[k]; w.first = T.first[k];
-    w.leaf = T.isleaf[k] ? (T.leaf_rank ? T.leaf_rank[k] : 0) : -1;
-    w.pad0 = w.pad1 = 0.0f;
+    const bool leaf = T.isleaf[k] != 0;
+    w.count = (T.count[k] & 0x7fffffff) | (leaf ? (int32_t)0x80000000u : 0);
+    w.end = T.end[k];
+    w.entry = (leaf && T.leaf_rank) ? T.leaf_rank[k] : T.first[k];
+    w.pad = 0.0f;
     nodes[k] = w;
 }
 
@@ -1324,7 +1329,7 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
     const int64_t cb = sink_cell[s];
     const float4* nq = reinterpret_cast<const float4*>(nodes);
     const float4 b0 = __ldg(nq + 4 * cb), b1 = __ldg(nq + 4 * cb + 2), b2 = __ldg(nq + 4 * cb + 3);
-    const double bx = b0.x, by = b0.y, bz = b0.z, bmaxB = b0.w;
+    const double bx = b0.x, by = b0.y, bz = b0.z, bmaxB = b2.z;
     const double lob0 = b1.x, lob1 = b1.y, lob2 = b1.z;
     const double hib0 = b1.w, hib1 = b2.x, hib2 = b2.y;
     const double gap_min2 = __dmul_rn(__dmul_rn(4.0, eps), eps);
@@ -1332,14 +1337,16 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
     int64_t wpp = FILL ? pp_off[s] : 0, wpc = FILL ? pc_off[s] : 0;
     int64_t k = 0;
     while (k < n_cells) {
-        const float4 q0 = __ldg(nq + 4 * k);
-        const int4 q3 = __ldg(reinterpret_cast<const int4*>(nq + 4 * k + 1));   // count, end, first, leaf
-        const int32_t cnt = q3.x, end = q3.y;
+        const float4 q0 = __ldg(nq + 4 * k);                                    // COM, count | leaf bit
+        const int4 q3 = __ldg(reinterpret_cast<const int4*>(nq + 4 * k + 1));   // ro (two words), end, entry
+        const int32_t cw = __float_as_int(q0.w), cnt = cw & 0x7fffffff, end = q3.z;
+        const bool leaf = cw < 0;
+        const double ro = __hiloint2double(q3.y, q3.x);
         bool accept = false;
         if (k != cb && cnt >= 2) {
             const double dx = __dsub_rn(bx, (double)q0.x), dy = __dsub_rn(by, (double)q0.y), dz = __dsub_rn(bz, (double)q0.z);
             const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
-            if (d > __dadd_rn(bmaxB, __ddiv_rn((double)q0.w, theta))) {
+            if (d > __dadd_rn(bmaxB, ro)) {
                 const float4 q1 = __ldg(nq + 4 * k + 2), q2 = __ldg(nq + 4 * k + 3);
                 const double lok0 = q1.x, lok1 = q1.y, lok2 = q1.z;
                 const double hik0 = q1.w, hik1 = q2.x, hik2 = q2.y;
@@ -1358,13 +1365,13 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
             if (FILL) pc_idx[wpc++] = (int32_t)k;
             ++npc;
             k = end;
-        } else if (q3.w >= 0) {   // a leaf joins the P-P list whole
+        } else if (leaf) {   // a leaf joins the P-P list whole
             if (leaf_refs) {
                 if (FILL) pp_idx[wpp++] = q3.w;
                 ++npp;
             } else {
                 if (FILL) {
-                    const int32_t f = q3.z;
+                    const int32_t f = q3.w;
                     for (int32_t j = 0; j < cnt; ++j) pp_idx[wpp++] = f + j;
                 }
                 npp += cnt;
