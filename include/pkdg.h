@@ -171,6 +171,58 @@ pkdg_status pkdg_gravity_eval_groups(pkdg_ctx *ctx, const pkdg_particles *partic
                                      const pkdg_list *pc, float eps, uint32_t flags, float *out_acc_pot,
                                      void *stream);
 
+/* pkdg_gravity_eval for callers that must not allocate device memory.
+ *
+ * Who that is.  A pkdg_ctx buys its workspace with cudaMalloc (pkdg_create, and again whenever a call brings a
+ * larger problem: "grows on demand" above, which also means a cudaFree).  Some hosts cannot live with that:
+ *   - a simulation that hands out ALL device memory itself at start-up and leaves nothing for a library to take
+ *     later (PKDGRAV3 pre-partitions its memory in just this way) -- a cudaMalloc in the middle of a
+ *     run fails there, or succeeds and starves the owner;
+ *   - a time-step loop that keeps several streams busy: cudaMalloc and cudaFree synchronise the whole device, so one
+ *     workspace growth stalls every stream, not just ours;
+ *   - code that runs where the CUDA allocator may not be called at all (a stretch of the program its authors have
+ *     declared allocation-free, for predictability or because it sits inside another library's callback).
+ * This entry point needs no pkdg_ctx and calls neither cudaMalloc nor cudaFree nor any CUDA routine that allocates:
+ * the bucket descriptors, the normalised cell records, the fp64 fix-up queue and the counters that the kernels of
+ * pkdg_gravity_eval keep in the context's workspace live here in one fixed array in device memory that is part of
+ * the library image (a file-scope `static __device__` array in pkdg.cu, PKDG_STATIC_SCRATCH_BYTES ~ 6.1 MB).  The
+ * price: every GPU on which this library's code is loaded holds those bytes until the process exits, whether or
+ * not this function is ever called, and the problem size is capped:
+ *     buckets->n <= PKDG_STATIC_MAX_BUCKETS, cells->n <= PKDG_STATIC_MAX_CELLS,
+ *     particles->n <= PKDG_STATIC_MAX_PARTICLES;
+ * anything larger is refused with PKDG_EINVAL and a text that names the limit (nothing is queued).  Cut a larger
+ * problem into bucket ranges yourself, or use a pkdg_ctx.
+ *
+ * Arguments, layouts, results and stream behaviour are those of pkdg_gravity_eval (the same kernels run; rows
+ * are bit-identical to it): all pointers are device pointers on `device`, the caller owns inputs and `out_acc_pot`,
+ * the call is asynchronous on `stream`.  Flags: PKDG_ACCUMULATE, PKDG_SKIP_PP, PKDG_SKIP_PC, PKDG_NO_FIXUP,
+ * PKDG_FIXUP_ALL; PKDG_PP_LEAVES and PKDG_VALIDATE need workspace of their own and are refused.  The fix-up
+ * threshold is the default kappa2 = 6.  There are no counters to read back (pkdg_get_stats needs a context):
+ * malformed buckets or list entries are skipped as in pkdg_gravity_eval but not reported -- validate the inputs
+ * once through a context if they come from an untrusted builder.
+ *
+ * First call on a device.  The first call for a given `device` (from any thread) looks up the device address of
+ * the array (on the host the array's name is only a handle, not an address a kernel could use), the SM count and
+ * the kernel's shared-memory opt-in, with that device current, and remembers them.  It allocates nothing either,
+ * but it does talk to the driver: make that first call once, early, outside any stream capture.  Later calls only
+ * queue two memsets and four kernels.
+ *
+ * Sharing.  There is ONE array per device and every call on that device uses it, from every thread and every
+ * stream.  It still holds what the previous call left; each call clears the counters it needs at zero itself
+ * (stream-ordered, before its kernels) and overwrites every descriptor, record and queue entry before reading it,
+ * so back-to-back calls on one stream are safe.  Two calls whose GPU work may OVERLAP (different streams without
+ * an event between them, or two host threads) race on the array and give wrong rows: order them.  Calls made
+ * through a pkdg_ctx need no such care: a context has its own workspace and never touches the array.
+ * Errors: PKDG_EINVAL (arguments, limits, flags), PKDG_ECUDA; the text is at pkdg_last_error(NULL). */
+#define PKDG_STATIC_MAX_BUCKETS 32768
+#define PKDG_STATIC_MAX_CELLS 32768
+#define PKDG_STATIC_MAX_PARTICLES 524288
+#define PKDG_STATIC_SCRATCH_BYTES (512 + 32 * PKDG_STATIC_MAX_BUCKETS + 128 * PKDG_STATIC_MAX_CELLS + \
+                                   16 * (PKDG_STATIC_MAX_BUCKETS + PKDG_STATIC_MAX_PARTICLES / 16 + 16))
+pkdg_status pkdg_gravity_eval_static(int device, const pkdg_particles *particles, const pkdg_cells *cells,
+                                     const pkdg_buckets *buckets, const pkdg_list *pp, const pkdg_list *pc,
+                                     float eps, uint32_t flags, float *out_acc_pot, void *stream);
+
 /* The FMM form of the path (PAPER.md:L57 cell-cell interactions, L69 fn 2 cell-particle
  * interactions, L71 "The local expansion of the potential about the sink's center of mass is actually done to
  * 5th order ... accumulating the CC and CP interactions"; readings A20-A22).  Every bucket b has four
@@ -305,7 +357,8 @@ pkdg_status pkdg_profile_read(pkdg_ctx *ctx, int64_t *n_launches_host, double *e
 int64_t pkdg_launch_count(const pkdg_ctx *ctx);
 
 const char *pkdg_status_string(pkdg_status s);
-/* Text of the last error on ctx; with ctx == NULL, why the calling thread's last pkdg_create failed. */
+/* Text of the last error on ctx; with ctx == NULL, why the calling thread's last pkdg_create or
+ * pkdg_gravity_eval_static failed (the two calls that have no context to hold the text). */
 const char *pkdg_last_error(const pkdg_ctx *ctx);
 void pkdg_version(int32_t *major, int32_t *minor);
 

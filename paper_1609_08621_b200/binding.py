@@ -28,7 +28,11 @@ OPT_KAPPA2 = 1
 CELL_FLOATS = 36
 CELLQ_FLOATS = 32
 
-EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
+STATIC_MAX_BUCKETS = 32768
+STATIC_MAX_CELLS = 32768
+STATIC_MAX_PARTICLES = 524288
+
+EXPORTS = ["pkdg_create", "pkdg_destroy", "pkdg_gravity_eval", "pkdg_gravity_eval_static", "pkdg_gravity_eval_range", "pkdg_gravity_eval_streamed",
            "pkdg_gravity_eval_host", "pkdg_gravity_eval_host_range", "pkdg_gravity_eval_groups",
            "pkdg_gravity_eval_host_groups", "pkdg_gravity_eval_fmm", "pkdg_build_lists_count", "pkdg_build_lists_fill",
            "pkdg_gravity_eval_tree_host", "pkdg_pack_export", "pkdg_chunk_bounds", "pkdg_prepare_cells_export",
@@ -84,6 +88,8 @@ def _load():
     L.pkdg_destroy.argtypes = [c_void_p]
     L.pkdg_gravity_eval.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
                                     POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_void_p]
+    L.pkdg_gravity_eval_static.argtypes = [c_int, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets),
+                                           POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p, c_void_p]
     L.pkdg_gravity_eval_range.argtypes = [c_void_p, POINTER(_Particles), POINTER(_Cells), POINTER(_Buckets), c_int64,
                                           c_int64, POINTER(_List), POINTER(_List), c_float, c_uint32, c_void_p,
                                           c_void_p]
@@ -187,6 +193,24 @@ def chunk_bounds(pp_off, pc_off, max_entries: int) -> np.ndarray:
     if s != 0:
         raise PkdgError(status_string(s))
     return bounds[: n.value + 1].copy()
+
+
+def gravity_eval_static(device, xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx, eps, out, flags=0,
+                        stream=None):
+    """pkdg_gravity_eval_static: pkdg_gravity_eval without a context and without any device allocation, for
+    hosts that own all device memory themselves or must not call the CUDA allocator where they call us.  The
+    workspace is a fixed array inside the library (about 6 MB per GPU, shared by every call on that GPU), so
+    the problem is limited to STATIC_MAX_BUCKETS / STATIC_MAX_CELLS / STATIC_MAX_PARTICLES and calls whose GPU
+    work could overlap must be ordered by the caller.  Asynchronous on `stream`; raises PkdgError (with the
+    limit in the text) for anything larger.  Marshalling only, like every function here."""
+    P, C, B, pp, pc = Context._structs(xyzm, cells, first, count, pp_off, pp_idx, pc_off, pc_idx)
+    _dt(out, "float32", "out")
+    s = _lib.pkdg_gravity_eval_static(int(device), byref(P), byref(C) if C else None, byref(B),
+                                      byref(pp) if pp else None, byref(pc) if pc else None, float(eps), int(flags),
+                                      _ptr(out), _stream_ptr(stream))
+    if s != 0:
+        raise PkdgError(f"{status_string(s)}: {_lib.pkdg_last_error(None).decode()}")
+    return out
 
 
 class Context:

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 
 #include "pkdg_kernels.cuh"
@@ -40,7 +41,28 @@ struct Slot {
 
 }  // namespace
 
-static thread_local std::string g_create_err;   // why the last pkdg_create of this thread failed
+static thread_local std::string g_create_err;   // why the last pkdg_create / pkdg_gravity_eval_static of this thread failed
+
+// ------------------------------------------------------------------------------------------------
+// Workspace of pkdg_gravity_eval_static: the one entry point for callers that must not allocate device memory
+// (include/pkdg.h says who they are).  A fixed array in the library's device image instead of cudaMalloc'ed
+// buffers; every GPU that loads this module carries it until the process ends.  On the HOST the name
+// g_static_scratch is only a handle for the runtime: its device address comes from cudaGetSymbolAddress, once
+// per device (static_setup), and only that address is ever handed to a kernel.
+//   [0, 256)    DevStats (the packer adds to it; nobody reads it back here)
+//   [256, 512)  work counter of the evaluation kernel, length of the fix-up queue
+//   then        bucket descriptors | normalised cell records | fix-up queue
+// ------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kStOffStats = 0, kStOffCounters = 256, kStOffDesc = 512;
+constexpr size_t kStOffCellq = kStOffDesc + sizeof(BucketDesc) * PKDG_STATIC_MAX_BUCKETS;
+constexpr size_t kStOffFixq = kStOffCellq + sizeof(float) * kCellQFloats * PKDG_STATIC_MAX_CELLS;
+constexpr int64_t kStFixCap = PKDG_STATIC_MAX_BUCKETS + PKDG_STATIC_MAX_PARTICLES / kTMax + 16;
+constexpr size_t kStBytes = kStOffFixq + sizeof(int4) * kStFixCap;
+static_assert(kStBytes == PKDG_STATIC_SCRATCH_BYTES, "include/pkdg.h states the size of the static workspace");
+static_assert(sizeof(DevStats) <= 256 && kStOffCellq % 256 == 0 && kStOffFixq % 256 == 0, "sections stay 256-byte aligned");
+}  // namespace
+static __device__ __align__(256) unsigned char g_static_scratch[kStBytes];
 
 struct pkdg_ctx {
     int device = 0;
@@ -451,6 +473,156 @@ pkdg_status pkdg_gravity_eval_range(pkdg_ctx* ctx, const pkdg_particles* P, cons
                                     int64_t b0, int64_t b1, const pkdg_list* pp, const pkdg_list* pc, float eps,
                                     uint32_t flags, float* out, void* stream) {
     return resident_impl(ctx, P, C, B, b0, b1, nullptr, pp, pc, eps, flags, out, stream);
+}
+
+// ------------------------------------------------------------------------------------------------
+// pkdg_gravity_eval_static: the resident call for hosts that cannot allocate (see include/pkdg.h).  Same four
+// kernels as resident_impl, in the same order and with the same launch shapes, but no pkdg_ctx and no cudaMalloc /
+// cudaFree anywhere below: all workspace pointers are offsets into g_static_scratch's device address.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+    bool ready = false;
+    unsigned char* base = nullptr;   // DEVICE address of g_static_scratch on this device
+    int num_sms = 0;
+    int per_sm = 0;                  // CTAs per SM of the bucket kernel (particle lists)
+};
+StaticDev g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;              // guards g_static_dev (set-up may be raced by two host threads)
+
+pkdg_status static_fail(pkdg_status s, const std::string& msg) {
+    g_create_err = "pkdg_gravity_eval_static: " + msg;
+    return s;
+}
+
+#define SCK(call)                                                                                  \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) return static_fail(PKDG_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+// Once per device, with that device current: where the array lives on THIS device, and what the launches need to
+// know.  None of these calls allocates; they do reach the driver, hence "first call outside stream capture".
+pkdg_status static_setup(int device, StaticDev** out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& d = g_static_dev[device];
+    if (!d.ready) {
+        unsigned char* base = nullptr;
+        SCK(cudaGetSymbolAddress((void**)&base, g_static_scratch));
+        if (!base || (reinterpret_cast<uintptr_t>(base) & 255u))
+            return static_fail(PKDG_ECUDA, "cudaGetSymbolAddress gave no usable device address for the static workspace");
+        int sms = 0, per_sm = 0;
+        SCK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+        auto kern = pkdg_evalb_kernel<kBucketWarps, kBucketMinBlocks, false>;
+        const int smem = kBucketWarps * (int)sizeof(WarpSmemB);
+        SCK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SCK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        SCK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kBucketWarps * 32, smem));
+        d.base = base; d.num_sms = sms; d.per_sm = per_sm < 1 ? 1 : per_sm;
+        d.ready = true;
+    }
+    *out = &d;
+    return PKDG_OK;
+}
+
+}  // namespace
+
+pkdg_status pkdg_gravity_eval_static(int device, const pkdg_particles* P, const pkdg_cells* C, const pkdg_buckets* B,
+                                     const pkdg_list* pp, const pkdg_list* pc, float eps, uint32_t flags, float* out,
+                                     void* stream) {
+    // arguments and limits first: a refused call has touched neither the device nor the array
+    if (device < 0 || device >= kStaticMaxDevices) return static_fail(PKDG_EINVAL, "device must be in 0..63");
+    if (!P || !B || !out) return static_fail(PKDG_EINVAL, "particles, buckets and out must not be NULL");
+    if (P->n < 0 || B->n < 0) return static_fail(PKDG_EINVAL, "negative size");
+    if (flags & ~(uint32_t)(PKDG_ACCUMULATE | PKDG_SKIP_PP | PKDG_SKIP_PC | PKDG_NO_FIXUP | PKDG_FIXUP_ALL))
+        return static_fail(PKDG_EINVAL, "only PKDG_ACCUMULATE, PKDG_SKIP_PP, PKDG_SKIP_PC, PKDG_NO_FIXUP and PKDG_FIXUP_ALL are "
+                                        "supported (PKDG_PP_LEAVES and PKDG_VALIDATE need workspace this call does not have)");
+    const bool has_pp = pp && pp->offsets;
+    const bool pc_given = pc && pc->offsets;
+    if (pc_given && (!C || C->n < 0 || (C->n > 0 && !C->rec) || C->stride_floats < PKDG_CELL_FLOATS))
+        return static_fail(PKDG_EINVAL, "P-C list given without valid cells (stride_floats >= 36)");
+    const int64_t nc = pc_given ? C->n : 0;
+    if (B->n > PKDG_STATIC_MAX_BUCKETS || nc > PKDG_STATIC_MAX_CELLS || P->n > PKDG_STATIC_MAX_PARTICLES) {
+        char msg[320];
+        snprintf(msg, sizeof msg,
+                 "problem too large for the static workspace: %lld buckets (limit %d), %lld cells (limit %d), %lld particles "
+                 "(limit %d); split it into bucket ranges or use pkdg_gravity_eval with a context",
+                 (long long)B->n, PKDG_STATIC_MAX_BUCKETS, (long long)nc, PKDG_STATIC_MAX_CELLS, (long long)P->n,
+                 PKDG_STATIC_MAX_PARTICLES);
+        return static_fail(PKDG_EINVAL, msg);
+    }
+    if (P->n > 0 && !P->xyzm) return static_fail(PKDG_EINVAL, "particles->xyzm is NULL");
+    if (B->n > 0 && (!B->first || !B->count)) return static_fail(PKDG_EINVAL, "buckets->first/count is NULL");
+    if (!aligned16(P->xyzm) || !aligned16(out)) return static_fail(PKDG_EINVAL, "xyzm and out must be 16-byte aligned");
+    if (B->n == 0) return PKDG_OK;
+
+    SCK(cudaSetDevice(device));
+    StaticDev* d = nullptr;
+    pkdg_status s = static_setup(device, &d);   // does work on the first call for this device only
+    if (s != PKDG_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool has_pc = pc_given && nc > 0;
+
+    DevStats* stats = reinterpret_cast<DevStats*>(d->base + kStOffStats);
+    unsigned int* counters = reinterpret_cast<unsigned int*>(d->base + kStOffCounters);   // [0] work, [1] fix-up queue length
+    BucketDesc* desc = reinterpret_cast<BucketDesc*>(d->base + kStOffDesc);
+    float* cellq = reinterpret_cast<float*>(d->base + kStOffCellq);
+    int4* fixq = reinterpret_cast<int4*>(d->base + kStOffFixq);
+
+    // The array keeps the previous call's contents.  What has to start at zero is cleared here, in stream order ahead
+    // of the kernels; descriptors [0, n_buckets), records [0, n_cells) and the queue entries below the queue length
+    // are all written by this call before anything reads them.
+    SCK(cudaMemsetAsync(stats, 0, sizeof(DevStats), st));
+    SCK(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned int), st));
+    if (has_pc) {
+        const int64_t blocks = (nc + kPrepThreads - 1) / kPrepThreads;
+        pkdg_prep_cells_kernel<<<(unsigned)blocks, kPrepThreads, 0, st>>>(C->rec, nc, C->stride_floats, cellq);
+    }
+    pkdg_pack_kernel<<<(unsigned)((B->n + 255) / 256), 256, 0, st>>>(
+        B->first, B->count, has_pp ? pp->offsets : nullptr, has_pc ? pc->offsets : nullptr, B->n, P->n, 0, 0, desc, stats,
+        counters, counters + 1, nullptr, nullptr, B->n);
+
+    EvalParams p;
+    p.xyzm = reinterpret_cast<const float4*>(P->xyzm);
+    p.cellq = reinterpret_cast<const float4*>(cellq);
+    p.desc = desc;
+    p.pp_idx = has_pp ? pp->idx : nullptr;
+    p.pc_idx = has_pc ? pc->idx : nullptr;
+    p.gfc = nullptr;
+    p.n_gbuckets = B->n;
+    p.out = reinterpret_cast<float4*>(out);
+    p.stats = stats;
+    p.work_counter = counters;
+    p.n_buckets = B->n; p.n_particles = P->n; p.n_cells = nc;
+    const float h = 2.0f * eps;
+    p.h2c = fmaxf(h * h, 1.0e-24f);
+    p.eps = eps;
+    p.flags = flags;
+    p.cells_raw = has_pc ? C->rec : nullptr;
+    p.cells_stride = has_pc ? C->stride_floats : PKDG_CELL_FLOATS;
+    p.fix_k = (flags & PKDG_NO_FIXUP) ? -1.0f : (flags & PKDG_FIXUP_ALL) ? 0.0f : kDefaultKappa2 * kDefaultKappa2;
+    p.fix_queue = fixq;
+    p.fix_count = counters + 1;
+    p.fix_cap = (unsigned)fix_capacity(B->n, P->n);   // <= kStFixCap by the limits above
+    p.g_first = nullptr; p.g_n = nullptr; p.n_groups = 0; p.g_base = 0;
+
+    {
+        const int smem = kBucketWarps * (int)sizeof(WarpSmemB);
+        int64_t grid = (int64_t)d->num_sms * d->per_sm;
+        const int64_t want = (B->n + kBucketWarps - 1) / kBucketWarps;
+        if (grid > want) grid = want;
+        pkdg_evalb_kernel<kBucketWarps, kBucketMinBlocks, false><<<(unsigned)grid, kBucketWarps * 32, smem, st>>>(p);
+    }
+    if (p.fix_k >= 0.0f) {
+        int64_t grid = B->n;
+        const int64_t full = (int64_t)d->num_sms * 16;
+        if (grid > full) grid = full;
+        pkdg_fixup_kernel<<<(unsigned)grid, kFixThreads, 0, st>>>(p);
+    }
+    SCK(cudaGetLastError());
+    return PKDG_OK;
 }
 
 // The FMM form of the path: the local expansion of every bucket from its C-C and C-P lists, evaluated at the
