@@ -862,37 +862,44 @@ static pkdg_status host_impl(pkdg_ctx* ctx, const pkdg_particles* Ph, const pkdg
     if (!ctx->own_stream) CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
     cudaStream_t st = ctx->own_stream;
     const bool has_pc = pch && pch->offsets && Ch && Ch->n > 0;
+    // all workspace first: nothing may fail between the first copy out of the caller's buffers and the
+    // synchronisation at the bottom except inside `run`, whose every way out passes that synchronisation
     if ((s = ensure(ctx, &ctx->e2e_xyzm, &ctx->e2e_np, Ph->n * 4)) != PKDG_OK) return s;
     if ((s = ensure(ctx, &ctx->e2e_out, &ctx->e2e_no, Ph->n * 4)) != PKDG_OK) return s;
-    if (Ph->n) CK(cudaMemcpyAsync(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * Ph->n, cudaMemcpyHostToDevice, st));
-    pkdg_cells Cd = {nullptr, 0, PKDG_CELL_FLOATS};
-    if (has_pc) {
-        if ((s = ensure(ctx, &ctx->e2e_cells, &ctx->e2e_nc, Ch->n * (int64_t)Ch->stride_floats)) != PKDG_OK) return s;
-        CK(cudaMemcpyAsync(ctx->e2e_cells, Ch->rec, sizeof(float) * Ch->n * Ch->stride_floats, cudaMemcpyHostToDevice, st));
-        Cd.rec = ctx->e2e_cells; Cd.n = Ch->n; Cd.stride_floats = Ch->stride_floats;
-    }
-    // tree-ordered sinks (every bucket of the range starts where the previous one ends: the rows form one run):
-    // each chunk's rows go back as soon as they are done and nothing else is copied.  Anything else: the caller's
-    // rows make a round trip, so that rows in no listed bucket keep their values.
-    bool run = Bh->n > 0;
-    for (int64_t b = 0; run && b < Bh->n; ++b) {
-        const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
-        run = Bh->count[b] >= 0 && Bh->first[b] >= 0 && end <= Ph->n && (b + 1 == Bh->n || end == (int64_t)Bh->first[b + 1]);
-    }
-    if (Ph->n && (!run || (flags & PKDG_ACCUMULATE))) {
-        int64_t r0 = 0, r1 = Ph->n;
-        if (run) { r0 = Bh->first[0]; r1 = (int64_t)Bh->first[Bh->n - 1] + Bh->count[Bh->n - 1]; }
-        if (r1 > r0)
-            CK(cudaMemcpyAsync(ctx->e2e_out + 4 * r0, out_host + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
-                               cudaMemcpyHostToDevice, st));
-    }
-    pkdg_particles Pd = {ctx->e2e_xyzm, Ph->n};
-    s = streamed_impl(ctx, &Pd, has_pc ? &Cd : nullptr, Bfull, rb0, rb1, Gh, pph, has_pc ? pch : nullptr, eps, flags,
-                      ctx->e2e_out, n_streams, max_entries, st, run ? out_host : nullptr);
-    if (s == PKDG_OK && !run && Ph->n) {
-        cudaError_t e = cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st);
-        if (e != cudaSuccess) s = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e));
-    }
+    if (has_pc && (s = ensure(ctx, &ctx->e2e_cells, &ctx->e2e_nc, Ch->n * (int64_t)Ch->stride_floats)) != PKDG_OK) return s;
+    auto run = [&]() -> pkdg_status {
+        pkdg_status s = PKDG_OK;
+        if (Ph->n) CK(cudaMemcpyAsync(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * Ph->n, cudaMemcpyHostToDevice, st));
+        pkdg_cells Cd = {nullptr, 0, PKDG_CELL_FLOATS};
+        if (has_pc) {
+            CK(cudaMemcpyAsync(ctx->e2e_cells, Ch->rec, sizeof(float) * Ch->n * Ch->stride_floats, cudaMemcpyHostToDevice, st));
+            Cd.rec = ctx->e2e_cells; Cd.n = Ch->n; Cd.stride_floats = Ch->stride_floats;
+        }
+        // tree-ordered sinks (every bucket of the range starts where the previous one ends: the rows form one run):
+        // each chunk's rows go back as soon as they are done and nothing else is copied.  Anything else: the caller's
+        // rows make a round trip, so that rows in no listed bucket keep their values.
+        bool one_run = Bh->n > 0;
+        for (int64_t b = 0; one_run && b < Bh->n; ++b) {
+            const int64_t end = (int64_t)Bh->first[b] + Bh->count[b];
+            one_run = Bh->count[b] >= 0 && Bh->first[b] >= 0 && end <= Ph->n && (b + 1 == Bh->n || end == (int64_t)Bh->first[b + 1]);
+        }
+        if (Ph->n && (!one_run || (flags & PKDG_ACCUMULATE))) {
+            int64_t r0 = 0, r1 = Ph->n;
+            if (one_run) { r0 = Bh->first[0]; r1 = (int64_t)Bh->first[Bh->n - 1] + Bh->count[Bh->n - 1]; }
+            if (r1 > r0)
+                CK(cudaMemcpyAsync(ctx->e2e_out + 4 * r0, out_host + 4 * r0, sizeof(float) * 4 * (size_t)(r1 - r0),
+                                   cudaMemcpyHostToDevice, st));
+        }
+        pkdg_particles Pd = {ctx->e2e_xyzm, Ph->n};
+        s = streamed_impl(ctx, &Pd, has_pc ? &Cd : nullptr, Bfull, rb0, rb1, Gh, pph, has_pc ? pch : nullptr, eps, flags,
+                          ctx->e2e_out, n_streams, max_entries, st, one_run ? out_host : nullptr);
+        if (s == PKDG_OK && !one_run && Ph->n) {
+            cudaError_t e = cudaMemcpyAsync(out_host, ctx->e2e_out, sizeof(float) * 4 * Ph->n, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) s = fail(ctx, PKDG_ECUDA, cudaGetErrorString(e));
+        }
+        return s;
+    };
+    s = run();
     // also on the error path: no copy that touches the caller's host buffers may still be in flight on return
     for (int i = 0; i < ctx->n_slots_live; ++i) cudaStreamSynchronize(ctx->slots[i].st);
     cudaError_t e = cudaStreamSynchronize(st);
