@@ -197,7 +197,7 @@ __global__ void pkdg_pack_kernel(const int32_t* __restrict__ first, const int32_
 // Group-shared lists (the walk stops at groups of up to 64 particles =
 // 4 buckets and resolves the checklist into ONE P-P and ONE P-C list per group).  One thread per group: the
 // work descriptor of every bucket of the group points at the group's lists.  Groups must tile the bucket range
-// in order; anything else is a bad entry and leaves the affected buckets without work.
+// in order; a group that does not is a bad entry and gets no work (neither here nor in pkdg_evalg_kernel).
 __global__ void pkdg_pack_groups_kernel(const int32_t* __restrict__ first, const int32_t* __restrict__ count,
                                         const int32_t* __restrict__ g_first, const int32_t* __restrict__ g_n,
                                         const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
@@ -212,9 +212,11 @@ __global__ void pkdg_pack_groups_kernel(const int32_t* __restrict__ first, const
     if (g < n_groups) {
         int64_t b0 = (int64_t)g_first[g] - bucket_base, nb = g_n[g];
         const int64_t want = g == 0 ? 0 : (int64_t)g_first[g - 1] - bucket_base + g_n[g - 1];
+        // a group that breaks the tiling gets no descriptors at all (its buckets keep the empty ones the caller's
+        // memset left) and pkdg_evalg_kernel skips it under the same test: two overlapping groups must not race
         if (nb < 0 || b0 != want || b0 + nb > n_buckets || (g == n_groups - 1 && b0 + nb != n_buckets)) {
             bad++;
-            if (b0 < 0 || nb < 0 || b0 + nb > n_buckets) nb = 0;
+            nb = 0;
         }
         int64_t p0 = pp_off ? pp_off[g] : 0, p1 = pp_off ? pp_off[g + 1] : 0;
         int64_t c0 = pc_off ? pc_off[g] : 0, c1 = pc_off ? pc_off[g + 1] : 0;
@@ -654,6 +656,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
         const int64_t gb0 = (int64_t)__ldg(p.g_first + gu) - p.g_base;
         const int gn = __ldg(p.g_n + gu);
         if (gn <= 0 || gb0 < 0 || gb0 + gn > p.n_buckets) continue;   // counted as a bad entry by the packer
+        {   // the packer's tiling test: a group that does not start where the previous one ends (or, being the last one,
+            // does not end where the buckets do) has no descriptors and is skipped
+            const int64_t want = gu == 0 ? 0 : (int64_t)__ldg(p.g_first + gu - 1) - p.g_base + __ldg(p.g_n + gu - 1);
+            if (gb0 != want || ((int64_t)gu == p.n_groups - 1 && gb0 + gn != p.n_buckets)) continue;
+        }
         const BucketDesc d0 = p.desc[gb0];                              // every bucket of the group names the group's lists
         const int pp_len = do_pp ? d0.pp_len : 0, pc_len = do_pc ? d0.pc_len : 0;
         int nt = 0;
@@ -802,7 +809,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) pkdg_evalg_kernel(const Eval
                     if (iB >= 0) { const float4 o = p.out[iB]; rB.x += o.x; rB.y += o.y; rB.z += o.z; rB.w += o.w; }
                 }
                 const float a2A = fmaf(rA.z, rA.z, fmaf(rA.y, rA.y, rA.x * rA.x)), a2B = fmaf(rB.z, rB.z, fmaf(rB.y, rB.y, rB.x * rB.x));
-                bool flagA = fix_on && iA >= 0 && s2.x >= p.fix_k * a2A, flagB = fix_on && iB >= 0 && s2.y >= p.fix_k * a2B;
+                const bool fix_all = p.fix_k == 0.0f;   // PKDG_FIXUP_ALL; otherwise a strict test: a sink with nothing to sum (S2 = |a| = 0) is not ill-conditioned
+                bool flagA = fix_on && iA >= 0 && (fix_all || s2.x > p.fix_k * a2A), flagB = fix_on && iB >= 0 && (fix_all || s2.y > p.fix_k * a2B);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const bool flag = h ? flagB : flagA;
@@ -1091,7 +1099,8 @@ __device__ __forceinline__ void bucket_pass(const EvalParams& p, WarpSmemB& S, c
         if (wB) { const float4 o = p.out[iB]; rB.x += o.x; rB.y += o.y; rB.z += o.z; rB.w += o.w; }
     }
     const float a2A = fmaf(rA.z, rA.z, fmaf(rA.y, rA.y, rA.x * rA.x)), a2B = fmaf(rB.z, rB.z, fmaf(rB.y, rB.y, rB.x * rB.x));
-    bool flagA = fix_on && wA && s2.x >= p.fix_k * a2A, flagB = fix_on && wB && s2.y >= p.fix_k * a2B;
+    const bool fix_all = p.fix_k == 0.0f;   // PKDG_FIXUP_ALL; otherwise a strict test: a sink with nothing to sum (S2 = |a| = 0) is not ill-conditioned
+    bool flagA = fix_on && wA && (fix_all || s2.x > p.fix_k * a2A), flagB = fix_on && wB && (fix_all || s2.y > p.fix_k * a2B);
     // one queue entry per (bucket, pass) in the fix-up kernel's format: sink t of the pass is bit 2 t
     const unsigned mask = __reduce_or_sync(0xffffffffu, ((unsigned)flagA << (4 * pair)) | ((unsigned)flagB << (4 * pair + 2)));
     if (mask) {

@@ -576,6 +576,19 @@ def test_group_shared_lists(ctx, torch, cfg1):
                             p.eps, out)
     torch.cuda.synchronize()
     assert ctx.get_stats(check=False)["bad_entries"] > 0
+    # group 3 now reaches into group 4's first bucket, so group 4 no longer starts where group 3 ends: it gets no
+    # work at all (its other buckets keep the caller's zeros) instead of racing with group 3 on the shared bucket;
+    # every group that tiles correctly evaluates as before
+    good = torch.zeros((p.n, 4), dtype=torch.float32, device="cuda")
+    ctx.gravity_eval_groups(t(p.xyzm), t(p.cells), t(p.first), t(p.count), t(gf), t(gn), t(ppo), t(ppi), t(pco), t(pci),
+                            p.eps, good)
+    torch.cuda.synchronize()
+    got, good = out.cpu().numpy(), good.cpu().numpy()
+    rows = lambda g0, g1: np.arange(p.first[gf[g0]], p.first[gf[g1 - 1] + gn[g1 - 1] - 1] + p.count[gf[g1 - 1] + gn[g1 - 1] - 1])
+    assert np.array_equal(got[rows(0, 3)], good[rows(0, 3)]) and np.array_equal(got[rows(5, len(gf))], good[rows(5, len(gf))])
+    if gn[4] > 1:
+        skipped = np.arange(p.first[gf[4] + 1], p.first[gf[4] + gn[4] - 1] + p.count[gf[4] + gn[4] - 1])
+        assert (got[skipped] == 0).all()
     with pytest.raises(binding.PkdgError):
         ctx.gravity_eval_host_groups(p.xyzm, p.cells, p.first, p.count, gf, bad_gn, ppo, ppi, pco, pci, p.eps,
                                      np.zeros((p.n, 4), np.float32))
