@@ -301,7 +301,10 @@ typedef struct {
  * owns the index arrays: _count writes the CSR offsets (n_sinks + 1 each, device) and returns the two totals
  * in totals_host[2] (synchronises; NULL = stay asynchronous); _fill writes the entries, in walk order.  With
  * PKDG_PP_LEAVES a P-P entry is the bucket index of the leaf instead of its particles.  Decisions are taken in
- * fp64 with IEEE operations and no contraction: offsets and indices are bit-identical to a host walk. */
+ * fp64 with IEEE operations and no contraction: offsets and indices are bit-identical to a host walk.
+ * Malformed tree input does not hang or read out of bounds: an end[k] outside (k, n_cells] is clamped into it and
+ * a sink_cell outside [0, n_cells) gets two empty lists; both are counted in pkdg_stats.bad_entries, which
+ * pkdg_get_stats reports (PKDG_EBADLIST) when called after _count and before the next evaluation call. */
 pkdg_status pkdg_build_lists_count(pkdg_ctx *ctx, const pkdg_tree *tree, const pkdg_cells *cells,
                                    const int32_t *sink_cell, int64_t n_sinks, double theta, double eps,
                                    uint32_t flags, int64_t *pp_offsets, int64_t *pc_offsets,
@@ -313,8 +316,10 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx *ctx, const pkdg_tree *tree, const pk
 
 /* End to end from the TREE (every buffer on the host, pinned for full speed): the lists are built on the device
  * (pkdg_build_lists_*, P-P entries as bucket references) and evaluated, so only particles, cells and the tree cross the
- * bus, not the lists.  tree_host holds host arrays (leaf_rank is ignored); buckets_host are the leaves as sinks,
- * contiguous runs of particles in ascending order, and bucket_cell_host[b] is the tree cell of bucket b.
+ * bus, not the lists.  tree_host holds host arrays (leaf_rank is ignored); buckets_host are ALL the leaves of the tree
+ * as sinks, contiguous runs of particles in ascending order, and bucket_cell_host[b] is the leaf cell of
+ * bucket b (a P-P source leaf is named by its bucket index, so a subset of the leaves is refused with PKDG_EINVAL; for
+ * a subset of sinks use pkdg_build_lists_* and pkdg_gravity_eval_range).
  * Tree, cells and buckets are copied first; the walk runs while the particles are still arriving; the evaluation is
  * cut into n_ranges (1..64; 4 is a good value) bucket ranges and the rows of a range are copied back while the next
  * range is evaluated.  Synchronous; rows of particles in no bucket keep the caller's values.  Flags: PKDG_NO_FIXUP,

@@ -994,10 +994,11 @@ static TreeView tree_view(const pkdg_tree* T, const pkdg_cells* C, bool leaves) 
 }
 
 // the walk's 64-byte cell records (workspace of the context)
-static pkdg_status walk_nodes(pkdg_ctx* ctx, const TreeView& v, double theta, cudaStream_t st) {
+static pkdg_status walk_nodes(pkdg_ctx* ctx, const TreeView& v, double theta, cudaStream_t st, bool count_bad) {
     pkdg_status s = ensure(ctx, &ctx->wnodes, &ctx->wnodes_cap, v.n_cells);
     if (s != PKDG_OK || v.n_cells == 0) return s;
-    pkdg_walk_nodes_kernel<<<(unsigned)((v.n_cells + 255) / 256), 256, 0, st>>>(v, theta, ctx->wnodes);
+    pkdg_walk_nodes_kernel<<<(unsigned)((v.n_cells + 255) / 256), 256, 0, st>>>(v, theta, ctx->wnodes,
+                                                                               count_bad ? ctx->stats : nullptr);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -1013,11 +1014,15 @@ pkdg_status pkdg_build_lists_count(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
-    if ((s = walk_nodes(ctx, v, theta, st)) != PKDG_OK) return s;
+    // malformed tree input (a subtree end that does not advance, a sink that is no cell of the tree) is counted in
+    // bad_entries: pkdg_get_stats after this call reports it (an evaluation call resets the counters)
+    ctx->last_stream = st; ctx->last_chunks = 1; ctx->last_buckets = n_sinks;
+    CK(cudaMemsetAsync(ctx->stats, 0, sizeof(DevStats), st));
+    if ((s = walk_nodes(ctx, v, theta, st, true)) != PKDG_OK) return s;
     if (n_sinks > 0) {
         pkdg_walk_kernel<false><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
             ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, pp_off, pc_off, nullptr,
-            nullptr, nullptr, nullptr);
+            nullptr, nullptr, nullptr, ctx->stats);
         ctx->launches++;
         CK(cudaGetLastError());
     }
@@ -1042,10 +1047,10 @@ pkdg_status pkdg_build_lists_fill(pkdg_ctx* ctx, const pkdg_tree* T, const pkdg_
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(ctx->device));
     const TreeView v = tree_view(T, C, (flags & PKDG_PP_LEAVES) != 0);
-    if ((s = walk_nodes(ctx, v, theta, st)) != PKDG_OK) return s;   // rebuilt here: the caller may have changed the tree since _count
+    if ((s = walk_nodes(ctx, v, theta, st, false)) != PKDG_OK) return s;   // rebuilt here: the caller may have changed the tree since _count
     pkdg_walk_kernel<true><<<(unsigned)((n_sinks + 127) / 128), 128, 0, st>>>(
         ctx->wnodes, v.n_cells, (flags & PKDG_PP_LEAVES) != 0, sink_cell, n_sinks, theta, eps, nullptr, nullptr, pp_off,
-        pc_off, pp_idx, pc_idx);
+        pc_off, pp_idx, pc_idx, nullptr);
     ctx->launches++;
     CK(cudaGetLastError());
     return PKDG_OK;
@@ -1071,6 +1076,20 @@ pkdg_status pkdg_gravity_eval_tree_host(pkdg_ctx* ctx, const pkdg_particles* Ph,
         if (Bh->count[b] < 0 || Bh->first[b] < 0 || end > np || (b + 1 < nb && end != (int64_t)Bh->first[b + 1]) ||
             bucket_cell_host[b] < 0 || bucket_cell_host[b] >= ncell)
             return fail(ctx, PKDG_EINVAL, "buckets must be contiguous runs in ascending order and name cells of the tree");
+        const int32_t c = bucket_cell_host[b];
+        if (!Th->isleaf[c] || Th->first[c] != Bh->first[b] || Th->count[c] != Bh->count[b])
+            return fail(ctx, PKDG_EINVAL, "bucket_cell_host[b] must be a leaf cell whose particle run is bucket b");
+    }
+    for (int64_t k = 0; k < ncell; ++k)   // the walk advances through end[]: it must move forward and stay inside
+        if (Th->end[k] <= k || Th->end[k] > ncell)
+            return fail(ctx, PKDG_EINVAL, "tree_host->end[k] must lie in (k, n_cells]");
+    // The walk names a P-P source leaf by its bucket index, so EVERY leaf must be a bucket.  The leaves partition the
+    // root's particle run; contiguous leaf runs that start and end where the root does are therefore all of them.
+    if (nb > 0 && ncell > 0) {
+        const int64_t r0 = Th->first[0], r1 = (int64_t)Th->first[0] + Th->count[0];
+        if ((int64_t)Bh->first[0] != r0 || (int64_t)Bh->first[nb - 1] + Bh->count[nb - 1] != r1)
+            return fail(ctx, PKDG_EINVAL, "buckets_host must be ALL leaves of the tree (a subset of sinks is not supported: "
+                                          "use pkdg_build_lists_* and pkdg_gravity_eval_range)");
     }
     CK(cudaSetDevice(ctx->device));
     if (!ctx->own_stream) CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
@@ -1109,7 +1128,9 @@ pkdg_status pkdg_gravity_eval_tree_host(pkdg_ctx* ctx, const pkdg_particles* Ph,
         CK(h2d(ctx->t_bfirst, Bh->first, 4 * nb, sa)); CK(h2d(ctx->t_bcount, Bh->count, 4 * nb, sa));
         CK(h2d(ctx->e2e_xyzm, Ph->xyzm, sizeof(float) * 4 * np, sb));
         CK(cudaEventRecord(ctx->t_ev[0], sb));
-        // leaf_rank[cell of bucket b] = b, then the walk (P-P entries as bucket references)
+        // leaf_rank[cell of bucket b] = b, then the walk (P-P entries as bucket references).  A cell no bucket names
+        // keeps 0x7f7f7f7f, which the packer counts as a bad entry (it cannot happen after the checks above).
+        CK(cudaMemsetAsync(ctx->t_rank, 0x7f, sizeof(int32_t) * (size_t)ncell, sa));
         pkdg_leaf_rank_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, sa>>>(ctx->t_sink, nb, ctx->t_rank);
         ctx->launches++;
         pkdg_tree Td = {ctx->t_first, ctx->t_count, ctx->t_end, ctx->t_isleaf, ctx->t_bblo, ctx->t_bbhi, ctx->t_rank, ncell};

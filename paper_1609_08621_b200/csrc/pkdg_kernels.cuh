@@ -1304,7 +1304,10 @@ struct __align__(16) WalkNode {     // first 32-byte sector: what every visit re
     float hiy, hiz, bmax, pad;
 };
 
-__global__ void pkdg_walk_nodes_kernel(const TreeView T, double theta, WalkNode* __restrict__ nodes) {
+// A subtree end outside (k, n_cells] would stall the walk (k = end must advance) or send it out of the array: it is
+// clamped into that range and counted as a bad entry, like every other malformed input of the library.
+__global__ void pkdg_walk_nodes_kernel(const TreeView T, double theta, WalkNode* __restrict__ nodes,
+                                       DevStats* __restrict__ stats) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= T.n_cells) return;
     const float* r = T.rec + k * (int64_t)T.stride;
@@ -1315,7 +1318,9 @@ __global__ void pkdg_walk_nodes_kernel(const TreeView T, double theta, WalkNode*
     w.hix = T.bbhi[3 * k]; w.hiy = T.bbhi[3 * k + 1]; w.hiz = T.bbhi[3 * k + 2];
     const bool leaf = T.isleaf[k] != 0;
     w.count = (T.count[k] & 0x7fffffff) | (leaf ? (int32_t)0x80000000u : 0);
-    w.end = T.end[k];
+    const int64_t e = T.end[k];
+    w.end = (int32_t)(e <= k ? k + 1 : e > T.n_cells ? T.n_cells : e);
+    if ((int64_t)w.end != e && stats) atomicAdd(&stats->bad_entries, 1ull);
     w.entry = (leaf && T.leaf_rank) ? T.leaf_rank[k] : T.first[k];
     w.pad = 0.0f;
     nodes[k] = w;
@@ -1332,10 +1337,15 @@ __global__ void pkdg_walk_kernel(const WalkNode* __restrict__ nodes, int64_t n_c
                                  const int32_t* __restrict__ sink_cell, int64_t n_sinks, double theta,
                                  double eps, int64_t* __restrict__ pp_len, int64_t* __restrict__ pc_len,
                                  const int64_t* __restrict__ pp_off, const int64_t* __restrict__ pc_off,
-                                 int32_t* __restrict__ pp_idx, int32_t* __restrict__ pc_idx) {
+                                 int32_t* __restrict__ pp_idx, int32_t* __restrict__ pc_idx,
+                                 DevStats* __restrict__ stats) {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_sinks) return;
     const int64_t cb = sink_cell[s];
+    if (cb < 0 || cb >= n_cells) {   // not a cell of this tree: empty lists, one bad entry (counted by the count pass)
+        if (!FILL) { pp_len[s] = 0; pc_len[s] = 0; if (stats) atomicAdd(&stats->bad_entries, 1ull); }
+        return;
+    }
     const float4* nq = reinterpret_cast<const float4*>(nodes);
     const float4 b0 = __ldg(nq + 4 * cb), b1 = __ldg(nq + 4 * cb + 2), b2 = __ldg(nq + 4 * cb + 3);
     const double bx = b0.x, by = b0.y, bz = b0.z, bmaxB = b2.z;

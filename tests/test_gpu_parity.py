@@ -643,6 +643,33 @@ def test_device_list_construction_is_bit_exact(ctx, torch, cfg1):
         _device_lists(ctx, torch, p, p.tree["leaf_cell"], -1.0, p.eps)
 
 
+def test_device_walk_survives_malformed_trees(ctx, torch, cfg1):
+    """A subtree end that does not advance and a sink that is no cell of the tree neither hang the walk nor send it
+    out of bounds: the walk finishes, the sink gets empty lists, and pkdg_get_stats counts both as bad entries."""
+    import copy
+    p = cfg1
+    lc = p.tree["leaf_cell"].astype(np.int32)
+    want = _device_lists(ctx, torch, p, lc, p.theta, p.eps)
+    assert ctx.get_stats()["bad_entries"] == 0
+    # sinks outside [0, n_cells)
+    sc = lc.copy(); sc[5] = p.cells.shape[0]; sc[9] = -3
+    got = _device_lists(ctx, torch, p, sc, p.theta, p.eps)
+    assert ctx.get_stats(check=False)["bad_entries"] == 2
+    lp, lq = np.diff(got[0]), np.diff(want[0])
+    assert lp[5] == 0 and lp[9] == 0 and np.diff(got[2])[5] == 0 and np.diff(got[2])[9] == 0
+    keep = np.ones(len(lc), bool); keep[[5, 9]] = False
+    assert np.array_equal(lp[keep], lq[keep])
+    # end[k] <= k (would never advance) and end[k] > n_cells (would leave the array)
+    q = copy.copy(p); q.tree = dict(p.tree); e = p.tree["end"].copy()
+    k_self = int(np.flatnonzero(p.tree["isleaf"] != 0)[3]); e[k_self] = k_self
+    k_far = int(np.flatnonzero(p.tree["isleaf"] != 0)[-1]); e[k_far] = p.cells.shape[0] + 1000
+    q.tree["end"] = e
+    got = _device_lists(ctx, torch, q, lc, p.theta, p.eps)      # returns: no hang; leaves' ends clamp to k + 1 / n_cells
+    assert ctx.get_stats(check=False)["bad_entries"] == 2
+    for a, b in zip(got, want):                                  # for a leaf, k + 1 (or n_cells for the last one) is the true end
+        assert np.array_equal(a, b)
+
+
 def test_tree_host_call_builds_lists_and_evaluates(ctx, torch, cfg1):
     """pkdg_gravity_eval_tree_host: every buffer on the host, lists built on the device.  Same bits as the resident
     call on the host generator's leaf-form lists (the device walk is bit-identical and ranges do not change a
@@ -666,16 +693,20 @@ def test_tree_host_call_builds_lists_and_evaluates(ctx, torch, cfg1):
             assert st["chunks"] == n_ranges and st["n_buckets"] == p.n_buckets
         ea, ep = rel_errors(out, ref)
         assert ea.max() <= TOL and ep.max() <= TOL, (p.name, ea.max(), ep.max())
-    # a subset of the buckets (a contiguous run): other rows untouched
+    # a subset of the leaves is refused (the walk names P-P source leaves by bucket index: every leaf must be a
+    # bucket), and so is a bucket that is not the particle run of the leaf cell it names; nothing is written
     p = cfg1
     tr = p.tree
     tree = {k: np.ascontiguousarray(tr[k]) for k in ("first", "count", "end", "isleaf", "bblo", "bbhi")}
-    b0, b1 = 100, 300
     out = np.full((p.n, 4), np.nan, np.float32)
-    ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, np.ascontiguousarray(p.first[b0:b1]), np.ascontiguousarray(p.count[b0:b1]),
-                               np.ascontiguousarray(tr["leaf_cell"][b0:b1].astype(np.int32)), p.theta, p.eps, out, n_ranges=2)
-    lo, hi = int(p.first[b0]), int(p.first[b1 - 1] + p.count[b1 - 1])
-    assert np.isfinite(out[lo:hi]).all() and np.isnan(out[:lo]).all() and np.isnan(out[hi:]).all()
+    for b0, b1 in ((100, 300), (0, p.n_buckets - 1), (1, p.n_buckets)):
+        with pytest.raises(binding.PkdgError, match="ALL leaves"):
+            ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, np.ascontiguousarray(p.first[b0:b1]), np.ascontiguousarray(p.count[b0:b1]),
+                                       np.ascontiguousarray(tr["leaf_cell"][b0:b1].astype(np.int32)), p.theta, p.eps, out, n_ranges=2)
+    wrong = np.ascontiguousarray(tr["leaf_cell"].astype(np.int32)); wrong[7] = 0   # the root is not a leaf
+    with pytest.raises(binding.PkdgError, match="leaf cell"):
+        ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, p.first, p.count, wrong, p.theta, p.eps, out)
+    assert np.isnan(out).all()
     with pytest.raises(binding.PkdgError):      # buckets out of order
         ctx.gravity_eval_tree_host(p.xyzm, p.cells, tree, np.ascontiguousarray(p.first[::-1]), np.ascontiguousarray(p.count[::-1]),
                                    np.ascontiguousarray(tr["leaf_cell"][::-1].astype(np.int32)), p.theta, p.eps, out)
