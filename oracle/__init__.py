@@ -64,6 +64,8 @@ def lib():
         L.orc_interactions.argtypes = [c_int64, c_void_p, c_void_p]
         L.orc_chunk_bounds.restype = c_int64
         L.orc_chunk_bounds.argtypes = [c_int64, c_void_p, c_void_p, c_int64, c_void_p]
+        L.orc_walk_lists.restype = c_int
+        L.orc_walk_lists.argtypes = [c_int64] + [c_void_p] * 10 + [c_int64, c_double, c_double, c_int, c_void_p, c_void_p]
         _lib = L
     return _lib
 
@@ -246,3 +248,32 @@ def chunk_bounds(pp_off, pc_off, max_entries: int) -> np.ndarray:
     bounds = np.zeros(nb + 2, np.int64)
     nc = lib().orc_chunk_bounds(nb, _p(pp_off), _p(pc_off), int(max_entries), _p(bounds))
     return bounds[: nc + 1].copy()
+
+
+def walk_lists(tree, cells, sink_cell, theta, eps, four=False, xyzm=None, leaf_rank=None):
+    """The tree walk written out (readings A6, A22): lists of every sink cell.
+
+    tree: dict of first, count, end, isleaf (int32 [n_cells], depth-first pre-order, subtree of k = [k, end[k]))
+    and bblo, bbhi (float32 [n_cells, 3]); cells: canonical records (COM, b_max).  sink_cell: the sink cells
+    (buckets, or group cells).  Returns [(off, idx)] for P-P, P-C (and C-P, C-C with four=True; xyzm needed).
+    leaf_rank: a rejected leaf's P-P entry is leaf_rank[k] (one bucket reference) instead of its particles."""
+    i32 = lambda a: _c(a, np.int32)
+    first, count, end, isleaf = i32(tree["first"]), i32(tree["count"]), i32(tree["end"]), i32(tree["isleaf"])
+    bblo, bbhi = _c(tree["bblo"], np.float32), _c(tree["bbhi"], np.float32)
+    cells = _c(cells, np.float32)
+    assert cells.ndim == 2 and cells.shape[1] == 36 and cells.shape[0] == first.shape[0]
+    sink_cell = i32(sink_cell); ns = sink_cell.shape[0]
+    xyzm = _c(xyzm, np.float32); leaf_rank = None if leaf_rank is None else i32(leaf_rank)
+    assert not four or xyzm is not None
+    nl = 4 if four else 2
+    off = [np.zeros(ns + 1, np.int64) for _ in range(nl)]
+    OffArr = c_void_p * 4
+    offp = OffArr(*([o.ctypes.data for o in off] + [None] * (4 - nl)))
+    args = (first.shape[0], _p(first), _p(count), _p(end), _p(isleaf), _p(cells), _p(bblo), _p(bbhi), _p(xyzm),
+            _p(leaf_rank), _p(sink_cell), ns, float(theta), float(eps), 1 if four else 0)
+    if lib().orc_walk_lists(*args, offp, None) != 0:
+        raise ValueError("malformed tree: a sink cell or an end[] out of range")
+    idx = [np.empty(int(o[-1]), np.int32) for o in off]
+    idxp = OffArr(*([i.ctypes.data for i in idx] + [None] * (4 - nl)))
+    lib().orc_walk_lists(*args, offp, idxp)
+    return list(zip(off, idx))

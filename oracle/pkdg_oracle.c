@@ -21,7 +21,10 @@
  * numpy; momentum conservation; Legendre series of an off-centre point mass;
  * (b/d)^5 convergence of a cloud's P-C field towards its direct sum; gradient
  * versus central differences; rotation covariance; trace invariance; tree +
- * lists versus direct summation; the paper's 655 -> 640 + 15 tile example.
+ * lists versus direct summation; the paper's 655 -> 640 + 15 tile example; the
+ * tree walk (orc_walk_lists, at the end of this file) against hand-built trees
+ * on either side of every threshold and a numpy evaluation of the acceptance
+ * inequality for every (sink, cell) pair.
  * No function here is "parity unpinned".
  *
  * No blocking, fusion or reordering: every loop is the definition written out.
@@ -537,4 +540,142 @@ int64_t orc_chunk_bounds(int64_t n_buckets, const int64_t *pp_off, const int64_t
     }
     bounds[++nc] = n_buckets;
     return nc;
+}
+
+/* ---------------------------------------------------------------------------
+ * Tree walk: which cells and particles end up on which list of a sink.
+ *
+ * PAPER.md:L65 (sec 3.1): the walk starts at the root with a checklist; every
+ * checklist element gets a case value -- open it, put it on the PP list, on the
+ * PC list, on the CC list, on the CP list, or keep it for the sink's children;
+ * cells are visited node-left-right.  L69: the opening radius of a cell is
+ * RO = b_max / theta; a cell-cell interaction is allowed when the centres are
+ * further apart than 1.5 RO_sink + RO_source, and multipoles are only used
+ * when the bounding boxes are at least two softening lengths apart; a particle
+ * is a source with RO_source = 0 (fn 2); the walk for a sink stops at group
+ * size g and resolves what is left into the lists.  The paper prints the CC /
+ * CP radius only; readings A6 (two lists) and A22 (four lists) fix
+ * the rest, and this is those readings written out as a RECURSIVE descent over
+ * explicit children -- one sink at a time, no checklist inheritance, no skip
+ * pointers -- so that each decision can be read off against the inequality:
+ *
+ *   visit(k):  if k may act on the sink as a whole (rule below) -> list it, done
+ *              else if k is a leaf -> its particles go on a particle list, done
+ *              else visit every child of k, left to right.
+ *
+ * Two lists (A6).  Cell k is a P-C source of sink cell B  iff
+ *     k != B,  count[k] >= 2,
+ *     |COM_B - COM_k| > b_max,B + RO_k,        RO_k = b_max,k / theta,
+ *     gap(bbox_B, bbox_k) >= 2 eps.
+ *   A rejected leaf's particles all go on the P-P list (B's own included; the
+ *   evaluation skips i = j by index).
+ * Four lists (A22).  With RO_B = b_max,B / theta:
+ *     C-C  iff k != B, count[k] >= 2, gap >= 2 eps, |COM_B - COM_k| > 1.5 RO_B + RO_k
+ *     P-C  else iff the two-list rule holds
+ *     a rejected leaf's particles one by one (RO_source = 0):
+ *     C-P  iff j is not in B, |COM_B - x_j| > 1.5 RO_B, gap(bbox_B, x_j) >= 2 eps
+ *     P-P  else.
+ * gap(.,.) is the Euclidean distance between two axis-aligned boxes (0 when they
+ * touch or overlap), compared squared.  All arithmetic in fp64 on the fp32
+ * inputs.  The tree comes as arrays in depth-first pre-order: cell k's subtree
+ * is cells [k, end[k]), so its children are k + 1, end[k + 1], end[end[k + 1]],
+ * ... below end[k].  The sink is ANY cell: a bucket (lists per bucket), or a
+ * cell of up to g particles (lists per group, L69).
+ *
+ * Pins (tests/test_oracle_walk_pins.py): hand-built three-cell trees on either
+ * side of every threshold (distance, 2 eps gap, count = 1, k = B, 1.5 RO_B);
+ * on N ~ 500 a numpy evaluation of the inequality for every (sink, cell) pair:
+ * every listed cell satisfies it, no ancestor of a listed cell or listed leaf
+ * does (the list is the coarsest admissible cover), every particle is covered
+ * exactly once.
+ * ------------------------------------------------------------------------- */
+typedef struct {
+    int64_t n_cells;
+    const int32_t *first, *count, *end, *isleaf;
+    const float *rec;   /* canonical records, stride 36: COM at [0..2], b_max at [35] */
+    const float *bblo, *bbhi;
+    const float *xyzm;  /* four-list walk only */
+    const int32_t *leaf_rank; /* two-list walk: non-NULL = a leaf's P-P entry is leaf_rank[k], once */
+    double theta, eps;
+    int64_t B;          /* the sink cell */
+    int four;           /* 0: lists 0 = P-P, 1 = P-C;  1: also 2 = C-P, 3 = C-C */
+    int32_t *out[4];    /* where to write (NULL = count only) */
+    int64_t n[4];       /* entries so far */
+} orc_walk;
+
+static void walk_emit(orc_walk *w, int list, int32_t v) {
+    if (w->out[list]) w->out[list][w->n[list]] = v;
+    w->n[list]++;
+}
+
+static double box_gap2(const float *loA, const float *hiA, const float *loB, const float *hiB) {
+    double g2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        double g = 0.0;
+        if ((double)loA[a] - (double)hiB[a] > g) g = (double)loA[a] - (double)hiB[a];   /* A lies above B */
+        if ((double)loB[a] - (double)hiA[a] > g) g = (double)loB[a] - (double)hiA[a];   /* A lies below B */
+        g2 += g * g;
+    }
+    return g2;
+}
+
+static double centre_dist(const float *a, const float *b) {
+    double dx = (double)a[0] - (double)b[0], dy = (double)a[1] - (double)b[1], dz = (double)a[2] - (double)b[2];
+    return sqrt(dx * dx + dy * dy + dz * dz);
+}
+
+/* 0: k may not act on the sink as a whole; 1: P-C; 3: C-C (four-list walk only) */
+static int walk_cell_rule(const orc_walk *w, int64_t k) {
+    if (k == w->B || w->count[k] < 2) return 0;
+    const float *rB = w->rec + 36 * w->B, *rk = w->rec + 36 * k;
+    const double two_eps = 2.0 * w->eps;
+    if (box_gap2(w->bblo + 3 * k, w->bbhi + 3 * k, w->bblo + 3 * w->B, w->bbhi + 3 * w->B) < two_eps * two_eps) return 0;
+    const double d = centre_dist(rB, rk);
+    const double RO_k = (double)rk[35] / w->theta, RO_B = (double)rB[35] / w->theta;
+    if (w->four && d > 1.5 * RO_B + RO_k) return 3;
+    if (d > (double)rB[35] + RO_k) return 1;
+    return 0;
+}
+
+static void walk_visit(orc_walk *w, int64_t k) {
+    const int rule = walk_cell_rule(w, k);
+    if (rule) { walk_emit(w, rule, (int32_t)k); return; }
+    if (w->isleaf[k]) {
+        if (!w->four && w->leaf_rank) { walk_emit(w, 0, w->leaf_rank[k]); return; }
+        for (int32_t t = 0; t < w->count[k]; ++t) {
+            const int32_t j = w->first[k] + t;
+            int cp = 0;
+            if (w->four && k != w->B) {   /* a source particle: RO_source = 0, its box is the point itself */
+                const float *xj = w->xyzm + 4 * (int64_t)j, *rB = w->rec + 36 * w->B;
+                const double two_eps = 2.0 * w->eps, RO_B = (double)rB[35] / w->theta;
+                cp = centre_dist(rB, xj) > 1.5 * RO_B &&
+                     box_gap2(xj, xj, w->bblo + 3 * w->B, w->bbhi + 3 * w->B) >= two_eps * two_eps;
+            }
+            walk_emit(w, cp ? 2 : 0, j);
+        }
+        return;
+    }
+    for (int64_t c = k + 1; c < w->end[k]; c = w->end[c]) walk_visit(w, c);   /* the children, left to right */
+}
+
+/* Lists of n_sinks sink cells.  off[q] = [n_sinks + 1] int64 (written), idx[q] = entries (NULL: only the offsets
+ * are computed -- call once to size, once to fill).  q = 0 P-P, 1 P-C, and with four != 0 also 2 C-P, 3 C-C.
+ * Returns 0, or -1 for a malformed tree (a sink or an end[] out of range). */
+int orc_walk_lists(int64_t n_cells, const int32_t *first, const int32_t *count, const int32_t *end,
+                   const int32_t *isleaf, const float *rec, const float *bblo, const float *bbhi,
+                   const float *xyzm, const int32_t *leaf_rank, const int32_t *sink_cell, int64_t n_sinks,
+                   double theta, double eps, int four, int64_t *const off[4], int32_t *const idx[4]) {
+    const int nl = four ? 4 : 2;
+    for (int64_t k = 0; k < n_cells; ++k)
+        if (end[k] <= k || end[k] > n_cells) return -1;
+    for (int q = 0; q < nl; ++q) off[q][0] = 0;
+    for (int64_t s = 0; s < n_sinks; ++s) {
+        if (sink_cell[s] < 0 || sink_cell[s] >= n_cells) return -1;
+        orc_walk w = {n_cells, first, count, end, isleaf, rec, bblo, bbhi, xyzm, leaf_rank, theta, eps, sink_cell[s],
+                      four, {0, 0, 0, 0}, {0, 0, 0, 0}};
+        for (int q = 0; q < nl; ++q) w.out[q] = idx && idx[q] ? idx[q] + off[q][s] : 0;
+        if (n_cells > 0) walk_visit(&w, 0);
+        for (int q = 0; q < nl; ++q) off[q][s + 1] = off[q][s] + w.n[q];
+    }
+    return 0;
 }

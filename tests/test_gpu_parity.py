@@ -614,26 +614,33 @@ def _device_lists(ctx, torch, p, sink_cell, theta, eps, flags=0):
 
 def test_device_list_construction_is_bit_exact(ctx, torch, cfg1):
     """the tree walk on the device (pkdg_build_lists_*) gives the SAME offsets and the
-    SAME indices as the host generator (integer work: bit-exact), for per-bucket lists, group-shared lists and
-    leaf-form P-P entries; theta = 0.7 and 0.55; octree and binary trees; the lists then evaluate to the same bits."""
+    SAME indices as the ORACLE's walk (oracle.walk_lists: the recursive statement of PAPER.md:L65-69 / readings A6,
+    pinned in tests/test_oracle_walk_pins.py) -- integer work, bit-exact -- for per-bucket lists, group-shared lists
+    and leaf-form P-P entries; theta = 0.7 and 0.55; octree and binary trees.  The input generator's lists (what the
+    other parity tests evaluate) are compared with the same oracle walk here at these sizes too."""
+    import oracle
     from paper_1609_08621_b200 import binding, inputs
-    from gpu_util import run_resident
+    flat = lambda w: (w[0][0], w[0][1], w[1][0], w[1][1])
     for p, theta in ((cfg1, 0.7), (inputs.config2(n=1 << 15), 0.7), (inputs.config3(32), 0.55), (inputs.config3(64), 0.7)):
         if theta != p.theta:
             p = inputs.with_lists(p, theta, p.eps)
+        want = flat(oracle.walk_lists(p.tree, p.cells, p.tree["leaf_cell"], theta, p.eps))
         got = _device_lists(ctx, torch, p, p.tree["leaf_cell"], theta, p.eps)
-        for a, b, name in zip(got, (p.pp_off, p.pp_idx, p.pc_off, p.pc_idx), ("pp_off", "pp_idx", "pc_off", "pc_idx")):
+        for a, b, c, name in zip(got, want, (p.pp_off, p.pp_idx, p.pc_off, p.pc_idx), ("pp_off", "pp_idx", "pc_off", "pc_idx")):
             assert a.dtype == b.dtype and np.array_equal(a, b), (p.name, name)
+            assert np.array_equal(c, b), (p.name, name, "generator")
         # group-shared lists
         gc, gf, gn = inputs.build_groups(p)
-        want = inputs.build_group_lists(p, gc, theta, p.eps)
+        want = flat(oracle.walk_lists(p.tree, p.cells, gc, theta, p.eps))
         got = _device_lists(ctx, torch, p, gc, theta, p.eps)
         for a, b in zip(got, want):
             assert np.array_equal(a, b), p.name
         # leaf-form entries: one bucket reference per leaf
-        lo, li = inputs.pp_leaves(p.n, p.first, p.count, p.pp_off, p.pp_idx)
+        rank = (np.cumsum(p.tree["isleaf"] != 0) - 1).astype(np.int32)
+        want = flat(oracle.walk_lists(p.tree, p.cells, p.tree["leaf_cell"], theta, p.eps, leaf_rank=rank))
         got = _device_lists(ctx, torch, p, p.tree["leaf_cell"], theta, p.eps, flags=binding.PP_LEAVES)
-        assert np.array_equal(got[0], lo) and np.array_equal(got[1], li) and np.array_equal(got[3], p.pc_idx)
+        for a, b in zip(got, want):
+            assert np.array_equal(a, b), (p.name, "leaf references")
     # empty sink set and bad arguments
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     p = cfg1
