@@ -65,7 +65,7 @@ def slice_lists(pp_off, pp_idx, pc_off, pc_idx, b0: int, b1: int):
             return None, None
         off = np.asarray(off)
         lo, hi = int(off[b0]), int(off[b1])
-        return (off[b0:b1 + 1] - lo).astype(np.int64), idx[lo:hi]
+        return (off[b0:b1 + 1] - lo).astype(np.int64), (None if idx is None else idx[lo:hi])   # idx None: offsets only
     ppo, ppi = cut(pp_off, pp_idx)
     pco, pci = cut(pc_off, pc_idx)
     return ppo, ppi, pco, pci

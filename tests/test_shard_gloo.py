@@ -33,9 +33,13 @@ def _worker(rank, world, port, ret):
         ref_p = inputs.config1(2048, seed=11)                     # what rank 0 owns (built everywhere only to compare)
         # the function bench.py --gpus N calls: rank 0's arrays are broadcast, every rank takes its piece
         g, piece = multigpu.distribute(ref_p if rank == 0 else None, dist, rank, world, "cpu", torch)
-        for k in ("xyzm", "cells", "first", "count", "pp_off", "pp_idx", "pc_off", "pc_idx"):
+        for k in ("xyzm", "cells", "first", "count", "pp_off", "pc_off"):
             assert np.array_equal(getattr(g, k).numpy(), getattr(ref_p, k)), k   # the broadcast delivered rank 0's bits
         assert g.eps == ref_p.eps
+        # list entries are NOT replicated: only the owner holds them whole, every rank holds its own range's
+        assert (g.pp_idx is None and g.pc_idx is None) if rank else (g.pp_idx is not None and g.pc_idx is not None)
+        for off, got, full in ((ref_p.pp_off, piece.pp_idx, ref_p.pp_idx), (ref_p.pc_off, piece.pc_idx, ref_p.pc_idx)):
+            assert np.array_equal(got.numpy(), full[off[piece.b0]:off[piece.b1]])
         # every rank derives the same cut
         tb = torch.from_numpy(piece.bounds.copy())
         tmax = tb.clone(); tmin = tb.clone()
