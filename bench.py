@@ -139,6 +139,16 @@ def oracle_sample(p, target_s: float, seed: int = 0):
     return inter / dt, dt, len(sel), inter, oracle.num_threads()
 
 
+def parallelism_string(world, scaling):
+    """What `config.parallelism` says; the same text in both arms (the arms are compared on `config`)."""
+    if world == 1:
+        return "1 GPU"
+    if scaling == "weak":
+        return f"{world} independent replicas"
+    return (f"{world} ranks, contiguous cost-balanced bucket ranges (shard.rank_piece), arrays replicated by one NCCL "
+            f"broadcast, no data-path collective")
+
+
 def run_reference(args, rank, world):
     if rank != 0:
         return
@@ -155,7 +165,7 @@ def run_reference(args, rank, world):
     line = {"impl": "reference", "metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
             "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(p, args.ng),
+            "config": dict(workload_config(p, args.ng), parallelism=parallelism_string(world, args.scaling)),
             "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -280,6 +290,8 @@ def run_ours(args, rank, world, local_rank):
     sampler.start()
     ms_step = timed(step, args.steps)
     clocks = sampler.stop()
+    sampler_x = ClockSampler(torch, local_rank)   # the extra keys below are timed too: their own clock record
+    sampler_x.start()
     n_eval, eval_ms_total, fix_ms_total = ctx.profile_read()
     ctx.profile_enable(False)
     launches = (ctx.launch_count() - launches0) // args.steps
@@ -636,6 +648,7 @@ def run_ours(args, rank, world, local_rank):
                        "criterion; every bucket keeps its own local expansion (no hierarchical sink side)"}
         del df, d_centre
 
+    clocks_x = sampler_x.stop()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -666,19 +679,51 @@ def run_ours(args, rank, world, local_rank):
                         "sample": f"{nsel} of {p.n_buckets} buckets evenly spread in tree order "
                                   f"({inter_s} interactions, {dt:.1f} s)"}
 
-    cfg["parallelism"] = (f"{world} ranks, contiguous cost-balanced bucket ranges (shard.rank_piece), arrays replicated by "
-                          f"one NCCL broadcast, no data-path collective") if strong else \
-                         ("1 GPU" if world == 1 else f"{world} independent replicas")
+    # ---- the other BASELINE.json configs that fit a default run (north_star: "uniform and clustered particle sets"):
+    # config 2 and three config-4 shapes through the resident call, kernel time from the library's CUDA events, each
+    # with its own clock record and a bounded oracle sample.  Not the headline: parity-test configs, measured.
+    configs = None
+    if world == 1 and not args.no_configs:
+        from paper_1609_08621_b200 import inputs as _inputs
+        configs = []
+        cases = [("configs[1]: N=2^20 Plummer mix, binary tree, theta=0.7", lambda: _inputs.config2()),
+                 ("configs[3]: 65536 buckets, P-P only, L_pp=4096", lambda: _inputs.config4(65536, 4096, 0)),
+                 ("configs[3]: 8192 buckets, P-C only, L_pc=2048", lambda: _inputs.config4(8192, 0, 2048)),
+                 ("configs[3]: 16384 buckets, fused, L_pp=L_pc=512", lambda: _inputs.config4(16384, 512, 512))]
+        keep = ("case", "n_particles", "n_buckets", "I_pp", "I_pc", "mean_L_pp", "mean_L_pc", "kernel_ms_median",
+                "step_ms_median", "interactions_per_s", "frac_fp32_fma_peak", "fixup_sinks", "clocks", "max_rel_err_acc",
+                "max_rel_err_pot", "n_sampled_particles", "oracle_sample")
+        for name, make in cases:
+            t0 = time.time()
+            q = make()
+            ln = report_case(name, q, ctx, torch, binding, peak_tflops, 40, flags, args.configs_cpu_seconds, quiet=True,
+                             modes=False)
+            c = {k: ln[k] for k in keep if k in ln}
+            c["mean_bucket_occupancy"] = round(float(q.count.mean()), 2)
+            c["gen_seconds"] = round(time.time() - t0 - 0.0, 1)
+            configs.append(c)
+            del q
+
+    cfg["parallelism"] = parallelism_string(world, args.scaling)
     line = {"metric": "P-P+P-C interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
             "steps": args.steps, "warmup": warm, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "strong" if (strong or world == 1) else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": cfg, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "config": cfg, "clocks": clocks, "clocks_extra_keys": clocks_x, "configs": configs, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu_baseline, "fixup": fixup, "rank_cost_shares": shares,
             "flops_per_s": flops / (ms_step * 1e-3), "frac_fp32_fma_peak": flops / (ms_step * 1e-3) / 1e12 / (peak_tflops * world),
             "paper_convention_tflops": (PAPER_F_PP * tot_pp + PAPER_F_PC * tot_pc) / (ms_step * 1e-3) / 1e12,
             "interactions_per_s": {"pp": tot_pp / (ms_step * 1e-3), "pc": tot_pc / (ms_step * 1e-3)},
             "gen_seconds": round(gen_s, 1), "flags": args.flags, "pp_leaves": leaves, "group_lists": groups,
             "device_lists": devlists, "fmm": fmm}
+    # `e2e` stays the plain call on the headline lists (the slowest host-buffer path: 2.2 GB of lists cross PCIe every
+    # step); the other host-buffer calls measured above move fewer bytes for the same forces -- name the fastest
+    cands = [("e2e", e2e), ("pp_leaves.e2e", (leaves or {}).get("e2e")), ("group_lists.e2e", (groups or {}).get("e2e")),
+             ("device_lists.tree_host_call", (devlists or {}).get("tree_host_call"))]
+    cands = [(k, v) for k, v in cands if v]
+    if cands:
+        k_best, v_best = min(cands, key=lambda kv: kv[1]["ms_per_step"])
+        line["e2e_best"] = {"key": k_best, "ms_per_step": v_best["ms_per_step"], "h2d_bytes_per_step": v_best.get("h2d_bytes_per_step"),
+                            "note": "fastest of the library's host-buffer calls on this workload; every candidate's own key has the details"}
     if fmm is not None:
         fmm["frac_fp32_fma_peak_local_kernel"] = fmm["local_expansion_tflops"] / peak_tflops
     if groups is not None:
@@ -695,8 +740,8 @@ def run_ours(args, rank, world, local_rank):
 # library's CUDA events, median of `reps`), the oracle timed and compared on a bounded sample of the
 # same buckets.  One JSON line per case; not the driver's contract line (that is the default mode).
 # ------------------------------------------------------------------------------------------------
-def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seconds, note=""):
-    dev = torch.device("cuda", 0)
+def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seconds, note="", quiet=False, modes=True):
+    dev = torch.device("cuda", torch.cuda.current_device())
     t = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     has_pc = p.cells is not None and p.cells.shape[0] > 0 and p.pc_off is not None
     d = dict(xyzm=t(p.xyzm), cells=t(p.cells) if has_pc else None, first=t(p.first), count=t(p.count),
@@ -708,6 +753,8 @@ def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seco
     for _ in range(3):
         step()
     torch.cuda.synchronize()
+    sampler = ClockSampler(torch, torch.cuda.current_device())   # clocks and throttle reasons over this case's timed calls
+    sampler.start()
     ctx.profile_read(); ctx.profile_enable(True)
     kms, sms_, fms = [], [], []
     for _ in range(reps):
@@ -732,7 +779,7 @@ def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seco
             "fixup_kernel_ms_median": float(np.median(fms))}
     line["frac_fp32_fma_peak_step"] = flops / (line["step_ms_median"] * 1e-3) / 1e12 / peak_tflops
     # the two other precision modes, timed whole-step (3 calls each): no fix-up at all; every sink in fp64
-    for key, fl in (("step_ms_no_fixup", flags | binding.NO_FIXUP), ("step_ms_fp64_all", flags | binding.FIXUP_ALL)):
+    for key, fl in ((("step_ms_no_fixup", flags | binding.NO_FIXUP), ("step_ms_fp64_all", flags | binding.FIXUP_ALL)) if modes else ()):
         ts = []
         for _ in range(3):
             e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -744,6 +791,7 @@ def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seco
         line[key] = float(np.median(ts))
     step()            # leave the default-mode result in `out` for the comparison below
     torch.cuda.synchronize()
+    line["clocks"] = sampler.stop()
     if cpu_seconds > 0:
         import oracle
         nb = p.n_buckets
@@ -772,7 +820,8 @@ def report_case(name, p, ctx, torch, binding, peak_tflops, reps, flags, cpu_seco
         line.update({"oracle_interactions_per_s": float(cost[sel].sum()) / dt, "oracle_cores": oracle.num_threads(),
                      "oracle_sample": f"{len(sel)} of {nb} buckets, {dt:.1f} s",
                      "max_rel_err_acc": float(ea.max()), "max_rel_err_pot": float(ep.max())})
-    print(json.dumps(line), flush=True)
+    if not quiet:
+        print(json.dumps(line), flush=True)
     del d, out
     torch.cuda.empty_cache()
     return line
@@ -923,6 +972,8 @@ def main():
     ap.add_argument("--no-groups", action="store_true", help="skip the extra group-shared-lists measurement")
     ap.add_argument("--no-fmm", action="store_true", help="skip the extra four-list (C-C / C-P local expansion) measurement")
     ap.add_argument("--no-device-lists", action="store_true", help="skip the extra device list-construction measurement")
+    ap.add_argument("--no-configs", action="store_true", help="skip the extra `configs` key (config 2 and three config-4 shapes)")
+    ap.add_argument("--configs-cpu-seconds", type=float, default=3.0, help="oracle sample per case of the `configs` key")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-chunk", type=int, default=1 << 23)

@@ -28,7 +28,7 @@ def test_reference_arm_prints_the_contract_line():
     assert d["impl"] == "reference" and d["dtype"] == "f64" and d["vs_baseline"] is None and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
-    assert "workload" in d["config"]
+    assert "workload" in d["config"] and d["config"]["parallelism"] == "1 GPU"   # the same key set as the product arm's config
 
 
 def test_reference_arm_other_ranks_exit_quietly():
@@ -54,7 +54,7 @@ import pytest
 def test_product_arm_line_on_gpu():
     """The product arm at a small lattice (same code path as the headline run): one JSON line with the
     keys the measurement contract asks for, a roofline fraction in (0, 1.05) and a counted launch number."""
-    r = _run(["--ng", "64", "--steps", "3", "--warmup", "3", "--cpu-seconds", "1"], timeout=600)
+    r = _run(["--ng", "64", "--steps", "3", "--warmup", "3", "--cpu-seconds", "1", "--configs-cpu-seconds", "1"], timeout=900)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1
@@ -71,3 +71,9 @@ def test_product_arm_line_on_gpu():
     assert d["e2e"]["value"] < d["value"]
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["pp_leaves"]["e2e"]["h2d_bytes_per_step"] < d["e2e"]["h2d_bytes_per_step"]
+    assert d["config"]["parallelism"] == "1 GPU" and "sm_mhz" in d["clocks_extra_keys"]
+    # the other configs, measured in the same run: each with its own clock record, a roofline fraction and parity
+    assert len(d["configs"]) == 4
+    for c in d["configs"]:
+        assert "sm_mhz" in c["clocks"] and 0.0 < c["frac_fp32_fma_peak"] < 1.05 and c["kernel_ms_median"] > 0
+        assert c["max_rel_err_acc"] <= 2e-5 and c["max_rel_err_pot"] <= 2e-5, c

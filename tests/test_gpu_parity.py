@@ -650,6 +650,33 @@ def test_device_list_construction_is_bit_exact(ctx, torch, cfg1):
         _device_lists(ctx, torch, p, p.tree["leaf_cell"], -1.0, p.eps)
 
 
+def test_two_contexts_on_two_devices_in_one_process(torch, cfg1):
+    """Function attributes (the dynamic shared-memory opt-in of the evaluation kernels) are per device and are set
+    per context; the static workspace of pkdg_gravity_eval_static exists once per device.  Two devices in one process
+    must therefore both work and agree bit for bit.  Skipped where only one GPU is visible."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    from paper_1609_08621_b200 import binding
+    from gpu_util import to_dev
+    p = cfg1
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            d = to_dev(p, torch, f"cuda:{dev}")
+            c = binding.Context(dev)
+            out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device=f"cuda:{dev}")
+            c.gravity_eval(d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"], d["pc_off"], d["pc_idx"],
+                           p.eps, out)
+            st_out = torch.full((p.n, 4), float("nan"), dtype=torch.float32, device=f"cuda:{dev}")
+            binding.gravity_eval_static(dev, d["xyzm"], d["cells"], d["first"], d["count"], d["pp_off"], d["pp_idx"],
+                                        d["pc_off"], d["pc_idx"], p.eps, st_out)
+            torch.cuda.synchronize(dev)
+            assert c.get_stats()["bad_entries"] == 0
+            outs.append((out.cpu().numpy(), st_out.cpu().numpy()))
+            c.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][0], outs[0][1]) and np.array_equal(outs[1][0], outs[1][1])
+
+
 def test_device_walk_survives_malformed_trees(ctx, torch, cfg1):
     """A subtree end that does not advance and a sink that is no cell of the tree neither hang the walk nor send it
     out of bounds: the walk finishes, the sink gets empty lists, and pkdg_get_stats counts both as bad entries."""
